@@ -1,0 +1,550 @@
+"""Pins for the CPU oracle.  CPU only.
+
+Each test checks oracle/ against something other than itself: values the paper prints (tests/golden/),
+closed forms, invariants, textbook / library routines (complex-exponential RoPE, torch's bf16 / fp8
+converters, Python list slicing), brute force on tiny inputs.  A plausible mistake anywhere in the oracle
+(dropped term, wrong sign or index, transposed operand, wrong pairing, off-by-one in the Delta rule)
+fails at least one of them.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import oracle as O
+from helpers import from_storage, golden, list_splice, rope_complex, to_storage
+from paper_2606_01065_b200 import synth
+
+H64 = synth.rope_inv_freq(64, 10000.0)
+
+
+# ----------------------------------------------------------------------------- small harness
+
+def run_oracle(dtype, pairing, Dc, Dr, P, L_old, dirs, rows_f64, repl_f64, inv_freq, mode=O.FRESH, seed=0,
+               scale=1.0, extra_pages=None):
+    """Build a shuffled paged pool holding rows_f64 [L_old, W], run the oracle, return (new rows [L_new, W] as
+    float64, BatchMap, old pool bytes, new pool bytes, stride)."""
+    rng = np.random.default_rng(seed)
+    n_old = -(-L_old // P)
+    grow = sum(d[2] for d in dirs)
+    n_pool = 2 * n_old + -(-grow // P) + 4 if extra_pages is None else n_old + extra_pages
+    perm = rng.permutation(n_pool).astype(np.int32)
+    pages, free = perm[:n_old], perm[n_old:]
+    if mode == O.ROTATE_ONLY:
+        free = (free.astype(np.int64)[:, None] * P + np.arange(P)[None, :]).reshape(-1).astype(np.int32)
+    W = Dc + Dr
+    stride = W * O.ELEM_BYTES[dtype]
+    pool = np.zeros((n_pool * P, stride), np.uint8)
+    pool[:] = rng.integers(0, 255, size=pool.shape, dtype=np.uint8) if dtype != O.F64 else 0
+    slot_old = pages.astype(np.int64)[np.arange(L_old) // P] * P + np.arange(L_old) % P
+    pool[slot_old] = to_storage(rows_f64, dtype, scale)
+    repl = to_storage(repl_f64, dtype, scale) if repl_f64 is not None and len(repl_f64) else np.zeros((1, stride), np.uint8)
+    full = []
+    row = 0
+    for (s, e, n) in dirs:
+        full.append((0, s, e, n, row, O.AMORTIZE))
+        row += n
+    bm = O.plan_batch(mode, P, [L_old], [0, n_old], pages, full, free)
+    assert bm.status == O.OK
+    old_flat = pool.reshape(-1)
+    new_flat = O.splice_layer(dtype, pairing, Dc, Dr, stride, inv_freq, scale, old_flat, repl.reshape(-1), bm)
+    new_pool = new_flat.reshape(pool.shape)
+    rm = bm.requests[0]
+    new_rows = from_storage(new_pool[rm.slot_new], dtype, scale)
+    return new_rows, bm, pool, new_pool, stride
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+# ----------------------------------------------------------------------------- P1: Delta / segment arithmetic
+
+def test_p1_paper_worked_example():
+    g = golden("paper_worked_example.txt")
+    pre, chunk, post, stub = g["pre_tokens"], g["chunk_tokens"], g["post_tokens"], g["stub_tokens"]
+    L_old = pre + chunk + post
+    segs = O.segments(L_old, [(pre, pre + chunk, stub, 0, O.AMORTIZE)])
+    assert L_old == 71 and segs.L_new == 25
+    assert segs.L_new - L_old == g["delta"] == -46
+    # (kind, src, dst, len, shift)
+    assert segs.as_tuples() == [(O.KEEP, 0, 0, 5, 0), (O.INSERT, 0, 5, 11, 0), (O.KEEP, 62, 16, 9, -46)]
+    # post tokens 62..70 -> 16..24
+    k = segs.as_tuples()[2]
+    assert [k[2] + q for q in range(k[3])] == list(range(16, 25))
+
+
+def test_p1_baseline_config_deltas():
+    # BASELINE.json configs 1-3: Delta = -568, -8064, cumulative (-1984, -18368, -18624), L_new = 112448
+    s = O.segments(4096, [(1000, 1600, 32, 0, 0)])
+    assert s.L_new - 4096 == -568
+    s = O.segments(32768, [(4096, 12288, 128, 0, 0)])
+    assert s.L_new - 32768 == -8064
+    L = 131072
+    s = O.segments(L, [(L // 16, L // 16 + 2048, 64, 0, 0), (L // 4, L // 4 + 16384, 0, 64, 0),
+                       (3 * L // 4, 3 * L // 4 + 512, 256, 64, 0)])
+    shifts = [t[4] for t in s.as_tuples() if t[0] == O.KEEP]
+    assert shifts == [0, -1984, -18368, -18624]
+    assert s.L_new == 112448
+    assert sum(t[3] for t in s.as_tuples() if t[0] == O.KEEP and t[4] != 0) == 103936  # SURVEY 8(d) moved rows
+    assert sum(t[3] for t in s.as_tuples() if t[0] == O.INSERT) == 320
+
+
+@pytest.mark.parametrize("seed", range(40))
+def test_p1_brute_force_list_slicing(seed):
+    """Edit shapes of the paper's randomised suite (1-2 spans, size U[8,200], |R| in
+    U[0, 2|span|], both signs) plus degenerate ones, against Python list slicing."""
+    rng = np.random.default_rng(seed)
+    L = int(rng.integers(1, 400))
+    k = int(rng.integers(0, 5))
+    cuts = np.sort(rng.integers(0, L + 1, size=2 * k))
+    dirs, row = [], 0
+    for j in range(k):
+        s, e = int(cuts[2 * j]), int(cuts[2 * j + 1])
+        n = int(rng.integers(0, 2 * (e - s) + 2)) if rng.random() < 0.8 else 0
+        dirs.append((s, e, n, row))
+        row += n
+    want = list_splice(L, dirs)
+    segs = O.segments(L, [(s, e, n, r, O.AMORTIZE) for (s, e, n, r) in dirs])
+    got = [None] * segs.L_new
+    for (kind, src, dst, ln, sh) in segs.as_tuples():
+        assert ln > 0
+        for q in range(ln):
+            assert got[dst + q] is None
+            got[dst + q] = ("o", src + q) if kind == O.KEEP else ("r", src + q)
+            if kind == O.KEEP:
+                assert (dst + q) - (src + q) == sh      # the rotation amount IS the position shift
+    assert got == want
+
+
+# ----------------------------------------------------------------------------- P11: allocation rules M1-M3
+
+@pytest.mark.parametrize("mode", [O.FRESH, O.INPLACE_MOVE, O.ROTATE_ONLY])
+@pytest.mark.parametrize("seed", range(25))
+def test_p11_maps_brute_force(mode, seed):
+    rng = np.random.default_rng(1000 + seed)
+    P = int(rng.choice([1, 2, 4, 8]))
+    n_req = int(rng.integers(1, 4))
+    seq_lens = [int(rng.integers(1, 90)) for _ in range(n_req)]
+    n_pages = [-(-L // P) for L in seq_lens]
+    pool_pages = sum(n_pages) * 3 + 40
+    perm = rng.permutation(pool_pages).astype(np.int32)
+    pages = perm[:sum(n_pages)]
+    free_pages = perm[sum(n_pages):]
+    free = free_pages if mode != O.ROTATE_ONLY else \
+        (free_pages.astype(np.int64)[:, None] * P + np.arange(P)[None, :]).reshape(-1).astype(np.int32)
+    pt = np.concatenate([[0], np.cumsum(n_pages)])
+    dirs, row = [], 0
+    per_req = []
+    for r, L in enumerate(seq_lens):
+        k = int(rng.integers(0, 4))
+        cuts = np.sort(rng.integers(0, L + 1, size=2 * k))
+        mine = []
+        for j in range(k):
+            s, e, n = int(cuts[2 * j]), int(cuts[2 * j + 1]), int(rng.integers(0, 12))
+            dirs.append((r, s, e, n, row, O.AMORTIZE))
+            mine.append((s, e, n, row))
+            row += n
+        per_req.append(mine)
+    bm = O.plan_batch(mode, P, seq_lens, pt, pages, dirs, free)
+    assert bm.status == O.OK
+    consumed = list(free[:bm.n_consumed])
+    used_free, all_released, live_slots = 0, [], []
+    for r, L in enumerate(seq_lens):
+        rm = bm.requests[r]
+        seq = list_splice(L, per_req[r])
+        assert rm.L_new == len(seq)
+        row_old = pages[pt[r]:pt[r + 1]]
+        idx_old = [int(row_old[t // P]) * P + t % P for t in range(L)]
+        assert list(rm.slot_old) == idx_old
+        assert list(O.slots_of(P, row_old, L)) == idx_old
+        if mode == O.ROTATE_ONLY:
+            # M3 by literal list slicing: kept tokens keep their slot, inserted rows take the next free SLOT ids
+            want, nfree = [], 0
+            for tok in seq:
+                if tok[0] == "o":
+                    want.append(idx_old[tok[1]])
+                else:
+                    want.append(int(free[used_free + nfree]))
+                    nfree += 1
+            assert list(rm.slot_new) == want
+            removed = sorted(set(range(L)) - {tok[1] for tok in seq if tok[0] == "o"})
+            assert list(rm.released) == [idx_old[t] for t in removed]
+            used_free += nfree
+        else:
+            n_old, n_new = n_pages[r], -(-rm.L_new // P)
+            if mode == O.FRESH:
+                keep = n_old if not per_req[r] else per_req[r][0][0] // P
+                want_pages = list(row_old[:keep]) + [int(x) for x in free[used_free:used_free + (0 if not per_req[r] else n_new - keep)]]
+                want_rel = [] if not per_req[r] else list(row_old[keep:])
+                used_free += 0 if not per_req[r] else n_new - keep
+            else:
+                keep = min(n_old, n_new)
+                want_pages = list(row_old[:keep]) + [int(x) for x in free[used_free:used_free + max(0, n_new - n_old)]]
+                want_rel = list(row_old[n_new:]) if n_new < n_old else []
+                used_free += max(0, n_new - n_old)
+            assert list(rm.new_pages) == want_pages
+            assert list(rm.released) == want_rel
+            assert list(rm.slot_new) == [int(want_pages[t // P]) * P + t % P for t in range(rm.L_new)]
+        live_slots += list(rm.slot_new)
+        all_released += list(rm.released)
+    assert used_free == bm.n_consumed
+    assert list(bm.released) == all_released
+    # every live new position maps to a distinct slot; released and live are disjoint
+    assert len(set(live_slots)) == len(live_slots)
+    if mode == O.ROTATE_ONLY:
+        assert not (set(all_released) & set(live_slots))
+    else:
+        live_pages = {s // P for s in live_slots}
+        assert not (set(int(x) for x in all_released) & live_pages)
+        assert set(int(x) for x in consumed) <= live_pages | set()
+
+
+def test_o1_validation_rules():
+    sl = [100, 50]
+    ok = [(0, 10, 20, 3, 0, 0), (0, 20, 30, 0, 3, 0), (1, 0, 50, 5, 3, 0)]
+    assert O.validate(sl, ok) == O.OK                                     # adjacency allowed
+    assert O.validate(sl, [(0, 10, 20, 0, 0, 0), (0, 15, 30, 0, 0, 0)]) == O.E_OVERLAP
+    assert O.validate(sl, [(0, 30, 40, 0, 0, 0), (0, 10, 20, 0, 0, 0)]) == O.E_UNSORTED
+    assert O.validate(sl, [(1, 0, 1, 0, 0, 0), (0, 10, 20, 0, 0, 0)]) == O.E_UNSORTED
+    assert O.validate(sl, [(0, 10, 101, 0, 0, 0)]) == O.E_RANGE
+    assert O.validate(sl, [(2, 0, 1, 0, 0, 0)]) == O.E_RANGE
+    assert O.validate(sl, [(0, 20, 10, 0, 0, 0)]) == O.E_INVALID
+    assert O.validate(sl, [(0, -1, 10, 0, 0, 0)]) == O.E_INVALID
+    assert O.validate(sl, [(0, 1, 10, -1, 0, 0)]) == O.E_INVALID
+    assert O.validate(sl, [(0, 1, 10, 0, 0, 7)]) == O.E_INVALID
+    assert O.validate(sl, [(0, 5, 5, 0, 0, 0), (0, 5, 5, 2, 0, 0), (0, 5, 9, 1, 2, 0)]) == O.OK   # no-op, insert, edit
+    assert O.validate(sl, []) == O.OK
+    # too few free ids
+    bm = O.plan_batch(O.FRESH, 4, [16], [0, 4], [0, 1, 2, 3], [(0, 4, 8, 0, 0, 0)], [9])
+    assert bm.status == O.E_NOFREE
+
+
+def test_forget_truncates():
+    segs = O.segments(100, [(10, 20, 4, 0, O.AMORTIZE), (50, 60, 3, 4, O.FORGET), (70, 80, 1, 7, O.AMORTIZE)])
+    assert segs.forget_trim == 50 - 6 and segs.L_new == 44
+    assert segs.as_tuples() == [(O.KEEP, 0, 0, 10, 0), (O.INSERT, 0, 10, 4, 0), (O.KEEP, 20, 14, 30, -6)]
+
+
+# ----------------------------------------------------------------------------- P2: identity
+
+@pytest.mark.parametrize("mode", [O.FRESH, O.INPLACE_MOVE, O.ROTATE_ONLY])
+def test_p2_identity(mode):
+    rng = np.random.default_rng(3)
+    L, Dc, Dr = 50, 8, 16
+    rows = rng.standard_normal((L, Dc + Dr))
+    rows[:, Dc:Dc + 4] = -0.0          # negative zeros in the rope band must survive a Delta=0 "rotation" (G19)
+    inv = synth.rope_inv_freq(Dr)
+    old_bytes = to_storage(rows, O.BF16)
+    # empty plan
+    new_rows, bm, pool, new_pool, _ = run_oracle(O.BF16, O.NEOX, Dc, Dr, 4, L, [], rows, None, inv, mode)
+    assert np.array_equal(pool, new_pool)
+    # zero-length no-op directive, and |R| == |span| (Delta = 0): every kept row is byte-identical
+    repl = rng.standard_normal((6, Dc + Dr))
+    for dirs in ([(20, 20, 0)], [(10, 16, 6)]):
+        new_rows, bm, pool, new_pool, _ = run_oracle(O.BF16, O.NEOX, Dc, Dr, 4, L, dirs, rows, repl, inv, mode)
+        rm = bm.requests[0]
+        assert rm.L_new == L
+        got = new_pool[rm.slot_new]
+        keep = np.ones(L, bool)
+        for (s, e, n) in dirs:
+            keep[s:s + n] = False
+        assert np.array_equal(got[keep], old_bytes[keep])
+        if dirs[0][2]:
+            assert np.array_equal(got[10:16], to_storage(repl, O.BF16))
+
+
+# ----------------------------------------------------------------------------- P4 / P8: rotation == fresh RoPE
+
+_PTS = golden("paper_rotation_points.txt")
+_DELTAS = [int(d) for d in _PTS["deltas"]] + [int(_PTS["delta_e2e_max"]), int(_PTS["delta_abs_max"]), 18624, 131071]
+
+
+@pytest.mark.parametrize("pairing", [O.NEOX, O.INTERLEAVED])
+@pytest.mark.parametrize("delta", _DELTAS + [-d for d in _DELTAS])
+def test_p4_rotation_equals_fresh_rope_f64(delta, pairing):
+    """K_pe[p] = R(p) k_raw[p]; after the splice K_pe_new[p + C] must equal R(p + C) k_raw[p] (Eq. 1 + closure,
+    PAPER.md:118-123, :509).  Sources include the paper's {10,100,1000,4000,8000,8836}."""
+    rng = np.random.default_rng(abs(delta))
+    Dc, Dr = 4, 64
+    src_pos = [int(s) for s in _PTS["sources"]]
+    L = max(src_pos) + 40
+    raw = rng.standard_normal((L, Dr))
+    kpe = rope_complex(raw, np.arange(L), H64, pairing)
+    rows = np.concatenate([rng.standard_normal((L, Dc)), kpe], axis=1)
+    if delta < 0:
+        dirs = [(2, 2 - delta, 0)] if 2 - delta < 10 else None
+        if dirs is None:      # large negative shift: prepend enough context so the span fits before p=10
+            pad = -delta
+            L2 = L + pad
+            raw2 = rng.standard_normal((L2, Dr))
+            raw2[pad:] = raw
+            kpe2 = rope_complex(raw2, np.arange(L2), H64, pairing)
+            rows2 = np.concatenate([rng.standard_normal((L2, Dc)), kpe2], axis=1)
+            new_rows, *_ = run_oracle(O.F64, pairing, Dc, Dr, 16, L2, [(1, 1 + pad, 0)], rows2, None, H64)
+            want = rope_complex(raw2[1 + pad:], np.arange(1 + pad, L2) + delta, H64, pairing)
+            assert np.allclose(new_rows[1:, Dc:], want, atol=1e-9, rtol=0)
+            assert np.array_equal(new_rows[1:, :Dc], rows2[1 + pad:, :Dc])
+            return
+        new_rows, *_ = run_oracle(O.F64, pairing, Dc, Dr, 16, L, dirs, rows, None, H64)
+        e = dirs[0][1]
+    else:
+        repl = rng.standard_normal((delta, Dc + Dr))
+        new_rows, *_ = run_oracle(O.F64, pairing, Dc, Dr, 16, L, [(5, 5, delta)], rows, repl, H64)
+        e = 5
+    for p in src_pos:
+        want = rope_complex(raw[p], p + delta, H64, pairing)
+        assert np.allclose(new_rows[p + delta, Dc:], want, atol=1e-9, rtol=0), (p, delta)
+        assert np.array_equal(new_rows[p + delta, :Dc], rows[p, :Dc])
+    assert np.allclose(new_rows[e + delta:, Dc:], rope_complex(raw[e:], np.arange(e, L) + delta, H64, pairing),
+                       atol=1e-9, rtol=0)
+
+
+@pytest.mark.parametrize("delta", [1, 21, 48, 76, 512, 2000, -4531, 6794])
+def test_p4_bf16_storage_within_paper_bound(delta):
+    """With bf16 storage the result must stay under the paper's single-rotation drift (4.7e-3 rel-L2,
+    PAPER.md:123; Table 8 d=64 rows).  fp64 trig => expected well below."""
+    bound = _PTS["bf16_single_rotation_rel_l2"]
+    rng = np.random.default_rng(7)
+    Dc, Dr, L = 4, 64, 9000
+    raw = rng.standard_normal((L, Dr))
+    rows = np.concatenate([rng.standard_normal((L, Dc)), rope_complex(raw, np.arange(L), H64)], axis=1)
+    if delta > 0:
+        dirs, e = [(5, 5, delta)], 5
+        repl = rng.standard_normal((delta, Dc + Dr))
+    else:
+        dirs, e = [(5, 5 - delta, 0)], 5 - delta
+        repl = None
+    new_rows, *_ = run_oracle(O.BF16, O.NEOX, Dc, Dr, 64, L, dirs, rows, repl, H64)
+    want = rope_complex(raw[e:], np.arange(e, L) + delta, H64)
+    got = new_rows[e + delta:, Dc:]
+    per_row = np.linalg.norm(got - want, axis=1) / np.linalg.norm(want, axis=1)
+    assert per_row.max() <= bound
+    assert rel_l2(got, want) <= 0.75 * bound
+
+
+# ----------------------------------------------------------------------------- P5: logits are preserved
+
+def test_p5_logits_relative_position():
+    """For every (query position m', key position n') after the edit, (R(m') q) . K_pe_new[n'] equals
+    Re sum_i q_i conj(k_i) exp(i (m'-n') theta_i) computed from the RAW key."""
+    rng = np.random.default_rng(11)
+    Dc, Dr, L = 2, 8, 40
+    inv = synth.rope_inv_freq(Dr, 100.0)
+    raw = rng.standard_normal((L, Dr))
+    rows = np.concatenate([rng.standard_normal((L, Dc)), rope_complex(raw, np.arange(L), inv)], axis=1)
+    dirs = [(5, 12, 2), (20, 21, 6)]
+    # replacement K_pe is roped at its FINAL position (G12); build it that way
+    raw_r = rng.standard_normal((8, Dr))
+    final_pos = np.array([5, 6] + [20 - 5 + q for q in range(6)])
+    repl = np.concatenate([rng.standard_normal((8, Dc)), rope_complex(raw_r, final_pos, inv)], axis=1)
+    new_rows, bm, *_ = run_oracle(O.F64, O.NEOX, Dc, Dr, 4, L, dirs, rows, repl, inv)
+    seq = list_splice(L, [(5, 12, 2, 0), (20, 21, 6, 2)])
+    assert len(seq) == new_rows.shape[0]
+    H = Dr // 2
+    th = inv.astype(np.float64)
+    q_raw = rng.standard_normal(Dr)
+    qc = q_raw[:H] + 1j * q_raw[H:]
+    for m in range(len(seq)):
+        q_m = rope_complex(q_raw, m, inv)
+        for n, tok in enumerate(seq):
+            k_raw = raw[tok[1]] if tok[0] == "o" else raw_r[tok[1]]
+            kc = k_raw[:H] + 1j * k_raw[H:]
+            want = float(np.real(np.sum(qc * np.conj(kc) * np.exp(1j * (m - n) * th))))
+            got = float(q_m @ new_rows[n, Dc:])
+            assert abs(got - want) < 1e-9
+
+
+# ----------------------------------------------------------------------------- P3: composition
+
+def test_p3_two_splices_equal_one_plan():
+    rng = np.random.default_rng(5)
+    Dc, Dr, L = 4, 64, 600
+    raw = rng.standard_normal((L, Dr))
+    rows = np.concatenate([rng.standard_normal((L, Dc)), rope_complex(raw, np.arange(L), H64)], axis=1)
+    repl1, repl2 = rng.standard_normal((7, Dc + Dr)), rng.standard_normal((40, Dc + Dr))
+    d1, d2 = (100, 180, 7), (300, 310, 40)
+    for dtype, tol in ((O.F64, 1e-12), (O.BF16, None)):
+        both, *_ = run_oracle(dtype, O.NEOX, Dc, Dr, 8, L, [d1, d2], rows, np.concatenate([repl1, repl2]), H64)
+        r1 = to_storage(rows, dtype), to_storage(repl1, dtype), to_storage(repl2, dtype)
+        step1, *_ = run_oracle(dtype, O.NEOX, Dc, Dr, 8, L, [d1], rows, repl1, H64)
+        sh = d1[2] - (d1[1] - d1[0])
+        step2, *_ = run_oracle(dtype, O.NEOX, Dc, Dr, 8, step1.shape[0], [(d2[0] + sh, d2[1] + sh, d2[2])], step1,
+                               repl2, H64)
+        assert step2.shape == both.shape
+        assert np.array_equal(step2[:, :Dc], both[:, :Dc])                  # latent bit-exact
+        if tol is not None:
+            assert np.abs(step2 - both).max() < tol                          # closure R(a)R(b)=R(a+b)
+        else:
+            tail = slice(d2[0] + sh + d2[2], None)                           # rows rotated twice vs once
+            assert rel_l2(step2[tail, Dc:], both[tail, Dc:]) <= _PTS["table6_n2_rel_l2"]
+            mid = slice(d1[0] + d1[2], d2[0] + sh)                           # rotated once in both: identical
+            assert np.array_equal(step2[mid], both[mid])
+        del r1
+
+
+# ----------------------------------------------------------------------------- P6: O4 vs O4'
+
+@pytest.mark.parametrize("seed", range(5))
+def test_p6_rotate_vs_brute_force_rerope(seed):
+    rng = np.random.default_rng(seed)
+    for _ in range(200):
+        a, b = rng.standard_normal(2)
+        p = float(rng.integers(0, 131072))
+        c = float(rng.integers(-18624, 18624))
+        th = float(H64[rng.integers(0, 32)])
+        x1 = O.rotate_pair(a, b, c * th)
+        x2 = O.rerope_pair(a, b, p, c, th)
+        assert math.hypot(x1[0] - x2[0], x1[1] - x2[1]) <= 1e-9 * math.hypot(a, b)
+
+
+# ----------------------------------------------------------------------------- P7: textbook reductions
+
+def test_p7_hand_rotation_and_periods():
+    # theta_0 = base^0 = 1: a shift of C is a rotation by C radians.  Hand values of cos(1), sin(1).
+    COS1, SIN1 = 0.5403023058681398, 0.8414709848078965
+    a2, b2 = O.rotate_pair(1.0, 0.0, 1.0)
+    assert abs(a2 - COS1) < 1e-15 and abs(b2 - SIN1) < 1e-15           # positive shift: (1,0) -> (cos, +sin)
+    a2, b2 = O.rotate_pair(0.0, 1.0, 1.0)
+    assert abs(a2 + SIN1) < 1e-15 and abs(b2 - COS1) < 1e-15
+    a2, b2 = O.rotate_pair(1.0, 0.0, math.pi / 2)
+    assert abs(a2) < 1e-15 and abs(b2 - 1.0) < 1e-15
+    for m in (1, 5, 1000):                                              # C*theta = 2 pi m  =>  identity
+        a2, b2 = O.rotate_pair(0.3, -1.7, 2.0 * math.pi * m)
+        tol = 2e-15 * (1.0 + 2.0 * math.pi * m)       # fp64 representation error of the angle itself
+        assert abs(a2 - 0.3) < tol and abs(b2 + 1.7) < tol
+
+
+@pytest.mark.parametrize("pairing", [O.NEOX, O.INTERLEAVED])
+def test_p7_layer_level_pairing_and_theta_index(pairing):
+    """Unit vector in pair i, shift C=+3: the only non-zero outputs are (cos 3 theta_i, sin 3 theta_i) at the
+    pair's two element indices -- pins pairing convention, theta indexing and sign."""
+    Dc, Dr, L = 2, 16, 6
+    H = Dr // 2
+    inv = synth.rope_inv_freq(Dr, 10000.0)
+    assert inv[0] == 1.0
+    for i in range(H):
+        rows = np.zeros((L, Dc + Dr))
+        ia, ib = (i, i + H) if pairing == O.NEOX else (2 * i, 2 * i + 1)
+        rows[:, Dc + ia] = 1.0
+        new_rows, *_ = run_oracle(O.F64, pairing, Dc, Dr, 2, L, [(1, 1, 3)], rows, np.zeros((3, Dc + Dr)), inv)
+        out = new_rows[4:, Dc:]                                          # old rows 1.. moved to 4..
+        want = np.zeros(Dr)
+        want[ia], want[ib] = math.cos(3 * float(inv[i])), math.sin(3 * float(inv[i]))
+        assert np.allclose(out, want[None, :], atol=1e-15, rtol=0)
+        assert np.array_equal(new_rows[0], rows[0])                      # prefix untouched
+
+
+def test_p7_norms_preserved():
+    rng = np.random.default_rng(2)
+    Dc, Dr, L = 4, 64, 300
+    rows = rng.standard_normal((L, Dc + Dr))
+    new_rows, *_ = run_oracle(O.F64, O.NEOX, Dc, Dr, 8, L, [(10, 100, 0)], rows, None, H64)
+    old_k, new_k = rows[100:, Dc:], new_rows[10:, Dc:]
+    assert np.allclose(np.hypot(old_k[:, :32], old_k[:, 32:]), np.hypot(new_k[:, :32], new_k[:, 32:]), atol=1e-12)
+    assert np.allclose(np.linalg.norm(old_k, axis=1), np.linalg.norm(new_k, axis=1), atol=1e-12)
+
+
+# ----------------------------------------------------------------------------- P9: bytes
+
+def test_p9_row_bytes_match_paper():
+    g = golden("paper_kv_bytes.txt")
+    w = synth.config(2)
+    assert w.latent_dim == g["kv_lora_rank"] and w.rope_dim == g["qk_rope_head_dim"]
+    assert w.n_layers == g["dsv2lite_layers"] and w.elem_bytes == g["bytes_per_dtype"]
+    assert w.row_bytes == 1152
+    per_tok = w.row_bytes * w.n_layers
+    assert per_tok == g["bytes_per_token"] == 31104
+    for n, key in ((256, "tokens_256_MB"), (128, "tokens_128_MB"), (896, "tokens_896_MB"), (1724, "slots_1724_MB"),
+                   (2111, "slots_2111_MB"), (3135, "slots_3135_MB")):
+        assert abs(n * per_tok / 1e6 - g[key]) < 0.06, key                # paper rounds to 2-3 digits (decimal MB)
+
+
+# ----------------------------------------------------------------------------- P10: codecs
+
+def test_p10_bf16_codec():
+    bits = np.arange(65536, dtype=np.uint16)
+    ref = torch.from_numpy(bits.view(np.int16).copy()).view(torch.bfloat16).to(torch.float64).numpy()
+    for h in range(65536):
+        d = O.bf16_decode(h)
+        if math.isnan(ref[h]):
+            assert math.isnan(d)
+            continue
+        assert d == ref[h] and math.copysign(1, d) == math.copysign(1, ref[h])
+        assert O.bf16_encode(d) == h                                        # exact values round-trip, +-0 kept
+    # fp32-exact inputs: torch's fp32->bf16 RNE is the library pin
+    rng = np.random.default_rng(0)
+    x = np.concatenate([rng.standard_normal(20000) * 10.0 ** rng.integers(-30, 30, 20000),
+                        np.array([0.0, -0.0, 1e-40, -1e-40, 3.38e38, 3.4e38, -3.4e38])]).astype(np.float32)
+    want = torch.from_numpy(x).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+    got = np.array([O.bf16_encode(float(v)) for v in x], np.uint16)
+    assert np.array_equal(got, want)
+    # bf16 subnormals (quantum 2^-133): random fp32 values there against torch, and ties by hand
+    sub = (rng.standard_normal(5000) * 2.0 ** -128).astype(np.float32)
+    want = torch.from_numpy(sub).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+    assert np.array_equal(np.array([O.bf16_encode(float(v)) for v in sub], np.uint16), want)
+    assert O.bf16_encode(2.0 ** -134) == 0x0000 and O.bf16_encode(2.0 ** -134 * 1.01) == 0x0001
+    assert O.bf16_encode(3 * 2.0 ** -134) == 0x0002 and O.bf16_encode(-2.0 ** -133) == 0x8001
+    # ties to even, by hand: 1 + 2^-8 is halfway between 1.0 (0x3F80) and 1 + 2^-7 (0x3F81) -> even mantissa
+    assert O.bf16_encode(1.0 + 2.0 ** -8) == 0x3F80
+    assert O.bf16_encode(1.0 + 3 * 2.0 ** -8) == 0x3F82
+    # direct rounding from fp64: just above the tie must round UP (a detour through fp32 would lose the 2^-30)
+    assert O.bf16_encode(1.0 + 2.0 ** -8 + 2.0 ** -30) == 0x3F81
+    assert O.bf16_encode(-(1.0 + 2.0 ** -8 - 2.0 ** -30)) == 0xBF80
+
+
+def test_p10_e4m3_codec():
+    bits = np.arange(256, dtype=np.uint8)
+    ref = torch.from_numpy(bits.copy()).view(torch.float8_e4m3fn).to(torch.float64).numpy()
+    for b in range(256):
+        d = O.e4m3_decode(b)
+        if math.isnan(ref[b]):
+            assert math.isnan(d) and (b & 0x7F) == 0x7F
+            continue
+        assert d == ref[b] and math.copysign(1, d) == math.copysign(1, ref[b])
+        assert O.e4m3_encode(d) == b
+    assert O.e4m3_decode(0x7E) == 448.0 and O.e4m3_decode(0x01) == 2.0 ** -9
+    rng = np.random.default_rng(1)
+    x = np.concatenate([rng.standard_normal(20000) * 10.0 ** rng.integers(-4, 3, 20000), [0.0, -0.0, 448.0, -448.0]])
+    x = np.clip(x, -448, 448).astype(np.float32)
+    want = torch.from_numpy(x).to(torch.float8_e4m3fn).view(torch.uint8).numpy()
+    got = np.array([O.e4m3_encode(float(v)) for v in x], np.uint8)
+    assert np.array_equal(got, want)
+    # saturation ("satfinite"), by hand: anything that would round past 448 stays 448, never NaN
+    for v, want_b in ((1000.0, 0x7E), (-1e9, 0xFE), (464.0, 0x7E), (449.0, 0x7E), (float("inf"), 0x7E)):
+        assert O.e4m3_encode(v) == want_b
+    # ties to even in the subnormals: 2^-10 is halfway between 0 and 2^-9 -> 0; 3*2^-10 between m=1 and m=2 -> m=2
+    assert O.e4m3_encode(2.0 ** -10) == 0x00 and O.e4m3_encode(3 * 2.0 ** -10) == 0x02
+    assert O.e4m3_encode(2.0 ** -10 + 2.0 ** -40) == 0x01
+    # normal tie: 1 + 1/16 between 1.0 (0x38) and 1.125 (0x39) -> even
+    assert O.e4m3_encode(1.0625) == 0x38 and O.e4m3_encode(1.1875) == 0x3A
+
+
+def test_fp8_layer_scale_semantics():
+    """fp8 path (G16): dequantise with the layer scale, rotate, requantise with the same scale;
+    latent bytes verbatim.  Pin: result equals quantising the textbook rotation of the dequantised values."""
+    rng = np.random.default_rng(9)
+    Dc, Dr, L, scale = 16, 64, 200, 0.011
+    rows = rng.standard_normal((L, Dc + Dr)) * 2.0
+    new_rows, bm, pool, new_pool, _ = run_oracle(O.FP8_E4M3, O.NEOX, Dc, Dr, 8, L, [(8, 40, 0)], rows, None, H64,
+                                                 scale=scale)
+    rm = bm.requests[0]
+    old_q = from_storage(pool[rm.slot_old], O.FP8_E4M3, scale)
+    want = rope_complex(old_q[40:, Dc:], -32, H64)
+    want_b = to_storage(want, O.FP8_E4M3, scale)
+    got_b = new_pool[rm.slot_new][8:, Dc:]
+    # torch quantises from fp32(want/scale); the oracle from fp64 -- allow the (rare) 1-ulp tie differences
+    o = got_b.astype(np.int16) - want_b.astype(np.int16)
+    assert np.abs(o).max() <= 1 and (o != 0).mean() < 5e-3
+    assert np.array_equal(new_pool[rm.slot_new][8:, :Dc], pool[rm.slot_old][40:, :Dc])
+
+
+def test_yarn_table_shape():
+    """G9: the YaRN table is an INPUT; sanity-pin its limits: high-frequency dims keep base freqs, low-frequency
+    dims are divided by the factor (40), and the ramp is monotone in between (low=10, high=23 for d=64)."""
+    y, r = synth.yarn_inv_freq(64, 10000.0, 40.0, 4096).astype(np.float64), synth.rope_inv_freq(64).astype(np.float64)
+    assert np.allclose(y[:11], r[:11], rtol=1e-6)
+    assert np.allclose(y[23:], r[23:] / 40.0, rtol=1e-6)
+    ratio = y / r
+    assert np.all(np.diff(ratio) <= 1e-6) and ratio[0] == 1.0
