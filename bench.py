@@ -1,0 +1,399 @@
+#!/usr/bin/env python
+"""bench.py -- Leyline splice throughput on one B200 (or N independent replicas), DESIGN.md "Measurement".
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload 3] [--mode fresh]
+
+One step = one pass of the whole hot path over the workload: leyline_plan on the host (a1), then
+leyline_splice on the stream: table upload, index / page-table rewrite (a2), fused gather -> rotate -> scatter
+with the replacement insert (a3 + a4; a0 is the released list the plan reports).  Default workload =
+BASELINE.json config 3 (DeepSeek-V3 shape: 61 layers x 131072 tokens, bf16, page 64, YaRN, three directives),
+FRESH mode.  The metric is splice GB/s counting algorithmic bytes read + written (plan.bytes_read +
+plan.bytes_written).  Rank 0 prints ONE JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "splice_throughput_read_plus_write"
+UNIT = "GB/s"
+MODES = {"fresh": 0, "inplace": 1, "rotate_only": 2}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="3", help="BASELINE.json config: 2, 3, 3m, 4, 5")
+    ap.add_argument("--mode", default="fresh", choices=list(MODES))
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the supplementary modes / workloads")
+    ap.add_argument("--kernel", type=int, default=0, help="leyline_tuning.kernel (0 auto, 1 row, 2 bulk)")
+    ap.add_argument("--tile-rows", type=int, default=0)
+    ap.add_argument("--ctas-per-sm", type=int, default=0)
+    return ap.parse_args()
+
+
+def workload_of(name: str, mode: str):
+    from paper_2606_01065_b200 import synth
+    cfg = int(name) if name.isdigit() else name
+    # FRESH compacts into pages of the same pool: the pool holds the live pages plus as many fresh ones
+    factor = 2.0 if mode == "fresh" else 1.25
+    return synth.config(cfg, pool_factor=factor)
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch device copy, read+write)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s, earlier measurement on this pool)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons while the timed region runs (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 3 + i and r[3 + i].lower().startswith("active") for r in self.rows)]
+        pw = [float(r[2]) for r in self.rows if len(r) > 2 and r[2].replace(".", "").isdigit()]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": reasons}
+
+
+# ----------------------------------------------------------------------------- our arm
+
+def dist_setup(n_gpus: int):
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    return rank, world, local
+
+
+def barrier(world: int):
+    import torch
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    torch.cuda.synchronize()
+
+
+def max_over_ranks(x: float, world: int) -> float:
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1):
+    """K timed steps of plan + splice on torch's current stream, CUDA events around the whole region and the
+    library's own events around the data-moving kernels of every step."""
+    import torch
+    from paper_2606_01065_b200 import binding as B
+    from paper_2606_01065_b200 import harness
+    desc, keep = cache.desc()
+    dev = cache.device
+    plan0 = harness.plan_workload(w, mode, desc)
+    info = plan0.info
+    pt = torch.empty(max(int(info.total_new_pages), 1), dtype=torch.int32, device=dev)
+    idx = torch.empty(max(int(info.total_new_tokens), 1), dtype=torch.int32, device=dev)
+    nbytes = int(info.bytes_read + info.bytes_written)
+    launches = 2 + (2 if mode != B.FRESH else 1)      # index x2 (page table, slot list; 1 for rotate-only) + movers
+    if mode == B.ROTATE_ONLY:
+        launches = 1 + 2
+    plan0.close()
+    plans, host_us = [], []
+
+    def step():
+        t0 = time.perf_counter()
+        plan = harness.plan_workload(w, mode, desc)
+        host_us.append((time.perf_counter() - t0) * 1e6)
+        if mode == B.ROTATE_ONLY:
+            B.leyline_rotate_inplace(plan, cache.pools, cache.repl, idx)
+        else:
+            B.leyline_splice(plan, cache.pools, cache.pools, cache.repl, pt, idx)
+        plans.append(plan)
+
+    for _ in range(warmup):
+        step()
+    barrier(world)
+    for p in plans:
+        p.close()
+    plans.clear()
+    host_us.clear()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    barrier(world)
+    ms = e0.elapsed_time(e1) / steps
+    kms = [p.kernel_ms() for p in plans]
+    for p in plans:
+        p.close()
+    del keep
+    return {"ms_per_step": ms, "kernel_ms": float(np.mean(kms)), "kernel_ms_min": float(np.min(kms)), "bytes": nbytes,
+            "plan_host_us": float(np.median(host_us)), "launches_per_step": launches,
+            "n_directives": len(w.directives), "rows_moved": int(info.rows_moved), "rows_inserted": int(info.rows_inserted)}
+
+
+def cpu_baseline(pools, repls, scales, w, mode: int, bytes_per_layer: int, budget_s: float = 12.0, max_layers: int = 8):
+    """The oracle as it stands (one thread, explicit per-token loops, fp64 libm trig) on whole layers of the same
+    workload, on this host.  `pools` / `repls`: callables returning a layer's bytes as a flat uint8 numpy array."""
+    import oracle as O
+    free = w.free_slots() if mode == O.ROTATE_ONLY else w.free_pages
+    t0 = time.perf_counter()
+    bm = O.plan_batch(mode, w.page_size, w.seq_lens, w.pt_offsets, w.pages, w.directives, free)
+    t_total = time.perf_counter() - t0
+    assert bm.status == O.OK
+    done = 0
+    while done < min(max_layers, w.n_layers) and t_total < budget_s:
+        old, repl = pools(done), repls(done)
+        t0 = time.perf_counter()
+        O.splice_layer(w.dtype, w.pairing, w.latent_dim, w.rope_dim, w.row_bytes, w.inv_freq, scales[done], old, repl, bm)
+        t_total += time.perf_counter() - t0
+        done += 1
+    return {"value": done * bytes_per_layer / t_total / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"{done} of {w.n_layers} layers of {w.name} ({done * bytes_per_layer / 1e9:.2f} GB read+written), "
+                      f"plan + per-layer splice, {t_total:.1f} s",
+            "seconds": t_total, "host_cpus": os.cpu_count()}
+
+
+def run_e2e(cache, w, steps: int, warmup: int = 1):
+    """Same metric through the public API with HOST buffers: every step copies each layer's pool and replacement
+    rows host -> device (pinned), plans on the host, splices, and reads each layer's pool back device -> host.
+    Layers are pipelined over three streams (copy-in, splice, copy-out) with a one-layer plan reused per layer."""
+    import torch
+    from paper_2606_01065_b200 import binding as B
+    from paper_2606_01065_b200 import synth
+    L = cache.n_layers
+    dev = cache.device
+    host_pool = [torch.empty(w.layer_bytes, dtype=torch.uint8, pin_memory=True) for _ in range(L)]
+    host_repl = [torch.empty(cache.repl[l].numel(), dtype=torch.uint8, pin_memory=True) for l in range(L)]
+    for l in range(L):
+        host_pool[l].copy_(cache.pools[l])
+        host_repl[l].copy_(cache.repl[l])
+    desc1, keep = B.make_desc(1, w.latent_dim, w.rope_dim, w.page_size, w.dtype, w.pairing, w.row_bytes, w.n_slots,
+                              w.inv_freq, [cache.scales[0]] if w.dtype == synth.DT_FP8 else None)
+    s_in, s_run, s_out = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    ev_in = [torch.cuda.Event() for _ in range(L)]
+    ev_run = [torch.cuda.Event() for _ in range(L)]
+    pt_host = idx_host = None
+    h2d = sum(t.numel() for t in host_pool) + sum(t.numel() for t in host_repl)
+    d2h = sum(t.numel() for t in host_pool)
+
+    def step():
+        nonlocal pt_host, idx_host
+        plan = B.leyline_plan(desc1, B.FRESH, w.seq_lens, w.pt_offsets, w.pages, w.directives, w.free_pages)
+        info = plan.info
+        pt = torch.empty(int(info.total_new_pages), dtype=torch.int32, device=dev)
+        idx = torch.empty(int(info.total_new_tokens), dtype=torch.int32, device=dev)
+        for l in range(L):
+            with torch.cuda.stream(s_in):
+                cache.pools[l].copy_(host_pool[l], non_blocking=True)
+                cache.repl[l].copy_(host_repl[l], non_blocking=True)
+                ev_in[l].record(s_in)
+            s_run.wait_event(ev_in[l])
+            B.leyline_splice(plan, [cache.pools[l]], [cache.pools[l]], [cache.repl[l]], pt if l == 0 else None,
+                             idx if l == 0 else None, stream=s_run)
+            ev_run[l].record(s_run)
+            s_out.wait_event(ev_run[l])
+            with torch.cuda.stream(s_out):
+                host_pool[l].copy_(cache.pools[l], non_blocking=True)
+        with torch.cuda.stream(s_run):
+            pt_host, idx_host = pt.cpu(), idx.cpu()
+        torch.cuda.synchronize()
+        plan.close()
+        return int(info.bytes_read + info.bytes_written) * L, pt.numel() * 4 + idx.numel() * 4
+
+    for _ in range(warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        nbytes, small = step()
+    dt = (time.perf_counter() - t0) / steps
+    del keep
+    return {"value": nbytes / dt / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h + small,
+            "ms_per_step": dt * 1e3, "steps": steps,
+            "note": "whole layer pools + replacement rows H2D, whole pools + page table + slot list D2H, pinned, "
+                    "3-stream per-layer pipeline; host wall clock around synchronised steps"}
+
+
+def run_ours(args):
+    import torch
+    from paper_2606_01065_b200 import binding as B
+    from paper_2606_01065_b200 import harness
+    from paper_2606_01065_b200 import synth
+    rank, world, local = dist_setup(args.gpus)
+    B.leyline_set_tuning(kernel=args.kernel, tile_rows=args.tile_rows, ctas_per_sm=args.ctas_per_sm, profile=1)
+    mode = MODES[args.mode]
+    w = workload_of(args.workload, args.mode)
+    cache = harness.DeviceCache(w, f"cuda:{local}")
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    r = time_splice(cache, w, mode, args.steps, args.warmup, world)
+    clocks = sampler.stop()
+    ms = max_over_ranks(r["ms_per_step"], world)
+    value = world * r["bytes"] / (ms * 1e-3) / 1e9
+    peak, peak_src = peaks()
+    kernel_gbs = r["bytes"] / (r["kernel_ms"] * 1e-3) / 1e9
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16" if w.dtype == 0 else "fp8_e4m3",
+        "data": "synthetic", "impl": "ours",
+        "config": {"workload": w.name, "mode": args.mode, "n_layers": w.n_layers, "seq_lens": f"{w.n_requests}x{w.seq_lens[0]}",
+                   "page_size": w.page_size, "directives": r["n_directives"], "rows_moved_per_layer": r["rows_moved"],
+                   "rows_inserted_per_layer": r["rows_inserted"], "bytes_read_plus_written": r["bytes"],
+                   "cache_flush": "none needed: each step streams %.2f GB, far larger than the 126 MB L2" % (r["bytes"] / 1e9),
+                   "replicas": world, "multi_gpu": "replicas only (the path has no exchange step)"},
+        "us_per_directive": ms * 1e3 / max(1, r["n_directives"]),
+        "pct_of_8TBps_nominal": 100.0 * value / world / 8000.0,
+        "plan_host_us": r["plan_host_us"],
+        "gpu_launches": r["launches_per_step"] * args.steps,
+        "clocks": clocks,
+        "roofline": {"bound": "hbm", "achieved": kernel_gbs, "peak": peak, "unit": UNIT, "frac": kernel_gbs / peak,
+                     "traffic": None, "kernel": "k_move (fused gather-rotate-scatter + insert)",
+                     "kernel_ms": r["kernel_ms"], "kernel_ms_best": r["kernel_ms_min"],
+                     "peak_source": peak_src, "frac_of_8TBps_nominal": kernel_gbs / 8000.0},
+    }
+    if rank == 0 and world == 1:
+        bytes_per_layer = r["bytes"] // w.n_layers
+        if not args.no_extras and args.workload == "3" and args.mode == "fresh":
+            extras = {}
+            for name, wl, md in (("cfg3_inplace", w, "inplace"), ("cfg3_rotate_only", w, "rotate_only"),
+                                 ("cfg3m_fresh", synth.config("3m", pool_factor=2.0), "fresh")):
+                cache.w = wl
+                x = time_splice(cache, wl, MODES[md], max(3, args.steps // 4), 2)
+                extras[name] = {"ms_per_step": x["ms_per_step"], "GBps": x["bytes"] / x["ms_per_step"] / 1e6,
+                                "kernel_GBps": x["bytes"] / x["kernel_ms"] / 1e6, "bytes": x["bytes"]}
+            cache.w = w
+            out["extras"] = extras
+        if not args.no_cpu_baseline:
+            out["cpu_baseline"] = cpu_baseline(lambda l: cache.pools[l].cpu().numpy(), lambda l: cache.repl[l].cpu().numpy(),
+                                               cache.scales, w, mode, bytes_per_layer)
+        if not args.no_e2e and mode == B.FRESH:
+            try:
+                out["e2e"] = run_e2e(cache, w, steps=min(args.steps, 3))
+            except Exception as ex:   # e.g. the host cannot pin that much memory: say so instead of inventing a number
+                out["e2e"] = {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
+                              "error": f"{type(ex).__name__}: {ex}"}
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(out))
+
+
+# ----------------------------------------------------------------------------- reference arm = the oracle
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on this host's cores; each step is a bounded sample (one
+    layer) of the same workload.  No CUDA library, no GPU work.  Under torchrun only rank 0 runs."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import torch
+    import oracle as O
+    from paper_2606_01065_b200 import synth
+    mode = MODES[args.mode]
+    w = workload_of(args.workload, args.mode)
+    buf = torch.empty(w.layer_bytes, dtype=torch.uint8)
+    scale = synth.fill_layer_(buf, w, 0)
+    rp = torch.empty(max(w.n_repl_rows, 1) * w.row_bytes, dtype=torch.uint8)
+    synth.fill_repl_(rp[: w.n_repl_rows * w.row_bytes], w, 0, scale)
+    old, repl = buf.numpy(), rp.numpy()
+    free = w.free_slots() if mode == O.ROTATE_ONLY else w.free_pages
+    E, W = w.elem_bytes, w.latent_dim + w.rope_dim
+    times = []
+    nbytes = 0
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        bm = O.plan_batch(mode, w.page_size, w.seq_lens, w.pt_offsets, w.pages, w.directives, free)
+        O.splice_layer(w.dtype, w.pairing, w.latent_dim, w.rope_dim, w.row_bytes, w.inv_freq, scale, old, repl, bm)
+        dt = time.perf_counter() - t0
+        if i >= args.warmup:
+            times.append(dt)
+        if not nbytes:
+            rows = 0
+            for r, rm in enumerate(bm.requests):
+                mine = [d for d in w.directives if d[0] == r]
+                k0P = (mine[0][1] // w.page_size) * w.page_size if mine else rm.L_new
+                for (k, s, d, n, c) in rm.segs.as_tuples():
+                    if k == O.INSERT:
+                        rows += n
+                    elif mode == O.FRESH:
+                        rows += max(0, d + n - max(d, k0P))
+                    elif c != 0:
+                        rows += n if mode == O.INPLACE_MOVE else 0
+            nbytes = 2 * rows * W * E
+            if mode == O.ROTATE_ONLY:
+                nbytes += 2 * sum(n for rm in bm.requests for (k, s, d, n, c) in rm.segs.as_tuples() if k == O.KEEP and c != 0) * w.rope_dim * E
+    ms = float(np.mean(times)) * 1e3
+    value = nbytes / (ms * 1e-3) / 1e9
+    sample = f"1 of {w.n_layers} layers of {w.name} per step ({nbytes / 1e9:.3f} GB read+written), plan + splice"
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "impl": "reference",
+        "config": {"workload": w.name, "mode": args.mode, "n_layers": w.n_layers, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                         "host_cpus": os.cpu_count()},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -1,0 +1,245 @@
+/*
+ * leyline.h -- C ABI of the B200-native Leyline splice library (libleyline.so).
+ *
+ * The library implements the data-parallel hot path of the KV-cache directive of
+ * "Leyline: KV Cache Directives for Agentic Inference" (arxiv/paper_2606_01065).
+ * Citations "PAPER.md:N" are lines of the paper text; "G<n>" / "M<n>" / "rule V" are the readings and
+ * rules listed in DESIGN.md.
+ *
+ * One directive D = (s_start, s_end, R, m) replaces the cached token span
+ * [s_start, s_end) of a request by |R| replacement tokens.  Applying it to an MLA cache means
+ * (PAPER.md:127 steps 1-3, PAPER.md:405 (a)-(d)):
+ *   (a) the span's KV slots are released;
+ *   (b) the replacement's precomputed KV rows are written at new positions [s_start, s_start+|R|);
+ *   (c) every downstream token i >= s_end is re-keyed to i + Delta, Delta = |R| - (s_end - s_start), and its
+ *       K_pe is rotated in closed form, K_pe_new = R(Delta) K_pe (Eq. (1)), latent untouched;
+ *   (d) nothing for Q.
+ * Several sorted, non-overlapping directives per request compose into one rotation per segment by the
+ * cumulative shift C_j = sum_{i<=j} Delta_i (R(a)R(b) = R(a+b)).
+ *
+ * Cache layout (caller-owned): per layer one pool of `n_slots` rows of
+ * `row_stride_bytes`; a row is `latent_dim` elements of c_kv followed by `rope_dim` elements of K_pe
+ * (bf16, or fp8 e4m3 with one fp32 scale per layer).  Page p of a layer is rows [p*page_size, (p+1)*page_size).
+ * A request's logical position t lives at slot  table[t / page_size] * page_size + t % page_size.
+ *
+ * Threading / streams: leyline_plan is pure host code (no CUDA call, no device needed).  leyline_splice and
+ * leyline_rotate_inplace upload the plan's tables on first use (stream-ordered), launch on the caller's
+ * stream and return without synchronising.  A plan may be in flight on one stream at a time.
+ * Nothing is thrown across the ABI: every entry point returns a leyline_status.
+ * There is no CPU fallback: without a CUDA device the two launch entry points return LEYLINE_E_CUDA.
+ */
+#ifndef LEYLINE_H_
+#define LEYLINE_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    LEYLINE_OK = 0,
+    LEYLINE_E_INVALID = 1,     /* NULL / negative / inconsistent argument */
+    LEYLINE_E_UNSORTED = 2,    /* directives not sorted by (request, start) */
+    LEYLINE_E_OVERLAP = 3,     /* two spans of one request overlap (rejected at apply time) */
+    LEYLINE_E_RANGE = 4,       /* request id or span outside the request */
+    LEYLINE_E_NOFREE = 5,      /* free list too short for the pages / slots the plan must consume */
+    LEYLINE_E_UNSUPPORTED = 6, /* geometry the kernels do not cover (see leyline_cache_desc) */
+    LEYLINE_E_CUDA = 7         /* CUDA runtime error (message via leyline_last_cuda_error) */
+} leyline_status;
+
+typedef enum { LEYLINE_BF16 = 0, LEYLINE_FP8_E4M3 = 1 } leyline_dtype;
+/* RoPE pairing: NEOX pairs element i with i + rope_dim/2, INTERLEAVED pairs 2i with 2i+1. */
+typedef enum { LEYLINE_ROPE_NEOX = 0, LEYLINE_ROPE_INTERLEAVED = 1 } leyline_pairing;
+/* FRESH        : the paper's dst_slots path: everything from the first edited page on is
+ *                compacted into pages taken from the free list; source pages are released, never written (M1).
+ * INPLACE_MOVE : rows move inside the request's own pages (growth appends free pages, shrink releases the
+ *                tail); overlapping source/destination handled by hazard-ordered tiles (M2).
+ * ROTATE_ONLY  : the paper's in-place path: no row moves, K_pe rotated where it sits, the
+ *                token-level slot index list is rewritten (M3). */
+typedef enum { LEYLINE_FRESH = 0, LEYLINE_INPLACE_MOVE = 1, LEYLINE_ROTATE_ONLY = 2 } leyline_mode;
+/* PAPER.md:98, :102.  FORGET truncates the request at the directive's start; no kernel work. */
+typedef enum { LEYLINE_AMORTIZE = 0, LEYLINE_FORGET = 1 } leyline_semantic;
+
+#define LEYLINE_MAX_LAYERS_PER_LAUNCH 128
+
+typedef struct {
+    int32_t n_layers;          /* >= 1 */
+    int32_t latent_dim;        /* c_kv elements per row (512 for DeepSeek MLA); latent bytes must be a multiple of 16 */
+    int32_t rope_dim;          /* K_pe elements per row (64); even; (rope_dim/2)*elem bytes a multiple of 16 for NEOX,
+                                  rope_dim*elem bytes a multiple of 16 for INTERLEAVED */
+    int32_t page_size;         /* tokens per page, power of two (1 = token-level slots) */
+    int32_t dtype;             /* leyline_dtype */
+    int32_t pairing;           /* leyline_pairing */
+    int64_t row_stride_bytes;  /* >= (latent_dim+rope_dim)*elem bytes, multiple of 16.  Bytes of a row beyond
+                                  (latent_dim+rope_dim)*elem (padding) are never read or written. */
+    int64_t pool_slots;        /* rows in each layer's pool (a multiple of page_size); page ids are validated
+                                  against pool_slots / page_size, slot ids against pool_slots */
+    const float* inv_freq;     /* HOST, [rope_dim/2]: THE theta_i in fp32 (YaRN etc. already applied; G9).
+                                  Copied by leyline_plan. */
+    const float* layer_scale;  /* HOST, [n_layers], fp8 only (may be NULL): per-layer dequantisation scale.  A splice
+                                  leaves it unchanged, so it cancels in x/scale*scale; it is validated (> 0, finite)
+                                  but not used by the kernels (G16). */
+} leyline_cache_desc;
+
+typedef struct {
+    int32_t request;           /* index into seq_lens */
+    int32_t repl_len;          /* |R| >= 0 */
+    int64_t start, end;        /* span [start, end) in ORIGINAL token indices of the request (G1) */
+    int64_t repl_row;          /* first row of this directive's replacement KV inside layer_repl[l] */
+    int32_t semantic;          /* leyline_semantic */
+    int32_t reserved_;         /* must be 0 */
+} leyline_directive;
+
+/* One segment of a request in new-position order (query result). */
+typedef struct {
+    int32_t request;
+    int32_t kind;              /* 0 = KEEP (old rows re-keyed and rotated), 1 = INSERT (replacement rows) */
+    int64_t src_begin;         /* KEEP: first old position; INSERT: first replacement row */
+    int64_t dst_begin;         /* first new position */
+    int64_t length;            /* > 0 (empty segments are omitted) */
+    int64_t shift;             /* KEEP: cumulative C_j (rotation amount = dst - src); INSERT: 0 */
+} leyline_segment;
+
+typedef struct {
+    int32_t mode;
+    int32_t n_requests;
+    int64_t total_new_tokens;  /* sum of new sequence lengths = length of the token-level index list */
+    int64_t total_new_pages;   /* sum of new page-table rows (0 for ROTATE_ONLY) */
+    int64_t n_free_consumed;   /* ids taken from the front of the free list */
+    int64_t n_released;        /* ids reported back (pages, or slots for ROTATE_ONLY) */
+    int64_t n_segments;
+    int64_t n_tiles;           /* device work items per layer (move tiles first, then insert tiles) */
+    int64_t n_move_tiles;
+    int64_t n_trig;            /* rows of the cos/sin table = distinct non-zero cumulative shifts */
+    int64_t rows_moved;        /* per layer: KEEP rows copied+rotated (FRESH / INPLACE_MOVE; includes FRESH's head copy) */
+    int64_t rows_inserted;     /* per layer: replacement rows written */
+    int64_t rows_rotated;      /* per layer: rows whose K_pe is rotated (shift != 0) */
+    int64_t bytes_read;        /* ALGORITHMIC bytes over all layers: (latent+rope)*elem per moved/inserted row,
+                                  rope*elem per in-place rotated row */
+    int64_t bytes_written;     /* same, written */
+    int64_t bytes_index;       /* 4 B per new token + 4 B per new page-table entry (once, not per layer) */
+} leyline_plan_info;
+
+typedef struct leyline_plan_s leyline_plan_t;
+
+/*
+ * leyline_plan -- the host planner (step a1).
+ *
+ *   desc          cache geometry (copied).
+ *   n_requests    number of requests; seq_lens[r] = cached tokens of request r (HOST).
+ *   pt_offsets    HOST [n_requests+1]: row r of the page table is pages[pt_offsets[r] .. pt_offsets[r+1]),
+ *                 at least ceil(seq_lens[r]/page_size) entries.
+ *   pages         HOST int32 page ids.
+ *   directives    HOST, sorted by (request, start), spans of one request non-overlapping (adjacent allowed).
+ *   free_ids      HOST int32: free PAGE ids (FRESH, INPLACE_MOVE) or free SLOT ids (ROTATE_ONLY); consumed front to
+ *                 back, requests in ascending order.  The library never allocates pool pages itself.
+ *   out           receives the plan (owned by the caller, release with leyline_plan_destroy).
+ *
+ * Every directive of every request is validated before any state is produced (all-or-none);
+ * on error *out is NULL.  Validation order is rule V of DESIGN.md (first failure wins, directives in order):
+ * request out of range -> RANGE; start<0 | end<start | repl_len<0 | repl_row<0 | bad semantic -> INVALID;
+ * end > seq_len -> RANGE; request or start decreasing -> UNSORTED; start < previous end -> OVERLAP;
+ * then free list too short -> NOFREE.  Accepted: start==end (pure insert), repl_len==0 (pure delete,
+ * PAPER.md:605), both (no-op), adjacent spans, start==0, requests without directives (untouched).
+ */
+leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t mode, int32_t n_requests,
+                            const int64_t* seq_lens, const int64_t* pt_offsets, const int32_t* pages,
+                            int32_t n_directives, const leyline_directive* directives, const int32_t* free_ids,
+                            int64_t n_free, leyline_plan_t** out);
+
+/* Plan queries (all HOST output buffers, sized from leyline_plan_info). */
+leyline_status leyline_plan_get_info(const leyline_plan_t* plan, leyline_plan_info* out);
+leyline_status leyline_plan_new_seq_lens(const leyline_plan_t* plan, int64_t* out /*[n_requests]*/);
+/* First FORGET directive's start in new coordinates per request, -1 if none. */
+leyline_status leyline_plan_forget_trim(const leyline_plan_t* plan, int64_t* out /*[n_requests]*/);
+/* Offsets of each request inside the token-level index list: [n_requests+1], prefix sums of new_seq_lens. */
+leyline_status leyline_plan_slot_offsets(const leyline_plan_t* plan, int64_t* out);
+/* New page tables (FRESH / INPLACE_MOVE; LEYLINE_E_INVALID for ROTATE_ONLY): offsets [n_requests+1] and ids. */
+leyline_status leyline_plan_new_pt_offsets(const leyline_plan_t* plan, int64_t* out);
+leyline_status leyline_plan_new_pages(const leyline_plan_t* plan, int32_t* out /*[total_new_pages]*/);
+/* Released ids, requests ascending: pages in ascending logical order (FRESH: old pages from the first edited
+ * page on; INPLACE_MOVE: tail pages) or, for ROTATE_ONLY, the slots of every removed old position in order.
+ * Their bytes are never written (PAPER.md:405(a); G14). */
+leyline_status leyline_plan_released(const leyline_plan_t* plan, int32_t* out /*[n_released]*/);
+leyline_status leyline_plan_segments(const leyline_plan_t* plan, leyline_segment* out /*[n_segments]*/);
+
+/* One device work item per layer (query result, for tests and tooling): `n_rows` rows that are consecutive in
+ * NEW logical position, `dst_pos .. dst_pos+n_rows` of `request`, read from OLD logical positions
+ * `src_pos ..` of the same request (or from replacement rows `src_pos ..` when LEYLINE_TILE_SRC_REPL is set).
+ * The device resolves positions to slots through the page tables, so a tile may straddle pages.  `trig` is the
+ * row of the cos/sin table that rotates the K_pe band (-1: byte copy).  Tiles are listed in TICKET order: the
+ * device hands them out in this order, layer fastest.  For INPLACE_MOVE a tile may store only after tiles
+ * [dep_lo, dep_hi] (indices into this list, all smaller than its own; empty when dep_lo > dep_hi) have
+ * finished LOADING the same layer: those are exactly the tiles whose source rows it overwrites (rule M2 of
+ * DESIGN.md).  Move tiles come first ([0, n_move_tiles)), replacement inserts after.  For ROTATE_ONLY the move
+ * tiles are the in-place K_pe rotations (src_pos = old position, dst_pos = new position, no row moves). */
+#define LEYLINE_TILE_SRC_REPL 1
+typedef struct {
+    int64_t src_pos;
+    int64_t dst_pos;
+    int32_t n_rows;
+    int32_t trig;
+    int32_t flags;
+    int32_t dep_lo, dep_hi;
+    int32_t request;
+} leyline_tile;
+leyline_status leyline_plan_tiles(const leyline_plan_t* plan, leyline_tile* out /*[n_tiles]*/);
+/* Shifts C of the cos/sin table rows: row g holds cos/sin(C_g * theta_i), i in [0, rope_dim/2). */
+leyline_status leyline_plan_trig_shifts(const leyline_plan_t* plan, int64_t* out /*[n_trig]*/);
+/* The table itself, [n_trig][2][rope_dim/2] fp32: cos then sin of C_g * theta_i (fp64 product and trig, rounded once). */
+leyline_status leyline_plan_trig_table(const leyline_plan_t* plan, float* out);
+
+/*
+ * leyline_splice -- execute a FRESH or INPLACE_MOVE plan on `cuda_stream` (steps a2-a4).
+ *
+ *   layer_src   HOST array of n_layers DEVICE pointers to the pools read (16-byte aligned).
+ *   layer_dst   HOST array of n_layers DEVICE pointers to the pools written.  May equal layer_src (fresh pages of
+ *               the same pool); MUST equal it for INPLACE_MOVE.
+ *   layer_repl  HOST array of n_layers DEVICE pointers to the replacement KV rows, [rows x row_stride_bytes] per
+ *               layer, K_pe already roped at its FINAL position (G12).  May be NULL iff the plan inserts no row.
+ *   dev_page_table_out  DEVICE int32 [total_new_pages] or NULL: receives the new page-table rows (concatenated,
+ *               leyline_plan_new_pt_offsets).
+ *   dev_slot_idx_out    DEVICE int32 [total_new_tokens] or NULL: receives the token-level slot of every new position.
+ *
+ * Kernels: index / page-table rewrite, then the fused gather -> rotate -> scatter (+ replacement insert).
+ * Asynchronous; only launch errors are returned.  Bytes the mode says are never written are never written.
+ */
+leyline_status leyline_splice(leyline_plan_t* plan, void* const* layer_src, void* const* layer_dst,
+                              const void* const* layer_repl, int32_t* dev_page_table_out, int32_t* dev_slot_idx_out,
+                              void* cuda_stream);
+
+/*
+ * leyline_rotate_inplace -- execute a ROTATE_ONLY plan (steps a2, a5): rotate the K_pe band of every downstream
+ * token where it sits (128 B of every 1152 B bf16 row), optionally copy the replacement rows into the consumed
+ * free slots (layer_repl == NULL: the caller already prefilled them), and write the new token-level index list.
+ */
+leyline_status leyline_rotate_inplace(leyline_plan_t* plan, void* const* layer_ptrs, const void* const* layer_repl,
+                                      int32_t* dev_slot_idx_out, void* cuda_stream);
+
+void leyline_plan_destroy(leyline_plan_t* plan);
+const char* leyline_strerror(leyline_status s);
+/* Text of the last CUDA error seen by this thread's calls into the library ("" if none). */
+const char* leyline_last_cuda_error(void);
+
+/* Process-wide tuning knobs (benchmarking; defaults are what bench.py reports).  Read by leyline_plan. */
+typedef struct {
+    int32_t kernel;        /* 0 = auto, 1 = row kernel (LDG/STG), 2 = bulk kernel (TMA bulk copies through smem) */
+    int32_t tile_rows;     /* rows per tile of the move/insert kernels, 0 = default */
+    int32_t ctas_per_sm;   /* row kernel only, 0 = default */
+    int32_t profile;       /* 1: record CUDA events around the data-moving kernels (leyline_plan_kernel_ms) */
+} leyline_tuning;
+leyline_status leyline_set_tuning(const leyline_tuning* t);
+leyline_status leyline_get_tuning(leyline_tuning* t);
+
+/* Device time of the data-moving kernels (a3+a4 / a5) of the plan's last launch, from CUDA events recorded on
+ * the launching stream when the plan was created with tuning.profile = 1.  Call after synchronising the stream. */
+leyline_status leyline_plan_kernel_ms(const leyline_plan_t* plan, float* ms);
+
+/* Library / build description, e.g. "leyline-b200 0.1 sm_100a". */
+const char* leyline_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LEYLINE_H_ */

@@ -1,0 +1,163 @@
+/*
+ * kernels_rows.cuh -- the register-staged ("row") kernels: steps a2, a3, a4, a5 of DESIGN.md.
+ *
+ *   k_index        a2  slot-index list / page-table rewrite (PAPER.md:135, :405(c) "re-keyed")
+ *   k_move_rows    a3+a4  gather -> rotate -> scatter of whole rows, replacement insert as extra tiles
+ *                  (PAPER.md:118-127, :405(b)(c)); with HAZARD = true it is the in-place mover of rule M2
+ *   k_rotate_band  a5  in-place rotation of the K_pe band only
+ *
+ * All three are persistent: CTAs pull (tile, layer) items from a ticket counter, layer fastest.
+ */
+#ifndef LEYLINE_KERNELS_ROWS_CUH_
+#define LEYLINE_KERNELS_ROWS_CUH_
+
+#include "device_common.cuh"
+
+namespace leyline {
+
+/* ------------------------------------------------------------------ a2 ---- */
+
+__global__ void __launch_bounds__(kThreads) k_index(const IndexParams p) {
+    for (long long o = blockIdx.x * (long long)blockDim.x + threadIdx.x; o < p.total;
+         o += (long long)gridDim.x * blockDim.x) {
+        int lo = 0, hi = p.n_runs - 1; /* last run with out_begin <= o */
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (__ldg(&p.runs[mid].out_begin) <= o) lo = mid; else hi = mid - 1;
+        }
+        const IdxRun r = p.runs[lo];
+        const int64_t q = o - r.out_begin;
+        int32_t v;
+        if (r.kind == 0) v = (int32_t)slot_of(p.tabs, r.tab, r.pos0 + q, p.page_shift);
+        else if (r.kind == 1) v = __ldg(p.tabs + r.tab + r.pos0 + q);
+        else v = __ldg(p.tabs + r.pos0 + q);
+        p.out[o] = v;
+    }
+}
+
+/* ------------------------------------------------------------------ a3 + a4 ---- */
+
+constexpr int kMaxTileRows = 32;
+constexpr int kLatPerThread = 8; /* 16-byte latent chunks a thread holds: tile_rows * lat_chunks <= 8 * 256 */
+
+/* LC / NB: latent / band chunks per row at compile time, or -1 to read them from the parameters. */
+template <int DT, int PAIRING, bool HAZARD, int LC_T, int NB_T>
+__global__ void __launch_bounds__(kThreads, 3) k_move_rows(const __grid_constant__ MoveParams p) {
+    __shared__ int64_t s_src[kMaxTileRows], s_dst[kMaxTileRows];
+    __shared__ long long s_item;
+    const int tid = threadIdx.x;
+    const int LC = LC_T >= 0 ? LC_T : p.lat_chunks;
+    const int NB = NB_T >= 0 ? NB_T : p.band_chunks;
+
+    for (;;) {
+        if (tid == 0) s_item = (long long)atomicAdd(p.ticket, 1ull);
+        __syncthreads();
+        const long long item = s_item;
+        if (item >= p.n_items) break;
+        const int tile_i = p.tile_begin + (int)(item / p.n_layers);
+        const int layer = (int)(item % p.n_layers);
+        const DevTile t = p.tiles[tile_i];
+        const bool from_repl = (t.flags & TILE_SRC_REPL) != 0;
+        if (tid < t.n_rows) {
+            s_src[tid] = (from_repl ? t.src_pos + tid : slot_of(p.tabs, t.src_tab, t.src_pos + tid, p.page_shift)) * p.stride;
+            s_dst[tid] = slot_of(p.tabs, t.dst_tab, t.dst_pos + tid, (t.flags & TILE_DST_TOKEN) ? 0 : p.page_shift) * p.stride;
+        }
+        __syncthreads();
+        const uint8_t* __restrict__ sbase = from_repl ? p.repl[layer] : p.src[layer];
+        uint8_t* __restrict__ dbase = p.dst[layer];
+
+        /* gather: every load of the tile is issued before anything is stored */
+        int4 lat[kLatPerThread];
+        const int n_lat = t.n_rows * LC;
+#pragma unroll
+        for (int k = 0; k < kLatPerThread; ++k) {
+            const int c = tid + k * kThreads;
+            if (c < n_lat) {
+                const int r = c / LC, col = c - r * LC;
+                const uint8_t* a = sbase + s_src[r] + col * 16;
+                lat[k] = HAZARD ? ld_coherent(a) : ld_stream(a);
+            }
+        }
+        const int br = tid / NB, bj = tid - br * NB;
+        const bool has_band = br < t.n_rows;
+        int4 band = make_int4(0, 0, 0, 0);
+        if (has_band) {
+            const uint8_t* a = sbase + s_src[br] + (LC + bj) * 16;
+            band = HAZARD ? ld_coherent(a) : ld_stream(a);
+        }
+
+        /* rotate (tile-uniform branch: C = 0 segments, head copies and inserts are byte copies, G19) */
+        if (t.trig >= 0) band = rotate_band_chunk<DT, PAIRING>(band, bj, NB, p.trig + (int64_t)t.trig * 2 * p.H, p.H, has_band);
+
+        if (HAZARD) {
+            /* rule M2: publish "loaded", then wait for the tiles whose source rows this tile overwrites */
+            __threadfence();
+            __syncthreads();
+            int32_t* flags = p.flags + p.layer0 + layer;
+            if (tid == 0) st_release(flags + (int64_t)tile_i * p.n_layers_total, 1);
+            for (int d = t.dep_lo + tid; d <= t.dep_hi; d += kThreads)
+                while (ld_acquire(flags + (int64_t)d * p.n_layers_total) == 0) __nanosleep(64);
+            __syncthreads();
+        }
+
+        /* scatter */
+#pragma unroll
+        for (int k = 0; k < kLatPerThread; ++k) {
+            const int c = tid + k * kThreads;
+            if (c < n_lat) {
+                const int r = c / LC, col = c - r * LC;
+                st_stream(dbase + s_dst[r] + col * 16, lat[k]);
+            }
+        }
+        if (has_band) st_stream(dbase + s_dst[br] + (LC + bj) * 16, band);
+    }
+}
+
+/* ------------------------------------------------------------------ a5 ---- */
+
+constexpr int kRotTileRows = 256; /* rows per in-place rotation tile (ROTATE_ONLY plans) */
+constexpr int kRotPerThread = 8;
+
+template <int DT, int PAIRING, int NB_T>
+__global__ void __launch_bounds__(kThreads, 4) k_rotate_band(const __grid_constant__ MoveParams p) {
+    __shared__ int64_t s_off[kRotTileRows];
+    __shared__ long long s_item;
+    const int tid = threadIdx.x;
+    const int NB = NB_T >= 0 ? NB_T : p.band_chunks;
+    const int per_pass = kThreads / NB; /* rows per pass */
+
+    for (;;) {
+        if (tid == 0) s_item = (long long)atomicAdd(p.ticket, 1ull);
+        __syncthreads();
+        const long long item = s_item;
+        if (item >= p.n_items) break;
+        const int tile_i = p.tile_begin + (int)(item / p.n_layers);
+        const int layer = (int)(item % p.n_layers);
+        const DevTile t = p.tiles[tile_i];
+        for (int r = tid; r < t.n_rows; r += kThreads)
+            s_off[r] = slot_of(p.tabs, t.src_tab, t.src_pos + r, p.page_shift) * p.stride + (int64_t)p.lat_chunks * 16;
+        __syncthreads();
+        uint8_t* __restrict__ base = p.dst[layer];
+        const float* __restrict__ trig_row = p.trig + (int64_t)t.trig * 2 * p.H;
+        const int r0 = tid / NB, j = tid - r0 * NB;
+        int4 v[kRotPerThread];
+#pragma unroll
+        for (int k = 0; k < kRotPerThread; ++k) {
+            const int r = r0 + k * per_pass;
+            if (r < t.n_rows) v[k] = ld_coherent(base + s_off[r] + j * 16);
+        }
+#pragma unroll
+        for (int k = 0; k < kRotPerThread; ++k) {
+            const int r = r0 + k * per_pass;
+            const bool active = r < t.n_rows;
+            if (k * per_pass < t.n_rows) { /* warp-uniform: the NeoX partner exchange needs the whole warp */
+                const int4 w = rotate_band_chunk<DT, PAIRING>(active ? v[k] : make_int4(0, 0, 0, 0), j, NB, trig_row, p.H, active);
+                if (active) st_stream(base + s_off[r] + j * 16, w);
+            }
+        }
+    }
+}
+
+}  // namespace leyline
+
+#endif /* LEYLINE_KERNELS_ROWS_CUH_ */

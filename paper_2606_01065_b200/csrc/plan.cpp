@@ -1,0 +1,483 @@
+/*
+ * plan.cpp -- leyline_plan: the host planner (step a1 of DESIGN.md).
+ *
+ * Pure host C++: no CUDA call, usable without a device.  Turns sorted, non-overlapping directives into
+ *   - per-request segments with cumulative shift C_j ("running position shift carried over"),
+ *   - the new slot / page map under rule M1 (FRESH), M2 (INPLACE_MOVE) or M3 (ROTATE_ONLY),
+ *   - device work items (tiles of <= tile_rows rows, consecutive in new position) in ticket order, with the
+ *     load->store dependencies that make in-place moves safe (rule M2),
+ *   - the cos/sin table of C_j * theta_i: product and trig in fp64, rounded once to fp32.
+ */
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <map>
+#include <new>
+
+#include "plan_internal.h"
+
+using leyline::DevTile;
+using leyline::IdxRun;
+
+namespace {
+
+leyline_tuning g_tuning = {0, 0, 0, 0};
+
+inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+struct Seg {
+    int32_t kind;  /* 0 KEEP, 1 INSERT */
+    int64_t src, dst, len, shift;
+};
+
+/* Segments of one request in new-position order.  Returns L_new. */
+int64_t build_segments(int64_t L_old, const leyline_directive* d, int32_t k, std::vector<Seg>& out, int64_t* trim) {
+    int64_t C = 0, pos = 0;
+    *trim = -1;
+    for (int32_t j = 0; j < k; ++j) {
+        if (d[j].start > pos) out.push_back({0, pos, pos + C, d[j].start - pos, C});
+        if (d[j].semantic == LEYLINE_FORGET) { /* truncate here, re-prefill is the caller's */
+            *trim = d[j].start + C;
+            return d[j].start + C;
+        }
+        if (d[j].repl_len > 0) out.push_back({1, d[j].repl_row, d[j].start + C, d[j].repl_len, 0});
+        C += (int64_t)d[j].repl_len - (d[j].end - d[j].start); /* Delta = |R| - (e - s) */
+        pos = d[j].end;
+    }
+    if (L_old > pos) out.push_back({0, pos, pos + C, L_old - pos, C});
+    return L_old + C;
+}
+
+leyline_status check_desc(const leyline_cache_desc* c, int* elem_bytes, int* page_shift) {
+    if (!c) return LEYLINE_E_INVALID;
+    if (c->n_layers < 1 || c->latent_dim < 0 || c->rope_dim < 2 || (c->rope_dim & 1)) return LEYLINE_E_INVALID;
+    if (c->page_size < 1 || (c->page_size & (c->page_size - 1))) return LEYLINE_E_INVALID;
+    if (c->dtype != LEYLINE_BF16 && c->dtype != LEYLINE_FP8_E4M3) return LEYLINE_E_INVALID;
+    if (c->pairing != LEYLINE_ROPE_NEOX && c->pairing != LEYLINE_ROPE_INTERLEAVED) return LEYLINE_E_INVALID;
+    if (!c->inv_freq) return LEYLINE_E_INVALID;
+    int E = c->dtype == LEYLINE_BF16 ? 2 : 1;
+    int64_t row = (int64_t)(c->latent_dim + c->rope_dim) * E;
+    if (c->row_stride_bytes < row || (c->row_stride_bytes & 15)) return LEYLINE_E_INVALID;
+    if (c->pool_slots < 0 || (c->pool_slots % c->page_size)) return LEYLINE_E_INVALID;
+    for (int i = 0; i < c->rope_dim / 2; ++i)
+        if (!std::isfinite(c->inv_freq[i])) return LEYLINE_E_INVALID;
+    if (c->dtype == LEYLINE_FP8_E4M3 && c->layer_scale)
+        for (int l = 0; l < c->n_layers; ++l)
+            if (!(c->layer_scale[l] > 0.f) || !std::isfinite(c->layer_scale[l])) return LEYLINE_E_INVALID;
+    /* what the kernels cover: 16-byte chunks, K_pe band of 2^k chunks (k <= 5), NeoX halves in whole chunks */
+    int64_t lat_bytes = (int64_t)c->latent_dim * E, band_bytes = (int64_t)c->rope_dim * E;
+    if ((lat_bytes & 15) || (band_bytes & 15)) return LEYLINE_E_UNSUPPORTED;
+    int64_t nb = band_bytes / 16;
+    if (nb > 32 || (nb & (nb - 1))) return LEYLINE_E_UNSUPPORTED;
+    if (c->pairing == LEYLINE_ROPE_NEOX && nb < 2) return LEYLINE_E_UNSUPPORTED;
+    if (lat_bytes / 16 > 2048) return LEYLINE_E_UNSUPPORTED;
+    int sh = 0;
+    while ((1 << sh) < c->page_size) ++sh;
+    *elem_bytes = E;
+    *page_shift = sh;
+    return LEYLINE_OK;
+}
+
+/* Rule V of DESIGN.md (same order as the paper's checks are stated: PAPER.md:98, :409, :635). */
+leyline_status check_directives(int32_t n_req, const int64_t* seq_lens, int32_t n_dir, const leyline_directive* d) {
+    for (int32_t i = 0; i < n_dir; ++i) {
+        if (d[i].request < 0 || d[i].request >= n_req) return LEYLINE_E_RANGE;
+        if (d[i].start < 0 || d[i].end < d[i].start || d[i].repl_len < 0 || d[i].repl_row < 0) return LEYLINE_E_INVALID;
+        if (d[i].semantic != LEYLINE_AMORTIZE && d[i].semantic != LEYLINE_FORGET) return LEYLINE_E_INVALID;
+        if (d[i].end > seq_lens[d[i].request]) return LEYLINE_E_RANGE;
+        if (i > 0) {
+            if (d[i].request < d[i - 1].request) return LEYLINE_E_UNSORTED;
+            if (d[i].request == d[i - 1].request) {
+                if (d[i].start < d[i - 1].start) return LEYLINE_E_UNSORTED;
+                if (d[i].start < d[i - 1].end) return LEYLINE_E_OVERLAP;
+            }
+        }
+    }
+    return LEYLINE_OK;
+}
+
+int choose_tile_rows(const leyline_cache_desc& c, int E, const leyline_tuning& t) {
+    int64_t lat_chunks = (int64_t)c.latent_dim * E / 16, nb = (int64_t)c.rope_dim * E / 16;
+    /* the row kernel keeps a whole tile in registers: <= 8 latent + 1 band chunk per thread, 256 threads */
+    int64_t cap = 32;
+    if (lat_chunks > 0) cap = std::min<int64_t>(cap, 2048 / lat_chunks);
+    cap = std::min<int64_t>(cap, 256 / nb);
+    if (cap < 1) cap = 1;
+    int64_t want = t.tile_rows > 0 ? t.tile_rows : 32;
+    return (int)std::max<int64_t>(1, std::min(want, cap));
+}
+
+/* split [dst0, dst0+len) into tiles whose boundaries are multiples of tile_rows in `align_pos` space */
+template <class F>
+void split_tiles(int64_t src0, int64_t dst0, int64_t len, int64_t align0, int tile_rows, F&& emit) {
+    int64_t done = 0;
+    while (done < len) {
+        int64_t a = align0 + done;
+        int64_t n = std::min<int64_t>(len - done, tile_rows - (a % tile_rows));
+        emit(src0 + done, dst0 + done, (int32_t)n);
+        done += n;
+    }
+}
+
+}  // namespace
+
+extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t mode, int32_t n_requests,
+                                       const int64_t* seq_lens, const int64_t* pt_offsets, const int32_t* pages,
+                                       int32_t n_directives, const leyline_directive* directives,
+                                       const int32_t* free_ids, int64_t n_free, leyline_plan_t** out) {
+    if (!out) return LEYLINE_E_INVALID;
+    *out = nullptr;
+    int E = 2, pshift = 0;
+    leyline_status st = check_desc(desc, &E, &pshift);
+    if (st != LEYLINE_OK) return st;
+    if (mode != LEYLINE_FRESH && mode != LEYLINE_INPLACE_MOVE && mode != LEYLINE_ROTATE_ONLY) return LEYLINE_E_INVALID;
+    if (n_requests < 0 || n_directives < 0 || n_free < 0) return LEYLINE_E_INVALID;
+    if (n_requests > 0 && (!seq_lens || !pt_offsets)) return LEYLINE_E_INVALID;
+    if (n_directives > 0 && !directives) return LEYLINE_E_INVALID;
+    if (n_free > 0 && !free_ids) return LEYLINE_E_INVALID;
+    const int64_t P = desc->page_size;
+    const int64_t pool_pages = desc->pool_slots / P;
+    for (int32_t r = 0; r < n_requests; ++r) {
+        if (seq_lens[r] < 0 || pt_offsets[r] < 0 || pt_offsets[r + 1] < pt_offsets[r]) return LEYLINE_E_INVALID;
+        int64_t need = ceil_div(seq_lens[r], P);
+        if (pt_offsets[r + 1] - pt_offsets[r] < need) return LEYLINE_E_INVALID;
+        if (need > 0 && !pages) return LEYLINE_E_INVALID;
+        for (int64_t p = 0; p < need; ++p) {
+            int32_t id = pages[pt_offsets[r] + p];
+            if (id < 0 || id >= pool_pages) return LEYLINE_E_RANGE;
+        }
+    }
+    const int64_t free_limit = mode == LEYLINE_ROTATE_ONLY ? desc->pool_slots : pool_pages;
+    st = check_directives(n_requests, seq_lens, n_directives, directives);
+    if (st != LEYLINE_OK) return st;
+
+    leyline_plan_s* pl = new (std::nothrow) leyline_plan_s();
+    if (!pl) return LEYLINE_E_INVALID;
+    pl->desc = *desc;
+    const int H = desc->rope_dim / 2;
+    pl->inv_freq.assign(desc->inv_freq, desc->inv_freq + H);
+    pl->desc.inv_freq = pl->inv_freq.data();
+    if (desc->layer_scale) pl->layer_scale.assign(desc->layer_scale, desc->layer_scale + desc->n_layers);
+    pl->desc.layer_scale = pl->layer_scale.empty() ? nullptr : pl->layer_scale.data();
+    pl->mode = mode;
+    pl->n_requests = n_requests;
+    pl->elem_bytes = E;
+    pl->page_shift = pshift;
+    pl->tuning = g_tuning;
+    pl->tile_rows = choose_tile_rows(*desc, E, g_tuning);
+    const int TR = pl->tile_rows;
+
+    /* tabs: old page tables first, one row per request */
+    std::vector<int32_t> old_tab_off(n_requests + 1, 0);
+    for (int32_t r = 0; r < n_requests; ++r) {
+        int64_t need = ceil_div(seq_lens[r], P);
+        old_tab_off[r] = (int32_t)pl->tabs.size();
+        pl->tabs.insert(pl->tabs.end(), pages + (need ? pt_offsets[r] : 0), pages + (need ? pt_offsets[r] : 0) + need);
+    }
+    old_tab_off[n_requests] = (int32_t)pl->tabs.size();
+
+    std::map<int64_t, int32_t> trig_of;
+    auto trig_index = [&](int64_t C) -> int32_t {
+        if (C == 0) return -1; /* G19: a zero shift is a byte copy, never arithmetic */
+        auto it = trig_of.find(C);
+        if (it != trig_of.end()) return it->second;
+        int32_t g = (int32_t)pl->trig_shifts.size();
+        trig_of.emplace(C, g);
+        pl->trig_shifts.push_back(C);
+        for (int i = 0; i < H; ++i) pl->trig.push_back((float)std::cos((double)C * (double)pl->inv_freq[i]));
+        for (int i = 0; i < H; ++i) pl->trig.push_back((float)std::sin((double)C * (double)pl->inv_freq[i]));
+        return g;
+    };
+
+    pl->old_seq_lens.assign(seq_lens, seq_lens + n_requests);
+    pl->new_seq_lens.resize(n_requests);
+    pl->forget_trim.resize(n_requests);
+    pl->slot_offsets.assign(n_requests + 1, 0);
+    pl->new_pt_offsets.assign(n_requests + 1, 0);
+
+    struct ReqWork { std::vector<Seg> segs; int64_t k0; int32_t new_tab; };
+    std::vector<ReqWork> work(n_requests);
+    std::vector<int32_t> token_lists;               /* ROTATE_ONLY: consumed free slots, in consumption order */
+    std::vector<DevTile> move_tiles, insert_tiles;
+    int64_t consumed = 0;
+    int32_t di = 0;
+    bool nofree = false, badfree = false;
+
+    auto take_free = [&]() -> int32_t {
+        if (consumed >= n_free) { nofree = true; return 0; }
+        int32_t id = free_ids[consumed++];
+        if (id < 0 || id >= free_limit) badfree = true;
+        return id;
+    };
+
+    /* pass 1: segments, maps, released lists (requests ascending, free ids front to back) */
+    for (int32_t r = 0; r < n_requests && !nofree; ++r) {
+        int32_t d0 = di;
+        while (di < n_directives && directives[di].request == r) ++di;
+        const int32_t k = di - d0;
+        const int64_t L_old = seq_lens[r];
+        ReqWork& w = work[r];
+        int64_t trim = -1;
+        const int64_t L_new = build_segments(L_old, directives + d0, k, w.segs, &trim);
+        pl->new_seq_lens[r] = L_new;
+        pl->forget_trim[r] = trim;
+        pl->slot_offsets[r + 1] = pl->slot_offsets[r] + L_new;
+        for (const Seg& s : w.segs)
+            pl->segments.push_back({r, s.kind, s.src, s.dst, s.len, s.shift});
+        const int64_t n_old = ceil_div(L_old, P), n_new = ceil_div(L_new, P);
+        const int32_t* old_row = pl->tabs.data() + old_tab_off[r];
+        if (mode == LEYLINE_FRESH) {
+            /* M1: pages before the first edited page kept, the rest compacted into fresh pages */
+            if (k == 0) {
+                w.k0 = n_old;
+                pl->new_pages.insert(pl->new_pages.end(), old_row, old_row + n_old);
+            } else {
+                w.k0 = directives[d0].start / P;
+                pl->new_pages.insert(pl->new_pages.end(), old_row, old_row + w.k0);
+                for (int64_t p = w.k0; p < n_new && !nofree; ++p) pl->new_pages.push_back(take_free());
+                for (int64_t p = w.k0; p < n_old; ++p) pl->released.push_back(old_row[p]);
+            }
+        } else if (mode == LEYLINE_INPLACE_MOVE) {
+            /* M2: identity on the common pages, growth appends, shrink releases the tail */
+            for (int64_t p = 0; p < n_new && !nofree; ++p) pl->new_pages.push_back(p < n_old ? old_row[p] : take_free());
+            for (int64_t p = n_new; p < n_old; ++p) pl->released.push_back(old_row[p]);
+        } else {
+            /* M3: no row moves; removed positions' slots are released in order */
+            int64_t pos = 0;
+            auto slot_old = [&](int64_t t) { return (int32_t)(((int64_t)old_row[t >> pshift] << pshift) | (t & (P - 1))); };
+            for (const Seg& s : w.segs) {
+                if (s.kind == 0) {
+                    for (int64_t t = pos; t < s.src; ++t) pl->released.push_back(slot_old(t));
+                    pos = s.src + s.len;
+                } else {
+                    for (int64_t q = 0; q < s.len && !nofree; ++q) token_lists.push_back(take_free());
+                }
+            }
+            for (int64_t t = pos; t < L_old; ++t) pl->released.push_back(slot_old(t));
+        }
+        pl->new_pt_offsets[r + 1] = (int64_t)pl->new_pages.size();
+    }
+    if (nofree || badfree) {
+        delete pl;
+        return nofree ? LEYLINE_E_NOFREE : LEYLINE_E_RANGE;
+    }
+
+    /* tabs: new page tables, then token-level lists */
+    const int32_t new_tab_base = (int32_t)pl->tabs.size();
+    pl->tabs.insert(pl->tabs.end(), pl->new_pages.begin(), pl->new_pages.end());
+    const int32_t token_base = (int32_t)pl->tabs.size();
+    pl->tabs.insert(pl->tabs.end(), token_lists.begin(), token_lists.end());
+
+    /* pass 2: tiles, index runs */
+    int64_t token_cursor = 0;
+    for (int32_t r = 0; r < n_requests; ++r) {
+        ReqWork& w = work[r];
+        const int32_t src_tab = old_tab_off[r];
+        const int32_t dst_tab = new_tab_base + (int32_t)pl->new_pt_offsets[r];
+        if (mode == LEYLINE_ROTATE_ONLY) {
+            for (const Seg& s : w.segs) {
+                if (s.kind == 0) {
+                    pl->slot_runs.push_back({pl->slot_offsets[r] + s.dst, s.len, s.src, src_tab, 0});
+                    int32_t g = trig_index(s.shift);
+                    if (g < 0) continue;
+                    split_tiles(s.src, s.dst, s.len, s.src, TR, [&](int64_t a, int64_t b, int32_t n) {
+                        move_tiles.push_back({a, b, src_tab, src_tab, n, g, 0, 0, -1, r});
+                    });
+                } else {
+                    int32_t list = token_base + (int32_t)token_cursor;
+                    pl->slot_runs.push_back({pl->slot_offsets[r] + s.dst, s.len, 0, list, 1});
+                    split_tiles(s.src, 0, s.len, 0, TR, [&](int64_t a, int64_t b, int32_t n) {
+                        insert_tiles.push_back({a, b, -1, list, n, -1, leyline::TILE_SRC_REPL | leyline::TILE_DST_TOKEN,
+                                                0, -1, r});
+                    });
+                    token_cursor += s.len;
+                }
+            }
+            continue;
+        }
+        if (pl->new_seq_lens[r] > 0)
+            pl->slot_runs.push_back({pl->slot_offsets[r], pl->new_seq_lens[r], 0, dst_tab, 0});
+        if (mode == LEYLINE_FRESH) {
+            const int64_t first = w.k0 * P; /* new positions >= first live in fresh pages and must be written */
+            for (const Seg& s : w.segs) {
+                if (s.kind == 1) {
+                    split_tiles(s.src, s.dst, s.len, s.dst, TR, [&](int64_t a, int64_t b, int32_t n) {
+                        insert_tiles.push_back({a, b, -1, dst_tab, n, -1, leyline::TILE_SRC_REPL, 0, -1, r});
+                    });
+                    continue;
+                }
+                int64_t skip = std::max<int64_t>(0, first - s.dst);
+                if (skip >= s.len) continue;
+                int32_t g = trig_index(s.shift);
+                split_tiles(s.src + skip, s.dst + skip, s.len - skip, s.dst + skip, TR,
+                            [&](int64_t a, int64_t b, int32_t n) {
+                                move_tiles.push_back({a, b, src_tab, dst_tab, n, g, 0, 0, -1, r});
+                            });
+            }
+        } else { /* INPLACE_MOVE, rule M2 */
+            std::vector<DevTile> left, right;
+            for (const Seg& s : w.segs) {
+                if (s.kind == 1) {
+                    split_tiles(s.src, s.dst, s.len, s.dst, TR, [&](int64_t a, int64_t b, int32_t n) {
+                        insert_tiles.push_back({a, b, -1, dst_tab, n, -1, leyline::TILE_SRC_REPL, 0, -1, r});
+                    });
+                    continue;
+                }
+                if (s.shift == 0) continue; /* stays where it is, bytes untouched */
+                int32_t g = trig_index(s.shift);
+                std::vector<DevTile>& grp = s.shift < 0 ? left : right;
+                split_tiles(s.src, s.dst, s.len, s.dst, TR, [&](int64_t a, int64_t b, int32_t n) {
+                    grp.push_back({a, b, src_tab, dst_tab, n, g, 0, 0, -1, r});
+                });
+            }
+            /* left-shifters ascending: a tile's destination covers source rows of tiles at lower positions */
+            const int32_t base_l = (int32_t)move_tiles.size();
+            for (size_t i = 0, lo = 0; i < left.size(); ++i) {
+                DevTile t = left[i];
+                const int64_t d0 = t.dst_pos, d1 = t.dst_pos + t.n_rows;
+                while (lo < i && left[lo].src_pos + left[lo].n_rows <= d0) ++lo;
+                size_t hi = lo; /* first tile at or after lo whose source starts at or past d1 */
+                while (hi < i && left[hi].src_pos < d1) ++hi;
+                t.dep_lo = base_l + (int32_t)lo;
+                t.dep_hi = base_l + (int32_t)hi - 1;
+                move_tiles.push_back(t);
+            }
+            /* right-shifters descending: destination covers source rows of tiles at higher positions */
+            const int32_t base_r = (int32_t)move_tiles.size();
+            std::reverse(right.begin(), right.end());
+            for (size_t i = 0, lo = 0; i < right.size(); ++i) {
+                DevTile t = right[i];
+                const int64_t d0 = t.dst_pos, d1 = t.dst_pos + t.n_rows;
+                while (lo < i && right[lo].src_pos >= d1) ++lo;
+                size_t hi = lo;
+                while (hi < i && right[hi].src_pos + right[hi].n_rows > d0) ++hi;
+                t.dep_lo = base_r + (int32_t)lo;
+                t.dep_hi = base_r + (int32_t)hi - 1;
+                move_tiles.push_back(t);
+            }
+        }
+    }
+    if (mode != LEYLINE_ROTATE_ONLY && !pl->new_pages.empty())
+        pl->page_runs.push_back({0, (int64_t)pl->new_pages.size(), new_tab_base, 0, 2});
+
+    leyline_plan_info& in = pl->info;
+    in.mode = mode;
+    in.n_requests = n_requests;
+    in.total_new_tokens = pl->slot_offsets[n_requests];
+    in.total_new_pages = mode == LEYLINE_ROTATE_ONLY ? 0 : (int64_t)pl->new_pages.size();
+    in.n_free_consumed = consumed;
+    in.n_released = (int64_t)pl->released.size();
+    in.n_segments = (int64_t)pl->segments.size();
+    in.n_move_tiles = (int64_t)move_tiles.size();
+    in.n_tiles = (int64_t)(move_tiles.size() + insert_tiles.size());
+    in.n_trig = (int64_t)pl->trig_shifts.size();
+    for (const DevTile& t : move_tiles) {
+        if (mode != LEYLINE_ROTATE_ONLY) in.rows_moved += t.n_rows;
+        if (t.trig >= 0) in.rows_rotated += t.n_rows;
+    }
+    for (const DevTile& t : insert_tiles) in.rows_inserted += t.n_rows;
+    const int64_t row_bytes = (int64_t)(desc->latent_dim + desc->rope_dim) * E, band_bytes = (int64_t)desc->rope_dim * E;
+    int64_t per_layer = (in.rows_moved + in.rows_inserted) * row_bytes;
+    if (mode == LEYLINE_ROTATE_ONLY) per_layer = in.rows_rotated * band_bytes + in.rows_inserted * row_bytes;
+    in.bytes_read = in.bytes_written = per_layer * desc->n_layers;
+    in.bytes_index = 4 * in.total_new_tokens + 4 * in.total_new_pages;
+    if (mode == LEYLINE_ROTATE_ONLY) pl->new_pages.clear();
+
+    pl->tiles = std::move(move_tiles);
+    pl->tiles.insert(pl->tiles.end(), insert_tiles.begin(), insert_tiles.end());
+    *out = pl;
+    return LEYLINE_OK;
+}
+
+/* ------------------------------------------------------------------ queries ---- */
+
+#define LEYLINE_GETTER(name, type, member)                                         \
+    extern "C" leyline_status name(const leyline_plan_t* plan, type* out) {        \
+        if (!plan || (!out && !plan->member.empty())) return LEYLINE_E_INVALID;    \
+        if (!plan->member.empty()) std::memcpy(out, plan->member.data(), plan->member.size() * sizeof(type)); \
+        return LEYLINE_OK;                                                         \
+    }
+
+extern "C" leyline_status leyline_plan_get_info(const leyline_plan_t* plan, leyline_plan_info* out) {
+    if (!plan || !out) return LEYLINE_E_INVALID;
+    *out = plan->info;
+    return LEYLINE_OK;
+}
+LEYLINE_GETTER(leyline_plan_new_seq_lens, int64_t, new_seq_lens)
+LEYLINE_GETTER(leyline_plan_forget_trim, int64_t, forget_trim)
+LEYLINE_GETTER(leyline_plan_slot_offsets, int64_t, slot_offsets)
+LEYLINE_GETTER(leyline_plan_released, int32_t, released)
+LEYLINE_GETTER(leyline_plan_segments, leyline_segment, segments)
+LEYLINE_GETTER(leyline_plan_trig_shifts, int64_t, trig_shifts)
+
+extern "C" leyline_status leyline_plan_new_pt_offsets(const leyline_plan_t* plan, int64_t* out) {
+    if (!plan || !out || plan->mode == LEYLINE_ROTATE_ONLY) return LEYLINE_E_INVALID;
+    std::memcpy(out, plan->new_pt_offsets.data(), plan->new_pt_offsets.size() * sizeof(int64_t));
+    return LEYLINE_OK;
+}
+
+extern "C" leyline_status leyline_plan_new_pages(const leyline_plan_t* plan, int32_t* out) {
+    if (!plan || plan->mode == LEYLINE_ROTATE_ONLY || (!out && !plan->new_pages.empty())) return LEYLINE_E_INVALID;
+    if (!plan->new_pages.empty()) std::memcpy(out, plan->new_pages.data(), plan->new_pages.size() * sizeof(int32_t));
+    return LEYLINE_OK;
+}
+
+extern "C" leyline_status leyline_plan_tiles(const leyline_plan_t* plan, leyline_tile* out) {
+    if (!plan || (!out && !plan->tiles.empty())) return LEYLINE_E_INVALID;
+    for (size_t i = 0; i < plan->tiles.size(); ++i) {
+        const DevTile& t = plan->tiles[i];
+        out[i].src_pos = t.src_pos;
+        out[i].dst_pos = t.dst_pos;
+        out[i].n_rows = t.n_rows;
+        out[i].trig = t.trig;
+        out[i].flags = t.flags & LEYLINE_TILE_SRC_REPL;
+        out[i].dep_lo = t.dep_lo;
+        out[i].dep_hi = t.dep_hi;
+        out[i].request = t.request;
+    }
+    return LEYLINE_OK;
+}
+
+/* cos/sin table rows, [n_trig][2][rope_dim/2] fp32 (tests check them against an independent fp64 evaluation) */
+extern "C" leyline_status leyline_plan_trig_table(const leyline_plan_t* plan, float* out) {
+    if (!plan || (!out && !plan->trig.empty())) return LEYLINE_E_INVALID;
+    if (!plan->trig.empty()) std::memcpy(out, plan->trig.data(), plan->trig.size() * sizeof(float));
+    return LEYLINE_OK;
+}
+
+extern "C" void leyline_plan_destroy(leyline_plan_t* plan) {
+    if (!plan) return;
+    leyline_plan_release_device_(plan);
+    delete plan;
+}
+
+extern "C" const char* leyline_strerror(leyline_status s) {
+    switch (s) {
+        case LEYLINE_OK: return "ok";
+        case LEYLINE_E_INVALID: return "invalid argument";
+        case LEYLINE_E_UNSORTED: return "directives not sorted by (request, start)";
+        case LEYLINE_E_OVERLAP: return "overlapping spans";
+        case LEYLINE_E_RANGE: return "request, span or id out of range";
+        case LEYLINE_E_NOFREE: return "free list too short";
+        case LEYLINE_E_UNSUPPORTED: return "cache geometry not supported by the kernels";
+        case LEYLINE_E_CUDA: return "CUDA error";
+    }
+    return "unknown status";
+}
+
+extern "C" leyline_status leyline_set_tuning(const leyline_tuning* t) {
+    if (!t) return LEYLINE_E_INVALID;
+    if (t->kernel < 0 || t->kernel > 2 || t->tile_rows < 0 || t->tile_rows > 32 || t->ctas_per_sm < 0 ||
+        t->ctas_per_sm > 32)
+        return LEYLINE_E_INVALID;
+    g_tuning = *t;
+    return LEYLINE_OK;
+}
+
+extern "C" leyline_status leyline_get_tuning(leyline_tuning* t) {
+    if (!t) return LEYLINE_E_INVALID;
+    *t = g_tuning;
+    return LEYLINE_OK;
+}
+
+extern "C" const char* leyline_version(void) { return "leyline-b200 0.1 sm_100a"; }

@@ -1,0 +1,85 @@
+/*
+ * plan_internal.h -- the plan object shared by the host planner (plan.cpp) and the launchers (splice.cu).
+ * Not part of the ABI.  See include/leyline.h for the contract and DESIGN.md for the rules (M1-M3, V).
+ */
+#ifndef LEYLINE_PLAN_INTERNAL_H_
+#define LEYLINE_PLAN_INTERNAL_H_
+
+#include <cstdint>
+#include <vector>
+
+#include "leyline.h"
+
+namespace leyline {
+
+/* Device work item: up to tile_rows rows that are consecutive in NEW logical position (one segment, hence one
+ * rotation).  Source and destination rows are located through int32 tables in `tabs`:
+ *   slot(pos) = tabs[tab + (pos >> shift)] << shift | (pos & ((1 << shift) - 1))
+ * with shift = log2(page_size) for page tables and 0 for token-level slot lists.  src_tab < 0: the source is
+ * the replacement buffer and src_pos is the row inside it. */
+struct DevTile {
+    int64_t src_pos;
+    int64_t dst_pos;
+    int32_t src_tab;
+    int32_t dst_tab;
+    int32_t n_rows;
+    int32_t trig;      /* row of the cos/sin table, -1 = byte copy */
+    int32_t flags;     /* bit 0: source is the replacement buffer; bit 1: dst table is token-level (shift 0) */
+    int32_t dep_lo;    /* INPLACE_MOVE: tiles [dep_lo, dep_hi] must have loaded (same layer) before this stores */
+    int32_t dep_hi;
+    int32_t request;
+};
+static_assert(sizeof(DevTile) == 48, "DevTile layout");
+
+enum : int32_t { TILE_SRC_REPL = 1, TILE_DST_TOKEN = 2 };
+
+/* One run of the token-level index list / page-table output (step a2). */
+struct IdxRun {
+    int64_t out_begin; /* first output element */
+    int64_t length;
+    int64_t pos0;      /* kind 0/1: first logical position; kind 2: first element of `tabs` to copy */
+    int32_t tab;       /* kind 0: page table offset in tabs; kind 1: token-level list offset */
+    int32_t kind;      /* 0 = via page table (shift = log2 P), 1 = via token-level list, 2 = raw copy of tabs */
+};
+static_assert(sizeof(IdxRun) == 32, "IdxRun layout");
+
+}  // namespace leyline
+
+struct leyline_plan_s {
+    leyline_cache_desc desc;            /* inv_freq / layer_scale pointers redirected to the copies below */
+    std::vector<float> inv_freq;
+    std::vector<float> layer_scale;
+    int32_t mode = 0;
+    int32_t n_requests = 0;
+    int32_t elem_bytes = 2;
+    int32_t page_shift = 0;
+    int32_t tile_rows = 32;
+    leyline_tuning tuning{};
+
+    std::vector<int64_t> old_seq_lens, new_seq_lens, forget_trim, slot_offsets, new_pt_offsets, old_pt_offsets;
+    std::vector<int32_t> new_pages;     /* concatenated new page-table rows (FRESH / INPLACE_MOVE) */
+    std::vector<int32_t> released;
+    std::vector<leyline_segment> segments;
+    std::vector<leyline::DevTile> tiles;   /* move tiles first, then insert tiles; ticket order */
+    std::vector<int64_t> trig_shifts;
+    std::vector<float> trig;            /* [n_trig][2][H]: cos then sin of C * theta_i, fp64 libm rounded to fp32 */
+    std::vector<int32_t> tabs;          /* old page tables ++ new page tables ++ token-level lists */
+    std::vector<leyline::IdxRun> slot_runs;  /* produce dev_slot_idx_out */
+    std::vector<leyline::IdxRun> page_runs;  /* produce dev_page_table_out */
+    leyline_plan_info info{};
+
+    /* device side (owned by splice.cu; created on first launch, freed by leyline_plan_destroy) */
+    void* d_blob = nullptr;             /* tiles | trig | tabs | slot_runs | page_runs */
+    int64_t off_tiles = 0, off_trig = 0, off_tabs = 0, off_slot_runs = 0, off_page_runs = 0, blob_bytes = 0;
+    void* d_scratch = nullptr;          /* [0,256): ticket counters; then hazard flags [n_move_tiles * n_layers] int32 */
+    int64_t scratch_bytes = 0;
+    int device = -1;
+    void* ev_start = nullptr;           /* cudaEvent_t pair around the data-moving kernels (tuning.profile) */
+    void* ev_stop = nullptr;
+    void* last_stream = nullptr;        /* stream of the last launch: the device tables are freed on it */
+};
+
+/* implemented in splice.cu; plan.cpp calls it from leyline_plan_destroy */
+extern "C" void leyline_plan_release_device_(leyline_plan_s* plan);
+
+#endif /* LEYLINE_PLAN_INTERNAL_H_ */

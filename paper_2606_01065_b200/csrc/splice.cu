@@ -1,0 +1,313 @@
+/*
+ * splice.cu -- leyline_splice / leyline_rotate_inplace: upload the plan's tables once, then launch
+ * the index rewrite (a2) and the fused gather -> rotate -> scatter (+ insert) kernels (a3, a4, a5) on the
+ * caller's stream.  No synchronisation, no CPU fallback: every failure is a LEYLINE_E_CUDA status.
+ */
+#include <cstdio>
+#include <cstring>
+#include <string>
+
+#include "kernels_rows.cuh"
+
+using namespace leyline;
+
+namespace {
+
+thread_local std::string g_last_error;
+
+bool cuda_ok(cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return true;
+    g_last_error = std::string(what) + ": " + cudaGetErrorString(e);
+    (void)cudaGetLastError(); /* clear the sticky-less error state */
+    return false;
+}
+#define CU(call) do { if (!cuda_ok((call), #call)) return LEYLINE_E_CUDA; } while (0)
+
+inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
+
+struct DeviceInfo { int device = -1; int sms = 0; };
+DeviceInfo g_dev;
+
+leyline_status ensure_device(leyline_plan_s* pl, cudaStream_t stream) {
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    if (g_dev.device != dev) {
+        cudaDeviceProp prop;
+        CU(cudaGetDeviceProperties(&prop, dev));
+        g_dev.device = dev;
+        g_dev.sms = prop.multiProcessorCount;
+    }
+    if (pl->d_blob || pl->device >= 0) {
+        if (pl->device != dev) { g_last_error = "plan was uploaded on another device"; return LEYLINE_E_CUDA; }
+        return LEYLINE_OK;
+    }
+    /* one blob: tiles | trig | tabs | slot_runs | page_runs, each 256-byte aligned */
+    int64_t off = 0;
+    auto place = [&](int64_t bytes) { int64_t o = off; off = align_up(off + bytes, 256); return o; };
+    pl->off_tiles = place((int64_t)pl->tiles.size() * sizeof(DevTile));
+    pl->off_trig = place((int64_t)pl->trig.size() * sizeof(float));
+    pl->off_tabs = place((int64_t)pl->tabs.size() * sizeof(int32_t));
+    pl->off_slot_runs = place((int64_t)pl->slot_runs.size() * sizeof(IdxRun));
+    pl->off_page_runs = place((int64_t)pl->page_runs.size() * sizeof(IdxRun));
+    pl->blob_bytes = off > 0 ? off : 256;
+    std::string host((size_t)pl->blob_bytes, '\0');
+    auto put = [&](int64_t o, const void* src, size_t bytes) { if (bytes) std::memcpy(&host[(size_t)o], src, bytes); };
+    put(pl->off_tiles, pl->tiles.data(), pl->tiles.size() * sizeof(DevTile));
+    put(pl->off_trig, pl->trig.data(), pl->trig.size() * sizeof(float));
+    put(pl->off_tabs, pl->tabs.data(), pl->tabs.size() * sizeof(int32_t));
+    put(pl->off_slot_runs, pl->slot_runs.data(), pl->slot_runs.size() * sizeof(IdxRun));
+    put(pl->off_page_runs, pl->page_runs.data(), pl->page_runs.size() * sizeof(IdxRun));
+    const int64_t n_flags = pl->mode == LEYLINE_INPLACE_MOVE ? pl->info.n_move_tiles * pl->desc.n_layers : 0;
+    pl->scratch_bytes = 256 + align_up(n_flags * (int64_t)sizeof(int32_t), 256);
+    CU(cudaMallocAsync(&pl->d_blob, (size_t)pl->blob_bytes, stream));
+    if (!cuda_ok(cudaMallocAsync(&pl->d_scratch, (size_t)pl->scratch_bytes, stream), "cudaMallocAsync(scratch)")) {
+        cudaFreeAsync(pl->d_blob, stream);
+        pl->d_blob = nullptr;
+        return LEYLINE_E_CUDA;
+    }
+    /* pageable source: the runtime stages it before returning, so `host` may go out of scope */
+    CU(cudaMemcpyAsync(pl->d_blob, host.data(), (size_t)pl->blob_bytes, cudaMemcpyHostToDevice, stream));
+    pl->device = dev;
+    return LEYLINE_OK;
+}
+
+template <class T>
+const T* blob_at(const leyline_plan_s* pl, int64_t off) {
+    return reinterpret_cast<const T*>(static_cast<const uint8_t*>(pl->d_blob) + off);
+}
+
+leyline_status launch_index(const leyline_plan_s* pl, const std::vector<IdxRun>& runs, int64_t off, int32_t* out,
+                            cudaStream_t stream) {
+    if (!out || runs.empty()) return LEYLINE_OK;
+    IndexParams ip;
+    ip.runs = blob_at<IdxRun>(pl, off);
+    ip.tabs = blob_at<int32_t>(pl, pl->off_tabs);
+    ip.out = out;
+    ip.total = runs.back().out_begin + runs.back().length;
+    ip.n_runs = (int32_t)runs.size();
+    ip.page_shift = pl->page_shift;
+    if (ip.total <= 0) return LEYLINE_OK;
+    long long blocks = (ip.total + kThreads - 1) / kThreads;
+    if (blocks > 8LL * g_dev.sms) blocks = 8LL * g_dev.sms;
+    k_index<<<(unsigned)blocks, kThreads, 0, stream>>>(ip);
+    CU(cudaGetLastError());
+    return LEYLINE_OK;
+}
+
+using MoveKernel = void (*)(const MoveParams);
+
+template <int DT, int PAIRING, bool HAZARD>
+MoveKernel pick_move_geom(const leyline_plan_s* pl) {
+    const int lc = pl->desc.latent_dim * pl->elem_bytes / 16, nb = pl->desc.rope_dim * pl->elem_bytes / 16;
+    if (DT == LEYLINE_BF16 && lc == 64 && nb == 8) return k_move_rows<DT, PAIRING, HAZARD, 64, 8>;
+    if (DT == LEYLINE_FP8_E4M3 && lc == 32 && nb == 4) return k_move_rows<DT, PAIRING, HAZARD, 32, 4>;
+    return k_move_rows<DT, PAIRING, HAZARD, -1, -1>;
+}
+template <int DT, int PAIRING>
+MoveKernel pick_move_hazard(const leyline_plan_s* pl, bool hazard) {
+    return hazard ? pick_move_geom<DT, PAIRING, true>(pl) : pick_move_geom<DT, PAIRING, false>(pl);
+}
+MoveKernel pick_move(const leyline_plan_s* pl, bool hazard) {
+    const bool neox = pl->desc.pairing == LEYLINE_ROPE_NEOX;
+    if (pl->desc.dtype == LEYLINE_BF16)
+        return neox ? pick_move_hazard<LEYLINE_BF16, LEYLINE_ROPE_NEOX>(pl, hazard)
+                    : pick_move_hazard<LEYLINE_BF16, LEYLINE_ROPE_INTERLEAVED>(pl, hazard);
+    return neox ? pick_move_hazard<LEYLINE_FP8_E4M3, LEYLINE_ROPE_NEOX>(pl, hazard)
+                : pick_move_hazard<LEYLINE_FP8_E4M3, LEYLINE_ROPE_INTERLEAVED>(pl, hazard);
+}
+
+MoveKernel pick_rotate(const leyline_plan_s* pl) {
+    const bool neox = pl->desc.pairing == LEYLINE_ROPE_NEOX;
+    const int nb = pl->desc.rope_dim * pl->elem_bytes / 16;
+    if (pl->desc.dtype == LEYLINE_BF16) {
+        if (nb == 8) return neox ? k_rotate_band<LEYLINE_BF16, LEYLINE_ROPE_NEOX, 8> : k_rotate_band<LEYLINE_BF16, LEYLINE_ROPE_INTERLEAVED, 8>;
+        return neox ? k_rotate_band<LEYLINE_BF16, LEYLINE_ROPE_NEOX, -1> : k_rotate_band<LEYLINE_BF16, LEYLINE_ROPE_INTERLEAVED, -1>;
+    }
+    if (nb == 4) return neox ? k_rotate_band<LEYLINE_FP8_E4M3, LEYLINE_ROPE_NEOX, 4> : k_rotate_band<LEYLINE_FP8_E4M3, LEYLINE_ROPE_INTERLEAVED, 4>;
+    return neox ? k_rotate_band<LEYLINE_FP8_E4M3, LEYLINE_ROPE_NEOX, -1> : k_rotate_band<LEYLINE_FP8_E4M3, LEYLINE_ROPE_INTERLEAVED, -1>;
+}
+
+}  // namespace
+
+namespace {
+
+struct OccCache { const void* fn; int smem; int blocks; };
+OccCache g_occ[64];
+int g_occ_n = 0;
+
+int occupancy(const void* fn, int smem) {
+    for (int i = 0; i < g_occ_n; ++i)
+        if (g_occ[i].fn == fn && g_occ[i].smem == smem) return g_occ[i].blocks;
+    int blocks = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks, fn, kThreads, (size_t)smem) != cudaSuccess || blocks < 1) {
+        (void)cudaGetLastError();
+        blocks = 1;
+    }
+    if (g_occ_n < 64) g_occ[g_occ_n++] = {fn, smem, blocks};
+    return blocks;
+}
+
+void fill_params(const leyline_plan_s* pl, MoveParams& mp, int32_t tile_begin, int64_t tile_count, int l0, int nl,
+                 void* const* layer_src, void* const* layer_dst, const void* const* layer_repl, int ticket_slot) {
+    std::memset(&mp, 0, sizeof(mp));
+    mp.tiles = blob_at<DevTile>(pl, pl->off_tiles);
+    mp.trig = blob_at<float>(pl, pl->off_trig);
+    mp.tabs = blob_at<int32_t>(pl, pl->off_tabs);
+    mp.ticket = reinterpret_cast<unsigned long long*>(pl->d_scratch) + ticket_slot;
+    mp.flags = reinterpret_cast<int32_t*>(static_cast<uint8_t*>(pl->d_scratch) + 256);
+    mp.n_items = (long long)tile_count * nl;
+    mp.stride = pl->desc.row_stride_bytes;
+    mp.tile_begin = tile_begin;
+    mp.n_layers = nl;
+    mp.layer0 = l0;
+    mp.n_layers_total = pl->desc.n_layers;
+    mp.page_shift = pl->page_shift;
+    mp.H = pl->desc.rope_dim / 2;
+    mp.lat_chunks = pl->desc.latent_dim * pl->elem_bytes / 16;
+    mp.band_chunks = pl->desc.rope_dim * pl->elem_bytes / 16;
+    for (int l = 0; l < nl; ++l) {
+        mp.src[l] = static_cast<const uint8_t*>(layer_src ? layer_src[l0 + l] : nullptr);
+        mp.dst[l] = static_cast<uint8_t*>(layer_dst[l0 + l]);
+        mp.repl[l] = static_cast<const uint8_t*>(layer_repl ? layer_repl[l0 + l] : nullptr);
+    }
+}
+
+/* Launch `fn` over tiles [tile_begin, tile_begin + tile_count) x all layers (chunks of kMaxLayers). */
+leyline_status run_tiles(leyline_plan_s* pl, MoveKernel fn, int smem, int max_ctas_per_sm, int32_t tile_begin,
+                         int64_t tile_count, void* const* layer_src, void* const* layer_dst,
+                         const void* const* layer_repl, cudaStream_t stream, int* ticket_slot) {
+    if (tile_count <= 0) return LEYLINE_OK;
+    const int L = pl->desc.n_layers;
+    for (int l0 = 0; l0 < L; l0 += kMaxLayers) {
+        const int nl = L - l0 < kMaxLayers ? L - l0 : kMaxLayers;
+        if (*ticket_slot >= 32) { g_last_error = "too many launches for one plan"; return LEYLINE_E_UNSUPPORTED; }
+        MoveParams mp;
+        fill_params(pl, mp, tile_begin, tile_count, l0, nl, layer_src, layer_dst, layer_repl, (*ticket_slot)++);
+        int per_sm = occupancy(reinterpret_cast<const void*>(fn), smem);
+        if (max_ctas_per_sm > 0 && per_sm > max_ctas_per_sm) per_sm = max_ctas_per_sm;
+        long long grid = (long long)g_dev.sms * per_sm;
+        if (grid > mp.n_items) grid = mp.n_items;
+        fn<<<(unsigned)grid, kThreads, (size_t)smem, stream>>>(mp);
+        CU(cudaGetLastError());
+    }
+    return LEYLINE_OK;
+}
+
+leyline_status check_layers(const leyline_plan_s* pl, const void* const* a, const char* what) {
+    if (!a) { g_last_error = std::string(what) + " is NULL"; return LEYLINE_E_INVALID; }
+    for (int l = 0; l < pl->desc.n_layers; ++l)
+        if (!a[l] || (reinterpret_cast<uintptr_t>(a[l]) & 15)) {
+            g_last_error = std::string(what) + ": NULL or not 16-byte aligned layer pointer";
+            return LEYLINE_E_INVALID;
+        }
+    return LEYLINE_OK;
+}
+
+leyline_status begin_call(leyline_plan_s* pl, cudaStream_t stream) {
+    leyline_status st = ensure_device(pl, stream);
+    if (st != LEYLINE_OK) return st;
+    pl->last_stream = stream;
+    CU(cudaMemsetAsync(pl->d_scratch, 0, (size_t)pl->scratch_bytes, stream));
+    if (pl->tuning.profile && !pl->ev_start) {
+        CU(cudaEventCreate(reinterpret_cast<cudaEvent_t*>(&pl->ev_start)));
+        CU(cudaEventCreate(reinterpret_cast<cudaEvent_t*>(&pl->ev_stop)));
+    }
+    return LEYLINE_OK;
+}
+
+}  // namespace
+
+extern "C" leyline_status leyline_splice(leyline_plan_t* pl, void* const* layer_src, void* const* layer_dst,
+                                         const void* const* layer_repl, int32_t* dev_page_table_out,
+                                         int32_t* dev_slot_idx_out, void* cuda_stream) {
+    g_last_error.clear();
+    if (!pl || pl->mode == LEYLINE_ROTATE_ONLY) return LEYLINE_E_INVALID;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const bool inplace = pl->mode == LEYLINE_INPLACE_MOVE;
+    const int64_t n_move = pl->info.n_move_tiles, n_ins = pl->info.n_tiles - n_move;
+    if (n_move + n_ins > 0) {
+        leyline_status st = check_layers(pl, layer_dst, "layer_dst");
+        if (st == LEYLINE_OK && n_move > 0) st = check_layers(pl, layer_src, "layer_src");
+        if (st == LEYLINE_OK && n_ins > 0) st = check_layers(pl, layer_repl, "layer_repl");
+        if (st != LEYLINE_OK) return st;
+        if (inplace && n_move > 0)
+            for (int l = 0; l < pl->desc.n_layers; ++l)
+                if (layer_src[l] != layer_dst[l]) {
+                    g_last_error = "INPLACE_MOVE needs layer_src == layer_dst";
+                    return LEYLINE_E_INVALID;
+                }
+    }
+    leyline_status st = begin_call(pl, stream);
+    if (st != LEYLINE_OK) return st;
+    /* a2: page-table rows and token-level slot list */
+    st = launch_index(pl, pl->page_runs, pl->off_page_runs, dev_page_table_out, stream);
+    if (st != LEYLINE_OK) return st;
+    st = launch_index(pl, pl->slot_runs, pl->off_slot_runs, dev_slot_idx_out, stream);
+    if (st != LEYLINE_OK) return st;
+    if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_start), stream));
+    int slot = 0;
+    const int cps = pl->tuning.ctas_per_sm;
+    if (inplace) {
+        /* a3 under rule M2 ordering, then a4 once every move has landed (stream order) */
+        st = run_tiles(pl, pick_move(pl, true), 0, cps, 0, n_move, layer_src, layer_dst, layer_repl, stream, &slot);
+        if (st != LEYLINE_OK) return st;
+        st = run_tiles(pl, pick_move(pl, false), 0, cps, (int32_t)n_move, n_ins, layer_src, layer_dst, layer_repl,
+                       stream, &slot);
+    } else {
+        /* a3 + a4 in one launch: fresh pages alias nothing */
+        st = run_tiles(pl, pick_move(pl, false), 0, cps, 0, n_move + n_ins, layer_src, layer_dst, layer_repl, stream,
+                       &slot);
+    }
+    if (st != LEYLINE_OK) return st;
+    if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_stop), stream));
+    return LEYLINE_OK;
+}
+
+extern "C" leyline_status leyline_rotate_inplace(leyline_plan_t* pl, void* const* layer_ptrs,
+                                                 const void* const* layer_repl, int32_t* dev_slot_idx_out,
+                                                 void* cuda_stream) {
+    g_last_error.clear();
+    if (!pl || pl->mode != LEYLINE_ROTATE_ONLY) return LEYLINE_E_INVALID;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const int64_t n_rot = pl->info.n_move_tiles, n_ins = layer_repl ? pl->info.n_tiles - n_rot : 0;
+    if (n_rot + n_ins > 0) {
+        leyline_status st = check_layers(pl, layer_ptrs, "layer_ptrs");
+        if (st == LEYLINE_OK && n_ins > 0) st = check_layers(pl, layer_repl, "layer_repl");
+        if (st != LEYLINE_OK) return st;
+    }
+    leyline_status st = begin_call(pl, stream);
+    if (st != LEYLINE_OK) return st;
+    st = launch_index(pl, pl->slot_runs, pl->off_slot_runs, dev_slot_idx_out, stream);
+    if (st != LEYLINE_OK) return st;
+    if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_start), stream));
+    int slot = 0;
+    /* a5: rotate where the rows sit; a4: replacement rows go to the consumed free slots (disjoint from a5's) */
+    st = run_tiles(pl, pick_rotate(pl), 0, pl->tuning.ctas_per_sm, 0, n_rot, nullptr, layer_ptrs, layer_repl, stream,
+                   &slot);
+    if (st != LEYLINE_OK) return st;
+    st = run_tiles(pl, pick_move(pl, false), 0, pl->tuning.ctas_per_sm, (int32_t)n_rot, n_ins, layer_ptrs, layer_ptrs,
+                   layer_repl, stream, &slot);
+    if (st != LEYLINE_OK) return st;
+    if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_stop), stream));
+    return LEYLINE_OK;
+}
+
+extern "C" leyline_status leyline_plan_kernel_ms(const leyline_plan_t* pl, float* ms) {
+    g_last_error.clear();
+    if (!pl || !ms || !pl->ev_start) return LEYLINE_E_INVALID;
+    CU(cudaEventElapsedTime(ms, static_cast<cudaEvent_t>(pl->ev_start), static_cast<cudaEvent_t>(pl->ev_stop)));
+    return LEYLINE_OK;
+}
+
+extern "C" void leyline_plan_release_device_(leyline_plan_s* pl) {
+    if (pl->ev_start) cudaEventDestroy(static_cast<cudaEvent_t>(pl->ev_start));
+    if (pl->ev_stop) cudaEventDestroy(static_cast<cudaEvent_t>(pl->ev_stop));
+    /* stream-ordered: freed after everything this plan launched on its stream, without a device sync */
+    if (pl->d_blob) cudaFreeAsync(pl->d_blob, static_cast<cudaStream_t>(pl->last_stream));
+    if (pl->d_scratch) cudaFreeAsync(pl->d_scratch, static_cast<cudaStream_t>(pl->last_stream));
+    pl->d_blob = pl->d_scratch = nullptr;
+    pl->ev_start = pl->ev_stop = nullptr;
+    if (pl->device >= 0) (void)cudaGetLastError();
+}
+
+extern "C" const char* leyline_last_cuda_error(void) { return g_last_error.c_str(); }

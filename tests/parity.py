@@ -1,0 +1,126 @@
+"""Test-only: compare the CUDA library (through the binding) with the CPU oracle on the same seeded inputs.
+
+The bar (BASELINE.json north_star):
+  * bit-exact: new sequence lengths, page-table rows, token-level slot list, released list, free ids consumed,
+    segments, every pool byte outside rotated K_pe bands (moved latent, C = 0 segments, replacement rows, and
+    every byte the mode never writes -- other requests, free pool, prefix pages, released pages);
+  * rotated bf16 K_pe: ordinal distance <= 2 bf16 ulp, or |g - o| <= 2^-20 * rho where the result cancels
+    (rho = norm of the input pair; fp32 rounding error does not shrink with the result);
+  * rotated fp8 K_pe: ordinal distance <= 1 e4m3 code (+0 == -0).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+import oracle as O
+from paper_2606_01065_b200 import synth
+
+
+def oracle_plan(w: synth.Workload, mode: int) -> O.BatchMap:
+    free = w.free_slots() if mode == O.ROTATE_ONLY else w.free_pages
+    return O.plan_batch(mode, w.page_size, w.seq_lens, w.pt_offsets, w.pages, w.directives, free)
+
+
+def assert_plan_equal(plan, bm: O.BatchMap, mode: int):
+    """Library plan (binding.Plan) vs oracle BatchMap: everything integer, bit-exact."""
+    assert bm.status == O.OK
+    np.testing.assert_array_equal(plan.new_seq_lens, bm.new_seq_lens)
+    assert plan.info.n_free_consumed == bm.n_consumed
+    np.testing.assert_array_equal(plan.released, bm.released)
+    segs = []
+    for r, rm in enumerate(bm.requests):
+        segs += [(r, k, s, d, n, c) for (k, s, d, n, c) in rm.segs.as_tuples()]
+    assert plan.segments == segs
+    np.testing.assert_array_equal(plan.forget_trim, [rm.segs.forget_trim for rm in bm.requests])
+    if mode != O.ROTATE_ONLY:
+        want = np.concatenate([rm.new_pages for rm in bm.requests]) if bm.requests else np.zeros(0, np.int32)
+        np.testing.assert_array_equal(plan.new_pages, want)
+        off = np.concatenate([[0], np.cumsum([len(rm.new_pages) for rm in bm.requests])])
+        np.testing.assert_array_equal(plan.new_pt_offsets, off)
+    off = np.concatenate([[0], np.cumsum([rm.L_new for rm in bm.requests])])
+    np.testing.assert_array_equal(plan.slot_offsets, off)
+
+
+def oracle_slot_list(bm: O.BatchMap) -> np.ndarray:
+    return np.concatenate([rm.slot_new for rm in bm.requests]).astype(np.int32) if bm.requests else np.zeros(0, np.int32)
+
+
+def _bf16_ord(bits: np.ndarray) -> np.ndarray:
+    b = bits.astype(np.int32)
+    mag = b & 0x7FFF
+    return np.where(b & 0x8000, -mag, mag)
+
+
+def _bf16_val(bits: np.ndarray) -> np.ndarray:
+    return (bits.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+
+
+def _e4m3_ord(b: np.ndarray) -> np.ndarray:
+    v = b.astype(np.int32)
+    mag = v & 0x7F
+    return np.where(v & 0x80, -mag, mag)
+
+
+def rotated_rows(w: synth.Workload, bm: O.BatchMap, mode: int):
+    """(new slot, old slot) of every row whose K_pe band is rotated (KEEP segments with shift != 0 that the mode
+    processes)."""
+    new_s, old_s = [], []
+    for rm in bm.requests:
+        for (kind, src, dst, ln, sh) in rm.segs.as_tuples():
+            if kind == O.KEEP and sh != 0:
+                new_s.append(rm.slot_new[dst:dst + ln])
+                old_s.append(rm.slot_old[src:src + ln])
+    if not new_s:
+        return np.zeros(0, np.int64), np.zeros(0, np.int64)
+    return np.concatenate(new_s).astype(np.int64), np.concatenate(old_s).astype(np.int64)
+
+
+def compare_layer(w: synth.Workload, bm: O.BatchMap, mode: int, old_pool: np.ndarray, gpu_pool: np.ndarray,
+                  repl: np.ndarray, scale: float = 1.0) -> dict:
+    """One layer, whole pool.  old_pool / gpu_pool / repl: flat uint8.  Asserts the bar and returns statistics."""
+    stride = w.row_bytes
+    E = w.elem_bytes
+    want = O.splice_layer(w.dtype, w.pairing, w.latent_dim, w.rope_dim, stride, w.inv_freq, scale, old_pool, repl, bm)
+    g = gpu_pool.reshape(-1, stride)
+    o = want.reshape(-1, stride)
+    new_s, old_s = rotated_rows(w, bm, mode)
+    band0 = w.latent_dim * E
+    # 1. everything outside rotated bands: bit-exact over the whole pool
+    mask = np.ones(g.shape, dtype=bool)
+    if len(new_s):
+        mask[new_s, band0:] = False
+    neq = (g != o) & mask
+    assert not neq.any(), f"{int(neq.sum())} bytes differ outside rotated K_pe bands (first rows {np.unique(np.nonzero(neq)[0])[:8]})"
+    stats = {"rotated_elems": 0, "max_ord": 0, "frac_equal": 1.0, "n_floor": 0}
+    if not len(new_s):
+        return stats
+    gb = np.ascontiguousarray(g[new_s, band0:])
+    ob = np.ascontiguousarray(o[new_s, band0:])
+    if w.dtype == synth.DT_BF16:
+        gbits, obits = gb.view(np.uint16), ob.view(np.uint16)
+        dist = np.abs(_bf16_ord(gbits) - _bf16_ord(obits))
+        bad = dist > 2
+        n_floor = 0
+        if bad.any():
+            # cancellation floor: |g - o| <= 2^-20 * rho, rho = norm of the INPUT pair
+            ib = np.ascontiguousarray(old_pool.reshape(-1, stride)[old_s, band0:]).view(np.uint16)
+            x = _bf16_val(ib)
+            H = w.rope_dim // 2
+            if w.pairing == synth.NEOX:
+                rho_h = np.sqrt(x[:, :H] ** 2 + x[:, H:] ** 2)
+                rho = np.concatenate([rho_h, rho_h], axis=1)
+            else:
+                rho_h = np.sqrt(x[:, 0::2] ** 2 + x[:, 1::2] ** 2)
+                rho = np.repeat(rho_h, 2, axis=1)
+            err = np.abs(_bf16_val(gbits) - _bf16_val(obits))
+            floor_ok = err <= (2.0 ** -20) * rho
+            n_floor = int((bad & floor_ok).sum())
+            really_bad = bad & ~floor_ok
+            assert not really_bad.any(), f"{int(really_bad.sum())} rotated bf16 elements beyond 2 ulp and the 2^-20 rho floor"
+        stats.update(rotated_elems=int(dist.size), max_ord=int(dist.max()), frac_equal=float((dist == 0).mean()),
+                     n_floor=n_floor)
+    else:
+        dist = np.abs(_e4m3_ord(gb) - _e4m3_ord(ob))
+        assert dist.max() <= 1, f"fp8 rotated K_pe: max ordinal distance {int(dist.max())} > 1"
+        stats.update(rotated_elems=int(dist.size), max_ord=int(dist.max()), frac_equal=float((dist == 0).mean()))
+    return stats

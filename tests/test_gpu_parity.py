@@ -1,0 +1,143 @@
+"""GPU parity: the CUDA library through its C ABI vs the CPU oracle, element by element, on the same seeded
+inputs (tests/parity.py states the bar).  Small and medium cases compare every layer and the whole pool
+(so every byte the mode must not write is checked too); the full BASELINE.json configs run in the launch
+configuration bench.py times (all layers, one call) and compare sampled layers completely."""
+import numpy as np
+import pytest
+import torch
+
+import oracle as O
+from parity import assert_plan_equal, compare_layer, oracle_plan, oracle_slot_list
+from paper_2606_01065_b200 import synth
+from test_plan_host import tiny_workload
+
+pytestmark = pytest.mark.gpu
+
+MODES = [O.FRESH, O.INPLACE_MOVE, O.ROTATE_ONLY]
+MODE_NAME = {O.FRESH: "fresh", O.INPLACE_MOVE: "inplace", O.ROTATE_ONLY: "rotate_only"}
+
+
+def run_and_compare(w, mode, check_layers=None, tuning=None):
+    from paper_2606_01065_b200 import binding as B
+    from paper_2606_01065_b200 import harness
+    if tuning:
+        B.leyline_set_tuning(**tuning)
+    try:
+        cache = harness.DeviceCache(w, "cuda:0")
+        check_layers = list(range(w.n_layers)) if check_layers is None else check_layers
+        old = {l: cache.pools[l].cpu().numpy() for l in check_layers}
+        plan, pt, idx = harness.run_workload(cache, mode)
+        torch.cuda.synchronize()
+    finally:
+        if tuning:
+            B.leyline_set_tuning()
+    bm = oracle_plan(w, mode)
+    assert_plan_equal(plan, bm, mode)
+    n_tok = int(plan.info.total_new_tokens)
+    np.testing.assert_array_equal(idx.cpu().numpy()[:n_tok], oracle_slot_list(bm))          # a2, bit-exact
+    if mode != O.ROTATE_ONLY:
+        n_pg = int(plan.info.total_new_pages)
+        want = np.concatenate([rm.new_pages for rm in bm.requests]) if n_pg else np.zeros(0, np.int32)
+        np.testing.assert_array_equal(pt.cpu().numpy()[:n_pg], want)
+    stats = []
+    for l in check_layers:
+        stats.append(compare_layer(w, bm, mode, old[l], cache.pools[l].cpu().numpy(), cache.repl[l].cpu().numpy(),
+                                   cache.scales[l]))
+    plan.close()
+    tot = sum(s["rotated_elems"] for s in stats)
+    if tot:
+        worst = max(s["max_ord"] for s in stats)
+        eq = sum(s["frac_equal"] * s["rotated_elems"] for s in stats) / tot
+        print(f"[parity] {w.name} {MODE_NAME[mode]}: rotated elems {tot}, max ordinal distance {worst}, "
+              f"bit-equal {eq:.6f}, cancellation-floor passes {sum(s['n_floor'] for s in stats)}")
+        if w.dtype == synth.DT_BF16:
+            assert eq > 0.99          # fp32 trig + one RNE: almost every element is the oracle's exact code
+    return stats
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_config1_all_modes(mode):
+    run_and_compare(synth.config(1, pool_factor=2.5), mode)
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("dtype", [synth.DT_BF16, synth.DT_FP8])
+@pytest.mark.parametrize("pairing", [synth.NEOX, synth.INTERLEAVED])
+def test_randomised_small(mode, dtype, pairing):
+    rng = np.random.default_rng(77 + 10 * mode + 3 * dtype + pairing)
+    for _ in range(12):
+        w = tiny_workload(rng, dtype=dtype)
+        w.pairing = pairing
+        run_and_compare(w, mode)
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("tile_rows", [1, 7, 32])
+def test_medium_many_tiles_ragged(mode, tile_rows):
+    """Several pages, ragged tails, tiles that straddle pages, growth and shrink in one request, YaRN thetas."""
+    w = synth.Workload("medium", 3, [3000, 1, 0, 2777], 16, inv_freq=synth.yarn_inv_freq(),
+                       directives=[(0, 5, 5, 40, 0, 0), (0, 100, 900, 3, 0, 0), (0, 1500, 1501, 333, 0, 0),
+                                   (0, 2990, 3000, 0, 0, 0),
+                                   (1, 0, 1, 0, 0, 0),
+                                   (3, 0, 17, 500, 0, 0), (3, 1000, 1700, 0, 0, 0), (3, 2776, 2777, 2, 0, 0)],
+                       seed=11, pool_factor=3.0, extra_pages=80).finalize()
+    run_and_compare(w, mode, tuning={"tile_rows": tile_rows})
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_identity_and_degenerate(mode):
+    # no directives at all, no-op directives, |R| = |span| (Delta = 0: everything downstream is a byte copy, G19)
+    for dirs in ([], [(0, 10, 10, 0, 0, 0)], [(0, 64, 128, 64, 0, 0)], [(0, 0, 0, 0, 0, 0), (0, 500, 500, 0, 0, 0)]):
+        w = synth.Workload("ident", 2, [500], 8, inv_freq=synth.rope_inv_freq(), directives=dirs, seed=3,
+                           pool_factor=3.0, extra_pages=16).finalize()
+        stats = run_and_compare(w, mode)
+        assert all(s["rotated_elems"] == 0 for s in stats)
+
+
+def test_special_values_survive():
+    """-0.0, subnormals and large magnitudes in K_pe: byte-exact where C = 0, within tolerance where rotated."""
+    from paper_2606_01065_b200 import binding as B
+    from paper_2606_01065_b200 import harness
+    w = synth.Workload("special", 1, [256], 4, inv_freq=synth.rope_inv_freq(), directives=[(0, 100, 110, 3, 0, 0)],
+                       seed=5, pool_factor=3.0, extra_pages=8).finalize()
+    cache = harness.DeviceCache(w, "cuda:0")
+    v = cache.pools[0].view(torch.int16)
+    # -0.0, +-smallest subnormal, largest subnormal, 2^125, smallest normal, 1.0
+    specials = torch.tensor([-32768, 1, -32767, 0x007F, 0x7E00, 0x0080, 0x3F80], dtype=torch.int16, device="cuda:0")
+    v[::13] = specials[torch.arange(v[::13].numel(), device="cuda:0") % len(specials)]
+    old = cache.pools[0].cpu().numpy()
+    plan, pt, idx = harness.run_workload(cache, B.FRESH)
+    torch.cuda.synchronize()
+    bm = oracle_plan(w, B.FRESH)
+    compare_layer(w, bm, B.FRESH, old, cache.pools[0].cpu().numpy(), cache.repl[0].cpu().numpy(), 1.0)
+
+
+@pytest.mark.parametrize("mode", [O.FRESH, O.ROTATE_ONLY, O.INPLACE_MOVE])
+def test_config2_dsv2lite(mode):
+    run_and_compare(synth.config(2, pool_factor=2.2), mode, check_layers=[0, 13, 26])
+
+
+@pytest.mark.parametrize("cfg", [3, "3m"])
+@pytest.mark.parametrize("mode", MODES)
+def test_config3_dsv3_full_size(cfg, mode):
+    run_and_compare(synth.config(cfg, pool_factor=2.0), mode, check_layers=[0, 37, 60])
+
+
+def test_config4_batched_inplace_full_size():
+    w = synth.config(4)           # 64 x 16K x 61 layers, one shared pool (~92 GB with the 25 % spare pages)
+    free, total = torch.cuda.mem_get_info(0)
+    if free < w.layer_bytes * w.n_layers * 1.08:
+        pytest.skip(f"needs {w.layer_bytes * w.n_layers / 2**30:.0f} GiB of device memory")
+    run_and_compare(w, O.INPLACE_MOVE, check_layers=[0, 60])
+
+
+def test_config4_batched_fresh_reduced_layers():
+    # FRESH on the batched workload needs a second set of pages; 61 layers of that do not fit next to the pool,
+    # so the same plan runs on 12 layers (layers are independent buffers under one plan)
+    w = synth.config(4, pool_factor=2.2, n_layers=12)
+    run_and_compare(w, O.FRESH, check_layers=[0, 11])
+
+
+@pytest.mark.parametrize("mode", [O.FRESH, O.INPLACE_MOVE, O.ROTATE_ONLY])
+def test_config5_fp8_full_size(mode):
+    run_and_compare(synth.config(5, pool_factor=2.2), mode, check_layers=[0, 60])

@@ -1,0 +1,267 @@
+"""Host-side tests of libleyline.so (no GPU): the C ABI exports what include/leyline.h declares, leyline_plan
+agrees bit-exactly with the oracle's O1-O3 on thousands of tiny randomised cases and on the five BASELINE.json
+configs, its error codes follow rule V, and the tile list with its load->store dependencies (rule M2) is a
+correct schedule for the in-place move -- checked by executing the tiles on integer row labels under random
+legal interleavings."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle as O
+from helpers import list_splice
+from parity import assert_plan_equal, oracle_plan
+from paper_2606_01065_b200 import binding as B
+from paper_2606_01065_b200 import synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+MODES = [B.FRESH, B.INPLACE_MOVE, B.ROTATE_ONLY]
+
+
+def test_abi_exports_every_declared_symbol():
+    text = open(os.path.join(ROOT, "include", "leyline.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    names = set(re.findall(r"\b(leyline_[a-z_0-9]+)\s*\(", text))
+    assert {"leyline_plan", "leyline_splice", "leyline_rotate_inplace", "leyline_plan_destroy"} <= names
+    lib = ctypes.CDLL(B.LIB_PATH)
+    for n in sorted(names):
+        assert hasattr(lib, n), f"{n} declared in leyline.h but not exported"
+    assert "sm_100a" in B.leyline_version()
+
+
+def test_enum_values_match_oracle_contract():
+    assert (B.OK, B.E_INVALID, B.E_UNSORTED, B.E_OVERLAP, B.E_RANGE, B.E_NOFREE, B.E_UNSUPPORTED) == \
+           (O.OK, O.E_INVALID, O.E_UNSORTED, O.E_OVERLAP, O.E_RANGE, O.E_NOFREE, O.E_UNSUPPORTED)
+    assert (B.FRESH, B.INPLACE_MOVE, B.ROTATE_ONLY) == (O.FRESH, O.INPLACE_MOVE, O.ROTATE_ONLY)
+
+
+def tiny_workload(rng, P=None, n_req=None, forget=False, dtype=synth.DT_BF16):
+    P = int(rng.choice([1, 2, 4, 8, 16])) if P is None else P
+    n_req = int(rng.integers(1, 4)) if n_req is None else n_req
+    seq_lens = [int(rng.integers(0, 150)) for _ in range(n_req)]
+    dirs = []
+    for r, L in enumerate(seq_lens):
+        k = int(rng.integers(0, 5))
+        cuts = np.sort(rng.integers(0, L + 1, size=2 * k))
+        for j in range(k):
+            s, e = int(cuts[2 * j]), int(cuts[2 * j + 1])
+            n = int(rng.integers(0, 2 * (e - s) + 3)) if rng.random() < 0.8 else 0
+            sem = B.FORGET if (forget and rng.random() < 0.15) else B.AMORTIZE
+            dirs.append((r, s, e, n, 0, sem))
+    w = synth.Workload("tiny", 2, seq_lens, P, dtype=dtype, inv_freq=synth.rope_inv_freq(64), directives=dirs,
+                       seed=int(rng.integers(1 << 30)), pool_factor=3.0, extra_pages=sum(d[3] for d in dirs) + 8)
+    return w.finalize()
+
+
+def make_plan(w, mode, n_layers=None):
+    d, keep = B.make_desc(n_layers or w.n_layers, w.latent_dim, w.rope_dim, w.page_size, w.dtype, w.pairing,
+                          w.row_bytes, w.n_slots, w.inv_freq)
+    free = w.free_slots() if mode == B.ROTATE_ONLY else w.free_pages
+    return B.leyline_plan(d, mode, w.seq_lens, w.pt_offsets, w.pages, w.directives, free)
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("block", range(8))
+def test_plan_matches_oracle_randomised(mode, block):
+    rng = np.random.default_rng(5000 + 100 * mode + block)
+    for _ in range(150):
+        w = tiny_workload(rng, forget=True)
+        bm = oracle_plan(w, mode)
+        assert bm.status == O.OK
+        with make_plan(w, mode) as plan:
+            assert_plan_equal(plan, bm, mode)
+            check_tiles_cover(plan, bm, w, mode)
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("cfg", [1, 2, 3, "3m", 4, 5])
+def test_plan_matches_oracle_on_baseline_configs(mode, cfg):
+    w = synth.config(cfg, pool_factor=2.2)
+    bm = oracle_plan(w, mode)
+    with make_plan(w, mode) as plan:
+        assert_plan_equal(plan, bm, mode)
+        check_tiles_cover(plan, bm, w, mode)
+        i = plan.info
+        E, W = w.elem_bytes, w.latent_dim + w.rope_dim
+        if mode != B.ROTATE_ONLY:
+            assert i.bytes_read == i.bytes_written == (i.rows_moved + i.rows_inserted) * W * E * w.n_layers
+        if cfg == 3 and mode == B.FRESH:   # (103,936 + 320) x 61 rows, 14.65 GB read + written
+            assert (i.rows_moved, i.rows_inserted, i.rows_rotated) == (103936, 320, 103936)
+            assert i.bytes_read + i.bytes_written == 2 * (103936 + 320) * 1152 * 61
+        if cfg == 4:
+            shifts = [s[5] for s in plan.segments if s[1] == 0]
+            assert sum(1 for r in range(64) if any(s[0] == r and s[1] == 0 and s[5] > 0 for s in plan.segments)) >= 8
+            assert any(c < 0 for c in shifts)
+
+
+def check_tiles_cover(plan, bm, w, mode):
+    """Tiles are exactly the rows the mode must touch, each once, with the right source, shift and trig row."""
+    tiles = plan.tiles
+    shifts = plan.trig_shifts
+    n_move = plan.info.n_move_tiles
+    seen = {}
+    for t_i, t in enumerate(tiles):
+        assert 1 <= t.n_rows <= (256 if (mode == B.ROTATE_ONLY and t_i < n_move) else 32)
+        is_repl = bool(t.flags & B.TILE_SRC_REPL)
+        assert is_repl == (t_i >= n_move)
+        for q in range(t.n_rows):
+            key = (t.request, "r" if is_repl else "o", t.src_pos + q)
+            assert key not in seen
+            seen[key] = (t.dst_pos + q, t.trig)
+        assert t.dep_lo >= 0 and t.dep_hi < t_i
+        if mode != B.INPLACE_MOVE:
+            assert t.dep_hi < t.dep_lo
+    want = {}
+    for r, rm in enumerate(bm.requests):
+        segs = rm.segs.as_tuples()
+        k0P = 0
+        if mode == B.FRESH:
+            mine = [d for d in w.directives if d[0] == r]
+            k0P = (mine[0][1] // w.page_size) * w.page_size if mine else rm.L_new
+        ins_cursor = 0
+        for (kind, src, dst, ln, sh) in segs:
+            for q in range(ln):
+                if kind == O.INSERT:
+                    want[(r, "r", src + q)] = (dst + q, None)
+                elif mode == B.FRESH and dst + q >= k0P:
+                    want[(r, "o", src + q)] = (dst + q, sh)
+                elif mode in (B.INPLACE_MOVE, B.ROTATE_ONLY) and sh != 0:
+                    want[(r, "o", src + q)] = (dst + q, sh)
+    assert set(seen) == set(want)
+    for key, (dst, trig) in seen.items():
+        wdst, wsh = want[key]
+        if key[1] == "o":
+            assert dst == wdst
+            assert (trig == -1 and wsh == 0) or (trig >= 0 and shifts[trig] == wsh)
+        else:
+            assert trig == -1
+            if mode != B.ROTATE_ONLY:
+                assert dst == wdst
+
+
+def test_trig_table_is_fp64_trig_rounded_once():
+    w = synth.config(3, pool_factor=2.2)
+    with make_plan(w, B.FRESH) as plan:
+        sh, tab = plan.trig_shifts, plan.trig_table
+        th = w.inv_freq.astype(np.float64)
+        for g, c in enumerate(sh):
+            # independent evaluation: exact integer-times-double product, numpy fp64 trig
+            phi = float(c) * th
+            np.testing.assert_array_equal(tab[g, 0], np.cos(phi).astype(np.float32))
+            np.testing.assert_array_equal(tab[g, 1], np.sin(phi).astype(np.float32))
+
+
+def test_error_codes_follow_rule_v():
+    w = tiny_workload(np.random.default_rng(1), P=4, n_req=2)
+    w.seq_lens = [40, 30]
+    w.directives = []
+    w.finalize()
+    d, keep = B.make_desc(2, 512, 64, 4, 0, 0, 1152, w.n_slots, w.inv_freq)
+
+    def status(dirs, mode=B.FRESH, free=None, desc=d):
+        try:
+            B.leyline_plan(desc, mode, w.seq_lens, w.pt_offsets, w.pages, dirs, w.free_pages if free is None else free).close()
+            return B.OK
+        except B.LeylineError as e:
+            return e.status
+
+    A = B.AMORTIZE
+    cases = [
+        ([], B.OK), ([(0, 5, 5, 0, 0, A)], B.OK), ([(0, 0, 40, 0, 0, A)], B.OK),
+        ([(0, 5, 10, 1, 0, A), (0, 10, 12, 0, 0, A)], B.OK),                 # adjacent spans accepted
+        ([(2, 0, 1, 0, 0, A)], B.E_RANGE), ([(-1, 0, 1, 0, 0, A)], B.E_RANGE),
+        ([(0, -1, 1, 0, 0, A)], B.E_INVALID), ([(0, 5, 4, 0, 0, A)], B.E_INVALID),
+        ([(0, 1, 2, -1, 0, A)], B.E_INVALID), ([(0, 1, 2, 0, -1, A)], B.E_INVALID), ([(0, 1, 2, 0, 0, 7)], B.E_INVALID),
+        ([(0, 30, 41, 0, 0, A)], B.E_RANGE), ([(1, 0, 31, 0, 0, A)], B.E_RANGE),
+        ([(1, 0, 1, 0, 0, A), (0, 0, 1, 0, 0, A)], B.E_UNSORTED),
+        ([(0, 10, 12, 0, 0, A), (0, 5, 6, 0, 0, A)], B.E_UNSORTED),
+        ([(0, 5, 10, 0, 0, A), (0, 9, 12, 0, 0, A)], B.E_OVERLAP),
+    ]
+    for dirs, want in cases:
+        assert status(dirs) == want, dirs
+        assert O.validate(w.seq_lens, dirs) == want, dirs                      # the oracle applies the same rule
+    assert status([(0, 0, 0, 400, 0, A)], free=w.free_pages[:3]) == B.E_NOFREE
+    assert status([(0, 0, 0, 5, 0, A)], mode=B.ROTATE_ONLY, free=w.free_slots()[:4]) == B.E_NOFREE
+    bad, k2 = B.make_desc(2, 512, 64, 3, 0, 0, 1152, w.n_slots, w.inv_freq)        # page size not a power of two
+    assert status([], desc=bad) == B.E_INVALID
+    bad, k3 = B.make_desc(2, 512, 63, 4, 0, 0, 1152, w.n_slots, w.inv_freq)        # odd rope_dim
+    assert status([], desc=bad) == B.E_INVALID
+    bad, k4 = B.make_desc(2, 500, 64, 4, 0, 0, 1136, w.n_slots, w.inv_freq)        # latent bytes not 16-byte chunks
+    assert status([], desc=bad) == B.E_UNSUPPORTED
+    bad, k5 = B.make_desc(2, 512, 64, 4, 0, 0, 1152, 8, w.inv_freq)                # page ids beyond the pool
+    assert status([]) == B.OK and status([], desc=bad) == B.E_RANGE
+
+
+# ----------------------------------------------------------------------------- rule M2 as a schedule
+
+def simulate_inplace(plan, w, rng):
+    """Execute the plan's tiles on integer row labels: a tile's LOAD may happen at any time, its STORE only after
+    its own load and the loads of tiles [dep_lo, dep_hi]; inserts run after every move.  The interleaving is a
+    random legal one.  Returns the pool of labels."""
+    P = w.page_size
+    pool = np.full(w.n_slots, -1, np.int64)
+    for r, L in enumerate(w.seq_lens):
+        row = w.pages[w.pt_offsets[r]:w.pt_offsets[r + 1]]
+        t = np.arange(L)
+        pool[row[t // P].astype(np.int64) * P + t % P] = r * 10 ** 6 + t            # label = (request, old position)
+    new_pages, off = plan.new_pages, plan.new_pt_offsets
+    tiles = plan.tiles
+    n_move = plan.info.n_move_tiles
+
+    def src_slots(t):
+        row = w.pages[w.pt_offsets[t.request]:w.pt_offsets[t.request + 1]]
+        p = t.src_pos + np.arange(t.n_rows)
+        return row[p // P].astype(np.int64) * P + p % P
+
+    def dst_slots(t):
+        row = new_pages[off[t.request]:off[t.request + 1]]
+        p = t.dst_pos + np.arange(t.n_rows)
+        return row[p // P].astype(np.int64) * P + p % P
+
+    loaded, stored, regs = set(), set(), {}
+    pending = list(range(n_move))
+    while len(stored) < n_move:
+        ready = []
+        for i in pending:
+            if i not in loaded:
+                ready.append(("L", i))
+            elif all(d in loaded for d in range(tiles[i].dep_lo, tiles[i].dep_hi + 1)):
+                ready.append(("S", i))
+        # bias towards stores so that missing dependencies actually bite
+        stores = [x for x in ready if x[0] == "S"]
+        op, i = stores[int(rng.integers(len(stores)))] if stores and rng.random() < 0.7 else ready[int(rng.integers(len(ready)))]
+        if op == "L":
+            regs[i] = pool[src_slots(tiles[i])].copy()
+            loaded.add(i)
+        else:
+            pool[dst_slots(tiles[i])] = regs.pop(i)
+            stored.add(i)
+            pending.remove(i)
+    for t in tiles[n_move:]:
+        pool[dst_slots(t)] = -(t.request * 10 ** 6 + t.src_pos + np.arange(t.n_rows)) - 2   # label = -(req, repl row) - 2
+    return pool
+
+
+@pytest.mark.parametrize("seed", range(60))
+def test_inplace_tiles_are_a_correct_schedule(seed):
+    rng = np.random.default_rng(9000 + seed)
+    w = tiny_workload(rng, P=int(rng.choice([1, 2, 4, 8])))
+    B.leyline_set_tuning(tile_rows=int(rng.choice([1, 2, 3, 5, 8, 32])))
+    try:
+        plan = make_plan(w, B.INPLACE_MOVE)
+    finally:
+        B.leyline_set_tuning()
+    with plan:
+        pool = simulate_inplace(plan, w, rng)
+        P = w.page_size
+        new_pages, off = plan.new_pages, plan.new_pt_offsets
+        for r, L in enumerate(w.seq_lens):
+            dirs = [(d[1], d[2], d[3], d[4]) for d in w.directives if d[0] == r]
+            want = list_splice(L, dirs)                                   # literal Python list slicing
+            row = new_pages[off[r]:off[r + 1]]
+            assert plan.new_seq_lens[r] == len(want)
+            for tpos, (kind, i) in enumerate(want):
+                got = pool[int(row[tpos // P]) * P + tpos % P]
+                assert got == (r * 10 ** 6 + i if kind == "o" else -(r * 10 ** 6 + i) - 2), (r, tpos, kind, i, got)
