@@ -64,6 +64,24 @@ def peaks():
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s, earlier measurement on this pool)"
 
 
+def ncu_traffic(workload: str, mode: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on (workload, mode), from the newest
+    committed `ncu --set full` summary under profiles/ (text, written from a capture; see profiles/README.md).
+    None when no capture of that kernel/workload exists."""
+    import csv
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_ncu_full_{kernel}_cfg{workload}_{mode}.csv")))
+    if not files:
+        return None, None
+    mult = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    tot = 0.0
+    with open(files[-1]) as f:
+        for row in csv.reader(f):
+            if len(row) == 3 and row[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                tot += float(row[2]) * mult.get(row[1], 1.0)
+    return (tot or None), os.path.relpath(files[-1], ROOT)
+
+
 class ClockSampler:
     """nvidia-smi clocks + throttle reasons while the timed region runs (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -286,6 +304,8 @@ def run_ours(args):
     value = world * r["bytes"] / (ms * 1e-3) / 1e9
     peak, peak_src = peaks()
     kernel_gbs = r["bytes"] / (r["kernel_ms"] * 1e-3) / 1e9
+    kname = "k_rotate_band" if mode == B.ROTATE_ONLY else "k_move_rows"
+    traffic, traffic_src = ncu_traffic(args.workload, args.mode, kname)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16" if w.dtype == 0 else "fp8_e4m3",
@@ -301,7 +321,8 @@ def run_ours(args):
         "gpu_launches": r["launches_per_step"] * args.steps,
         "clocks": clocks,
         "roofline": {"bound": "hbm", "achieved": kernel_gbs, "peak": peak, "unit": UNIT, "frac": kernel_gbs / peak,
-                     "traffic": None, "kernel": "k_move (fused gather-rotate-scatter + insert)",
+                     "traffic": traffic, "traffic_source": traffic_src, "algorithmic_bytes": r["bytes"],
+                     "kernel": kname + (" (fused gather-rotate-scatter + insert)" if kname == "k_move_rows" else " (in-place K_pe rotation)"),
                      "kernel_ms": r["kernel_ms"], "kernel_ms_best": r["kernel_ms_min"],
                      "peak_source": peak_src, "frac_of_8TBps_nominal": kernel_gbs / 8000.0},
     }
