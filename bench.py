@@ -44,6 +44,8 @@ def parse_args():
     ap.add_argument("--kernel", type=int, default=0, help="leyline_tuning.kernel (0 auto, 1 row, 2 bulk)")
     ap.add_argument("--tile-rows", type=int, default=0)
     ap.add_argument("--ctas-per-sm", type=int, default=0)
+    ap.add_argument("--stages", type=int, default=0, help="leyline_tuning.stages (bulk kernel)")
+    ap.add_argument("--layer-group", type=int, default=0, help="leyline_tuning.layer_group (bulk kernel)")
     return ap.parse_args()
 
 
@@ -200,7 +202,8 @@ def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1):
     del keep
     return {"ms_per_step": ms, "kernel_ms": float(np.mean(kms)), "kernel_ms_min": float(np.min(kms)), "bytes": nbytes,
             "plan_host_us": float(np.median(host_us)), "launches_per_step": launches,
-            "n_directives": len(w.directives), "rows_moved": int(info.rows_moved), "rows_inserted": int(info.rows_inserted)}
+            "n_directives": len(w.directives), "rows_moved": int(info.rows_moved), "rows_inserted": int(info.rows_inserted),
+            "mover": int(info.mover), "tile_rows": int(info.tile_rows)}
 
 
 def cpu_baseline(pools, repls, scales, w, mode: int, bytes_per_layer: int, budget_s: float = 12.0, max_layers: int = 8):
@@ -291,7 +294,8 @@ def run_ours(args):
     from paper_2606_01065_b200 import harness
     from paper_2606_01065_b200 import synth
     rank, world, local = dist_setup(args.gpus)
-    B.leyline_set_tuning(kernel=args.kernel, tile_rows=args.tile_rows, ctas_per_sm=args.ctas_per_sm, profile=1)
+    B.leyline_set_tuning(kernel=args.kernel, tile_rows=args.tile_rows, ctas_per_sm=args.ctas_per_sm, profile=1,
+                         stages=args.stages, layer_group=args.layer_group)
     mode = MODES[args.mode]
     w = workload_of(args.workload, args.mode)
     cache = harness.DeviceCache(w, f"cuda:{local}")
@@ -304,7 +308,7 @@ def run_ours(args):
     value = world * r["bytes"] / (ms * 1e-3) / 1e9
     peak, peak_src = peaks()
     kernel_gbs = r["bytes"] / (r["kernel_ms"] * 1e-3) / 1e9
-    kname = "k_rotate_band" if mode == B.ROTATE_ONLY else "k_move_rows"
+    kname = "k_rotate_band" if mode == B.ROTATE_ONLY else ("k_move_bulk" if r["mover"] == 2 else "k_move_rows")
     traffic, traffic_src = ncu_traffic(args.workload, args.mode, kname)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -322,7 +326,8 @@ def run_ours(args):
         "clocks": clocks,
         "roofline": {"bound": "hbm", "achieved": kernel_gbs, "peak": peak, "unit": UNIT, "frac": kernel_gbs / peak,
                      "traffic": traffic, "traffic_source": traffic_src, "algorithmic_bytes": r["bytes"],
-                     "kernel": kname + (" (fused gather-rotate-scatter + insert)" if kname == "k_move_rows" else " (in-place K_pe rotation)"),
+                     "kernel": kname + (" (in-place K_pe rotation)" if kname == "k_rotate_band" else " (fused gather-rotate-scatter + insert)"),
+                     "tile_rows": r["tile_rows"],
                      "kernel_ms": r["kernel_ms"], "kernel_ms_best": r["kernel_ms_min"],
                      "peak_source": peak_src, "frac_of_8TBps_nominal": kernel_gbs / 8000.0},
     }

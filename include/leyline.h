@@ -119,6 +119,8 @@ typedef struct {
                                   rope*elem per in-place rotated row */
     int64_t bytes_written;     /* same, written */
     int64_t bytes_index;       /* 4 B per new token + 4 B per new page-table entry (once, not per layer) */
+    int64_t tile_rows;         /* rows per device work item chosen for this plan */
+    int64_t mover;             /* a3/a4 kernel this plan launches: 1 = k_move_rows, 2 = k_move_bulk (see leyline_tuning) */
 } leyline_plan_info;
 
 typedef struct leyline_plan_s leyline_plan_t;
@@ -224,10 +226,13 @@ const char* leyline_last_cuda_error(void);
 
 /* Process-wide tuning knobs (benchmarking; defaults are what bench.py reports).  Read by leyline_plan. */
 typedef struct {
-    int32_t kernel;        /* 0 = auto, 1 = row kernel (LDG/STG), 2 = bulk kernel (TMA bulk copies through smem) */
-    int32_t tile_rows;     /* rows per tile of the move/insert kernels, 0 = default */
+    int32_t kernel;        /* a3/a4 mover: 0 = auto (bulk when pages hold >= 16 unpadded rows), 1 = row kernel (LDG/STG
+                              through registers), 2 = bulk kernel (TMA 1-D bulk copies through shared memory) */
+    int32_t tile_rows;     /* rows per tile of the move/insert kernels, 0 = default (row kernel <= 32, bulk <= 64) */
     int32_t ctas_per_sm;   /* row kernel only, 0 = default */
     int32_t profile;       /* 1: record CUDA events around the data-moving kernels (leyline_plan_kernel_ms) */
+    int32_t stages;        /* bulk kernel only: shared-memory stages per CTA, 0 = as many as fit (at most 8) */
+    int32_t layer_group;   /* bulk kernel only: layers per work item (one stage each), 0 = default */
 } leyline_tuning;
 leyline_status leyline_set_tuning(const leyline_tuning* t);
 leyline_status leyline_get_tuning(leyline_tuning* t);

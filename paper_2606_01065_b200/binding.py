@@ -44,7 +44,7 @@ class PlanInfo(C.Structure):
     _fields_ = [("mode", C.c_int32), ("n_requests", C.c_int32)] + [
         (n, C.c_int64) for n in ("total_new_tokens", "total_new_pages", "n_free_consumed", "n_released", "n_segments",
                                  "n_tiles", "n_move_tiles", "n_trig", "rows_moved", "rows_inserted", "rows_rotated",
-                                 "bytes_read", "bytes_written", "bytes_index")]
+                                 "bytes_read", "bytes_written", "bytes_index", "tile_rows", "mover")]
 
 
 class Tile(C.Structure):
@@ -53,7 +53,8 @@ class Tile(C.Structure):
 
 
 class Tuning(C.Structure):
-    _fields_ = [("kernel", C.c_int32), ("tile_rows", C.c_int32), ("ctas_per_sm", C.c_int32), ("profile", C.c_int32)]
+    _fields_ = [("kernel", C.c_int32), ("tile_rows", C.c_int32), ("ctas_per_sm", C.c_int32), ("profile", C.c_int32),
+                ("stages", C.c_int32), ("layer_group", C.c_int32)]
 
 
 class LeylineError(RuntimeError):
@@ -111,15 +112,17 @@ def leyline_version() -> str:
     return _lib.leyline_version().decode()
 
 
-def leyline_set_tuning(kernel: int = 0, tile_rows: int = 0, ctas_per_sm: int = 0, profile: int = 0):
-    t = Tuning(kernel, tile_rows, ctas_per_sm, profile)
+def leyline_set_tuning(kernel: int = 0, tile_rows: int = 0, ctas_per_sm: int = 0, profile: int = 0, stages: int = 0,
+                       layer_group: int = 0):
+    t = Tuning(kernel, tile_rows, ctas_per_sm, profile, stages, layer_group)
     _check(_lib.leyline_set_tuning(C.byref(t)), "leyline_set_tuning")
 
 
 def leyline_get_tuning() -> dict:
     t = Tuning()
     _check(_lib.leyline_get_tuning(C.byref(t)), "leyline_get_tuning")
-    return {"kernel": t.kernel, "tile_rows": t.tile_rows, "ctas_per_sm": t.ctas_per_sm, "profile": t.profile}
+    return {"kernel": t.kernel, "tile_rows": t.tile_rows, "ctas_per_sm": t.ctas_per_sm, "profile": t.profile,
+            "stages": t.stages, "layer_group": t.layer_group}
 
 
 def _arr(x, dtype):

@@ -21,7 +21,7 @@ using leyline::IdxRun;
 
 namespace {
 
-leyline_tuning g_tuning = {0, 0, 0, 0};
+leyline_tuning g_tuning = {0, 0, 0, 0, 0, 0};
 
 inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
@@ -96,8 +96,24 @@ leyline_status check_directives(int32_t n_req, const int64_t* seq_lens, int32_t 
     return LEYLINE_OK;
 }
 
-int choose_tile_rows(const leyline_cache_desc& c, int E, const leyline_tuning& t) {
+/* Which mover runs a3/a4.  The bulk kernel moves contiguous runs of rows with TMA 1-D copies, so it needs runs:
+ * pages of >= 16 rows and unpadded rows (padding must never be written); otherwise, and for the a5 in-place
+ * rotation, the register-staged row kernel is used.  tuning.kernel = 1 / 2 forces one of them. */
+bool choose_bulk(const leyline_cache_desc& c, int E, const leyline_tuning& t, int mode) {
+    if (mode == LEYLINE_ROTATE_ONLY) return false;
+    if (t.kernel == 1) return false;
+    if (t.kernel == 2) return true;
+    return c.page_size >= 16 && c.row_stride_bytes == (int64_t)(c.latent_dim + c.rope_dim) * E;
+}
+
+int choose_tile_rows(const leyline_cache_desc& c, int E, const leyline_tuning& t, bool bulk) {
     int64_t lat_chunks = (int64_t)c.latent_dim * E / 16, nb = (int64_t)c.rope_dim * E / 16;
+    if (bulk) {
+        /* bulk kernel: one shared-memory stage holds a tile; default ~36 KB per stage, at most 64 rows */
+        int64_t row = (int64_t)(c.latent_dim + c.rope_dim) * E;
+        int64_t want = t.tile_rows > 0 ? t.tile_rows : std::max<int64_t>(1, 36864 / row);
+        return (int)std::max<int64_t>(1, std::min<int64_t>({want, (int64_t)64, 65536 / row}));
+    }
     /* the row kernel keeps a whole tile in registers: <= 8 latent + 1 band chunk per thread, 256 threads */
     int64_t cap = 32;
     if (lat_chunks > 0) cap = std::min<int64_t>(cap, 2048 / lat_chunks);
@@ -164,7 +180,8 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
     pl->elem_bytes = E;
     pl->page_shift = pshift;
     pl->tuning = g_tuning;
-    pl->tile_rows = choose_tile_rows(*desc, E, g_tuning);
+    pl->use_bulk = choose_bulk(*desc, E, g_tuning, mode);
+    pl->tile_rows = choose_tile_rows(*desc, E, g_tuning, pl->use_bulk);
     const int TR = pl->tile_rows;
 
     /* tabs: old page tables first, one row per request */
@@ -381,6 +398,8 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
     if (mode == LEYLINE_ROTATE_ONLY) per_layer = in.rows_rotated * band_bytes + in.rows_inserted * row_bytes;
     in.bytes_read = in.bytes_written = per_layer * desc->n_layers;
     in.bytes_index = 4 * in.total_new_tokens + 4 * in.total_new_pages;
+    in.tile_rows = pl->tile_rows;
+    in.mover = pl->use_bulk ? 2 : 1;
     if (mode == LEYLINE_ROTATE_ONLY) pl->new_pages.clear();
 
     pl->tiles = std::move(move_tiles);
@@ -467,8 +486,9 @@ extern "C" const char* leyline_strerror(leyline_status s) {
 
 extern "C" leyline_status leyline_set_tuning(const leyline_tuning* t) {
     if (!t) return LEYLINE_E_INVALID;
-    if (t->kernel < 0 || t->kernel > 2 || t->tile_rows < 0 || t->tile_rows > 32 || t->ctas_per_sm < 0 ||
-        t->ctas_per_sm > 32)
+    if (t->kernel < 0 || t->kernel > 2 || t->tile_rows < 0 || t->tile_rows > 64 || t->ctas_per_sm < 0 ||
+        t->ctas_per_sm > 32 || t->stages < 0 || t->stages > 8 || t->layer_group < 0 ||
+        t->layer_group > LEYLINE_MAX_LAYERS_PER_LAUNCH)
         return LEYLINE_E_INVALID;
     g_tuning = *t;
     return LEYLINE_OK;

@@ -54,6 +54,7 @@ struct leyline_plan_s {
     int32_t elem_bytes = 2;
     int32_t page_shift = 0;
     int32_t tile_rows = 32;
+    bool use_bulk = false;              /* a3/a4 run on k_move_bulk (TMA bulk copies) instead of k_move_rows */
     leyline_tuning tuning{};
 
     std::vector<int64_t> old_seq_lens, new_seq_lens, forget_trim, slot_offsets, new_pt_offsets, old_pt_offsets;

@@ -7,6 +7,7 @@
 #include <cstring>
 #include <string>
 
+#include "kernels_bulk.cuh"
 #include "kernels_rows.cuh"
 
 using namespace leyline;
@@ -25,7 +26,7 @@ bool cuda_ok(cudaError_t e, const char* what) {
 
 inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
-struct DeviceInfo { int device = -1; int sms = 0; };
+struct DeviceInfo { int device = -1; int sms = 0; int smem_optin = 0; };
 DeviceInfo g_dev;
 
 leyline_status ensure_device(leyline_plan_s* pl, cudaStream_t stream) {
@@ -36,6 +37,7 @@ leyline_status ensure_device(leyline_plan_s* pl, cudaStream_t stream) {
         CU(cudaGetDeviceProperties(&prop, dev));
         g_dev.device = dev;
         g_dev.sms = prop.multiProcessorCount;
+        g_dev.smem_optin = (int)prop.sharedMemPerBlockOptin;
     }
     if (pl->d_blob || pl->device >= 0) {
         if (pl->device != dev) { g_last_error = "plan was uploaded on another device"; return LEYLINE_E_CUDA; }
@@ -116,6 +118,18 @@ MoveKernel pick_move(const leyline_plan_s* pl, bool hazard) {
                 : pick_move_hazard<LEYLINE_FP8_E4M3, LEYLINE_ROPE_INTERLEAVED>(pl, hazard);
 }
 
+using BulkKernel = void (*)(const MoveParams, int, int, int, int);
+
+template <int DT>
+BulkKernel pick_bulk_dt(const leyline_plan_s* pl, bool hazard) {
+    const bool neox = pl->desc.pairing == LEYLINE_ROPE_NEOX;
+    if (hazard) return neox ? k_move_bulk<DT, LEYLINE_ROPE_NEOX, true> : k_move_bulk<DT, LEYLINE_ROPE_INTERLEAVED, true>;
+    return neox ? k_move_bulk<DT, LEYLINE_ROPE_NEOX, false> : k_move_bulk<DT, LEYLINE_ROPE_INTERLEAVED, false>;
+}
+BulkKernel pick_bulk(const leyline_plan_s* pl, bool hazard) {
+    return pl->desc.dtype == LEYLINE_BF16 ? pick_bulk_dt<LEYLINE_BF16>(pl, hazard) : pick_bulk_dt<LEYLINE_FP8_E4M3>(pl, hazard);
+}
+
 MoveKernel pick_rotate(const leyline_plan_s* pl) {
     const bool neox = pl->desc.pairing == LEYLINE_ROPE_NEOX;
     const int nb = pl->desc.rope_dim * pl->elem_bytes / 16;
@@ -193,6 +207,39 @@ leyline_status run_tiles(leyline_plan_s* pl, MoveKernel fn, int smem, int max_ct
     return LEYLINE_OK;
 }
 
+/* Same, with the bulk kernel: one persistent CTA per SM, a ring of shared-memory stages of one tile each. */
+leyline_status run_tiles_bulk(leyline_plan_s* pl, bool hazard, int32_t tile_begin, int64_t tile_count,
+                              void* const* layer_src, void* const* layer_dst, const void* const* layer_repl,
+                              cudaStream_t stream, int* ticket_slot) {
+    if (tile_count <= 0) return LEYLINE_OK;
+    const int L = pl->desc.n_layers;
+    const int row_bytes = (pl->desc.latent_dim + pl->desc.rope_dim) * pl->elem_bytes;
+    const int stage_bytes = pl->tile_rows * row_bytes;
+    BulkKernel fn = pick_bulk(pl, hazard);
+    cudaFuncAttributes fa;
+    CU(cudaFuncGetAttributes(&fa, reinterpret_cast<const void*>(fn)));
+    int stages = (g_dev.smem_optin - (int)fa.sharedSizeBytes - 1024) / stage_bytes;
+    if (pl->tuning.stages > 0 && stages > pl->tuning.stages) stages = pl->tuning.stages;
+    if (stages > kBulkMaxStages) stages = kBulkMaxStages;
+    if (stages < 3) { g_last_error = "bulk kernel: tile does not fit three shared-memory stages"; return LEYLINE_E_UNSUPPORTED; }
+    const int smem = stages * stage_bytes;
+    CU(cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    for (int l0 = 0; l0 < L; l0 += kMaxLayers) {
+        const int nl = L - l0 < kMaxLayers ? L - l0 : kMaxLayers;
+        if (*ticket_slot >= 32) { g_last_error = "too many launches for one plan"; return LEYLINE_E_UNSUPPORTED; }
+        MoveParams mp;
+        fill_params(pl, mp, tile_begin, tile_count, l0, nl, layer_src, layer_dst, layer_repl, (*ticket_slot)++);
+        int group = pl->tuning.layer_group > 0 ? pl->tuning.layer_group : 4;
+        if (group > nl) group = nl;
+        mp.n_items = (long long)tile_count * ((nl + group - 1) / group);
+        long long grid = g_dev.sms;
+        if (grid > mp.n_items) grid = mp.n_items;
+        fn<<<(unsigned)grid, hazard ? kBulkThreadsHazard : kBulkThreadsWS, (size_t)smem, stream>>>(mp, stages, stage_bytes, row_bytes, group);
+        CU(cudaGetLastError());
+    }
+    return LEYLINE_OK;
+}
+
 leyline_status check_layers(const leyline_plan_s* pl, const void* const* a, const char* what) {
     if (!a) { g_last_error = std::string(what) + " is NULL"; return LEYLINE_E_INVALID; }
     for (int l = 0; l < pl->desc.n_layers; ++l)
@@ -247,7 +294,16 @@ extern "C" leyline_status leyline_splice(leyline_plan_t* pl, void* const* layer_
     if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_start), stream));
     int slot = 0;
     const int cps = pl->tuning.ctas_per_sm;
-    if (inplace) {
+    if (pl->use_bulk) {
+        /* bulk kernel (TMA 1-D copies through shared memory); inserts after the moves for INPLACE_MOVE */
+        if (inplace) {
+            st = run_tiles_bulk(pl, true, 0, n_move, layer_src, layer_dst, layer_repl, stream, &slot);
+            if (st != LEYLINE_OK) return st;
+            st = run_tiles_bulk(pl, false, (int32_t)n_move, n_ins, layer_src, layer_dst, layer_repl, stream, &slot);
+        } else {
+            st = run_tiles_bulk(pl, false, 0, n_move + n_ins, layer_src, layer_dst, layer_repl, stream, &slot);
+        }
+    } else if (inplace) {
         /* a3 under rule M2 ordering, then a4 once every move has landed (stream order) */
         st = run_tiles(pl, pick_move(pl, true), 0, cps, 0, n_move, layer_src, layer_dst, layer_repl, stream, &slot);
         if (st != LEYLINE_OK) return st;

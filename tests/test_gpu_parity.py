@@ -15,6 +15,9 @@ pytestmark = pytest.mark.gpu
 
 MODES = [O.FRESH, O.INPLACE_MOVE, O.ROTATE_ONLY]
 MODE_NAME = {O.FRESH: "fresh", O.INPLACE_MOVE: "inplace", O.ROTATE_ONLY: "rotate_only"}
+# leyline_tuning.kernel: the a3/a4 mover.  1 = k_move_rows (register-staged), 2 = k_move_bulk (TMA bulk copies through
+# shared memory); 0 = the planner's choice (bulk when pages hold >= 16 unpadded rows), which is what bench.py times.
+MOVERS = [1, 2]
 
 
 def run_and_compare(w, mode, check_layers=None, tuning=None):
@@ -56,24 +59,26 @@ def run_and_compare(w, mode, check_layers=None, tuning=None):
 
 
 @pytest.mark.parametrize("mode", MODES)
-def test_config1_all_modes(mode):
-    run_and_compare(synth.config(1, pool_factor=2.5), mode)
+@pytest.mark.parametrize("mover", [0] + MOVERS)
+def test_config1_all_modes(mode, mover):
+    run_and_compare(synth.config(1, pool_factor=2.5), mode, tuning={"kernel": mover})
 
 
 @pytest.mark.parametrize("mode", MODES)
 @pytest.mark.parametrize("dtype", [synth.DT_BF16, synth.DT_FP8])
 @pytest.mark.parametrize("pairing", [synth.NEOX, synth.INTERLEAVED])
-def test_randomised_small(mode, dtype, pairing):
+@pytest.mark.parametrize("mover", MOVERS)
+def test_randomised_small(mode, dtype, pairing, mover):
     rng = np.random.default_rng(77 + 10 * mode + 3 * dtype + pairing)
     for _ in range(12):
         w = tiny_workload(rng, dtype=dtype)
         w.pairing = pairing
-        run_and_compare(w, mode)
+        run_and_compare(w, mode, tuning={"kernel": mover})
 
 
 @pytest.mark.parametrize("mode", MODES)
-@pytest.mark.parametrize("tile_rows", [1, 7, 32])
-def test_medium_many_tiles_ragged(mode, tile_rows):
+@pytest.mark.parametrize("mover,tile_rows", [(1, 1), (1, 7), (1, 32), (2, 1), (2, 7), (2, 32), (2, 64)])
+def test_medium_many_tiles_ragged(mode, mover, tile_rows):
     """Several pages, ragged tails, tiles that straddle pages, growth and shrink in one request, YaRN thetas."""
     w = synth.Workload("medium", 3, [3000, 1, 0, 2777], 16, inv_freq=synth.yarn_inv_freq(),
                        directives=[(0, 5, 5, 40, 0, 0), (0, 100, 900, 3, 0, 0), (0, 1500, 1501, 333, 0, 0),
@@ -81,7 +86,18 @@ def test_medium_many_tiles_ragged(mode, tile_rows):
                                    (1, 0, 1, 0, 0, 0),
                                    (3, 0, 17, 500, 0, 0), (3, 1000, 1700, 0, 0, 0), (3, 2776, 2777, 2, 0, 0)],
                        seed=11, pool_factor=3.0, extra_pages=80).finalize()
-    run_and_compare(w, mode, tuning={"tile_rows": tile_rows})
+    run_and_compare(w, mode, tuning={"kernel": mover, "tile_rows": tile_rows})
+
+
+@pytest.mark.parametrize("mode", [O.FRESH, O.INPLACE_MOVE])
+@pytest.mark.parametrize("stages,layer_group", [(3, 1), (4, 3), (8, 8)])
+def test_bulk_ring_geometry(mode, stages, layer_group):
+    """The bulk mover's shared-memory ring at its smallest and largest depth, layer groups that do not divide the
+    layer count (5 layers), growth and shrink in one request."""
+    w = synth.Workload("ring", 5, [2100, 900], 16, inv_freq=synth.yarn_inv_freq(),
+                       directives=[(0, 7, 40, 300, 0, 0), (0, 900, 1700, 5, 0, 0), (1, 100, 101, 77, 0, 0)],
+                       seed=21, pool_factor=3.0, extra_pages=60).finalize()
+    run_and_compare(w, mode, tuning={"kernel": 2, "tile_rows": 16, "stages": stages, "layer_group": layer_group})
 
 
 @pytest.mark.parametrize("mode", MODES)
@@ -112,15 +128,22 @@ def test_special_values_survive():
     compare_layer(w, bm, B.FRESH, old, cache.pools[0].cpu().numpy(), cache.repl[0].cpu().numpy(), 1.0)
 
 
-@pytest.mark.parametrize("mode", [O.FRESH, O.ROTATE_ONLY, O.INPLACE_MOVE])
-def test_config2_dsv2lite(mode):
-    run_and_compare(synth.config(2, pool_factor=2.2), mode, check_layers=[0, 13, 26])
+@pytest.mark.parametrize("mode,mover", [(O.FRESH, 1), (O.FRESH, 2), (O.ROTATE_ONLY, 0), (O.INPLACE_MOVE, 1),
+                                        (O.INPLACE_MOVE, 2)])
+def test_config2_dsv2lite(mode, mover):
+    run_and_compare(synth.config(2, pool_factor=2.2), mode, check_layers=[0, 13, 26], tuning={"kernel": mover})
 
 
 @pytest.mark.parametrize("cfg", [3, "3m"])
 @pytest.mark.parametrize("mode", MODES)
 def test_config3_dsv3_full_size(cfg, mode):
+    # default tuning = the launch configuration bench.py times (bulk mover for FRESH / INPLACE_MOVE)
     run_and_compare(synth.config(cfg, pool_factor=2.0), mode, check_layers=[0, 37, 60])
+
+
+@pytest.mark.parametrize("mode", [O.FRESH, O.INPLACE_MOVE])
+def test_config3m_row_mover_full_size(mode):
+    run_and_compare(synth.config("3m", pool_factor=2.0), mode, check_layers=[0, 60], tuning={"kernel": 1})
 
 
 def test_config4_batched_inplace_full_size():

@@ -103,7 +103,7 @@ def check_tiles_cover(plan, bm, w, mode):
     n_move = plan.info.n_move_tiles
     seen = {}
     for t_i, t in enumerate(tiles):
-        assert 1 <= t.n_rows <= (256 if (mode == B.ROTATE_ONLY and t_i < n_move) else 32)
+        assert 1 <= t.n_rows <= plan.info.tile_rows <= 64
         is_repl = bool(t.flags & B.TILE_SRC_REPL)
         assert is_repl == (t_i >= n_move)
         for q in range(t.n_rows):
