@@ -123,34 +123,25 @@ class ClockSampler:
 # ----------------------------------------------------------------------------- our arm
 
 def dist_setup(n_gpus: int):
+    """One process per GPU (torchrun exports RANK / LOCAL_RANK / WORLD_SIZE); nccl only carries the timing contract's
+    barrier and max-over-ranks -- the splice itself has no exchange step (paper_2606_01065_b200/replicas.py)."""
     import torch
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2606_01065_b200 import replicas as R
+    local = R.env_rank()[2]
     torch.cuda.set_device(local)
-    if world > 1:
-        import torch.distributed as dist
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    return rank, world, local
+    return R.init("nccl", torch.device("cuda", local))
 
 
 def barrier(world: int):
     import torch
-    if world > 1:
-        import torch.distributed as dist
-        dist.barrier()
-    torch.cuda.synchronize()
+    from paper_2606_01065_b200 import replicas as R
+    R.barrier(world, torch.device("cuda", torch.cuda.current_device()))
 
 
 def max_over_ranks(x: float, world: int) -> float:
-    if world == 1:
-        return x
     import torch
-    import torch.distributed as dist
-    t = torch.tensor([x], dtype=torch.float64, device="cuda")
-    dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    return float(t.item())
+    from paper_2606_01065_b200 import replicas as R
+    return R.max_over_ranks(x, world, torch.device("cuda", torch.cuda.current_device()))
 
 
 def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1):
@@ -352,10 +343,8 @@ def run_ours(args):
             except Exception as ex:   # e.g. the host cannot pin that much memory: say so instead of inventing a number
                 out["e2e"] = {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
                               "error": f"{type(ex).__name__}: {ex}"}
-    if world > 1:
-        import torch.distributed as dist
-        dist.barrier()
-        dist.destroy_process_group()
+    from paper_2606_01065_b200 import replicas as R
+    R.finish(world)
     if rank == 0:
         print(json.dumps(out))
 
