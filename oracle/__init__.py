@@ -267,25 +267,27 @@ def plan_batch(mode: int, P: int, seq_lens, pt_offsets, pages, directives, free_
 # ----------------------------------------------------------------------------- O4
 
 def apply_layer(dtype: int, pairing: int, Dc: int, Dr: int, stride: int, inv_freq: np.ndarray, scale: float,
-                old_pool: np.ndarray, new_pool: np.ndarray, repl: np.ndarray | None, rm: RequestMap) -> int:
-    """One request, one layer.  old_pool (uint8, pristine) is read, new_pool (uint8) is written in place."""
+                old_pool: np.ndarray, new_pool: np.ndarray, repl: np.ndarray | None, rm: RequestMap,
+                n_heads: int = 1) -> int:
+    """One request, one layer.  old_pool (uint8, pristine) is read, new_pool (uint8) is written in place.
+    A row is Dc position-free elements + n_heads heads of Dr rotated elements (n_heads = 1: MLA)."""
     assert old_pool.dtype == np.uint8 and new_pool.dtype == np.uint8
     assert old_pool.flags.c_contiguous and new_pool.flags.c_contiguous
     inv = np.ascontiguousarray(inv_freq, dtype=np.float32)
     s = rm.segs
     rp = _p(np.ascontiguousarray(repl)) if repl is not None else None
-    return lib().ora_apply_layer(C.c_int(dtype), C.c_int(pairing), C.c_int32(Dc), C.c_int32(Dr), C.c_int64(stride),
-                                 _p(inv), C.c_float(scale), _p(old_pool), _p(new_pool), rp, C.c_int32(len(s)),
+    return lib().ora_apply_layer(C.c_int(dtype), C.c_int(pairing), C.c_int32(Dc), C.c_int32(Dr), C.c_int32(n_heads),
+                                 C.c_int64(stride), _p(inv), C.c_float(scale), _p(old_pool), _p(new_pool), rp, C.c_int32(len(s)),
                                  _p(s.kind), _p(s.src), _p(s.dst), _p(s.len), _p(s.shift), _p(_i64(rm.slot_old)),
                                  _p(_i64(rm.slot_new)))
 
 
 def splice_layer(dtype: int, pairing: int, Dc: int, Dr: int, stride: int, inv_freq: np.ndarray, scale: float,
-                 old_pool: np.ndarray, repl: np.ndarray | None, bm: BatchMap) -> np.ndarray:
+                 old_pool: np.ndarray, repl: np.ndarray | None, bm: BatchMap, n_heads: int = 1) -> np.ndarray:
     """All requests of a batch on one layer: returns the new pool (a copy of old_pool with every live new
     position of every request written).  Requests never alias, so their order is irrelevant here."""
     new_pool = old_pool.copy()
     for rm in bm.requests:
-        st = apply_layer(dtype, pairing, Dc, Dr, stride, inv_freq, scale, old_pool, new_pool, repl, rm)
+        st = apply_layer(dtype, pairing, Dc, Dr, stride, inv_freq, scale, old_pool, new_pool, repl, rm, n_heads)
         assert st == OK, st
     return new_pool

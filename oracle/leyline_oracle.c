@@ -287,47 +287,54 @@ void ora_rerope_pair(double a, double b, double p, double C, double theta, doubl
 
 /* One layer.  old_pool is a pristine snapshot, new_pool a separate buffer (pre-filled by the caller),
  * so no ordering or hazard logic exists here.  slot_old[t] / slot_new[t'] are token-level slots of old /
- * new logical positions.  For every segment, for every token (explicit loop):
+ * new logical positions.  A row is Dc position-free elements followed by n_heads heads of Dr rotated elements:
+ * n_heads = 1 is MLA's K_pe band; n_heads = kv_heads with Dc = 0 is the GQA / MHA degenerate case
+ * "qk_nope_head_dim=0 ... rotates the full 128-dim K" ("the rotation must act across
+ * all d_K dimensions per token"), every head using the same theta_i (RoPE is applied per head, Su et al.).
+ * For every segment, for every token (explicit loop):
  *   latent  : Dc*E bytes copied verbatim, never decoded                     ("K_nope and V preserved")
- *   K_pe    : shift C == 0 -> Dr*E bytes verbatim (G19: -0 must survive);
- *             else for i in [0,H): pair (i, i+H) NeoX or (2i, 2i+1) interleaved,
+ *   K_pe    : shift C == 0 -> n_heads*Dr*E bytes verbatim (G19: -0 must survive);
+ *             else for every head h, for i in [0,H): pair (i, i+H) NeoX or (2i, 2i+1)
+ *             interleaved inside the head,
  *             phi = (double)C * (double)inv_freq[i], rotate in fp64, encode by direct RNE.
  *             fp8: x = decode(byte)*scale, rotate, encode(x'/scale) saturating (G16).
  *   INSERT  : W*E bytes verbatim from the replacement buffer row repl_row+q (its K_pe is already roped
  *             at the final position, G12; PAPER.md:127 step 2).
  * Bytes of a row beyond W*E (row padding) are not touched. */
-int ora_apply_layer(int dtype, int pairing, int32_t Dc, int32_t Dr, int64_t stride, const float* inv_freq,
-                    float scale_f, const uint8_t* old_pool, uint8_t* new_pool, const uint8_t* repl, int32_t n_seg,
-                    const int32_t* kind, const int64_t* src, const int64_t* dst, const int64_t* len,
-                    const int64_t* shift, const int64_t* slot_old, const int64_t* slot_new) {
+int ora_apply_layer(int dtype, int pairing, int32_t Dc, int32_t Dr, int32_t n_heads, int64_t stride,
+                    const float* inv_freq, float scale_f, const uint8_t* old_pool, uint8_t* new_pool,
+                    const uint8_t* repl, int32_t n_seg, const int32_t* kind, const int64_t* src, const int64_t* dst,
+                    const int64_t* len, const int64_t* shift, const int64_t* slot_old, const int64_t* slot_new) {
     int E = elem_bytes(dtype);
     int32_t H = Dr / 2;
     double scale = (dtype == ORA_FP8_E4M3) ? (double)scale_f : 1.0;
-    if (Dr % 2 != 0) return ORA_E_UNSUPPORTED;
+    if (Dr % 2 != 0 || n_heads < 1) return ORA_E_UNSUPPORTED;
     for (int32_t g = 0; g < n_seg; ++g) {
         for (int64_t q = 0; q < len[g]; ++q) {
             uint8_t* out = new_pool + slot_new[dst[g] + q] * stride;
             if (kind[g] == ORA_INSERT) {
-                memcpy(out, repl + (src[g] + q) * stride, (size_t)(Dc + Dr) * E);
+                memcpy(out, repl + (src[g] + q) * stride, (size_t)(Dc + (int64_t)n_heads * Dr) * E);
                 continue;
             }
             const uint8_t* in = old_pool + slot_old[src[g] + q] * stride;
             memcpy(out, in, (size_t)Dc * E); /* latent */
-            const uint8_t* kin = in + (int64_t)Dc * E;
-            uint8_t* kout = out + (int64_t)Dc * E;
             if (shift[g] == 0) {
-                memcpy(kout, kin, (size_t)Dr * E);
+                memcpy(out + (int64_t)Dc * E, in + (int64_t)Dc * E, (size_t)n_heads * Dr * E);
                 continue;
             }
-            for (int32_t i = 0; i < H; ++i) {
-                int64_t ia = (pairing == ORA_NEOX) ? i : 2 * i;
-                int64_t ib = (pairing == ORA_NEOX) ? i + H : 2 * i + 1;
-                double a = load_elem(dtype, kin, ia, scale), b = load_elem(dtype, kin, ib, scale);
-                double phi = (double)shift[g] * (double)inv_freq[i];
-                double a2, b2;
-                ora_rotate_pair(a, b, phi, &a2, &b2);
-                store_elem(dtype, kout, ia, a2, scale);
-                store_elem(dtype, kout, ib, b2, scale);
+            for (int32_t h = 0; h < n_heads; ++h) {
+                const uint8_t* kin = in + ((int64_t)Dc + (int64_t)h * Dr) * E;
+                uint8_t* kout = out + ((int64_t)Dc + (int64_t)h * Dr) * E;
+                for (int32_t i = 0; i < H; ++i) {
+                    int64_t ia = (pairing == ORA_NEOX) ? i : 2 * i;
+                    int64_t ib = (pairing == ORA_NEOX) ? i + H : 2 * i + 1;
+                    double a = load_elem(dtype, kin, ia, scale), b = load_elem(dtype, kin, ib, scale);
+                    double phi = (double)shift[g] * (double)inv_freq[i];
+                    double a2, b2;
+                    ora_rotate_pair(a, b, phi, &a2, &b2);
+                    store_elem(dtype, kout, ia, a2, scale);
+                    store_elem(dtype, kout, ib, b2, scale);
+                }
             }
         }
     }

@@ -38,7 +38,9 @@ struct MoveParams {
     int32_t page_shift;
     int32_t H;                    /* rope_dim / 2 */
     int32_t lat_chunks;           /* 16-byte chunks of latent per row */
-    int32_t band_chunks;          /* 16-byte chunks of K_pe per row (power of two) */
+    int32_t band_chunks;          /* 16-byte chunks of the rotated band per row = n_heads * head_chunks */
+    int32_t n_heads;              /* heads in the rotated band (1 for MLA's K_pe; kv_heads for full-width K) */
+    int32_t head_chunks;          /* 16-byte chunks per head (rope_dim * elem bytes / 16) */
     const uint8_t* src[kMaxLayers];
     uint8_t* dst[kMaxLayers];
     const uint8_t* repl[kMaxLayers];
@@ -185,6 +187,54 @@ __device__ __forceinline__ int4 rotate_chunk_interleaved(const int4& mine, const
         r[2 * q + 1] = __fmaf_rn(a, s[q], b * c[q]);
     }
     return Codec<DT>::pack(r);
+}
+
+/* ---- the rotation of a PAIR of 16-byte chunks held by one thread (no lane exchange) ----
+ * NeoX: `lo` = elements [q*N, q*N+N) of a head's first half, `hi` = the same elements of its second half;
+ *       c / s = cos / sin of those N pairs (trig_row + q*N, trig_row + H + q*N).
+ * Interleaved: `lo` = chunk q of the head, `hi` = chunk q + half; each holds N/2 whole pairs;
+ *       c[0..N/2) / s[0..N/2) belong to lo (pairs q*N/2 ..), c[N/2..N) / s[N/2..N) to hi (pairs (q+half)*N/2 ..).
+ * Same fp32 expressions as rotate_chunk_neox / rotate_chunk_interleaved: a' = fma(b, -s, a*c), b' = fma(a, s, b*c). */
+template <int DT, int PAIRING>
+__device__ __forceinline__ void rotate_chunk_pair(int4& lo, int4& hi, const float* c, const float* s) {
+    constexpr int N = Codec<DT>::kElems;
+    float a[N], b[N];
+    Codec<DT>::unpack(lo, a);
+    Codec<DT>::unpack(hi, b);
+    if (PAIRING == LEYLINE_ROPE_NEOX) {
+#pragma unroll
+        for (int e = 0; e < N; ++e) {
+            const float x = a[e], y = b[e];
+            a[e] = __fmaf_rn(y, -s[e], x * c[e]);
+            b[e] = __fmaf_rn(x, s[e], y * c[e]);
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < N / 2; ++q) {
+            const float x0 = a[2 * q], y0 = a[2 * q + 1], x1 = b[2 * q], y1 = b[2 * q + 1];
+            a[2 * q] = __fmaf_rn(y0, -s[q], x0 * c[q]);
+            a[2 * q + 1] = __fmaf_rn(x0, s[q], y0 * c[q]);
+            b[2 * q] = __fmaf_rn(y1, -s[N / 2 + q], x1 * c[N / 2 + q]);
+            b[2 * q + 1] = __fmaf_rn(x1, s[N / 2 + q], y1 * c[N / 2 + q]);
+        }
+    }
+    lo = Codec<DT>::pack(a);
+    hi = Codec<DT>::pack(b);
+}
+
+/* cos / sin registers for pair column q of a head (see rotate_chunk_pair): N floats each. */
+template <int DT, int PAIRING>
+__device__ __forceinline__ void load_pair_trig(const float* __restrict__ trig_row, int H, int q, int half, float* c, float* s) {
+    constexpr int N = Codec<DT>::kElems;
+    if (PAIRING == LEYLINE_ROPE_NEOX) {
+        load_floats(trig_row + q * N, c, N);
+        load_floats(trig_row + H + q * N, s, N);
+    } else {
+        load_floats(trig_row + q * (N / 2), c, N / 2);
+        load_floats(trig_row + H + q * (N / 2), s, N / 2);
+        load_floats(trig_row + (q + half) * (N / 2), c + N / 2, N / 2);
+        load_floats(trig_row + H + (q + half) * (N / 2), s + N / 2, N / 2);
+    }
 }
 
 __device__ __forceinline__ int4 shfl_xor_int4(const int4& v, int lane_mask) {

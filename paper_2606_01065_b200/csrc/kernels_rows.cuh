@@ -6,7 +6,8 @@
  *                  (PAPER.md:118-127, :405(b)(c)); with HAZARD = true it is the in-place mover of rule M2
  *   k_rotate_band  a5  in-place rotation of the K_pe band only
  *
- * All three are persistent: CTAs pull (tile, layer) items from a ticket counter, layer fastest.
+ * k_move_rows is persistent (CTAs pull (tile, layer) items from a ticket counter, layer fastest); k_rotate_band
+ * and k_index take their items round-robin.
  */
 #ifndef LEYLINE_KERNELS_ROWS_CUH_
 #define LEYLINE_KERNELS_ROWS_CUH_
@@ -115,44 +116,76 @@ __global__ void __launch_bounds__(kThreads, 3) k_move_rows(const __grid_constant
 
 /* ------------------------------------------------------------------ a5 ---- */
 
-constexpr int kRotTileRows = 256; /* rows per in-place rotation tile (ROTATE_ONLY plans) */
-constexpr int kRotPerThread = 8;
+/* In-place rotation of the band where the rows sit.  Only `band` bytes of every row move (128 B of a
+ * 1152-B bf16 MLA row), so the kernel is a strided gather/scatter: what matters is many independent 16-byte
+ * accesses in flight and few instructions around them.  A work unit is a (row, pair column): the 16-byte chunk q
+ * of a head's first half and its partner chunk q + half, both held by ONE thread, so no lane exchange, no shared
+ * memory and no barrier is needed.  One block handles one (tile, layer) item = kRotUnroll units per thread, all
+ * loads issued before the first store; items are assigned round-robin (static), no atomics.
+ * FIXED: the pair columns per row divide the block size, so a thread keeps one column (cos/sin stay in registers). */
+constexpr int kRotUnroll = 4;
+constexpr int kRotUnitsPerItem = kThreads * kRotUnroll; /* the planner sizes ROTATE_ONLY tiles to <= this many units */
 
-template <int DT, int PAIRING, int NB_T>
-__global__ void __launch_bounds__(kThreads, 4) k_rotate_band(const __grid_constant__ MoveParams p) {
-    __shared__ int64_t s_off[kRotTileRows];
-    __shared__ long long s_item;
+template <int DT, int PAIRING, bool FIXED>
+__global__ void __launch_bounds__(kThreads, 3) k_rotate_band(const __grid_constant__ MoveParams p) {
+    constexpr int N = Codec<DT>::kElems;
     const int tid = threadIdx.x;
-    const int NB = NB_T >= 0 ? NB_T : p.band_chunks;
-    const int per_pass = kThreads / NB; /* rows per pass */
-
-    for (;;) {
-        if (tid == 0) s_item = (long long)atomicAdd(p.ticket, 1ull);
-        __syncthreads();
-        const long long item = s_item;
-        if (item >= p.n_items) break;
+    const int half = p.head_chunks >> 1;   /* pair columns per head */
+    const int cols = p.n_heads * half;     /* pair columns per row */
+    const int64_t band0 = (int64_t)p.lat_chunks * 16;
+    const int rows_per_pass = FIXED ? kThreads / cols : 0;
+    int col_f = 0, r_f = 0, q_f = 0, chunk_f = 0;
+    if (FIXED) {
+        r_f = tid / cols;
+        col_f = tid - r_f * cols;
+        const int head = col_f / half;
+        q_f = col_f - head * half;
+        chunk_f = head * p.head_chunks + q_f;
+    }
+    for (long long item = blockIdx.x; item < p.n_items; item += gridDim.x) {
         const int tile_i = p.tile_begin + (int)(item / p.n_layers);
         const int layer = (int)(item % p.n_layers);
         const DevTile t = p.tiles[tile_i];
-        for (int r = tid; r < t.n_rows; r += kThreads)
-            s_off[r] = slot_of(p.tabs, t.src_tab, t.src_pos + r, p.page_shift) * p.stride + (int64_t)p.lat_chunks * 16;
-        __syncthreads();
         uint8_t* __restrict__ base = p.dst[layer];
         const float* __restrict__ trig_row = p.trig + (int64_t)t.trig * 2 * p.H;
-        const int r0 = tid / NB, j = tid - r0 * NB;
-        int4 v[kRotPerThread];
+        const int total = t.n_rows * cols;
+        int4 lo[kRotUnroll], hi[kRotUnroll];
+        uint8_t* addr[kRotUnroll];
+        int qs[kRotUnroll];
 #pragma unroll
-        for (int k = 0; k < kRotPerThread; ++k) {
-            const int r = r0 + k * per_pass;
-            if (r < t.n_rows) v[k] = ld_coherent(base + s_off[r] + j * 16);
+        for (int k = 0; k < kRotUnroll; ++k) {
+            int r, chunk;
+            bool active;
+            if (FIXED) {
+                r = r_f + k * rows_per_pass;
+                chunk = chunk_f;
+                qs[k] = q_f;
+                active = r < t.n_rows;
+            } else {
+                const int u = tid + k * kThreads;
+                r = u / cols;
+                const int col = u - r * cols;
+                const int head = col / half;
+                qs[k] = col - head * half;
+                chunk = head * p.head_chunks + qs[k];
+                active = u < total;
+            }
+            addr[k] = nullptr;
+            if (active) {
+                addr[k] = base + slot_of(p.tabs, t.src_tab, t.src_pos + r, p.page_shift) * p.stride + band0 + (int64_t)chunk * 16;
+                lo[k] = ld_coherent(addr[k]);
+                hi[k] = ld_coherent(addr[k] + half * 16);
+            }
         }
+        float c[N], s[N];
+        if (FIXED) load_pair_trig<DT, PAIRING>(trig_row, p.H, q_f, half, c, s);
 #pragma unroll
-        for (int k = 0; k < kRotPerThread; ++k) {
-            const int r = r0 + k * per_pass;
-            const bool active = r < t.n_rows;
-            if (k * per_pass < t.n_rows) { /* warp-uniform: the NeoX partner exchange needs the whole warp */
-                const int4 w = rotate_band_chunk<DT, PAIRING>(active ? v[k] : make_int4(0, 0, 0, 0), j, NB, trig_row, p.H, active);
-                if (active) st_stream(base + s_off[r] + j * 16, w);
+        for (int k = 0; k < kRotUnroll; ++k) {
+            if (addr[k]) {
+                if (!FIXED) load_pair_trig<DT, PAIRING>(trig_row, p.H, qs[k], half, c, s);
+                rotate_chunk_pair<DT, PAIRING>(lo[k], hi[k], c, s);
+                st_stream(addr[k], lo[k]);
+                st_stream(addr[k] + half * 16, hi[k]);
             }
         }
     }
