@@ -36,7 +36,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="3", help="BASELINE.json config: 2, 3, 3m, 4, 5")
+    ap.add_argument("--workload", default="3", help="BASELINE.json config: 2, 3, 3m, 4, 5; full-width K: gqa, mha96")
     ap.add_argument("--mode", default="fresh", choices=list(MODES))
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -210,7 +210,8 @@ def cpu_baseline(pools, repls, scales, w, mode: int, bytes_per_layer: int, budge
     while done < min(max_layers, w.n_layers) and t_total < budget_s:
         old, repl = pools(done), repls(done)
         t0 = time.perf_counter()
-        O.splice_layer(w.dtype, w.pairing, w.latent_dim, w.rope_dim, w.row_bytes, w.inv_freq, scales[done], old, repl, bm)
+        O.splice_layer(w.dtype, w.pairing, w.latent_dim, w.rope_dim, w.row_bytes, w.inv_freq, scales[done], old, repl, bm,
+                       n_heads=w.rope_heads)
         t_total += time.perf_counter() - t0
         done += 1
     return {"value": done * bytes_per_layer / t_total / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
@@ -234,7 +235,7 @@ def run_e2e(cache, w, steps: int, warmup: int = 1):
         host_pool[l].copy_(cache.pools[l])
         host_repl[l].copy_(cache.repl[l])
     desc1, keep = B.make_desc(1, w.latent_dim, w.rope_dim, w.page_size, w.dtype, w.pairing, w.row_bytes, w.n_slots,
-                              w.inv_freq, [cache.scales[0]] if w.dtype == synth.DT_FP8 else None)
+                              w.inv_freq, [cache.scales[0]] if w.dtype == synth.DT_FP8 else None, rope_heads=w.rope_heads)
     s_in, s_run, s_out = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
     ev_in = [torch.cuda.Event() for _ in range(L)]
     ev_run = [torch.cuda.Event() for _ in range(L)]
@@ -367,13 +368,14 @@ def run_reference(args):
     synth.fill_repl_(rp[: w.n_repl_rows * w.row_bytes], w, 0, scale)
     old, repl = buf.numpy(), rp.numpy()
     free = w.free_slots() if mode == O.ROTATE_ONLY else w.free_pages
-    E, W = w.elem_bytes, w.latent_dim + w.rope_dim
+    E, W = w.elem_bytes, w.row_elems
     times = []
     nbytes = 0
     for i in range(args.warmup + args.steps):
         t0 = time.perf_counter()
         bm = O.plan_batch(mode, w.page_size, w.seq_lens, w.pt_offsets, w.pages, w.directives, free)
-        O.splice_layer(w.dtype, w.pairing, w.latent_dim, w.rope_dim, w.row_bytes, w.inv_freq, scale, old, repl, bm)
+        O.splice_layer(w.dtype, w.pairing, w.latent_dim, w.rope_dim, w.row_bytes, w.inv_freq, scale, old, repl, bm,
+                       n_heads=w.rope_heads)
         dt = time.perf_counter() - t0
         if i >= args.warmup:
             times.append(dt)
@@ -391,7 +393,7 @@ def run_reference(args):
                         rows += n if mode == O.INPLACE_MOVE else 0
             nbytes = 2 * rows * W * E
             if mode == O.ROTATE_ONLY:
-                nbytes += 2 * sum(n for rm in bm.requests for (k, s, d, n, c) in rm.segs.as_tuples() if k == O.KEEP and c != 0) * w.rope_dim * E
+                nbytes += 2 * sum(n for rm in bm.requests for (k, s, d, n, c) in rm.segs.as_tuples() if k == O.KEEP and c != 0) * w.rope_heads * w.rope_dim * E
     ms = float(np.mean(times)) * 1e3
     value = nbytes / (ms * 1e-3) / 1e9
     sample = f"1 of {w.n_layers} layers of {w.name} per step ({nbytes / 1e9:.3f} GB read+written), plan + splice"

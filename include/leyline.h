@@ -65,14 +65,20 @@ typedef enum { LEYLINE_AMORTIZE = 0, LEYLINE_FORGET = 1 } leyline_semantic;
 
 typedef struct {
     int32_t n_layers;          /* >= 1 */
-    int32_t latent_dim;        /* c_kv elements per row (512 for DeepSeek MLA); latent bytes must be a multiple of 16 */
-    int32_t rope_dim;          /* K_pe elements per row (64); even; (rope_dim/2)*elem bytes a multiple of 16 for NEOX,
-                                  rope_dim*elem bytes a multiple of 16 for INTERLEAVED */
+    int32_t latent_dim;        /* position-free elements at the start of a row (c_kv: 512 for DeepSeek MLA; 0 for a
+                                  GQA/MHA K pool; a V pool's elements when K and V share a row); bytes a multiple of 16 */
+    int32_t rope_dim;          /* rotated elements per HEAD (64 for MLA's K_pe; head_dim 128 / 96 for full-width K,
+                                  PAPER.md:223, :515, Table 8 :533-541); even; (rope_dim/2)*elem bytes a multiple of 16 */
     int32_t page_size;         /* tokens per page, power of two (1 = token-level slots) */
     int32_t dtype;             /* leyline_dtype */
-    int32_t pairing;           /* leyline_pairing */
-    int64_t row_stride_bytes;  /* >= (latent_dim+rope_dim)*elem bytes, multiple of 16.  Bytes of a row beyond
-                                  (latent_dim+rope_dim)*elem (padding) are never read or written. */
+    int32_t pairing;           /* leyline_pairing (inside each head) */
+    int32_t rope_heads;        /* heads in the rotated band, each rope_dim elements, all using the same inv_freq; 0 reads
+                                  as 1.  1 = MLA (one shared K_pe per token); kv_heads = the GQA/MHA degenerate case
+                                  "qk_nope_head_dim=0 rotates the full K".  Row = latent_dim +
+                                  rope_heads*rope_dim elements. */
+    int32_t reserved_;         /* must be 0 */
+    int64_t row_stride_bytes;  /* >= (latent_dim + rope_heads*rope_dim)*elem bytes, multiple of 16.  Bytes of a row
+                                  beyond that (padding) are never read or written. */
     int64_t pool_slots;        /* rows in each layer's pool (a multiple of page_size); page ids are validated
                                   against pool_slots / page_size, slot ids against pool_slots */
     const float* inv_freq;     /* HOST, [rope_dim/2]: THE theta_i in fp32 (YaRN etc. already applied; G9).
@@ -119,7 +125,8 @@ typedef struct {
                                   rope*elem per in-place rotated row */
     int64_t bytes_written;     /* same, written */
     int64_t bytes_index;       /* 4 B per new token + 4 B per new page-table entry (once, not per layer) */
-    int64_t tile_rows;         /* rows per device work item chosen for this plan */
+    int64_t tile_rows;         /* rows per device work item of the a3/a4 mover chosen for this plan */
+    int64_t rot_tile_rows;     /* ROTATE_ONLY: rows per in-place rotation work item (a5), else 0 */
     int64_t mover;             /* a3/a4 kernel this plan launches: 1 = k_move_rows, 2 = k_move_bulk (see leyline_tuning) */
 } leyline_plan_info;
 
@@ -212,8 +219,8 @@ leyline_status leyline_splice(leyline_plan_t* plan, void* const* layer_src, void
                               void* cuda_stream);
 
 /*
- * leyline_rotate_inplace -- execute a ROTATE_ONLY plan (steps a2, a5): rotate the K_pe band of every downstream
- * token where it sits (128 B of every 1152 B bf16 row), optionally copy the replacement rows into the consumed
+ * leyline_rotate_inplace -- execute a ROTATE_ONLY plan (steps a2, a5): rotate the band of every downstream
+ * token where it sits (128 B of every 1152 B bf16 MLA row; the whole row of a full-width K pool), optionally copy the replacement rows into the consumed
  * free slots (layer_repl == NULL: the caller already prefilled them), and write the new token-level index list.
  */
 leyline_status leyline_rotate_inplace(leyline_plan_t* plan, void* const* layer_ptrs, const void* const* layer_repl,
@@ -226,8 +233,10 @@ const char* leyline_last_cuda_error(void);
 
 /* Process-wide tuning knobs (benchmarking; defaults are what bench.py reports).  Read by leyline_plan. */
 typedef struct {
-    int32_t kernel;        /* a3/a4 mover: 0 = auto (bulk when pages hold >= 16 unpadded rows), 1 = row kernel (LDG/STG
-                              through registers), 2 = bulk kernel (TMA 1-D bulk copies through shared memory) */
+    int32_t kernel;        /* a3/a4 mover: 0 = auto (bulk when pages hold >= 16 unpadded rows, or when the band is not a
+                              single head of 2^k <= 32 chunks), 1 = row kernel (LDG/STG through registers; single-head
+                              bands of 2^k chunks only, else LEYLINE_E_UNSUPPORTED), 2 = bulk kernel (TMA 1-D bulk
+                              copies through shared memory) */
     int32_t tile_rows;     /* rows per tile of the move/insert kernels, 0 = default (row kernel <= 32, bulk <= 64) */
     int32_t ctas_per_sm;   /* row kernel only, 0 = default */
     int32_t profile;       /* 1: record CUDA events around the data-moving kernels (leyline_plan_kernel_ms) */

@@ -26,7 +26,7 @@ TILE_SRC_REPL = 1
 class CacheDesc(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("latent_dim", C.c_int32), ("rope_dim", C.c_int32),
                 ("page_size", C.c_int32), ("dtype", C.c_int32), ("pairing", C.c_int32),
-                ("row_stride_bytes", C.c_int64), ("pool_slots", C.c_int64),
+                ("rope_heads", C.c_int32), ("reserved_", C.c_int32), ("row_stride_bytes", C.c_int64), ("pool_slots", C.c_int64),
                 ("inv_freq", C.POINTER(C.c_float)), ("layer_scale", C.POINTER(C.c_float))]
 
 
@@ -44,7 +44,7 @@ class PlanInfo(C.Structure):
     _fields_ = [("mode", C.c_int32), ("n_requests", C.c_int32)] + [
         (n, C.c_int64) for n in ("total_new_tokens", "total_new_pages", "n_free_consumed", "n_released", "n_segments",
                                  "n_tiles", "n_move_tiles", "n_trig", "rows_moved", "rows_inserted", "rows_rotated",
-                                 "bytes_read", "bytes_written", "bytes_index", "tile_rows", "mover")]
+                                 "bytes_read", "bytes_written", "bytes_index", "tile_rows", "rot_tile_rows", "mover")]
 
 
 class Tile(C.Structure):
@@ -134,11 +134,12 @@ def _ptr(a: np.ndarray):
 
 
 def make_desc(n_layers, latent_dim, rope_dim, page_size, dtype, pairing, row_stride_bytes, pool_slots, inv_freq,
-              layer_scale=None):
-    """Returns (CacheDesc, keepalive) -- keep `keepalive` referenced while the desc is in use."""
+              layer_scale=None, rope_heads=1):
+    """Returns (CacheDesc, keepalive) -- keep `keepalive` referenced while the desc is in use.
+    Row = latent_dim + rope_heads * rope_dim elements (rope_heads = 1: MLA; kv_heads: full-width K)."""
     inv = _arr(inv_freq, np.float32)
     sc = _arr(layer_scale, np.float32) if layer_scale is not None else None
-    d = CacheDesc(n_layers, latent_dim, rope_dim, page_size, dtype, pairing, row_stride_bytes, pool_slots,
+    d = CacheDesc(n_layers, latent_dim, rope_dim, page_size, dtype, pairing, rope_heads, 0, row_stride_bytes, pool_slots,
                   inv.ctypes.data_as(C.POINTER(C.c_float)),
                   sc.ctypes.data_as(C.POINTER(C.c_float)) if sc is not None else None)
     return d, (inv, sc)

@@ -83,26 +83,29 @@ __device__ __forceinline__ void named_bar_sync(int id, int n_threads) {
 
 /* ------------------------------------------------------------------ a3 + a4 ---- */
 
+/* warp 0 = producer; warps 1..cwarps = consumers (warp 1 also stores), cwarps = 4 for MLA's narrow band, 8 when the
+ * band is most of the row (full-width K); HAZARD adds 4 warps that publish "loaded" and poll dependencies (rule M2),
+ * round-robin over stages, and a last warp that watches the stages land in order. */
 constexpr int kBulkConsumerWarps = 4;
-constexpr int kBulkConsumers = 32 * kBulkConsumerWarps;
-constexpr int kBulkThreadsWS = 32 + kBulkConsumers; /* warp 0 = producer, warps 1..4 = consumers (warp 1 also stores) */
-constexpr int kBulkHazardWarps = 4; /* + warps 5..8: publish "loaded" and poll dependencies (rule M2), round-robin over stages */
-constexpr int kBulkThreadsHazard = kBulkThreadsWS + 32 * (kBulkHazardWarps + 1); /* last warp: in-order landing watcher */
+constexpr int kBulkMaxConsumerWarps = 8;
+constexpr int kBulkHazardWarps = 4;
+constexpr int kBulkMaxThreadsWS = 32 * (1 + kBulkMaxConsumerWarps);
+constexpr int kBulkMaxThreadsHazard = kBulkMaxThreadsWS + 32 * (kBulkHazardWarps + 1);
 
 /* Work item = (tile, group of `layer_group` consecutive layers), group fastest: the producer resolves the tile's rows
  * once and issues one stage per layer of the group. */
 template <int DT, int PAIRING, bool HAZARD>
-__global__ void __launch_bounds__(HAZARD ? kBulkThreadsHazard : kBulkThreadsWS, 1) k_move_bulk(const __grid_constant__ MoveParams p, const int n_stages,
-                                                                 const int stage_bytes, const int row_bytes,
-                                                                 const int layer_group) {
+__global__ void __launch_bounds__(HAZARD ? kBulkMaxThreadsHazard : kBulkMaxThreadsWS, 1)
+k_move_bulk(const __grid_constant__ MoveParams p, const int n_stages, const int stage_bytes, const int row_bytes,
+            const int layer_group, const int cwarps) {
     extern __shared__ __align__(128) uint8_t smem[];
     __shared__ BulkStageInfo s_info[kBulkMaxStages];
     __shared__ __align__(8) uint64_t s_full[kBulkMaxStages], s_empty[kBulkMaxStages], s_deps[kBulkMaxStages];
     __shared__ volatile int s_end_it;    /* iteration index of the end marker, -1 while the producer still has work */
     __shared__ volatile int s_loaded_it; /* HAZARD: stages [0, s_loaded_it) have landed (written by the watcher warp, in order) */
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int NB = p.band_chunks;
     const int band0 = p.lat_chunks * 16;
+    const int n_consumers = 32 * cwarps;
     constexpr int N = Codec<DT>::kElems;
 
     if (tid == 0) {
@@ -184,7 +187,7 @@ __global__ void __launch_bounds__(HAZARD ? kBulkThreadsHazard : kBulkThreadsWS, 
         return;
     }
 
-    if (HAZARD && warp == 1 + kBulkConsumerWarps + kBulkHazardWarps) {
+    if (HAZARD && warp == 1 + cwarps + kBulkHazardWarps) {
         /* ---------------- watcher: waits for the stages in ring order (so its parity waits never alias) and counts
          * the landed ones for the hazard warps, ahead of the consumers ---------------- */
         for (int it = 0;; ++it) {
@@ -195,12 +198,12 @@ __global__ void __launch_bounds__(HAZARD ? kBulkThreadsHazard : kBulkThreadsWS, 
         }
         return;
     }
-    if (HAZARD && warp >= 1 + kBulkConsumerWarps) {
+    if (HAZARD && warp >= 1 + cwarps) {
         /* ---------------- hazard warps (rule M2), off the consumers' critical path: once a stage's rows are in shared
          * memory publish "loaded" for (tile, layer), then wait until every tile whose source rows this tile
          * overwrites has published too, and tell the storing warp through the stage's s_deps barrier.  The release
          * fence and the acquire poll cost more than a tile's time slot, so several warps take the stages in turn. - */
-        for (int it = warp - (1 + kBulkConsumerWarps);; it += kBulkHazardWarps) {
+        for (int it = warp - (1 + cwarps);; it += kBulkHazardWarps) {
             const int stage = it % n_stages;
             /* Gate on the consumers' in-order count of landed stages, not on the mbarrier parity: this warp skips
              * iterations, and a parity wait on a phase that is more than one ahead would alias. */
@@ -233,33 +236,26 @@ __global__ void __launch_bounds__(HAZARD ? kBulkThreadsHazard : kBulkThreadsWS, 
         if (n_rows == 0) break;
         uint8_t* stage_mem = smem + (size_t)stage * stage_bytes;
         if (info.trig >= 0) {
+            /* a unit = (row, pair column): chunk q of a head's first half and its partner q + half, both rotated by
+             * this thread (rotate_chunk_pair), so no two threads touch the same bytes */
             const float* __restrict__ trig_row = p.trig + (int64_t)info.trig * 2 * p.H;
-            const int total = n_rows * NB;
-            for (int c0 = cwarp * 32; c0 < total; c0 += kBulkConsumers) { /* warp-uniform trip count */
-                const int c = c0 + lane;
-                const bool active = c < total;
-                const int r = c / NB, j = c - r * NB;
-                int4* band = reinterpret_cast<int4*>(stage_mem + (size_t)r * row_bytes + band0);
-                int4 out = make_int4(0, 0, 0, 0);
-                if (active) {
-                    const int4 mine = band[j];
-                    if (PAIRING == LEYLINE_ROPE_NEOX) {
-                        const int half = NB >> 1;
-                        const int4 other = band[j ^ half];
-                        const int jj = j & (half - 1);
-                        out = rotate_chunk_neox<DT>(mine, other, trig_row + jj * N, trig_row + p.H + jj * N,
-                                                    j < half ? -1.0f : 1.0f);
-                    } else {
-                        out = rotate_chunk_interleaved<DT>(mine, trig_row + j * (N / 2), trig_row + p.H + j * (N / 2));
-                    }
-                }
-                /* partner chunks of a row sit in the same warp (NB divides 32): every read precedes every write */
-                __syncwarp();
-                if (active) band[j] = out;
+            const int half = p.head_chunks >> 1;
+            const int cols = p.n_heads * half;
+            const int total = n_rows * cols;
+            for (int u = cwarp * 32 + lane; u < total; u += n_consumers) {
+                const int r = u / cols, col = u - r * cols;
+                const int head = col / half, q = col - head * half;
+                int4* band = reinterpret_cast<int4*>(stage_mem + (size_t)r * row_bytes + band0) + head * p.head_chunks + q;
+                int4 lo = band[0], hi = band[half];
+                float c[N], sn[N];
+                load_pair_trig<DT, PAIRING>(trig_row, p.H, q, half, c, sn);
+                rotate_chunk_pair<DT, PAIRING>(lo, hi, c, sn);
+                band[0] = lo;
+                band[half] = hi;
             }
             fence_proxy_async_smem(); /* generic-proxy writes -> visible to the bulk store's async-proxy reads */
         }
-        named_bar_sync(1, kBulkConsumers);
+        named_bar_sync(1, n_consumers);
         if (cwarp == 0) {
             if (HAZARD) mbar_wait(&s_deps[stage], (uint32_t)((it / n_stages) & 1)); /* sources I overwrite are loaded */
             uint8_t* __restrict__ dbase = p.dst[info.layer];

@@ -124,10 +124,10 @@ __global__ void __launch_bounds__(kThreads, 3) k_move_rows(const __grid_constant
  * loads issued before the first store; items are assigned round-robin (static), no atomics.
  * FIXED: the pair columns per row divide the block size, so a thread keeps one column (cos/sin stay in registers). */
 constexpr int kRotUnroll = 4;
-constexpr int kRotUnitsPerItem = kThreads * kRotUnroll; /* the planner sizes ROTATE_ONLY tiles to <= this many units */
+static_assert(kRotUnitsPerItem == kThreads * kRotUnroll, "the planner sizes ROTATE_ONLY tiles to <= this many units");
 
 template <int DT, int PAIRING, bool FIXED>
-__global__ void __launch_bounds__(kThreads, 3) k_rotate_band(const __grid_constant__ MoveParams p) {
+__global__ void __launch_bounds__(kThreads, DT == LEYLINE_FP8_E4M3 ? 2 : 3) k_rotate_band(const __grid_constant__ MoveParams p) {
     constexpr int N = Codec<DT>::kElems;
     const int tid = threadIdx.x;
     const int half = p.head_chunks >> 1;   /* pair columns per head */

@@ -48,15 +48,26 @@ int64_t build_segments(int64_t L_old, const leyline_directive* d, int32_t k, std
     return L_old + C;
 }
 
+inline int heads_of(const leyline_cache_desc& c) { return c.rope_heads > 0 ? c.rope_heads : 1; }
+inline int64_t row_elems(const leyline_cache_desc& c) { return (int64_t)c.latent_dim + (int64_t)heads_of(c) * c.rope_dim; }
+
+/* The register-staged row kernel covers one head of 2^k <= 32 chunks (partner by lane xor); everything else (several
+ * heads, head_dim 96 = 12 chunks, ...) runs on the bulk mover, whose band loop is generic. */
+bool row_kernel_ok(const leyline_cache_desc& c, int E) {
+    const int64_t nb = (int64_t)c.rope_dim * E / 16;
+    return heads_of(c) == 1 && nb <= 32 && (nb & (nb - 1)) == 0 && (int64_t)c.latent_dim * E / 16 <= 2048;
+}
+
 leyline_status check_desc(const leyline_cache_desc* c, int* elem_bytes, int* page_shift) {
     if (!c) return LEYLINE_E_INVALID;
     if (c->n_layers < 1 || c->latent_dim < 0 || c->rope_dim < 2 || (c->rope_dim & 1)) return LEYLINE_E_INVALID;
+    if (c->rope_heads < 0 || c->reserved_ != 0) return LEYLINE_E_INVALID;
     if (c->page_size < 1 || (c->page_size & (c->page_size - 1))) return LEYLINE_E_INVALID;
     if (c->dtype != LEYLINE_BF16 && c->dtype != LEYLINE_FP8_E4M3) return LEYLINE_E_INVALID;
     if (c->pairing != LEYLINE_ROPE_NEOX && c->pairing != LEYLINE_ROPE_INTERLEAVED) return LEYLINE_E_INVALID;
     if (!c->inv_freq) return LEYLINE_E_INVALID;
     int E = c->dtype == LEYLINE_BF16 ? 2 : 1;
-    int64_t row = (int64_t)(c->latent_dim + c->rope_dim) * E;
+    int64_t row = row_elems(*c) * E;
     if (c->row_stride_bytes < row || (c->row_stride_bytes & 15)) return LEYLINE_E_INVALID;
     if (c->pool_slots < 0 || (c->pool_slots % c->page_size)) return LEYLINE_E_INVALID;
     for (int i = 0; i < c->rope_dim / 2; ++i)
@@ -64,13 +75,11 @@ leyline_status check_desc(const leyline_cache_desc* c, int* elem_bytes, int* pag
     if (c->dtype == LEYLINE_FP8_E4M3 && c->layer_scale)
         for (int l = 0; l < c->n_layers; ++l)
             if (!(c->layer_scale[l] > 0.f) || !std::isfinite(c->layer_scale[l])) return LEYLINE_E_INVALID;
-    /* what the kernels cover: 16-byte chunks, K_pe band of 2^k chunks (k <= 5), NeoX halves in whole chunks */
-    int64_t lat_bytes = (int64_t)c->latent_dim * E, band_bytes = (int64_t)c->rope_dim * E;
-    if ((lat_bytes & 15) || (band_bytes & 15)) return LEYLINE_E_UNSUPPORTED;
-    int64_t nb = band_bytes / 16;
-    if (nb > 32 || (nb & (nb - 1))) return LEYLINE_E_UNSUPPORTED;
-    if (c->pairing == LEYLINE_ROPE_NEOX && nb < 2) return LEYLINE_E_UNSUPPORTED;
-    if (lat_bytes / 16 > 2048) return LEYLINE_E_UNSUPPORTED;
+    /* what the kernels cover: 16-byte chunks; a head is an even number of chunks (a thread rotates chunk q of the
+     * first half together with chunk q + half), at most 64; at most 128 heads; rows of at most 64 KB */
+    int64_t lat_bytes = (int64_t)c->latent_dim * E, head_bytes = (int64_t)c->rope_dim * E;
+    if ((lat_bytes & 15) || (head_bytes & 31)) return LEYLINE_E_UNSUPPORTED;
+    if (head_bytes / 16 > 64 || heads_of(*c) > 128 || row > 65536) return LEYLINE_E_UNSUPPORTED;
     int sh = 0;
     while ((1 << sh) < c->page_size) ++sh;
     *elem_bytes = E;
@@ -96,21 +105,22 @@ leyline_status check_directives(int32_t n_req, const int64_t* seq_lens, int32_t 
     return LEYLINE_OK;
 }
 
-/* Which mover runs a3/a4.  The bulk kernel moves contiguous runs of rows with TMA 1-D copies, so it needs runs:
- * pages of >= 16 rows and unpadded rows (padding must never be written); otherwise, and for the a5 in-place
- * rotation, the register-staged row kernel is used.  tuning.kernel = 1 / 2 forces one of them. */
+/* Which mover runs a3/a4 (and ROTATE_ONLY's inserts).  The bulk kernel moves contiguous runs of rows with TMA 1-D
+ * copies, so it pays with runs: pages of >= 16 rows and unpadded rows (padding must never be written); otherwise the
+ * register-staged row kernel is used where it covers the band geometry.  tuning.kernel = 1 / 2 forces one of them. */
 bool choose_bulk(const leyline_cache_desc& c, int E, const leyline_tuning& t, int mode) {
+    if (!row_kernel_ok(c, E)) return true;
     if (mode == LEYLINE_ROTATE_ONLY) return false;
     if (t.kernel == 1) return false;
     if (t.kernel == 2) return true;
-    return c.page_size >= 16 && c.row_stride_bytes == (int64_t)(c.latent_dim + c.rope_dim) * E;
+    return c.page_size >= 16 && c.row_stride_bytes == row_elems(c) * E;
 }
 
 int choose_tile_rows(const leyline_cache_desc& c, int E, const leyline_tuning& t, bool bulk) {
     int64_t lat_chunks = (int64_t)c.latent_dim * E / 16, nb = (int64_t)c.rope_dim * E / 16;
     if (bulk) {
         /* bulk kernel: one shared-memory stage holds a tile; default ~36 KB per stage, at most 64 rows */
-        int64_t row = (int64_t)(c.latent_dim + c.rope_dim) * E;
+        int64_t row = row_elems(c) * E;
         int64_t want = t.tile_rows > 0 ? t.tile_rows : std::max<int64_t>(1, 36864 / row);
         return (int)std::max<int64_t>(1, std::min<int64_t>({want, (int64_t)64, 65536 / row}));
     }
@@ -120,6 +130,14 @@ int choose_tile_rows(const leyline_cache_desc& c, int E, const leyline_tuning& t
     cap = std::min<int64_t>(cap, 256 / nb);
     if (cap < 1) cap = 1;
     int64_t want = t.tile_rows > 0 ? t.tile_rows : 32;
+    return (int)std::max<int64_t>(1, std::min(want, cap));
+}
+
+/* Rows per k_rotate_band work item: as many as fill the block's kRotUnitsPerItem (row, pair column) units. */
+int choose_rot_tile_rows(const leyline_cache_desc& c, int E, const leyline_tuning& t) {
+    const int64_t cols = (int64_t)heads_of(c) * ((int64_t)c.rope_dim * E / 32);
+    int64_t cap = std::max<int64_t>(1, leyline::kRotUnitsPerItem / cols);
+    int64_t want = t.tile_rows > 0 ? t.tile_rows : cap;
     return (int)std::max<int64_t>(1, std::min(want, cap));
 }
 
@@ -180,9 +198,18 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
     pl->elem_bytes = E;
     pl->page_shift = pshift;
     pl->tuning = g_tuning;
+    pl->desc.rope_heads = heads_of(*desc);
+    pl->n_heads = heads_of(*desc);
+    pl->head_chunks = desc->rope_dim * E / 16;
+    if (g_tuning.kernel == 1 && !row_kernel_ok(*desc, E)) { /* forced row kernel on a band it does not cover */
+        delete pl;
+        return LEYLINE_E_UNSUPPORTED;
+    }
     pl->use_bulk = choose_bulk(*desc, E, g_tuning, mode);
     pl->tile_rows = choose_tile_rows(*desc, E, g_tuning, pl->use_bulk);
+    pl->rot_tile_rows = mode == LEYLINE_ROTATE_ONLY ? choose_rot_tile_rows(*desc, E, g_tuning) : 0;
     const int TR = pl->tile_rows;
+    const int TR_ROT = pl->rot_tile_rows;
 
     /* tabs: old page tables first, one row per request */
     std::vector<int32_t> old_tab_off(n_requests + 1, 0);
@@ -297,7 +324,7 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
                     pl->slot_runs.push_back({pl->slot_offsets[r] + s.dst, s.len, s.src, src_tab, 0});
                     int32_t g = trig_index(s.shift);
                     if (g < 0) continue;
-                    split_tiles(s.src, s.dst, s.len, s.src, TR, [&](int64_t a, int64_t b, int32_t n) {
+                    split_tiles(s.src, s.dst, s.len, s.src, TR_ROT, [&](int64_t a, int64_t b, int32_t n) {
                         move_tiles.push_back({a, b, src_tab, src_tab, n, g, 0, 0, -1, r});
                     });
                 } else {
@@ -393,12 +420,13 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
         if (t.trig >= 0) in.rows_rotated += t.n_rows;
     }
     for (const DevTile& t : insert_tiles) in.rows_inserted += t.n_rows;
-    const int64_t row_bytes = (int64_t)(desc->latent_dim + desc->rope_dim) * E, band_bytes = (int64_t)desc->rope_dim * E;
+    const int64_t row_bytes = row_elems(*desc) * E, band_bytes = (int64_t)heads_of(*desc) * desc->rope_dim * E;
     int64_t per_layer = (in.rows_moved + in.rows_inserted) * row_bytes;
     if (mode == LEYLINE_ROTATE_ONLY) per_layer = in.rows_rotated * band_bytes + in.rows_inserted * row_bytes;
     in.bytes_read = in.bytes_written = per_layer * desc->n_layers;
     in.bytes_index = 4 * in.total_new_tokens + 4 * in.total_new_pages;
     in.tile_rows = pl->tile_rows;
+    in.rot_tile_rows = pl->rot_tile_rows;
     in.mover = pl->use_bulk ? 2 : 1;
     if (mode == LEYLINE_ROTATE_ONLY) pl->new_pages.clear();
 

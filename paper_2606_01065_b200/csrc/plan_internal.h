@@ -33,6 +33,10 @@ static_assert(sizeof(DevTile) == 48, "DevTile layout");
 
 enum : int32_t { TILE_SRC_REPL = 1, TILE_DST_TOKEN = 2 };
 
+/* k_rotate_band (a5): (row, pair column) units one block handles = 256 threads x 4; ROTATE_ONLY tiles hold at most
+ * this many units, i.e. rot_tile_rows = kRotUnitsPerItem / (rope_heads * head_chunks / 2) rows. */
+constexpr int kRotUnitsPerItem = 1024;
+
 /* One run of the token-level index list / page-table output (step a2). */
 struct IdxRun {
     int64_t out_begin; /* first output element */
@@ -54,6 +58,9 @@ struct leyline_plan_s {
     int32_t elem_bytes = 2;
     int32_t page_shift = 0;
     int32_t tile_rows = 32;
+    int32_t rot_tile_rows = 0;          /* ROTATE_ONLY: rows per k_rotate_band work item */
+    int32_t n_heads = 1;                /* heads in the rotated band (desc.rope_heads, 0 read as 1) */
+    int32_t head_chunks = 8;            /* 16-byte chunks per head */
     bool use_bulk = false;              /* a3/a4 run on k_move_bulk (TMA bulk copies) instead of k_move_rows */
     leyline_tuning tuning{};
 

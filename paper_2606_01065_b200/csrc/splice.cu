@@ -100,7 +100,7 @@ using MoveKernel = void (*)(const MoveParams);
 
 template <int DT, int PAIRING, bool HAZARD>
 MoveKernel pick_move_geom(const leyline_plan_s* pl) {
-    const int lc = pl->desc.latent_dim * pl->elem_bytes / 16, nb = pl->desc.rope_dim * pl->elem_bytes / 16;
+    const int lc = pl->desc.latent_dim * pl->elem_bytes / 16, nb = pl->head_chunks; /* row kernel: one head */
     if (DT == LEYLINE_BF16 && lc == 64 && nb == 8) return k_move_rows<DT, PAIRING, HAZARD, 64, 8>;
     if (DT == LEYLINE_FP8_E4M3 && lc == 32 && nb == 4) return k_move_rows<DT, PAIRING, HAZARD, 32, 4>;
     return k_move_rows<DT, PAIRING, HAZARD, -1, -1>;
@@ -118,7 +118,7 @@ MoveKernel pick_move(const leyline_plan_s* pl, bool hazard) {
                 : pick_move_hazard<LEYLINE_FP8_E4M3, LEYLINE_ROPE_INTERLEAVED>(pl, hazard);
 }
 
-using BulkKernel = void (*)(const MoveParams, int, int, int, int);
+using BulkKernel = void (*)(const MoveParams, int, int, int, int, int);
 
 template <int DT>
 BulkKernel pick_bulk_dt(const leyline_plan_s* pl, bool hazard) {
@@ -130,15 +130,17 @@ BulkKernel pick_bulk(const leyline_plan_s* pl, bool hazard) {
     return pl->desc.dtype == LEYLINE_BF16 ? pick_bulk_dt<LEYLINE_BF16>(pl, hazard) : pick_bulk_dt<LEYLINE_FP8_E4M3>(pl, hazard);
 }
 
-MoveKernel pick_rotate(const leyline_plan_s* pl) {
+template <int DT>
+MoveKernel pick_rotate_dt(const leyline_plan_s* pl, bool fixed) {
     const bool neox = pl->desc.pairing == LEYLINE_ROPE_NEOX;
-    const int nb = pl->desc.rope_dim * pl->elem_bytes / 16;
-    if (pl->desc.dtype == LEYLINE_BF16) {
-        if (nb == 8) return neox ? k_rotate_band<LEYLINE_BF16, LEYLINE_ROPE_NEOX, 8> : k_rotate_band<LEYLINE_BF16, LEYLINE_ROPE_INTERLEAVED, 8>;
-        return neox ? k_rotate_band<LEYLINE_BF16, LEYLINE_ROPE_NEOX, -1> : k_rotate_band<LEYLINE_BF16, LEYLINE_ROPE_INTERLEAVED, -1>;
-    }
-    if (nb == 4) return neox ? k_rotate_band<LEYLINE_FP8_E4M3, LEYLINE_ROPE_NEOX, 4> : k_rotate_band<LEYLINE_FP8_E4M3, LEYLINE_ROPE_INTERLEAVED, 4>;
-    return neox ? k_rotate_band<LEYLINE_FP8_E4M3, LEYLINE_ROPE_NEOX, -1> : k_rotate_band<LEYLINE_FP8_E4M3, LEYLINE_ROPE_INTERLEAVED, -1>;
+    if (fixed) return neox ? k_rotate_band<DT, LEYLINE_ROPE_NEOX, true> : k_rotate_band<DT, LEYLINE_ROPE_INTERLEAVED, true>;
+    return neox ? k_rotate_band<DT, LEYLINE_ROPE_NEOX, false> : k_rotate_band<DT, LEYLINE_ROPE_INTERLEAVED, false>;
+}
+/* a5.  FIXED when the pair columns of a row divide the block (a thread then keeps one column and its cos/sin). */
+MoveKernel pick_rotate(const leyline_plan_s* pl) {
+    const int cols = pl->n_heads * (pl->head_chunks / 2);
+    const bool fixed = cols <= kThreads && kThreads % cols == 0;
+    return pl->desc.dtype == LEYLINE_BF16 ? pick_rotate_dt<LEYLINE_BF16>(pl, fixed) : pick_rotate_dt<LEYLINE_FP8_E4M3>(pl, fixed);
 }
 
 }  // namespace
@@ -178,7 +180,9 @@ void fill_params(const leyline_plan_s* pl, MoveParams& mp, int32_t tile_begin, i
     mp.page_shift = pl->page_shift;
     mp.H = pl->desc.rope_dim / 2;
     mp.lat_chunks = pl->desc.latent_dim * pl->elem_bytes / 16;
-    mp.band_chunks = pl->desc.rope_dim * pl->elem_bytes / 16;
+    mp.n_heads = pl->n_heads;
+    mp.head_chunks = pl->head_chunks;
+    mp.band_chunks = pl->n_heads * pl->head_chunks;
     for (int l = 0; l < nl; ++l) {
         mp.src[l] = static_cast<const uint8_t*>(layer_src ? layer_src[l0 + l] : nullptr);
         mp.dst[l] = static_cast<uint8_t*>(layer_dst[l0 + l]);
@@ -207,14 +211,37 @@ leyline_status run_tiles(leyline_plan_s* pl, MoveKernel fn, int smem, int max_ct
     return LEYLINE_OK;
 }
 
+/* a5: k_rotate_band takes its (tile, layer) items round-robin; enough blocks that the hardware scheduler balances. */
+leyline_status run_rotate(leyline_plan_s* pl, int32_t tile_begin, int64_t tile_count, void* const* layer_ptrs,
+                          cudaStream_t stream, int* ticket_slot) {
+    if (tile_count <= 0) return LEYLINE_OK;
+    const int L = pl->desc.n_layers;
+    MoveKernel fn = pick_rotate(pl);
+    for (int l0 = 0; l0 < L; l0 += kMaxLayers) {
+        const int nl = L - l0 < kMaxLayers ? L - l0 : kMaxLayers;
+        MoveParams mp;
+        fill_params(pl, mp, tile_begin, tile_count, l0, nl, nullptr, layer_ptrs, nullptr, *ticket_slot);
+        const int per_sm = occupancy(reinterpret_cast<const void*>(fn), 0);
+        long long grid = (long long)g_dev.sms * per_sm * 8;
+        if (grid > mp.n_items) grid = mp.n_items;
+        fn<<<(unsigned)grid, kThreads, 0, stream>>>(mp);
+        CU(cudaGetLastError());
+    }
+    return LEYLINE_OK;
+}
+
 /* Same, with the bulk kernel: one persistent CTA per SM, a ring of shared-memory stages of one tile each. */
 leyline_status run_tiles_bulk(leyline_plan_s* pl, bool hazard, int32_t tile_begin, int64_t tile_count,
                               void* const* layer_src, void* const* layer_dst, const void* const* layer_repl,
                               cudaStream_t stream, int* ticket_slot) {
     if (tile_count <= 0) return LEYLINE_OK;
     const int L = pl->desc.n_layers;
-    const int row_bytes = (pl->desc.latent_dim + pl->desc.rope_dim) * pl->elem_bytes;
+    const int row_bytes = (pl->desc.latent_dim + pl->n_heads * pl->desc.rope_dim) * pl->elem_bytes;
     const int stage_bytes = pl->tile_rows * row_bytes;
+    /* consumer warps rotate the band in shared memory: 4 keep up with MLA's 1/9 of the bytes, a band that is most of
+     * the row (full-width K) needs more issue slots */
+    const int cwarps = (int64_t)pl->n_heads * pl->desc.rope_dim * 4 <= (int64_t)pl->desc.latent_dim + (int64_t)pl->n_heads * pl->desc.rope_dim
+                           ? kBulkConsumerWarps : kBulkMaxConsumerWarps;
     BulkKernel fn = pick_bulk(pl, hazard);
     cudaFuncAttributes fa;
     CU(cudaFuncGetAttributes(&fa, reinterpret_cast<const void*>(fn)));
@@ -234,7 +261,8 @@ leyline_status run_tiles_bulk(leyline_plan_s* pl, bool hazard, int32_t tile_begi
         mp.n_items = (long long)tile_count * ((nl + group - 1) / group);
         long long grid = g_dev.sms;
         if (grid > mp.n_items) grid = mp.n_items;
-        fn<<<(unsigned)grid, hazard ? kBulkThreadsHazard : kBulkThreadsWS, (size_t)smem, stream>>>(mp, stages, stage_bytes, row_bytes, group);
+        const int threads = 32 * (1 + cwarps + (hazard ? kBulkHazardWarps + 1 : 0));
+        fn<<<(unsigned)grid, threads, (size_t)smem, stream>>>(mp, stages, stage_bytes, row_bytes, group, cwarps);
         CU(cudaGetLastError());
     }
     return LEYLINE_OK;
@@ -338,11 +366,13 @@ extern "C" leyline_status leyline_rotate_inplace(leyline_plan_t* pl, void* const
     if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_start), stream));
     int slot = 0;
     /* a5: rotate where the rows sit; a4: replacement rows go to the consumed free slots (disjoint from a5's) */
-    st = run_tiles(pl, pick_rotate(pl), 0, pl->tuning.ctas_per_sm, 0, n_rot, nullptr, layer_ptrs, layer_repl, stream,
-                   &slot);
+    st = run_rotate(pl, 0, n_rot, layer_ptrs, stream, &slot);
     if (st != LEYLINE_OK) return st;
-    st = run_tiles(pl, pick_move(pl, false), 0, pl->tuning.ctas_per_sm, (int32_t)n_rot, n_ins, layer_ptrs, layer_ptrs,
-                   layer_repl, stream, &slot);
+    if (pl->use_bulk)
+        st = run_tiles_bulk(pl, false, (int32_t)n_rot, n_ins, layer_ptrs, layer_ptrs, layer_repl, stream, &slot);
+    else
+        st = run_tiles(pl, pick_move(pl, false), 0, pl->tuning.ctas_per_sm, (int32_t)n_rot, n_ins, layer_ptrs, layer_ptrs,
+                       layer_repl, stream, &slot);
     if (st != LEYLINE_OK) return st;
     if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_stop), stream));
     return LEYLINE_OK;

@@ -37,7 +37,8 @@ class DeviceCache:
     def desc(self):
         w = self.w
         return B.make_desc(self.n_layers, w.latent_dim, w.rope_dim, w.page_size, w.dtype, w.pairing, w.row_bytes,
-                           w.n_slots, w.inv_freq, self.scales if w.dtype == synth.DT_FP8 else None)
+                           w.n_slots, w.inv_freq, self.scales if w.dtype == synth.DT_FP8 else None,
+                           rope_heads=w.rope_heads)
 
     def nbytes(self):
         return sum(p.numel() for p in self.pools) + sum(r.numel() for r in self.repl)

@@ -63,7 +63,8 @@ class Workload:
     dtype: int = DT_BF16
     pairing: int = NEOX
     latent_dim: int = 512
-    rope_dim: int = 64
+    rope_dim: int = 64                  # rotated elements per head
+    rope_heads: int = 1                 # heads in the rotated band (1 = MLA K_pe; kv_heads = full-width K)
     inv_freq: np.ndarray = None         # fp32 [rope_dim/2]
     # (request, start, end, repl_len, repl_row, semantic), sorted by (request, start)
     directives: list = field(default_factory=list)
@@ -83,7 +84,11 @@ class Workload:
 
     @property
     def row_bytes(self):
-        return (self.latent_dim + self.rope_dim) * self.elem_bytes
+        return self.row_elems * self.elem_bytes
+
+    @property
+    def row_elems(self):
+        return self.latent_dim + self.rope_heads * self.rope_dim
 
     @property
     def n_slots(self):
@@ -193,6 +198,26 @@ def config(n: int, **over) -> Workload:
                      (r, 3 * L // 4, 3 * L // 4 + 512, 256, 0, AMORTIZE)]
         w = Workload("cfg5_fp8_8x64K_61L", 61, [L] * n_req, 64, dtype=DT_FP8,
                      inv_freq=yarn_inv_freq(64, 10000.0, 40.0, 4096), directives=dirs, seed=5)
+    elif n == "gqa":
+        # full-width K rotation.  K pool of a Llama-3.1-8B-style GQA model:
+        # 32 layers, 8 kv heads x head_dim 128 (2048-B bf16 rows, all of it rotated), rope_theta 5e5 (Table 8 row 3,
+        # PAPER.md:537), NeoX pairing, one request of 128K tokens, config 3's three directives.  V is position-free
+        # and would be spliced as a latent-only pool with the same plan; it is not part of this workload.
+        L = 131072
+        w = Workload("gqa_llama31_32L_128K_8x128", 32, [L], 64, latent_dim=0, rope_dim=128, rope_heads=8,
+                     inv_freq=rope_inv_freq(128, 5.0e5),
+                     directives=[(0, L // 16, L // 16 + 2048, 64, 0, AMORTIZE),
+                                 (0, L // 4, L // 4 + 16384, 0, 0, AMORTIZE),
+                                 (0, 3 * L // 4, 3 * L // 4 + 512, 256, 0, AMORTIZE)], seed=6)
+    elif n == "mha96":
+        # Phi-3-style MHA K pool: 32 heads x head_dim 96 (12 chunks per head: not a power of two), theta 1e4
+        # (Table 8 row 5), 32 layers x 32K tokens, misaligned replacements
+        L = 32768
+        w = Workload("mha_phi3_32L_32K_32x96", 32, [L], 64, latent_dim=0, rope_dim=96, rope_heads=32,
+                     inv_freq=rope_inv_freq(96, 1.0e4),
+                     directives=[(0, L // 16, L // 16 + 2048, 67, 0, AMORTIZE),
+                                 (0, L // 4, L // 4 + 4096, 3, 0, AMORTIZE),
+                                 (0, 3 * L // 4, 3 * L // 4 + 512, 251, 0, AMORTIZE)], seed=7)
     else:
         raise ValueError(n)
     for k, v in over.items():
@@ -219,7 +244,7 @@ def fill_layer_(buf, w: Workload, layer: int, seed_base: int | None = None):
     seed = (w.seed if seed_base is None else seed_base) * 1000003 + layer
     g = torch.Generator(device=buf.device)
     g.manual_seed(seed)
-    n_elem = w.n_slots * (w.latent_dim + w.rope_dim)
+    n_elem = w.n_slots * w.row_elems
     if w.dtype == DT_BF16:
         view = buf.view(torch.bfloat16)
         assert view.numel() == n_elem
@@ -240,7 +265,7 @@ def fill_repl_(buf, w: Workload, layer: int, scale: float = 1.0):
         return
     g = torch.Generator(device=buf.device)
     g.manual_seed(1 * 1000003 + 7 * layer + 1 + w.seed * 31)
-    n_elem = w.n_repl_rows * (w.latent_dim + w.rope_dim)
+    n_elem = w.n_repl_rows * w.row_elems
     if w.dtype == DT_BF16:
         buf.view(torch.bfloat16).normal_(0.0, 1.0, generator=g)
         return

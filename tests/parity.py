@@ -80,7 +80,8 @@ def compare_layer(w: synth.Workload, bm: O.BatchMap, mode: int, old_pool: np.nda
     """One layer, whole pool.  old_pool / gpu_pool / repl: flat uint8.  Asserts the bar and returns statistics."""
     stride = w.row_bytes
     E = w.elem_bytes
-    want = O.splice_layer(w.dtype, w.pairing, w.latent_dim, w.rope_dim, stride, w.inv_freq, scale, old_pool, repl, bm)
+    want = O.splice_layer(w.dtype, w.pairing, w.latent_dim, w.rope_dim, stride, w.inv_freq, scale, old_pool, repl, bm,
+                          n_heads=w.rope_heads)
     g = gpu_pool.reshape(-1, stride)
     o = want.reshape(-1, stride)
     new_s, old_s = rotated_rows(w, bm, mode)
@@ -104,14 +105,15 @@ def compare_layer(w: synth.Workload, bm: O.BatchMap, mode: int, old_pool: np.nda
         if bad.any():
             # cancellation floor: |g - o| <= 2^-20 * rho, rho = norm of the INPUT pair
             ib = np.ascontiguousarray(old_pool.reshape(-1, stride)[old_s, band0:]).view(np.uint16)
-            x = _bf16_val(ib)
+            x = _bf16_val(ib).reshape(len(old_s), w.rope_heads, w.rope_dim)      # pairs live inside a head
             H = w.rope_dim // 2
             if w.pairing == synth.NEOX:
-                rho_h = np.sqrt(x[:, :H] ** 2 + x[:, H:] ** 2)
-                rho = np.concatenate([rho_h, rho_h], axis=1)
+                rho_h = np.sqrt(x[..., :H] ** 2 + x[..., H:] ** 2)
+                rho = np.concatenate([rho_h, rho_h], axis=-1)
             else:
-                rho_h = np.sqrt(x[:, 0::2] ** 2 + x[:, 1::2] ** 2)
-                rho = np.repeat(rho_h, 2, axis=1)
+                rho_h = np.sqrt(x[..., 0::2] ** 2 + x[..., 1::2] ** 2)
+                rho = np.repeat(rho_h, 2, axis=-1)
+            rho = rho.reshape(len(old_s), -1)
             err = np.abs(_bf16_val(gbits) - _bf16_val(obits))
             floor_ok = err <= (2.0 ** -20) * rho
             n_floor = int((bad & floor_ok).sum())

@@ -164,3 +164,41 @@ def test_config4_batched_fresh_reduced_layers():
 @pytest.mark.parametrize("mode", [O.FRESH, O.INPLACE_MOVE, O.ROTATE_ONLY])
 def test_config5_fp8_full_size(mode):
     run_and_compare(synth.config(5, pool_factor=2.2), mode, check_layers=[0, 60])
+
+
+# ----------------------------------------------------------------------------- full-width K
+
+def heads_workload(name, heads, d, latent, dtype, pairing, theta, page=16, layers=2):
+    return synth.Workload(name, layers, [2100, 900, 64], page, dtype=dtype, pairing=pairing, latent_dim=latent, rope_dim=d,
+                          rope_heads=heads, inv_freq=synth.rope_inv_freq(d, theta),
+                          directives=[(0, 7, 40, 300, 0, 0), (0, 900, 1700, 5, 0, 0), (1, 100, 101, 77, 0, 0),
+                                      (2, 0, 64, 1, 0, 0)],
+                          seed=31, pool_factor=3.0, extra_pages=60).finalize()
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("pairing", [synth.NEOX, synth.INTERLEAVED])
+@pytest.mark.parametrize("heads,d,latent,dtype,theta", [
+    (8, 128, 0, synth.DT_BF16, 5.0e5),      # GQA, Llama-3.1-style (Table 8 row 3)
+    (8, 128, 0, synth.DT_FP8, 1.0e6),       # GQA, Qwen-3-style, fp8 storage
+    (4, 96, 0, synth.DT_BF16, 1.0e4),       # Phi-3-style head_dim 96: 12 chunks per head
+    (3, 96, 64, synth.DT_BF16, 1.0e4),      # odd head count behind a position-free prefix (K and V sharing a row)
+    (2, 64, 512, synth.DT_BF16, 1.0e4),     # two rotated heads behind an MLA-sized latent
+    (1, 32, 16, synth.DT_FP8, 1.0e4),       # smallest band the kernels take: one head of two chunks
+])
+def test_full_width_heads(mode, pairing, heads, d, latent, dtype, theta):
+    run_and_compare(heads_workload("heads", heads, d, latent, dtype, pairing, theta), mode)
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("page", [1, 4])
+def test_full_width_small_pages(mode, page):
+    """Token-level slots / tiny pages: the bulk mover degenerates to one copy per row, inserts of ROTATE_ONLY too."""
+    run_and_compare(heads_workload("heads_p", 8, 128, 0, synth.DT_BF16, synth.NEOX, 5.0e5, page=page), mode)
+
+
+@pytest.mark.parametrize("cfg", ["gqa", "mha96"])
+@pytest.mark.parametrize("mode", MODES)
+def test_full_width_full_size(cfg, mode):
+    w = synth.config(cfg, pool_factor=2.0)
+    run_and_compare(w, mode, check_layers=[0, w.n_layers - 1])

@@ -57,7 +57,7 @@ def tiny_workload(rng, P=None, n_req=None, forget=False, dtype=synth.DT_BF16):
 
 def make_plan(w, mode, n_layers=None):
     d, keep = B.make_desc(n_layers or w.n_layers, w.latent_dim, w.rope_dim, w.page_size, w.dtype, w.pairing,
-                          w.row_bytes, w.n_slots, w.inv_freq)
+                          w.row_bytes, w.n_slots, w.inv_freq, rope_heads=w.rope_heads)
     free = w.free_slots() if mode == B.ROTATE_ONLY else w.free_pages
     return B.leyline_plan(d, mode, w.seq_lens, w.pt_offsets, w.pages, w.directives, free)
 
@@ -84,7 +84,7 @@ def test_plan_matches_oracle_on_baseline_configs(mode, cfg):
         assert_plan_equal(plan, bm, mode)
         check_tiles_cover(plan, bm, w, mode)
         i = plan.info
-        E, W = w.elem_bytes, w.latent_dim + w.rope_dim
+        E, W = w.elem_bytes, w.row_elems
         if mode != B.ROTATE_ONLY:
             assert i.bytes_read == i.bytes_written == (i.rows_moved + i.rows_inserted) * W * E * w.n_layers
         if cfg == 3 and mode == B.FRESH:   # (103,936 + 320) x 61 rows, 14.65 GB read + written
@@ -103,8 +103,12 @@ def check_tiles_cover(plan, bm, w, mode):
     n_move = plan.info.n_move_tiles
     seen = {}
     for t_i, t in enumerate(tiles):
-        assert 1 <= t.n_rows <= plan.info.tile_rows <= 64
         is_repl = bool(t.flags & B.TILE_SRC_REPL)
+        if mode == B.ROTATE_ONLY and not is_repl:     # a5 work items: <= 1024 (row, pair column) units per block
+            assert 1 <= t.n_rows <= plan.info.rot_tile_rows
+            assert plan.info.rot_tile_rows * w.rope_heads * (w.rope_dim * w.elem_bytes // 32) <= 1024 or plan.info.rot_tile_rows == 1
+        else:
+            assert 1 <= t.n_rows <= plan.info.tile_rows <= 64
         assert is_repl == (t_i >= n_move)
         for q in range(t.n_rows):
             key = (t.request, "r" if is_repl else "o", t.src_pos + q)
@@ -265,3 +269,46 @@ def test_inplace_tiles_are_a_correct_schedule(seed):
             for tpos, (kind, i) in enumerate(want):
                 got = pool[int(row[tpos // P]) * P + tpos % P]
                 assert got == (r * 10 ** 6 + i if kind == "o" else -(r * 10 ** 6 + i) - 2), (r, tpos, kind, i, got)
+
+
+def test_heads_descriptor_rules():
+    """rope_heads: 0 reads as 1; row = latent + heads * rope_dim; a head must be an even number of 16-byte chunks;
+    the row kernel (tuning.kernel = 1) only takes one head of 2^k chunks."""
+    w = synth.Workload("h", 1, [100], 16, latent_dim=0, rope_dim=128, rope_heads=8, inv_freq=synth.rope_inv_freq(128, 5e5),
+                       directives=[(0, 10, 20, 3, 0, 0)], seed=1, pool_factor=3.0, extra_pages=4).finalize()
+    for mode in MODES:
+        bm = oracle_plan(w, mode)
+        with make_plan(w, mode) as plan:
+            assert_plan_equal(plan, bm, mode)
+            i = plan.info
+            assert i.mover == 2                                   # several heads: the bulk mover
+            row = 8 * 128 * 2
+            if mode == B.ROTATE_ONLY:
+                assert i.bytes_read == (i.rows_rotated * row + i.rows_inserted * row) * w.n_layers
+                assert i.rot_tile_rows == 1024 // (8 * 8)
+            else:
+                assert i.bytes_read == (i.rows_moved + i.rows_inserted) * row * w.n_layers
+    inv = synth.rope_inv_freq(128, 5e5)
+    # stride must cover all heads
+    d, k = B.make_desc(1, 0, 128, 16, 0, 0, 128 * 2, w.n_slots, inv, rope_heads=8)
+    with pytest.raises(B.LeylineError) as e:
+        B.leyline_plan(d, B.FRESH, w.seq_lens, w.pt_offsets, w.pages, w.directives, w.free_pages)
+    assert e.value.status == 1
+    # a head of one 16-byte chunk (8 bf16 elements) cannot be split into two half-chunks
+    d, k = B.make_desc(1, 0, 8, 16, 0, 1, 16, w.n_slots, synth.rope_inv_freq(8), rope_heads=1)
+    with pytest.raises(B.LeylineError) as e:
+        B.leyline_plan(d, B.FRESH, w.seq_lens, w.pt_offsets, w.pages, w.directives, w.free_pages)
+    assert e.value.status == 6
+    # forced row kernel on a multi-head band
+    B.leyline_set_tuning(kernel=1)
+    try:
+        d, k = B.make_desc(1, 0, 128, 16, 0, 0, 2048, w.n_slots, inv, rope_heads=8)
+        with pytest.raises(B.LeylineError) as e:
+            B.leyline_plan(d, B.FRESH, w.seq_lens, w.pt_offsets, w.pages, w.directives, w.free_pages)
+        assert e.value.status == 6
+    finally:
+        B.leyline_set_tuning()
+    # rope_heads = 0 is the MLA default
+    d, k = B.make_desc(1, 512, 64, 16, 0, 0, 1152, w.n_slots, synth.rope_inv_freq(64), rope_heads=0)
+    with B.leyline_plan(d, B.FRESH, w.seq_lens, w.pt_offsets, w.pages, w.directives, w.free_pages) as plan:
+        assert plan.info.bytes_read == (plan.info.rows_moved + plan.info.rows_inserted) * 1152
