@@ -133,52 +133,53 @@ __global__ void __launch_bounds__(kThreads, DT == LEYLINE_FP8_E4M3 ? 2 : 3) k_ro
     const int half = p.head_chunks >> 1;   /* pair columns per head */
     const int cols = p.n_heads * half;     /* pair columns per row */
     const int64_t band0 = (int64_t)p.lat_chunks * 16;
-    const int rows_per_pass = FIXED ? kThreads / cols : 0;
-    int col_f = 0, r_f = 0, q_f = 0, chunk_f = 0;
-    if (FIXED) {
-        r_f = tid / cols;
-        col_f = tid - r_f * cols;
-        const int head = col_f / half;
-        q_f = col_f - head * half;
-        chunk_f = head * p.head_chunks + q_f;
+    /* what a thread's unit k is does not depend on the item: row-in-tile, 16-byte chunk of the band, pair column */
+    int rk[kRotUnroll], chunk[kRotUnroll], qs[kRotUnroll];
+#pragma unroll
+    for (int k = 0; k < kRotUnroll; ++k) {
+        const int u = FIXED ? tid : tid + k * kThreads;
+        const int r = u / cols, col = u - r * cols;
+        const int head = col / half;
+        qs[k] = col - head * half;
+        chunk[k] = head * p.head_chunks + qs[k];
+        rk[k] = FIXED ? r + k * (kThreads / cols) : r;
     }
-    for (long long item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+    /* The rows of an item are found through tile -> page table -> slot, two dependent look-ups before the first
+     * byte of data can be requested.  The loop is software-pipelined: the NEXT item's slots are resolved while the
+     * current item's band loads are in flight, so that chain never leaves the memory system idle. */
+    struct Item { int32_t slot[kRotUnroll]; int32_t layer, trig; };
+    auto resolve = [&](long long item, Item& it) {
         const int tile_i = p.tile_begin + (int)(item / p.n_layers);
-        const int layer = (int)(item % p.n_layers);
+        it.layer = (int)(item % p.n_layers);
         const DevTile t = p.tiles[tile_i];
-        uint8_t* __restrict__ base = p.dst[layer];
-        const float* __restrict__ trig_row = p.trig + (int64_t)t.trig * 2 * p.H;
-        const int total = t.n_rows * cols;
+        it.trig = t.trig;
+#pragma unroll
+        for (int k = 0; k < kRotUnroll; ++k)
+            it.slot[k] = rk[k] < t.n_rows ? (int32_t)slot_of(p.tabs, t.src_tab, t.src_pos + rk[k], p.page_shift) : -1;
+    };
+    long long item = blockIdx.x;
+    if (item >= p.n_items) return;
+    Item cur, nxt;
+    resolve(item, cur);
+    for (;;) {
+        uint8_t* __restrict__ base = p.dst[cur.layer];
         int4 lo[kRotUnroll], hi[kRotUnroll];
         uint8_t* addr[kRotUnroll];
-        int qs[kRotUnroll];
 #pragma unroll
         for (int k = 0; k < kRotUnroll; ++k) {
-            int r, chunk;
-            bool active;
-            if (FIXED) {
-                r = r_f + k * rows_per_pass;
-                chunk = chunk_f;
-                qs[k] = q_f;
-                active = r < t.n_rows;
-            } else {
-                const int u = tid + k * kThreads;
-                r = u / cols;
-                const int col = u - r * cols;
-                const int head = col / half;
-                qs[k] = col - head * half;
-                chunk = head * p.head_chunks + qs[k];
-                active = u < total;
-            }
             addr[k] = nullptr;
-            if (active) {
-                addr[k] = base + slot_of(p.tabs, t.src_tab, t.src_pos + r, p.page_shift) * p.stride + band0 + (int64_t)chunk * 16;
+            if (cur.slot[k] >= 0) {
+                addr[k] = base + (int64_t)cur.slot[k] * p.stride + band0 + (int64_t)chunk[k] * 16;
                 lo[k] = ld_coherent(addr[k]);
                 hi[k] = ld_coherent(addr[k] + half * 16);
             }
         }
+        const long long next = item + gridDim.x;
+        const bool more = next < p.n_items;
+        if (more) resolve(next, nxt);
+        const float* __restrict__ trig_row = p.trig + (int64_t)cur.trig * 2 * p.H;
         float c[N], s[N];
-        if (FIXED) load_pair_trig<DT, PAIRING>(trig_row, p.H, q_f, half, c, s);
+        if (FIXED) load_pair_trig<DT, PAIRING>(trig_row, p.H, qs[0], half, c, s);
 #pragma unroll
         for (int k = 0; k < kRotUnroll; ++k) {
             if (addr[k]) {
@@ -188,6 +189,9 @@ __global__ void __launch_bounds__(kThreads, DT == LEYLINE_FP8_E4M3 ? 2 : 3) k_ro
                 st_stream(addr[k] + half * 16, hi[k]);
             }
         }
+        if (!more) break;
+        cur = nxt;
+        item = next;
     }
 }
 
