@@ -157,9 +157,9 @@ def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1):
     pt = torch.empty(max(int(info.total_new_pages), 1), dtype=torch.int32, device=dev)
     idx = torch.empty(max(int(info.total_new_tokens), 1), dtype=torch.int32, device=dev)
     nbytes = int(info.bytes_read + info.bytes_written)
-    launches = 2 + (2 if mode != B.FRESH else 1)      # index x2 (page table, slot list; 1 for rotate-only) + movers
-    if mode == B.ROTATE_ONLY:
-        launches = 1 + 2
+    # k_index (page table + slot list, one launch) + the movers: FRESH one k_move_bulk; INPLACE_MOVE moves then
+    # inserts; ROTATE_ONLY k_rotate_band then the insert tiles
+    launches = 1 + (1 if mode == B.FRESH else 2)
     plan0.close()
     plans, host_us = [], []
 
@@ -197,9 +197,11 @@ def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1):
             "mover": int(info.mover), "tile_rows": int(info.tile_rows)}
 
 
-def cpu_baseline(pools, repls, scales, w, mode: int, bytes_per_layer: int, budget_s: float = 12.0, max_layers: int = 8):
+def cpu_baseline(pools, repls, scales, w, mode: int, bytes_per_layer: int, budget_s: float = 15.0, max_layers: int = 1 << 30):
     """The oracle as it stands (one thread, explicit per-token loops, fp64 libm trig) on whole layers of the same
-    workload, on this host.  `pools` / `repls`: callables returning a layer's bytes as a flat uint8 numpy array."""
+    workload, on this host, until about `budget_s` seconds of oracle time are spent (a bounded sample: whole layers,
+    which are independent given the plan).  `pools` / `repls`: callables returning a layer's bytes as a flat uint8
+    numpy array."""
     import oracle as O
     free = w.free_slots() if mode == O.ROTATE_ONLY else w.free_pages
     t0 = time.perf_counter()

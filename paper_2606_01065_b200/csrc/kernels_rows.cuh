@@ -18,9 +18,10 @@ namespace leyline {
 
 /* ------------------------------------------------------------------ a2 ---- */
 
-__global__ void __launch_bounds__(kThreads) k_index(const IndexParams p) {
-    for (long long o = blockIdx.x * (long long)blockDim.x + threadIdx.x; o < p.total;
-         o += (long long)gridDim.x * blockDim.x) {
+/* One launch writes both outputs: blocks [0, blocks_a) produce `a` (page-table rows), the rest `b` (token-level slot
+ * list); either may be empty (total = 0). */
+__device__ __forceinline__ void index_body(const IndexParams& p, long long block, long long n_blocks) {
+    for (long long o = block * blockDim.x + threadIdx.x; o < p.total; o += n_blocks * blockDim.x) {
         int lo = 0, hi = p.n_runs - 1; /* last run with out_begin <= o */
         while (lo < hi) {
             const int mid = (lo + hi + 1) >> 1;
@@ -34,6 +35,11 @@ __global__ void __launch_bounds__(kThreads) k_index(const IndexParams p) {
         else v = __ldg(p.tabs + r.pos0 + q);
         p.out[o] = v;
     }
+}
+
+__global__ void __launch_bounds__(kThreads) k_index(const IndexParams a, const IndexParams b, const int blocks_a) {
+    if ((int)blockIdx.x < blocks_a) index_body(a, blockIdx.x, blocks_a);
+    else index_body(b, blockIdx.x - blocks_a, gridDim.x - blocks_a);
 }
 
 /* ------------------------------------------------------------------ a3 + a4 ---- */

@@ -79,7 +79,7 @@ struct leyline_plan_s {
     /* device side (owned by splice.cu; created on first launch, freed by leyline_plan_destroy) */
     void* d_blob = nullptr;             /* tiles | trig | tabs | slot_runs | page_runs */
     int64_t off_tiles = 0, off_trig = 0, off_tabs = 0, off_slot_runs = 0, off_page_runs = 0, blob_bytes = 0;
-    void* d_scratch = nullptr;          /* [0,256): ticket counters; then hazard flags [n_move_tiles * n_layers] int32 */
+    void* d_scratch = nullptr;          /* tail of d_blob: [0,256) ticket counters; then hazard flags [n_move_tiles * n_layers] int32 */
     int64_t scratch_bytes = 0;
     int device = -1;
     void* ev_start = nullptr;           /* cudaEvent_t pair around the data-moving kernels (tuning.profile) */

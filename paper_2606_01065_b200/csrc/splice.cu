@@ -5,7 +5,9 @@
  */
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
+#include <vector>
 
 #include "kernels_bulk.cuh"
 #include "kernels_rows.cuh"
@@ -29,6 +31,50 @@ inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 struct DeviceInfo { int device = -1; int sms = 0; int smem_optin = 0; };
 DeviceInfo g_dev;
 
+/* ---- pinned staging for the plan upload ----
+ * A pageable source makes the runtime stage the tables itself (an extra host copy, and a DMA that cannot start
+ * before it); at 48 B per 32-row tile that upload is the largest fixed cost of a call.  Buffers are recycled: each
+ * goes back to the pool right after its copy is enqueued, guarded by an event the next user checks. */
+struct PinnedBuf { void* p = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; int device = -1; };
+std::mutex g_pin_mu;
+std::vector<PinnedBuf> g_pin_pool;
+constexpr size_t kPinMinBytes = 256 << 10, kPinMaxPooled = 32;
+
+PinnedBuf pin_acquire(size_t bytes, int dev) {
+    {
+        std::lock_guard<std::mutex> lk(g_pin_mu);
+        for (size_t i = 0; i < g_pin_pool.size(); ++i) {
+            PinnedBuf b = g_pin_pool[i];
+            if (b.cap >= bytes && b.device == dev && cudaEventQuery(b.ev) == cudaSuccess) {
+                g_pin_pool.erase(g_pin_pool.begin() + (long)i);
+                return b;
+            }
+        }
+        (void)cudaGetLastError(); /* cudaErrorNotReady from a busy buffer is not an error */
+    }
+    PinnedBuf b;
+    size_t cap = kPinMinBytes;
+    while (cap < bytes) cap <<= 1;
+    if (cudaHostAlloc(&b.p, cap, cudaHostAllocDefault) != cudaSuccess ||
+        cudaEventCreateWithFlags(&b.ev, cudaEventDisableTiming) != cudaSuccess) {
+        (void)cudaGetLastError();
+        if (b.p) cudaFreeHost(b.p);
+        return PinnedBuf{}; /* caller falls back to a pageable source */
+    }
+    b.cap = cap;
+    b.device = dev;
+    return b;
+}
+
+void pin_release(PinnedBuf b, cudaStream_t stream) {
+    cudaEventRecord(b.ev, stream);
+    std::lock_guard<std::mutex> lk(g_pin_mu);
+    if (g_pin_pool.size() < kPinMaxPooled) { g_pin_pool.push_back(b); return; }
+    cudaEventSynchronize(b.ev);
+    cudaEventDestroy(b.ev);
+    cudaFreeHost(b.p);
+}
+
 leyline_status ensure_device(leyline_plan_s* pl, cudaStream_t stream) {
     int dev = 0;
     CU(cudaGetDevice(&dev));
@@ -43,7 +89,7 @@ leyline_status ensure_device(leyline_plan_s* pl, cudaStream_t stream) {
         if (pl->device != dev) { g_last_error = "plan was uploaded on another device"; return LEYLINE_E_CUDA; }
         return LEYLINE_OK;
     }
-    /* one blob: tiles | trig | tabs | slot_runs | page_runs, each 256-byte aligned */
+    /* one allocation: tiles | trig | tabs | slot_runs | page_runs | scratch, each 256-byte aligned */
     int64_t off = 0;
     auto place = [&](int64_t bytes) { int64_t o = off; off = align_up(off + bytes, 256); return o; };
     pl->off_tiles = place((int64_t)pl->tiles.size() * sizeof(DevTile));
@@ -52,23 +98,29 @@ leyline_status ensure_device(leyline_plan_s* pl, cudaStream_t stream) {
     pl->off_slot_runs = place((int64_t)pl->slot_runs.size() * sizeof(IdxRun));
     pl->off_page_runs = place((int64_t)pl->page_runs.size() * sizeof(IdxRun));
     pl->blob_bytes = off > 0 ? off : 256;
-    std::string host((size_t)pl->blob_bytes, '\0');
-    auto put = [&](int64_t o, const void* src, size_t bytes) { if (bytes) std::memcpy(&host[(size_t)o], src, bytes); };
+    const int64_t n_flags = pl->mode == LEYLINE_INPLACE_MOVE ? pl->info.n_move_tiles * pl->desc.n_layers : 0;
+    pl->scratch_bytes = 256 + align_up(n_flags * (int64_t)sizeof(int32_t), 256);
+    PinnedBuf pin = pin_acquire((size_t)pl->blob_bytes, dev);
+    std::string pageable;
+    if (!pin.p) pageable.resize((size_t)pl->blob_bytes);
+    uint8_t* host = pin.p ? static_cast<uint8_t*>(pin.p) : reinterpret_cast<uint8_t*>(&pageable[0]);
+    auto put = [&](int64_t o, const void* src, size_t bytes) { if (bytes) std::memcpy(host + o, src, bytes); };
     put(pl->off_tiles, pl->tiles.data(), pl->tiles.size() * sizeof(DevTile));
     put(pl->off_trig, pl->trig.data(), pl->trig.size() * sizeof(float));
     put(pl->off_tabs, pl->tabs.data(), pl->tabs.size() * sizeof(int32_t));
     put(pl->off_slot_runs, pl->slot_runs.data(), pl->slot_runs.size() * sizeof(IdxRun));
     put(pl->off_page_runs, pl->page_runs.data(), pl->page_runs.size() * sizeof(IdxRun));
-    const int64_t n_flags = pl->mode == LEYLINE_INPLACE_MOVE ? pl->info.n_move_tiles * pl->desc.n_layers : 0;
-    pl->scratch_bytes = 256 + align_up(n_flags * (int64_t)sizeof(int32_t), 256);
-    CU(cudaMallocAsync(&pl->d_blob, (size_t)pl->blob_bytes, stream));
-    if (!cuda_ok(cudaMallocAsync(&pl->d_scratch, (size_t)pl->scratch_bytes, stream), "cudaMallocAsync(scratch)")) {
-        cudaFreeAsync(pl->d_blob, stream);
+    if (!cuda_ok(cudaMallocAsync(&pl->d_blob, (size_t)(pl->blob_bytes + pl->scratch_bytes), stream), "cudaMallocAsync(plan tables)")) {
+        if (pin.p) pin_release(pin, stream);
         pl->d_blob = nullptr;
         return LEYLINE_E_CUDA;
     }
-    /* pageable source: the runtime stages it before returning, so `host` may go out of scope */
-    CU(cudaMemcpyAsync(pl->d_blob, host.data(), (size_t)pl->blob_bytes, cudaMemcpyHostToDevice, stream));
+    pl->d_scratch = static_cast<uint8_t*>(pl->d_blob) + pl->blob_bytes;
+    /* pinned source: a plain stream-ordered DMA; pageable fallback: the runtime stages it before returning */
+    const bool ok = cuda_ok(cudaMemcpyAsync(pl->d_blob, host, (size_t)pl->blob_bytes, cudaMemcpyHostToDevice, stream),
+                            "cudaMemcpyAsync(plan tables)");
+    if (pin.p) pin_release(pin, stream);
+    if (!ok) return LEYLINE_E_CUDA;
     pl->device = dev;
     return LEYLINE_OK;
 }
@@ -78,20 +130,30 @@ const T* blob_at(const leyline_plan_s* pl, int64_t off) {
     return reinterpret_cast<const T*>(static_cast<const uint8_t*>(pl->d_blob) + off);
 }
 
-leyline_status launch_index(const leyline_plan_s* pl, const std::vector<IdxRun>& runs, int64_t off, int32_t* out,
-                            cudaStream_t stream) {
-    if (!out || runs.empty()) return LEYLINE_OK;
+IndexParams index_params(const leyline_plan_s* pl, const std::vector<IdxRun>& runs, int64_t off, int32_t* out) {
     IndexParams ip;
+    std::memset(&ip, 0, sizeof(ip));
+    if (!out || runs.empty()) return ip;
     ip.runs = blob_at<IdxRun>(pl, off);
     ip.tabs = blob_at<int32_t>(pl, pl->off_tabs);
     ip.out = out;
     ip.total = runs.back().out_begin + runs.back().length;
     ip.n_runs = (int32_t)runs.size();
     ip.page_shift = pl->page_shift;
-    if (ip.total <= 0) return LEYLINE_OK;
-    long long blocks = (ip.total + kThreads - 1) / kThreads;
-    if (blocks > 8LL * g_dev.sms) blocks = 8LL * g_dev.sms;
-    k_index<<<(unsigned)blocks, kThreads, 0, stream>>>(ip);
+    return ip;
+}
+
+/* a2: page-table rows and token-level slot list in ONE launch (either output may be NULL). */
+leyline_status launch_index(const leyline_plan_s* pl, int32_t* page_table_out, int32_t* slot_idx_out, cudaStream_t stream) {
+    const IndexParams a = index_params(pl, pl->page_runs, pl->off_page_runs, page_table_out);
+    const IndexParams b = index_params(pl, pl->slot_runs, pl->off_slot_runs, slot_idx_out);
+    auto blocks_of = [](const IndexParams& ip) {
+        long long n = (ip.total + kThreads - 1) / kThreads;
+        return n > 4LL * g_dev.sms ? 4LL * g_dev.sms : n;
+    };
+    const long long na = blocks_of(a), nb = blocks_of(b);
+    if (na + nb == 0) return LEYLINE_OK;
+    k_index<<<(unsigned)(na + nb), kThreads, 0, stream>>>(a, b, (int)na);
     CU(cudaGetLastError());
     return LEYLINE_OK;
 }
@@ -315,9 +377,7 @@ extern "C" leyline_status leyline_splice(leyline_plan_t* pl, void* const* layer_
     leyline_status st = begin_call(pl, stream);
     if (st != LEYLINE_OK) return st;
     /* a2: page-table rows and token-level slot list */
-    st = launch_index(pl, pl->page_runs, pl->off_page_runs, dev_page_table_out, stream);
-    if (st != LEYLINE_OK) return st;
-    st = launch_index(pl, pl->slot_runs, pl->off_slot_runs, dev_slot_idx_out, stream);
+    st = launch_index(pl, dev_page_table_out, dev_slot_idx_out, stream);
     if (st != LEYLINE_OK) return st;
     if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_start), stream));
     int slot = 0;
@@ -361,7 +421,7 @@ extern "C" leyline_status leyline_rotate_inplace(leyline_plan_t* pl, void* const
     }
     leyline_status st = begin_call(pl, stream);
     if (st != LEYLINE_OK) return st;
-    st = launch_index(pl, pl->slot_runs, pl->off_slot_runs, dev_slot_idx_out, stream);
+    st = launch_index(pl, nullptr, dev_slot_idx_out, stream);
     if (st != LEYLINE_OK) return st;
     if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_start), stream));
     int slot = 0;
@@ -389,8 +449,7 @@ extern "C" void leyline_plan_release_device_(leyline_plan_s* pl) {
     if (pl->ev_start) cudaEventDestroy(static_cast<cudaEvent_t>(pl->ev_start));
     if (pl->ev_stop) cudaEventDestroy(static_cast<cudaEvent_t>(pl->ev_stop));
     /* stream-ordered: freed after everything this plan launched on its stream, without a device sync */
-    if (pl->d_blob) cudaFreeAsync(pl->d_blob, static_cast<cudaStream_t>(pl->last_stream));
-    if (pl->d_scratch) cudaFreeAsync(pl->d_scratch, static_cast<cudaStream_t>(pl->last_stream));
+    if (pl->d_blob) cudaFreeAsync(pl->d_blob, static_cast<cudaStream_t>(pl->last_stream)); /* tables + scratch */
     pl->d_blob = pl->d_scratch = nullptr;
     pl->ev_start = pl->ev_stop = nullptr;
     if (pl->device >= 0) (void)cudaGetLastError();
