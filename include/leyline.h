@@ -226,6 +226,17 @@ leyline_status leyline_splice(leyline_plan_t* plan, void* const* layer_src, void
 leyline_status leyline_rotate_inplace(leyline_plan_t* plan, void* const* layer_ptrs, const void* const* layer_repl,
                                       int32_t* dev_slot_idx_out, void* cuda_stream);
 
+/*
+ * leyline_plan_prefetch -- OPTIONAL: start uploading the plan's device tables (tiles, cos/sin table, page tables,
+ * index runs; SURVEY.md section 3(3) "one small H2D copy") on a library-owned copy stream of the CURRENT device and
+ * return at once.  The first leyline_splice / leyline_rotate_inplace of the plan then only waits for that copy's
+ * event on its own stream instead of issuing the copy there, so the upload overlaps whatever the device is still
+ * running (the scheduler plans turn n+1 while turn n executes).  Without this call the tables are uploaded by the
+ * first launch, in order on its stream.  Idempotent; a no-op once the tables are on the device.
+ * Returns LEYLINE_E_CUDA without a device (the plan itself stays valid and usable for queries).
+ */
+leyline_status leyline_plan_prefetch(leyline_plan_t* plan);
+
 void leyline_plan_destroy(leyline_plan_t* plan);
 const char* leyline_strerror(leyline_status s);
 /* Text of the last CUDA error seen by this thread's calls into the library ("" if none). */

@@ -86,6 +86,8 @@ def _load() -> C.CDLL:
     L.leyline_rotate_inplace.argtypes = [vp, vp, vp, vp, vp]
     L.leyline_plan_kernel_ms.restype = C.c_int
     L.leyline_plan_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    L.leyline_plan_prefetch.restype = C.c_int
+    L.leyline_plan_prefetch.argtypes = [vp]
     L.leyline_plan_destroy.restype = None
     L.leyline_plan_destroy.argtypes = [vp]
     L.leyline_strerror.restype = C.c_char_p
@@ -191,6 +193,11 @@ class Plan:
         _check(_lib.leyline_plan_tiles(self._h, C.cast(buf, C.c_void_p)), "leyline_plan_tiles")
         return list(buf)
 
+    def prefetch(self):
+        """leyline.h: leyline_plan_prefetch -- start the table upload on the library's copy stream."""
+        _check(_lib.leyline_plan_prefetch(self._h), "leyline_plan_prefetch")
+        return self
+
     def kernel_ms(self) -> float:
         ms = C.c_float()
         _check(_lib.leyline_plan_kernel_ms(self._h, C.byref(ms)), "leyline_plan_kernel_ms")
@@ -234,15 +241,29 @@ def leyline_plan(desc: CacheDesc, mode: int, seq_lens, pt_offsets, pages, direct
     return Plan(h.value, len(sl), desc.rope_dim)
 
 
+class LayerPointers:
+    """A host array of per-layer device pointers, marshalled once (``layer_pointers``) and reusable across calls;
+    keeps the tensors alive."""
+
+    def __init__(self, layers):
+        self.n = len(layers)
+        self.array = (C.c_void_p * self.n)()
+        for i, t in enumerate(layers):
+            self.array[i] = int(t) if isinstance(t, int) else t.data_ptr()
+        self.keep = layers
+
+
+def layer_pointers(layers) -> LayerPointers:
+    return LayerPointers(layers)
+
+
 def _ptr_array(layers, n_layers: int, what: str):
     if layers is None:
         return None, None
-    if len(layers) != n_layers:
-        raise ValueError(f"{what}: expected {n_layers} layers, got {len(layers)}")
-    arr = (C.c_void_p * n_layers)()
-    for i, t in enumerate(layers):
-        arr[i] = int(t) if isinstance(t, int) else t.data_ptr()
-    return arr, layers
+    lp = layers if isinstance(layers, LayerPointers) else LayerPointers(layers)
+    if lp.n != n_layers:
+        raise ValueError(f"{what}: expected {n_layers} layers, got {lp.n}")
+    return lp.array, lp
 
 
 def _stream_handle(stream):
@@ -260,7 +281,7 @@ def leyline_splice(plan: Plan, layer_src, layer_dst, layer_repl=None, page_table
                    stream=None, n_layers: int | None = None):
     """leyline.h: leyline_splice.  layer_* are sequences of device tensors (or raw device pointers), one per
     layer; *_out are int32 device tensors or None.  Asynchronous on `stream` (default: torch's current)."""
-    n = n_layers if n_layers is not None else len(layer_dst)
+    n = n_layers if n_layers is not None else (layer_dst.n if isinstance(layer_dst, LayerPointers) else len(layer_dst))
     a, _k1 = _ptr_array(layer_src, n, "layer_src")
     b, _k2 = _ptr_array(layer_dst, n, "layer_dst")
     c, _k3 = _ptr_array(layer_repl, n, "layer_repl")
@@ -270,7 +291,7 @@ def leyline_splice(plan: Plan, layer_src, layer_dst, layer_repl=None, page_table
 
 def leyline_rotate_inplace(plan: Plan, layers, layer_repl=None, slot_idx_out=None, stream=None):
     """leyline.h: leyline_rotate_inplace."""
-    n = len(layers)
+    n = layers.n if isinstance(layers, LayerPointers) else len(layers)
     a, _k1 = _ptr_array(layers, n, "layer_ptrs")
     c, _k3 = _ptr_array(layer_repl, n, "layer_repl")
     st = _lib.leyline_rotate_inplace(plan._h, a, c, _dev_ptr(slot_idx_out), _stream_handle(stream))

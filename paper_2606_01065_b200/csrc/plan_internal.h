@@ -85,6 +85,8 @@ struct leyline_plan_s {
     void* ev_start = nullptr;           /* cudaEvent_t pair around the data-moving kernels (tuning.profile) */
     void* ev_stop = nullptr;
     void* last_stream = nullptr;        /* stream of the last launch: the device tables are freed on it */
+    void* ev_uploaded = nullptr;        /* leyline_plan_prefetch: cudaEvent_t recorded after the upload on the copy stream */
+    bool scratch_clean = false;         /* the upload path already zeroed d_scratch; the first launch skips its memset */
 };
 
 /* implemented in splice.cu; plan.cpp calls it from leyline_plan_destroy */

@@ -5,6 +5,7 @@
  */
 #include <cstdio>
 #include <cstring>
+#include <deque>
 #include <mutex>
 #include <string>
 #include <vector>
@@ -75,7 +76,39 @@ void pin_release(PinnedBuf b, cudaStream_t stream) {
     cudaFreeHost(b.p);
 }
 
-leyline_status ensure_device(leyline_plan_s* pl, cudaStream_t stream) {
+/* ---- device memory for the plan tables ----
+ * A pool of its own: allocations made on the copy stream (leyline_plan_prefetch) must never pick up a dependency
+ * on the work of the stream that freed the previous plan's tables, which the default pool is allowed to insert. */
+struct PlanPool { int device = -1; cudaMemPool_t pool = nullptr; cudaStream_t copy_stream = nullptr; };
+std::deque<PlanPool> g_plan_pools; /* deque: references stay valid as devices are added */
+
+PlanPool* plan_pool(int dev) {
+    std::lock_guard<std::mutex> lk(g_pin_mu);
+    for (auto& pp : g_plan_pools)
+        if (pp.device == dev) return &pp;
+    PlanPool pp;
+    pp.device = dev;
+    cudaMemPoolProps props;
+    std::memset(&props, 0, sizeof(props));
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    if (cudaMemPoolCreate(&pp.pool, &props) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+    int off = 0;
+    unsigned long long keep = ~0ull; /* keep freed blocks cached: a plan per turn is the steady state */
+    cudaMemPoolSetAttribute(pp.pool, cudaMemPoolReuseAllowInternalDependencies, &off);
+    cudaMemPoolSetAttribute(pp.pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    if (cudaStreamCreateWithFlags(&pp.copy_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        (void)cudaGetLastError();
+        cudaMemPoolDestroy(pp.pool);
+        return nullptr;
+    }
+    g_plan_pools.push_back(pp);
+    return &g_plan_pools.back();
+}
+
+leyline_status device_info(int* dev_out) {
     int dev = 0;
     CU(cudaGetDevice(&dev));
     if (g_dev.device != dev) {
@@ -85,10 +118,12 @@ leyline_status ensure_device(leyline_plan_s* pl, cudaStream_t stream) {
         g_dev.sms = prop.multiProcessorCount;
         g_dev.smem_optin = (int)prop.sharedMemPerBlockOptin;
     }
-    if (pl->d_blob || pl->device >= 0) {
-        if (pl->device != dev) { g_last_error = "plan was uploaded on another device"; return LEYLINE_E_CUDA; }
-        return LEYLINE_OK;
-    }
+    *dev_out = dev;
+    return LEYLINE_OK;
+}
+
+/* Allocate tables + scratch, copy the tables and zero the scratch, all stream-ordered on `stream`. */
+leyline_status upload_tables(leyline_plan_s* pl, int dev, cudaStream_t stream) {
     /* one allocation: tiles | trig | tabs | slot_runs | page_runs | scratch, each 256-byte aligned */
     int64_t off = 0;
     auto place = [&](int64_t bytes) { int64_t o = off; off = align_up(off + bytes, 256); return o; };
@@ -110,19 +145,37 @@ leyline_status ensure_device(leyline_plan_s* pl, cudaStream_t stream) {
     put(pl->off_tabs, pl->tabs.data(), pl->tabs.size() * sizeof(int32_t));
     put(pl->off_slot_runs, pl->slot_runs.data(), pl->slot_runs.size() * sizeof(IdxRun));
     put(pl->off_page_runs, pl->page_runs.data(), pl->page_runs.size() * sizeof(IdxRun));
-    if (!cuda_ok(cudaMallocAsync(&pl->d_blob, (size_t)(pl->blob_bytes + pl->scratch_bytes), stream), "cudaMallocAsync(plan tables)")) {
+    PlanPool* pp = plan_pool(dev);
+    const size_t total = (size_t)(pl->blob_bytes + pl->scratch_bytes);
+    const cudaError_t e = pp ? cudaMallocFromPoolAsync(&pl->d_blob, total, pp->pool, stream) : cudaMallocAsync(&pl->d_blob, total, stream);
+    if (!cuda_ok(e, "cudaMallocAsync(plan tables)")) {
         if (pin.p) pin_release(pin, stream);
         pl->d_blob = nullptr;
         return LEYLINE_E_CUDA;
     }
     pl->d_scratch = static_cast<uint8_t*>(pl->d_blob) + pl->blob_bytes;
     /* pinned source: a plain stream-ordered DMA; pageable fallback: the runtime stages it before returning */
-    const bool ok = cuda_ok(cudaMemcpyAsync(pl->d_blob, host, (size_t)pl->blob_bytes, cudaMemcpyHostToDevice, stream),
-                            "cudaMemcpyAsync(plan tables)");
+    bool ok = cuda_ok(cudaMemcpyAsync(pl->d_blob, host, (size_t)pl->blob_bytes, cudaMemcpyHostToDevice, stream),
+                      "cudaMemcpyAsync(plan tables)");
     if (pin.p) pin_release(pin, stream);
+    ok = ok && cuda_ok(cudaMemsetAsync(pl->d_scratch, 0, (size_t)pl->scratch_bytes, stream), "cudaMemsetAsync(scratch)");
     if (!ok) return LEYLINE_E_CUDA;
+    pl->scratch_clean = true;
     pl->device = dev;
     return LEYLINE_OK;
+}
+
+leyline_status ensure_device(leyline_plan_s* pl, cudaStream_t stream) {
+    int dev = 0;
+    leyline_status st = device_info(&dev);
+    if (st != LEYLINE_OK) return st;
+    if (pl->d_blob || pl->device >= 0) {
+        if (pl->device != dev) { g_last_error = "plan was uploaded on another device"; return LEYLINE_E_CUDA; }
+        /* prefetched tables: order this stream after the copy (cheap once the event has completed) */
+        if (pl->ev_uploaded) CU(cudaStreamWaitEvent(stream, static_cast<cudaEvent_t>(pl->ev_uploaded), 0));
+        return LEYLINE_OK;
+    }
+    return upload_tables(pl, dev, stream);
 }
 
 template <class T>
@@ -344,7 +397,8 @@ leyline_status begin_call(leyline_plan_s* pl, cudaStream_t stream) {
     leyline_status st = ensure_device(pl, stream);
     if (st != LEYLINE_OK) return st;
     pl->last_stream = stream;
-    CU(cudaMemsetAsync(pl->d_scratch, 0, (size_t)pl->scratch_bytes, stream));
+    if (!pl->scratch_clean) CU(cudaMemsetAsync(pl->d_scratch, 0, (size_t)pl->scratch_bytes, stream));
+    pl->scratch_clean = false; /* tickets and hazard flags are consumed by this launch */
     if (pl->tuning.profile && !pl->ev_start) {
         CU(cudaEventCreate(reinterpret_cast<cudaEvent_t*>(&pl->ev_start)));
         CU(cudaEventCreate(reinterpret_cast<cudaEvent_t*>(&pl->ev_stop)));
@@ -438,6 +492,23 @@ extern "C" leyline_status leyline_rotate_inplace(leyline_plan_t* pl, void* const
     return LEYLINE_OK;
 }
 
+extern "C" leyline_status leyline_plan_prefetch(leyline_plan_t* pl) {
+    g_last_error.clear();
+    if (!pl) return LEYLINE_E_INVALID;
+    if (pl->d_blob || pl->device >= 0) return LEYLINE_OK;
+    int dev = 0;
+    leyline_status st = device_info(&dev);
+    if (st != LEYLINE_OK) return st;
+    PlanPool* pp = plan_pool(dev);
+    if (!pp) { g_last_error = "could not create the plan-table pool / copy stream"; return LEYLINE_E_CUDA; }
+    st = upload_tables(pl, dev, pp->copy_stream);
+    if (st != LEYLINE_OK) return st;
+    CU(cudaEventCreateWithFlags(reinterpret_cast<cudaEvent_t*>(&pl->ev_uploaded), cudaEventDisableTiming));
+    CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_uploaded), pp->copy_stream));
+    pl->last_stream = pp->copy_stream; /* until a launch replaces it: a never-launched plan frees its tables there */
+    return LEYLINE_OK;
+}
+
 extern "C" leyline_status leyline_plan_kernel_ms(const leyline_plan_t* pl, float* ms) {
     g_last_error.clear();
     if (!pl || !ms || !pl->ev_start) return LEYLINE_E_INVALID;
@@ -448,6 +519,8 @@ extern "C" leyline_status leyline_plan_kernel_ms(const leyline_plan_t* pl, float
 extern "C" void leyline_plan_release_device_(leyline_plan_s* pl) {
     if (pl->ev_start) cudaEventDestroy(static_cast<cudaEvent_t>(pl->ev_start));
     if (pl->ev_stop) cudaEventDestroy(static_cast<cudaEvent_t>(pl->ev_stop));
+    if (pl->ev_uploaded) cudaEventDestroy(static_cast<cudaEvent_t>(pl->ev_uploaded));
+    pl->ev_uploaded = nullptr;
     /* stream-ordered: freed after everything this plan launched on its stream, without a device sync */
     if (pl->d_blob) cudaFreeAsync(pl->d_blob, static_cast<cudaStream_t>(pl->last_stream)); /* tables + scratch */
     pl->d_blob = pl->d_scratch = nullptr;

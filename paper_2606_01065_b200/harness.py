@@ -49,7 +49,7 @@ def plan_workload(w: synth.Workload, mode: int, desc) -> B.Plan:
     return B.leyline_plan(desc, mode, w.seq_lens, w.pt_offsets, w.pages, w.directives, free)
 
 
-def run_workload(cache: DeviceCache, mode: int, stream=None, want_idx=True):
+def run_workload(cache: DeviceCache, mode: int, stream=None, want_idx=True, prefetch=False, launches=1):
     """Plan + launch one splice of the cache's workload in `mode` (in place on cache.pools unless cache.dst is
     set and the mode is FRESH).  Returns (plan, page_table_out, slot_idx_out) -- device int32 tensors."""
     d, keep = cache.desc()
@@ -57,10 +57,13 @@ def run_workload(cache: DeviceCache, mode: int, stream=None, want_idx=True):
     dev = cache.device
     pt = torch.empty(max(int(plan.info.total_new_pages), 1), dtype=torch.int32, device=dev) if want_idx else None
     idx = torch.empty(max(int(plan.info.total_new_tokens), 1), dtype=torch.int32, device=dev) if want_idx else None
-    if mode == B.ROTATE_ONLY:
-        B.leyline_rotate_inplace(plan, cache.pools, cache.repl, idx, stream)
-    else:
-        dst = cache.dst if (cache.dst is not None and mode == B.FRESH) else cache.pools
-        B.leyline_splice(plan, cache.pools, dst, cache.repl, pt, idx, stream)
+    if prefetch:
+        plan.prefetch()
+    for _ in range(launches):     # FRESH never writes what it reads, so launching a plan again repeats the result
+        if mode == B.ROTATE_ONLY:
+            B.leyline_rotate_inplace(plan, cache.pools, cache.repl, idx, stream)
+        else:
+            dst = cache.dst if (cache.dst is not None and mode == B.FRESH) else cache.pools
+            B.leyline_splice(plan, cache.pools, dst, cache.repl, pt, idx, stream)
     del keep
     return plan, pt, idx

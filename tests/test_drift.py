@@ -1,0 +1,197 @@
+"""Chained-rotation drift (App. F, Table 6).
+
+The closure R(a)R(b) = R(a+b) is exact in real arithmetic; with bf16 storage every splice rounds the rotated K_pe
+once more.  App. F chains N random-delta rotations (|delta| <= 512, running position kept inside the cache) on
+K of shape [8, 32, 64] and reports the rel-L2 / max-abs distance to fresh RoPE at the final position (Table 6,
+tests/golden/paper_table6.txt).  Here the chain is N successive *splices*: each turn replaces the leading scratch
+region [0, S) of a request by S + delta tokens, so the 32 tracked tokens behind it move by delta, on 8 layers.
+
+CPU (not gpu): the oracle's chain against what the paper and the mathematics fix --
+  * fp64 storage: N = 100 chained splices equal ONE rotation by the summed delta to 1e-11 (closure);
+  * bf16 storage: drift vs fresh RoPE stays below every Table 6 row (the paper's path is bf16 throughout, ours
+    rounds once per rotation), grows sub-linearly (random walk) and not slower than the rounding floor.
+GPU: the same chain through leyline_plan + leyline_rotate_inplace (ROTATE_ONLY, token-level slots, the paper's
+in-place DynamicCache path), in lockstep with the oracle: integer results bit-exact every turn,
+drift statistics of the two chains agree, and both sit under Table 6.
+"""
+import numpy as np
+import pytest
+
+import oracle as O
+from helpers import from_storage, golden, rope_complex, to_storage
+from paper_2606_01065_b200 import synth
+
+T6 = golden("paper_table6.txt")
+H64 = synth.rope_inv_freq(64, 10000.0)
+N_LAYERS, N_TRACKED, DC, DR = 8, 32, 8, 64          # [batch = 8 layers, 32 tracked tokens, head_dim 64]
+CACHE = 8192                                         # "running position constrained to the cache range"
+
+
+def chain_deltas(rng, n, s0):
+    """n signed deltas in [-512, 512] (never 0) keeping the scratch length S in [1, CACHE - N_TRACKED)."""
+    out, s = [], s0
+    while len(out) < n:
+        d = int(rng.integers(-T6["delta_abs_max"], T6["delta_abs_max"] + 1))
+        if d != 0 and 1 <= s + d < CACHE - N_TRACKED:
+            out.append(d)
+            s += d
+    return out
+
+
+def initial_rows(rng, s0):
+    """Per layer: [s0 + N_TRACKED, DC + DR] float64 rows; K_pe = textbook RoPE of raw keys at positions 0..L-1."""
+    L = s0 + N_TRACKED
+    raw = rng.standard_normal((N_LAYERS, L, DR))
+    lat = rng.standard_normal((N_LAYERS, L, DC))
+    rows = np.concatenate([lat, rope_complex(raw, np.arange(L)[None, :], H64)], axis=2)
+    return raw, rows
+
+
+class OracleChain:
+    """State of one chain on the CPU oracle: token-level pool per layer (page size 1), the request's slot list."""
+
+    def __init__(self, dtype, rows, n_slots, seed):
+        self.dtype, self.stride = dtype, (DC + DR) * O.ELEM_BYTES[dtype]
+        L = rows.shape[1]
+        rng = np.random.default_rng(seed)
+        self.n_slots = n_slots
+        self.order = rng.permutation(n_slots).astype(np.int32)     # allocation order of the pool's slots
+        self.idx = self.order[:L].copy()
+        self.pools = []
+        for l in range(N_LAYERS):
+            pool = np.zeros((n_slots, self.stride), np.uint8)
+            pool[self.idx] = to_storage(rows[l], dtype)
+            self.pools.append(pool.reshape(-1))
+
+    def free_list(self):
+        live = np.zeros(self.n_slots, bool)
+        live[self.idx] = True
+        return self.order[~live[self.order]]
+
+    def step_inputs(self, S, delta):
+        L = len(self.idx)
+        return [L], np.array([0, L], np.int64), self.idx, [(0, 0, S, S + delta, 0, O.AMORTIZE)], self.free_list()
+
+    def step(self, S, delta, repl):
+        seq, pto, pages, dirs, free = self.step_inputs(S, delta)
+        bm = O.plan_batch(O.ROTATE_ONLY, 1, seq, pto, pages, dirs, free)
+        assert bm.status == O.OK
+        self.pools = [O.splice_layer(self.dtype, O.NEOX, DC, DR, self.stride, H64, 1.0, self.pools[l], repl[l], bm)
+                      for l in range(N_LAYERS)]
+        self.idx = bm.requests[0].slot_new.astype(np.int32)
+        return bm
+
+    def tracked(self):
+        rows = [from_storage(p.reshape(-1, self.stride)[self.idx[-N_TRACKED:]], self.dtype) for p in self.pools]
+        return np.stack(rows)[:, :, DC:]
+
+
+def fresh_reference(raw, s0, deltas):
+    """(b) of PAPER.md:455: fresh RoPE of the raw keys at the target position, fp64."""
+    S = s0 + sum(deltas)
+    return rope_complex(raw[:, s0:s0 + N_TRACKED], (S + np.arange(N_TRACKED))[None, :], H64)
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def run_oracle_chain(dtype, n, seed):
+    rng = np.random.default_rng(1000 + seed)
+    s0 = int(rng.integers(1024, 4096))
+    deltas = chain_deltas(rng, n, s0)
+    raw, rows = initial_rows(rng, s0)
+    ch = OracleChain(dtype, rows, 2 * CACHE, seed)
+    repl = [rng.integers(0, 255, size=CACHE * ch.stride, dtype=np.uint8) if dtype != O.F64
+            else np.zeros(CACHE * ch.stride, np.uint8) for _ in range(N_LAYERS)]
+    S = s0
+    for d in deltas:
+        ch.step(S, d, repl)
+        S += d
+    return ch, raw, rows, s0, deltas
+
+
+def test_closure_over_100_chained_splices_f64():
+    ch, raw, rows, s0, deltas = run_oracle_chain(O.F64, 100, 0)
+    got = ch.tracked()
+    one = rope_complex(rows[:, s0:, DC:], np.full((1, N_TRACKED), float(sum(deltas))), H64)   # (a): one rotation by the sum
+    assert np.abs(got - one).max() < 1e-11
+    assert np.abs(got - fresh_reference(raw, s0, deltas)).max() < 1e-11
+
+
+def test_bf16_drift_stays_under_table6_and_is_a_random_walk():
+    ns = [int(n) for n in T6["n_values"]]
+    mean_rel, worst_abs = {}, {}
+    for n in ns:
+        rels, mabs = [], []
+        for seed in range(3):
+            ch, raw, rows, s0, deltas = run_oracle_chain(O.BF16, n, seed)
+            ref = fresh_reference(raw, s0, deltas)
+            got = ch.tracked()
+            rels.append(rel_l2(got, ref))
+            mabs.append(float(np.abs(got - ref).max()))
+        mean_rel[n], worst_abs[n] = float(np.mean(rels)), max(mabs)
+    for n, bound_rel, bound_abs in zip(ns, T6["rel_l2"], T6["max_abs"]):
+        assert mean_rel[n] <= bound_rel, (n, mean_rel[n], bound_rel)
+        assert worst_abs[n] <= bound_abs, (n, worst_abs[n], bound_abs)
+    # one RNE to bf16 per rotation: an element's rounding error is uniform in +-ulp/2, ulp/|x| in (2^-8, 2^-7], so one
+    # rounding contributes between 2^-8/sqrt(12) and 2^-7/sqrt(12) of rel-L2; the N+1 independent roundings of a chain
+    # (the stored K_pe itself is one) add in quadrature -- a random walk, never linear growth
+    lo, hi = 2.0 ** -8 / np.sqrt(12.0), 2.0 ** -7 / np.sqrt(12.0)
+    for n in ns:
+        assert lo * np.sqrt(n + 1) <= mean_rel[n] <= hi * np.sqrt(n + 1), (n, mean_rel[n])
+    growth = mean_rel[100] / mean_rel[2]
+    assert 3.0 < growth < 9.0, growth          # sqrt(101/3) = 5.8; the paper measures 6.1x
+    assert abs(growth - T6["growth_n2_to_n100"]) / T6["growth_n2_to_n100"] < 0.35
+
+
+# ----------------------------------------------------------------------------- GPU chain
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n", [2, 20, 100])
+def test_gpu_chain_matches_oracle_chain(n):
+    import torch
+    from paper_2606_01065_b200 import binding as B
+    seed = 7
+    rng = np.random.default_rng(1000 + seed)
+    s0 = int(rng.integers(1024, 4096))
+    deltas = chain_deltas(rng, n, s0)
+    raw, rows = initial_rows(rng, s0)
+    ch = OracleChain(O.BF16, rows, 2 * CACHE, seed)
+    repl = [rng.integers(0, 255, size=CACHE * ch.stride, dtype=np.uint8) for _ in range(N_LAYERS)]
+    dev = torch.device("cuda:0")
+    pools = [torch.from_numpy(p.copy()).to(dev) for p in ch.pools]
+    repl_d = [torch.from_numpy(r).to(dev) for r in repl]
+    desc, keep = B.make_desc(N_LAYERS, DC, DR, 1, B.BF16, B.NEOX, ch.stride, ch.n_slots, H64)
+    idx = ch.idx.copy()
+    out = torch.empty(CACHE, dtype=torch.int32, device=dev)
+    S = s0
+    for d in deltas:
+        seq, pto, pages, dirs, free = ch.step_inputs(S, d)
+        np.testing.assert_array_equal(pages, idx)                   # the two chains hold the same slot list
+        plan = B.leyline_plan(desc, B.ROTATE_ONLY, seq, pto, idx, dirs, free)
+        B.leyline_rotate_inplace(plan, pools, repl_d, out)
+        bm = ch.step(S, d, repl)
+        L_new = int(plan.new_seq_lens[0])
+        idx = out[:L_new].cpu().numpy()
+        np.testing.assert_array_equal(idx, ch.idx)                  # a2 bit-exact on every turn
+        np.testing.assert_array_equal(plan.released, bm.released)
+        plan.close()
+        S += d
+    del keep
+    ref = fresh_reference(raw, s0, deltas)
+    got_o = ch.tracked()
+    got_g = np.stack([from_storage(p.cpu().numpy().reshape(-1, ch.stride)[idx[-N_TRACKED:]], O.BF16) for p in pools])
+    lat_o = np.stack([p.reshape(-1, ch.stride)[ch.idx][:, :DC * 2] for p in ch.pools])
+    lat_g = np.stack([p.cpu().numpy().reshape(-1, ch.stride)[idx][:, :DC * 2] for p in pools])
+    np.testing.assert_array_equal(lat_g, lat_o)                     # latent bytes never drift
+    got_g = got_g[:, :, DC:]
+    rg, ro = rel_l2(got_g, ref), rel_l2(got_o, ref)
+    bound = float(np.interp(n, T6["n_values"], T6["rel_l2"]))
+    print(f"[drift] N={n}: rel-L2 vs fresh  gpu {rg:.3e}  oracle {ro:.3e}  paper Table 6 {bound:.1e};  "
+          f"max-abs gpu {np.abs(got_g - ref).max():.3e} oracle {np.abs(got_o - ref).max():.3e};  "
+          f"gpu vs oracle chain rel-L2 {rel_l2(got_g, got_o):.3e}")
+    assert rg <= bound and ro <= bound
+    assert abs(rg - ro) <= 0.05 * ro                                # same random walk, statistically
+    # the chains differ only where a rounding decision differed (<= 1 ulp per turn, < 1 % of elements per turn)
+    assert rel_l2(got_g, got_o) <= 0.5 * ro

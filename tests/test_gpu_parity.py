@@ -20,7 +20,7 @@ MODE_NAME = {O.FRESH: "fresh", O.INPLACE_MOVE: "inplace", O.ROTATE_ONLY: "rotate
 MOVERS = [1, 2]
 
 
-def run_and_compare(w, mode, check_layers=None, tuning=None):
+def run_and_compare(w, mode, check_layers=None, tuning=None, **launch):
     from paper_2606_01065_b200 import binding as B
     from paper_2606_01065_b200 import harness
     if tuning:
@@ -29,7 +29,7 @@ def run_and_compare(w, mode, check_layers=None, tuning=None):
         cache = harness.DeviceCache(w, "cuda:0")
         check_layers = list(range(w.n_layers)) if check_layers is None else check_layers
         old = {l: cache.pools[l].cpu().numpy() for l in check_layers}
-        plan, pt, idx = harness.run_workload(cache, mode)
+        plan, pt, idx = harness.run_workload(cache, mode, **launch)
         torch.cuda.synchronize()
     finally:
         if tuning:
@@ -98,6 +98,20 @@ def test_bulk_ring_geometry(mode, stages, layer_group):
                        directives=[(0, 7, 40, 300, 0, 0), (0, 900, 1700, 5, 0, 0), (1, 100, 101, 77, 0, 0)],
                        seed=21, pool_factor=3.0, extra_pages=60).finalize()
     run_and_compare(w, mode, tuning={"kernel": 2, "tile_rows": 16, "stages": stages, "layer_group": layer_group})
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("mover", MOVERS)
+def test_prefetched_tables(mode, mover):
+    """leyline_plan_prefetch: tables uploaded on the library's copy stream, the launch only waits on the event."""
+    rng = np.random.default_rng(77)
+    run_and_compare(tiny_workload(rng, P=16, n_req=3), mode, tuning={"kernel": mover}, prefetch=True)
+
+
+@pytest.mark.parametrize("prefetch", [False, True])
+def test_relaunching_a_fresh_plan_repeats_the_result(prefetch):
+    """The second launch of a plan must zero its ticket counters itself (the upload zeroes them only once)."""
+    run_and_compare(synth.config(1, pool_factor=2.5), O.FRESH, prefetch=prefetch, launches=3)
 
 
 @pytest.mark.parametrize("mode", MODES)

@@ -55,6 +55,20 @@ def tiny_workload(rng, P=None, n_req=None, forget=False, dtype=synth.DT_BF16):
     return w.finalize()
 
 
+def test_prefetch_without_a_device_fails_loudly_and_keeps_the_plan():
+    """No CPU fallback: without a CUDA device the upload is refused with LEYLINE_E_CUDA; host queries still work."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("needs a box without a GPU")
+    w = tiny_workload(np.random.default_rng(3), P=4, n_req=2)
+    plan = make_plan(w, B.FRESH)
+    with pytest.raises(B.LeylineError) as ei:
+        plan.prefetch()
+    assert ei.value.status == B.E_CUDA
+    assert len(plan.new_seq_lens) == 2
+    plan.close()
+
+
 def make_plan(w, mode, n_layers=None):
     d, keep = B.make_desc(n_layers or w.n_layers, w.latent_dim, w.rope_dim, w.page_size, w.dtype, w.pairing,
                           w.row_bytes, w.n_slots, w.inv_freq, rope_heads=w.rope_heads)
