@@ -46,6 +46,7 @@ def parse_args():
     ap.add_argument("--ctas-per-sm", type=int, default=0)
     ap.add_argument("--stages", type=int, default=0, help="leyline_tuning.stages (bulk kernel)")
     ap.add_argument("--layer-group", type=int, default=0, help="leyline_tuning.layer_group (bulk kernel)")
+    ap.add_argument("--consumer-warps", type=int, default=0, help="leyline_tuning.consumer_warps (bulk kernel)")
     return ap.parse_args()
 
 
@@ -294,7 +295,7 @@ def run_ours(args):
     from paper_2606_01065_b200 import synth
     rank, world, local = dist_setup(args.gpus)
     B.leyline_set_tuning(kernel=args.kernel, tile_rows=args.tile_rows, ctas_per_sm=args.ctas_per_sm, profile=1,
-                         stages=args.stages, layer_group=args.layer_group)
+                         stages=args.stages, layer_group=args.layer_group, consumer_warps=args.consumer_warps)
     mode = MODES[args.mode]
     w = workload_of(args.workload, args.mode)
     cache = harness.DeviceCache(w, f"cuda:{local}")

@@ -253,6 +253,8 @@ typedef struct {
     int32_t profile;       /* 1: record CUDA events around the data-moving kernels (leyline_plan_kernel_ms) */
     int32_t stages;        /* bulk kernel only: shared-memory stages per CTA, 0 = as many as fit (at most 8) */
     int32_t layer_group;   /* bulk kernel only: layers per work item (one stage each), 0 = default */
+    int32_t consumer_warps;/* bulk kernel only: warps that rotate the band in shared memory, 0 = default (4 for MLA's
+                              narrow band, more when the band is most of the row), at most 16 */
 } leyline_tuning;
 leyline_status leyline_set_tuning(const leyline_tuning* t);
 leyline_status leyline_get_tuning(leyline_tuning* t);

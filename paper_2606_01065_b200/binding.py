@@ -54,7 +54,7 @@ class Tile(C.Structure):
 
 class Tuning(C.Structure):
     _fields_ = [("kernel", C.c_int32), ("tile_rows", C.c_int32), ("ctas_per_sm", C.c_int32), ("profile", C.c_int32),
-                ("stages", C.c_int32), ("layer_group", C.c_int32)]
+                ("stages", C.c_int32), ("layer_group", C.c_int32), ("consumer_warps", C.c_int32)]
 
 
 class LeylineError(RuntimeError):
@@ -115,8 +115,8 @@ def leyline_version() -> str:
 
 
 def leyline_set_tuning(kernel: int = 0, tile_rows: int = 0, ctas_per_sm: int = 0, profile: int = 0, stages: int = 0,
-                       layer_group: int = 0):
-    t = Tuning(kernel, tile_rows, ctas_per_sm, profile, stages, layer_group)
+                       layer_group: int = 0, consumer_warps: int = 0):
+    t = Tuning(kernel, tile_rows, ctas_per_sm, profile, stages, layer_group, consumer_warps)
     _check(_lib.leyline_set_tuning(C.byref(t)), "leyline_set_tuning")
 
 
@@ -124,7 +124,8 @@ def leyline_get_tuning() -> dict:
     t = Tuning()
     _check(_lib.leyline_get_tuning(C.byref(t)), "leyline_get_tuning")
     return {"kernel": t.kernel, "tile_rows": t.tile_rows, "ctas_per_sm": t.ctas_per_sm, "profile": t.profile,
-            "stages": t.stages, "layer_group": t.layer_group}
+            "stages": t.stages, "layer_group": t.layer_group,
+            "consumer_warps": t.consumer_warps}
 
 
 def _arr(x, dtype):

@@ -21,7 +21,7 @@ using leyline::IdxRun;
 
 namespace {
 
-leyline_tuning g_tuning = {0, 0, 0, 0, 0, 0};
+leyline_tuning g_tuning = {0, 0, 0, 0, 0, 0, 0};
 
 inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
@@ -119,9 +119,10 @@ bool choose_bulk(const leyline_cache_desc& c, int E, const leyline_tuning& t, in
 int choose_tile_rows(const leyline_cache_desc& c, int E, const leyline_tuning& t, bool bulk) {
     int64_t lat_chunks = (int64_t)c.latent_dim * E / 16, nb = (int64_t)c.rope_dim * E / 16;
     if (bulk) {
-        /* bulk kernel: one shared-memory stage holds a tile; default ~36 KB per stage, at most 64 rows */
+        /* bulk kernel: one shared-memory stage holds a tile; default ~36 KB per stage (48 KB for rows of 2 KB and
+         * more, measured on the full-width K pools: fewer, larger stages amortise the per-stage hand-offs), <= 64 rows */
         int64_t row = row_elems(c) * E;
-        int64_t want = t.tile_rows > 0 ? t.tile_rows : std::max<int64_t>(1, 36864 / row);
+        int64_t want = t.tile_rows > 0 ? t.tile_rows : std::max<int64_t>(1, (row >= 2048 ? 49152 : 36864) / row);
         return (int)std::max<int64_t>(1, std::min<int64_t>({want, (int64_t)64, 65536 / row}));
     }
     /* the row kernel keeps a whole tile in registers: <= 8 latent + 1 band chunk per thread, 256 threads */
@@ -516,7 +517,7 @@ extern "C" leyline_status leyline_set_tuning(const leyline_tuning* t) {
     if (!t) return LEYLINE_E_INVALID;
     if (t->kernel < 0 || t->kernel > 2 || t->tile_rows < 0 || t->tile_rows > 64 || t->ctas_per_sm < 0 ||
         t->ctas_per_sm > 32 || t->stages < 0 || t->stages > 8 || t->layer_group < 0 ||
-        t->layer_group > LEYLINE_MAX_LAYERS_PER_LAUNCH)
+        t->layer_group > LEYLINE_MAX_LAYERS_PER_LAUNCH || t->consumer_warps < 0 || t->consumer_warps > 16)
         return LEYLINE_E_INVALID;
     g_tuning = *t;
     return LEYLINE_OK;

@@ -355,8 +355,10 @@ leyline_status run_tiles_bulk(leyline_plan_s* pl, bool hazard, int32_t tile_begi
     const int stage_bytes = pl->tile_rows * row_bytes;
     /* consumer warps rotate the band in shared memory: 4 keep up with MLA's 1/9 of the bytes, a band that is most of
      * the row (full-width K) needs more issue slots */
-    const int cwarps = (int64_t)pl->n_heads * pl->desc.rope_dim * 4 <= (int64_t)pl->desc.latent_dim + (int64_t)pl->n_heads * pl->desc.rope_dim
-                           ? kBulkConsumerWarps : kBulkMaxConsumerWarps;
+    int cwarps = (int64_t)pl->n_heads * pl->desc.rope_dim * 4 <= (int64_t)pl->desc.latent_dim + (int64_t)pl->n_heads * pl->desc.rope_dim
+                     ? kBulkConsumerWarps : kBulkWideConsumerWarps;
+    if (pl->tuning.consumer_warps > 0) cwarps = pl->tuning.consumer_warps;
+    if (cwarps > kBulkMaxConsumerWarps) cwarps = kBulkMaxConsumerWarps;
     BulkKernel fn = pick_bulk(pl, hazard);
     cudaFuncAttributes fa;
     CU(cudaFuncGetAttributes(&fa, reinterpret_cast<const void*>(fn)));
