@@ -86,6 +86,10 @@ typedef struct {
     const float* layer_scale;  /* HOST, [n_layers], fp8 only (may be NULL): per-layer dequantisation scale.  A splice
                                   leaves it unchanged, so it cancels in x/scale*scale; it is validated (> 0, finite)
                                   but not used by the kernels (G16). */
+    const int32_t* layer_pairing; /* HOST, [n_layers] of leyline_pairing, or NULL: per-layer override of `pairing`
+                                  (the paper's helper "reads is_neox_style per layer"; G20).  Layers of one
+                                  convention are launched together, so a mixed cache costs one extra launch per mover.
+                                  Copied by leyline_plan. */
 } leyline_cache_desc;
 
 typedef struct {

@@ -27,7 +27,8 @@ class CacheDesc(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("latent_dim", C.c_int32), ("rope_dim", C.c_int32),
                 ("page_size", C.c_int32), ("dtype", C.c_int32), ("pairing", C.c_int32),
                 ("rope_heads", C.c_int32), ("reserved_", C.c_int32), ("row_stride_bytes", C.c_int64), ("pool_slots", C.c_int64),
-                ("inv_freq", C.POINTER(C.c_float)), ("layer_scale", C.POINTER(C.c_float))]
+                ("inv_freq", C.POINTER(C.c_float)), ("layer_scale", C.POINTER(C.c_float)),
+                ("layer_pairing", C.POINTER(C.c_int32))]
 
 
 class Directive(C.Structure):
@@ -137,15 +138,19 @@ def _ptr(a: np.ndarray):
 
 
 def make_desc(n_layers, latent_dim, rope_dim, page_size, dtype, pairing, row_stride_bytes, pool_slots, inv_freq,
-              layer_scale=None, rope_heads=1):
+              layer_scale=None, rope_heads=1, layer_pairing=None):
     """Returns (CacheDesc, keepalive) -- keep `keepalive` referenced while the desc is in use.
     Row = latent_dim + rope_heads * rope_dim elements (rope_heads = 1: MLA; kv_heads: full-width K)."""
     inv = _arr(inv_freq, np.float32)
     sc = _arr(layer_scale, np.float32) if layer_scale is not None else None
+    lp = _arr(layer_pairing, np.int32) if layer_pairing is not None else None
+    if lp is not None and len(lp) != n_layers:
+        raise ValueError(f"layer_pairing: expected {n_layers} entries, got {len(lp)}")
     d = CacheDesc(n_layers, latent_dim, rope_dim, page_size, dtype, pairing, rope_heads, 0, row_stride_bytes, pool_slots,
                   inv.ctypes.data_as(C.POINTER(C.c_float)),
-                  sc.ctypes.data_as(C.POINTER(C.c_float)) if sc is not None else None)
-    return d, (inv, sc)
+                  sc.ctypes.data_as(C.POINTER(C.c_float)) if sc is not None else None,
+                  lp.ctypes.data_as(C.POINTER(C.c_int32)) if lp is not None else None)
+    return d, (inv, sc, lp)
 
 
 class Plan:

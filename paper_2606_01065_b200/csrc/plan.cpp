@@ -66,6 +66,9 @@ leyline_status check_desc(const leyline_cache_desc* c, int* elem_bytes, int* pag
     if (c->dtype != LEYLINE_BF16 && c->dtype != LEYLINE_FP8_E4M3) return LEYLINE_E_INVALID;
     if (c->pairing != LEYLINE_ROPE_NEOX && c->pairing != LEYLINE_ROPE_INTERLEAVED) return LEYLINE_E_INVALID;
     if (!c->inv_freq) return LEYLINE_E_INVALID;
+    if (c->layer_pairing)
+        for (int l = 0; l < c->n_layers; ++l)
+            if (c->layer_pairing[l] != LEYLINE_ROPE_NEOX && c->layer_pairing[l] != LEYLINE_ROPE_INTERLEAVED) return LEYLINE_E_INVALID;
     int E = c->dtype == LEYLINE_BF16 ? 2 : 1;
     int64_t row = row_elems(*c) * E;
     if (c->row_stride_bytes < row || (c->row_stride_bytes & 15)) return LEYLINE_E_INVALID;
@@ -194,6 +197,8 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
     pl->desc.inv_freq = pl->inv_freq.data();
     if (desc->layer_scale) pl->layer_scale.assign(desc->layer_scale, desc->layer_scale + desc->n_layers);
     pl->desc.layer_scale = pl->layer_scale.empty() ? nullptr : pl->layer_scale.data();
+    if (desc->layer_pairing) pl->layer_pairing.assign(desc->layer_pairing, desc->layer_pairing + desc->n_layers);
+    pl->desc.layer_pairing = pl->layer_pairing.empty() ? nullptr : pl->layer_pairing.data();
     pl->mode = mode;
     pl->n_requests = n_requests;
     pl->elem_bytes = E;

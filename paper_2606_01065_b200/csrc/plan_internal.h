@@ -53,6 +53,7 @@ struct leyline_plan_s {
     leyline_cache_desc desc;            /* inv_freq / layer_scale pointers redirected to the copies below */
     std::vector<float> inv_freq;
     std::vector<float> layer_scale;
+    std::vector<int32_t> layer_pairing; /* per-layer override of desc.pairing, or empty */
     int32_t mode = 0;
     int32_t n_requests = 0;
     int32_t elem_bytes = 2;

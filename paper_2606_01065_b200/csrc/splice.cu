@@ -4,6 +4,7 @@
  * caller's stream.  No synchronisation, no CPU fallback: every failure is a LEYLINE_E_CUDA status.
  */
 #include <cstdio>
+#include <algorithm>
 #include <cstring>
 #include <deque>
 #include <mutex>
@@ -224,8 +225,8 @@ template <int DT, int PAIRING>
 MoveKernel pick_move_hazard(const leyline_plan_s* pl, bool hazard) {
     return hazard ? pick_move_geom<DT, PAIRING, true>(pl) : pick_move_geom<DT, PAIRING, false>(pl);
 }
-MoveKernel pick_move(const leyline_plan_s* pl, bool hazard) {
-    const bool neox = pl->desc.pairing == LEYLINE_ROPE_NEOX;
+MoveKernel pick_move(const leyline_plan_s* pl, int pairing, bool hazard) {
+    const bool neox = pairing == LEYLINE_ROPE_NEOX;
     if (pl->desc.dtype == LEYLINE_BF16)
         return neox ? pick_move_hazard<LEYLINE_BF16, LEYLINE_ROPE_NEOX>(pl, hazard)
                     : pick_move_hazard<LEYLINE_BF16, LEYLINE_ROPE_INTERLEAVED>(pl, hazard);
@@ -236,26 +237,26 @@ MoveKernel pick_move(const leyline_plan_s* pl, bool hazard) {
 using BulkKernel = void (*)(const MoveParams, int, int, int, int, int);
 
 template <int DT>
-BulkKernel pick_bulk_dt(const leyline_plan_s* pl, bool hazard) {
-    const bool neox = pl->desc.pairing == LEYLINE_ROPE_NEOX;
+BulkKernel pick_bulk_dt(int pairing, bool hazard) {
+    const bool neox = pairing == LEYLINE_ROPE_NEOX;
     if (hazard) return neox ? k_move_bulk<DT, LEYLINE_ROPE_NEOX, true> : k_move_bulk<DT, LEYLINE_ROPE_INTERLEAVED, true>;
     return neox ? k_move_bulk<DT, LEYLINE_ROPE_NEOX, false> : k_move_bulk<DT, LEYLINE_ROPE_INTERLEAVED, false>;
 }
-BulkKernel pick_bulk(const leyline_plan_s* pl, bool hazard) {
-    return pl->desc.dtype == LEYLINE_BF16 ? pick_bulk_dt<LEYLINE_BF16>(pl, hazard) : pick_bulk_dt<LEYLINE_FP8_E4M3>(pl, hazard);
+BulkKernel pick_bulk(const leyline_plan_s* pl, int pairing, bool hazard) {
+    return pl->desc.dtype == LEYLINE_BF16 ? pick_bulk_dt<LEYLINE_BF16>(pairing, hazard) : pick_bulk_dt<LEYLINE_FP8_E4M3>(pairing, hazard);
 }
 
 template <int DT>
-MoveKernel pick_rotate_dt(const leyline_plan_s* pl, bool fixed) {
-    const bool neox = pl->desc.pairing == LEYLINE_ROPE_NEOX;
+MoveKernel pick_rotate_dt(int pairing, bool fixed) {
+    const bool neox = pairing == LEYLINE_ROPE_NEOX;
     if (fixed) return neox ? k_rotate_band<DT, LEYLINE_ROPE_NEOX, true> : k_rotate_band<DT, LEYLINE_ROPE_INTERLEAVED, true>;
     return neox ? k_rotate_band<DT, LEYLINE_ROPE_NEOX, false> : k_rotate_band<DT, LEYLINE_ROPE_INTERLEAVED, false>;
 }
 /* a5.  FIXED when the pair columns of a row divide the block (a thread then keeps one column and its cos/sin). */
-MoveKernel pick_rotate(const leyline_plan_s* pl) {
+MoveKernel pick_rotate(const leyline_plan_s* pl, int pairing) {
     const int cols = pl->n_heads * (pl->head_chunks / 2);
     const bool fixed = cols <= kThreads && kThreads % cols == 0;
-    return pl->desc.dtype == LEYLINE_BF16 ? pick_rotate_dt<LEYLINE_BF16>(pl, fixed) : pick_rotate_dt<LEYLINE_FP8_E4M3>(pl, fixed);
+    return pl->desc.dtype == LEYLINE_BF16 ? pick_rotate_dt<LEYLINE_BF16>(pairing, fixed) : pick_rotate_dt<LEYLINE_FP8_E4M3>(pairing, fixed);
 }
 
 }  // namespace
@@ -278,8 +279,30 @@ int occupancy(const void* fn, int smem) {
     return blocks;
 }
 
-void fill_params(const leyline_plan_s* pl, MoveParams& mp, int32_t tile_begin, int64_t tile_count, int l0, int nl,
+/* Layers that one launch can serve: same pairing convention ("per layer"; G20), at most kMaxLayers.
+ * `flag_base` numbers the launch's layers uniquely inside the call (hazard-flag column). */
+struct LayerChunk { int pairing; int flag_base; std::vector<int> layers; };
+
+std::vector<LayerChunk> layer_chunks(const leyline_plan_s* pl) {
+    std::vector<LayerChunk> out;
+    const int L = pl->desc.n_layers;
+    int base = 0;
+    for (int conv = 0; conv < 2; ++conv) {
+        std::vector<int> mine;
+        for (int l = 0; l < L; ++l)
+            if ((pl->layer_pairing.empty() ? pl->desc.pairing : pl->layer_pairing[l]) == conv) mine.push_back(l);
+        for (size_t i = 0; i < mine.size(); i += kMaxLayers) {
+            const size_t n = std::min<size_t>(kMaxLayers, mine.size() - i);
+            out.push_back({conv, base, std::vector<int>(mine.begin() + (long)i, mine.begin() + (long)(i + n))});
+            base += (int)n;
+        }
+    }
+    return out;
+}
+
+void fill_params(const leyline_plan_s* pl, MoveParams& mp, int32_t tile_begin, int64_t tile_count, const LayerChunk& lc,
                  void* const* layer_src, void* const* layer_dst, const void* const* layer_repl, int ticket_slot) {
+    const int nl = (int)lc.layers.size(), l0 = lc.flag_base;
     std::memset(&mp, 0, sizeof(mp));
     mp.tiles = blob_at<DevTile>(pl, pl->off_tiles);
     mp.trig = blob_at<float>(pl, pl->off_trig);
@@ -299,23 +322,22 @@ void fill_params(const leyline_plan_s* pl, MoveParams& mp, int32_t tile_begin, i
     mp.head_chunks = pl->head_chunks;
     mp.band_chunks = pl->n_heads * pl->head_chunks;
     for (int l = 0; l < nl; ++l) {
-        mp.src[l] = static_cast<const uint8_t*>(layer_src ? layer_src[l0 + l] : nullptr);
-        mp.dst[l] = static_cast<uint8_t*>(layer_dst[l0 + l]);
-        mp.repl[l] = static_cast<const uint8_t*>(layer_repl ? layer_repl[l0 + l] : nullptr);
+        mp.src[l] = static_cast<const uint8_t*>(layer_src ? layer_src[lc.layers[l]] : nullptr);
+        mp.dst[l] = static_cast<uint8_t*>(layer_dst[lc.layers[l]]);
+        mp.repl[l] = static_cast<const uint8_t*>(layer_repl ? layer_repl[lc.layers[l]] : nullptr);
     }
 }
 
 /* Launch `fn` over tiles [tile_begin, tile_begin + tile_count) x all layers (chunks of kMaxLayers). */
-leyline_status run_tiles(leyline_plan_s* pl, MoveKernel fn, int smem, int max_ctas_per_sm, int32_t tile_begin,
+leyline_status run_tiles(leyline_plan_s* pl, bool hazard, int smem, int max_ctas_per_sm, int32_t tile_begin,
                          int64_t tile_count, void* const* layer_src, void* const* layer_dst,
                          const void* const* layer_repl, cudaStream_t stream, int* ticket_slot) {
     if (tile_count <= 0) return LEYLINE_OK;
-    const int L = pl->desc.n_layers;
-    for (int l0 = 0; l0 < L; l0 += kMaxLayers) {
-        const int nl = L - l0 < kMaxLayers ? L - l0 : kMaxLayers;
+    for (const LayerChunk& lc : layer_chunks(pl)) {
         if (*ticket_slot >= 32) { g_last_error = "too many launches for one plan"; return LEYLINE_E_UNSUPPORTED; }
+        MoveKernel fn = pick_move(pl, lc.pairing, hazard);
         MoveParams mp;
-        fill_params(pl, mp, tile_begin, tile_count, l0, nl, layer_src, layer_dst, layer_repl, (*ticket_slot)++);
+        fill_params(pl, mp, tile_begin, tile_count, lc, layer_src, layer_dst, layer_repl, (*ticket_slot)++);
         int per_sm = occupancy(reinterpret_cast<const void*>(fn), smem);
         if (max_ctas_per_sm > 0 && per_sm > max_ctas_per_sm) per_sm = max_ctas_per_sm;
         long long grid = (long long)g_dev.sms * per_sm;
@@ -330,12 +352,10 @@ leyline_status run_tiles(leyline_plan_s* pl, MoveKernel fn, int smem, int max_ct
 leyline_status run_rotate(leyline_plan_s* pl, int32_t tile_begin, int64_t tile_count, void* const* layer_ptrs,
                           cudaStream_t stream, int* ticket_slot) {
     if (tile_count <= 0) return LEYLINE_OK;
-    const int L = pl->desc.n_layers;
-    MoveKernel fn = pick_rotate(pl);
-    for (int l0 = 0; l0 < L; l0 += kMaxLayers) {
-        const int nl = L - l0 < kMaxLayers ? L - l0 : kMaxLayers;
+    for (const LayerChunk& lc : layer_chunks(pl)) {
+        MoveKernel fn = pick_rotate(pl, lc.pairing);
         MoveParams mp;
-        fill_params(pl, mp, tile_begin, tile_count, l0, nl, nullptr, layer_ptrs, nullptr, *ticket_slot);
+        fill_params(pl, mp, tile_begin, tile_count, lc, nullptr, layer_ptrs, nullptr, *ticket_slot);
         const int per_sm = occupancy(reinterpret_cast<const void*>(fn), 0);
         long long grid = (long long)g_dev.sms * per_sm * 8;
         if (grid > mp.n_items) grid = mp.n_items;
@@ -350,7 +370,6 @@ leyline_status run_tiles_bulk(leyline_plan_s* pl, bool hazard, int32_t tile_begi
                               void* const* layer_src, void* const* layer_dst, const void* const* layer_repl,
                               cudaStream_t stream, int* ticket_slot) {
     if (tile_count <= 0) return LEYLINE_OK;
-    const int L = pl->desc.n_layers;
     const int row_bytes = (pl->desc.latent_dim + pl->n_heads * pl->desc.rope_dim) * pl->elem_bytes;
     const int stage_bytes = pl->tile_rows * row_bytes;
     /* consumer warps rotate the band in shared memory: 4 keep up with MLA's 1/9 of the bytes, a band that is most of
@@ -359,20 +378,20 @@ leyline_status run_tiles_bulk(leyline_plan_s* pl, bool hazard, int32_t tile_begi
                      ? kBulkConsumerWarps : kBulkWideConsumerWarps;
     if (pl->tuning.consumer_warps > 0) cwarps = pl->tuning.consumer_warps;
     if (cwarps > kBulkMaxConsumerWarps) cwarps = kBulkMaxConsumerWarps;
-    BulkKernel fn = pick_bulk(pl, hazard);
-    cudaFuncAttributes fa;
-    CU(cudaFuncGetAttributes(&fa, reinterpret_cast<const void*>(fn)));
-    int stages = (g_dev.smem_optin - (int)fa.sharedSizeBytes - 1024) / stage_bytes;
-    if (pl->tuning.stages > 0 && stages > pl->tuning.stages) stages = pl->tuning.stages;
-    if (stages > kBulkMaxStages) stages = kBulkMaxStages;
-    if (stages < 3) { g_last_error = "bulk kernel: tile does not fit three shared-memory stages"; return LEYLINE_E_UNSUPPORTED; }
-    const int smem = stages * stage_bytes;
-    CU(cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    for (int l0 = 0; l0 < L; l0 += kMaxLayers) {
-        const int nl = L - l0 < kMaxLayers ? L - l0 : kMaxLayers;
+    for (const LayerChunk& lc : layer_chunks(pl)) {
+        const int nl = (int)lc.layers.size();
+        BulkKernel fn = pick_bulk(pl, lc.pairing, hazard);
+        cudaFuncAttributes fa;
+        CU(cudaFuncGetAttributes(&fa, reinterpret_cast<const void*>(fn)));
+        int stages = (g_dev.smem_optin - (int)fa.sharedSizeBytes - 1024) / stage_bytes;
+        if (pl->tuning.stages > 0 && stages > pl->tuning.stages) stages = pl->tuning.stages;
+        if (stages > kBulkMaxStages) stages = kBulkMaxStages;
+        if (stages < 3) { g_last_error = "bulk kernel: tile does not fit three shared-memory stages"; return LEYLINE_E_UNSUPPORTED; }
+        const int smem = stages * stage_bytes;
+        CU(cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         if (*ticket_slot >= 32) { g_last_error = "too many launches for one plan"; return LEYLINE_E_UNSUPPORTED; }
         MoveParams mp;
-        fill_params(pl, mp, tile_begin, tile_count, l0, nl, layer_src, layer_dst, layer_repl, (*ticket_slot)++);
+        fill_params(pl, mp, tile_begin, tile_count, lc, layer_src, layer_dst, layer_repl, (*ticket_slot)++);
         int group = pl->tuning.layer_group > 0 ? pl->tuning.layer_group : 4;
         if (group > nl) group = nl;
         mp.n_items = (long long)tile_count * ((nl + group - 1) / group);
@@ -449,13 +468,13 @@ extern "C" leyline_status leyline_splice(leyline_plan_t* pl, void* const* layer_
         }
     } else if (inplace) {
         /* a3 under rule M2 ordering, then a4 once every move has landed (stream order) */
-        st = run_tiles(pl, pick_move(pl, true), 0, cps, 0, n_move, layer_src, layer_dst, layer_repl, stream, &slot);
+        st = run_tiles(pl, true, 0, cps, 0, n_move, layer_src, layer_dst, layer_repl, stream, &slot);
         if (st != LEYLINE_OK) return st;
-        st = run_tiles(pl, pick_move(pl, false), 0, cps, (int32_t)n_move, n_ins, layer_src, layer_dst, layer_repl,
+        st = run_tiles(pl, false, 0, cps, (int32_t)n_move, n_ins, layer_src, layer_dst, layer_repl,
                        stream, &slot);
     } else {
         /* a3 + a4 in one launch: fresh pages alias nothing */
-        st = run_tiles(pl, pick_move(pl, false), 0, cps, 0, n_move + n_ins, layer_src, layer_dst, layer_repl, stream,
+        st = run_tiles(pl, false, 0, cps, 0, n_move + n_ins, layer_src, layer_dst, layer_repl, stream,
                        &slot);
     }
     if (st != LEYLINE_OK) return st;
@@ -487,7 +506,7 @@ extern "C" leyline_status leyline_rotate_inplace(leyline_plan_t* pl, void* const
     if (pl->use_bulk)
         st = run_tiles_bulk(pl, false, (int32_t)n_rot, n_ins, layer_ptrs, layer_ptrs, layer_repl, stream, &slot);
     else
-        st = run_tiles(pl, pick_move(pl, false), 0, pl->tuning.ctas_per_sm, (int32_t)n_rot, n_ins, layer_ptrs, layer_ptrs,
+        st = run_tiles(pl, false, 0, pl->tuning.ctas_per_sm, (int32_t)n_rot, n_ins, layer_ptrs, layer_ptrs,
                        layer_repl, stream, &slot);
     if (st != LEYLINE_OK) return st;
     if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_stop), stream));

@@ -38,7 +38,8 @@ class DeviceCache:
         w = self.w
         return B.make_desc(self.n_layers, w.latent_dim, w.rope_dim, w.page_size, w.dtype, w.pairing, w.row_bytes,
                            w.n_slots, w.inv_freq, self.scales if w.dtype == synth.DT_FP8 else None,
-                           rope_heads=w.rope_heads)
+                           rope_heads=w.rope_heads,
+                           layer_pairing=None if w.layer_pairing is None else [w.layer_pairing[l] for l in self.layer_ids])
 
     def nbytes(self):
         return sum(p.numel() for p in self.pools) + sum(r.numel() for r in self.repl)

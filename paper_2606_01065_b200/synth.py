@@ -62,6 +62,7 @@ class Workload:
     page_size: int
     dtype: int = DT_BF16
     pairing: int = NEOX
+    layer_pairing: list = None          # per-layer override of `pairing` ("per layer"), or None
     latent_dim: int = 512
     rope_dim: int = 64                  # rotated elements per head
     rope_heads: int = 1                 # heads in the rotated band (1 = MLA K_pe; kv_heads = full-width K)
@@ -101,6 +102,9 @@ class Workload:
     @property
     def n_requests(self):
         return len(self.seq_lens)
+
+    def pairing_of(self, layer: int) -> int:
+        return self.pairing if self.layer_pairing is None else int(self.layer_pairing[layer])
 
     def free_slots(self) -> np.ndarray:
         """Token-level free slot ids (for ROTATE_ONLY): the slots of the free pages, in free-list order."""

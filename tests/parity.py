@@ -76,11 +76,12 @@ def rotated_rows(w: synth.Workload, bm: O.BatchMap, mode: int):
 
 
 def compare_layer(w: synth.Workload, bm: O.BatchMap, mode: int, old_pool: np.ndarray, gpu_pool: np.ndarray,
-                  repl: np.ndarray, scale: float = 1.0) -> dict:
+                  repl: np.ndarray, scale: float = 1.0, layer: int = 0) -> dict:
     """One layer, whole pool.  old_pool / gpu_pool / repl: flat uint8.  Asserts the bar and returns statistics."""
     stride = w.row_bytes
     E = w.elem_bytes
-    want = O.splice_layer(w.dtype, w.pairing, w.latent_dim, w.rope_dim, stride, w.inv_freq, scale, old_pool, repl, bm,
+    pairing = w.pairing_of(layer)
+    want = O.splice_layer(w.dtype, pairing, w.latent_dim, w.rope_dim, stride, w.inv_freq, scale, old_pool, repl, bm,
                           n_heads=w.rope_heads)
     g = gpu_pool.reshape(-1, stride)
     o = want.reshape(-1, stride)
@@ -107,7 +108,7 @@ def compare_layer(w: synth.Workload, bm: O.BatchMap, mode: int, old_pool: np.nda
             ib = np.ascontiguousarray(old_pool.reshape(-1, stride)[old_s, band0:]).view(np.uint16)
             x = _bf16_val(ib).reshape(len(old_s), w.rope_heads, w.rope_dim)      # pairs live inside a head
             H = w.rope_dim // 2
-            if w.pairing == synth.NEOX:
+            if pairing == synth.NEOX:
                 rho_h = np.sqrt(x[..., :H] ** 2 + x[..., H:] ** 2)
                 rho = np.concatenate([rho_h, rho_h], axis=-1)
             else:

@@ -45,7 +45,7 @@ def run_and_compare(w, mode, check_layers=None, tuning=None, **launch):
     stats = []
     for l in check_layers:
         stats.append(compare_layer(w, bm, mode, old[l], cache.pools[l].cpu().numpy(), cache.repl[l].cpu().numpy(),
-                                   cache.scales[l]))
+                                   cache.scales[l], layer=l))
     plan.close()
     tot = sum(s["rotated_elems"] for s in stats)
     if tot:
@@ -98,6 +98,28 @@ def test_bulk_ring_geometry(mode, stages, layer_group):
                        directives=[(0, 7, 40, 300, 0, 0), (0, 900, 1700, 5, 0, 0), (1, 100, 101, 77, 0, 0)],
                        seed=21, pool_factor=3.0, extra_pages=60).finalize()
     run_and_compare(w, mode, tuning={"kernel": 2, "tile_rows": 16, "stages": stages, "layer_group": layer_group})
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("dtype", [synth.DT_BF16, synth.DT_FP8])
+@pytest.mark.parametrize("mover", MOVERS)
+def test_per_layer_pairing(mode, dtype, mover):
+    """the pairing helper "reads is_neox_style per layer" -- a cache whose layers mix the two conventions
+    (G20): each layer must be rotated with its own pairing, in every mode, in one call."""
+    rng = np.random.default_rng(133)
+    w = tiny_workload(rng, P=16, n_req=3, dtype=dtype)
+    w.n_layers = 5
+    w.layer_pairing = [synth.NEOX, synth.INTERLEAVED, synth.INTERLEAVED, synth.NEOX, synth.INTERLEAVED]
+    w.pairing = synth.NEOX
+    run_and_compare(w, mode, tuning={"kernel": mover})
+
+
+def test_per_layer_pairing_one_convention_only():
+    """All layers interleaved through the per-layer array while the cache-wide flag says NeoX: the array wins."""
+    w = synth.config(1, pool_factor=2.5)
+    w.layer_pairing = [synth.INTERLEAVED, synth.INTERLEAVED]
+    for mode in MODES:
+        run_and_compare(w, mode)
 
 
 @pytest.mark.parametrize("mode", MODES)

@@ -55,6 +55,22 @@ def tiny_workload(rng, P=None, n_req=None, forget=False, dtype=synth.DT_BF16):
     return w.finalize()
 
 
+def test_layer_pairing_is_validated():
+    w = tiny_workload(np.random.default_rng(4), P=4, n_req=1)
+
+    def plan_with(lp):
+        d, keep = B.make_desc(w.n_layers, w.latent_dim, w.rope_dim, w.page_size, w.dtype, w.pairing, w.row_bytes,
+                              w.n_slots, w.inv_freq, layer_pairing=lp)
+        return B.leyline_plan(d, B.FRESH, w.seq_lens, w.pt_offsets, w.pages, w.directives, w.free_pages)
+
+    plan_with([B.NEOX, B.INTERLEAVED]).close()
+    with pytest.raises(B.LeylineError) as ei:
+        plan_with([B.NEOX, 7])
+    assert ei.value.status == B.E_INVALID
+    with pytest.raises(ValueError):
+        plan_with([B.NEOX])
+
+
 def test_prefetch_without_a_device_fails_loudly_and_keeps_the_plan():
     """No CPU fallback: without a CUDA device the upload is refused with LEYLINE_E_CUDA; host queries still work."""
     import torch
