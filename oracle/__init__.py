@@ -20,6 +20,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "leyline_oracle.c")
+_SRC_CDC = os.path.join(_HERE, "cdc_oracle.c")     # discovery side, wrapped by oracle/cdc.py
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 OK, E_INVALID, E_UNSORTED, E_OVERLAP, E_RANGE, E_NOFREE, E_UNSUPPORTED = range(7)
@@ -33,9 +34,10 @@ ELEM_BYTES = {BF16: 2, FP8_E4M3: 1, F64: 8}
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (IEEE semantics: no fast-math, no FMA contraction)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    srcs = [_SRC, _SRC_CDC]
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(f) for f in srcs):
         cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
-               "-o", _LIB, _SRC, "-lm"]
+               "-o", _LIB, *srcs, "-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 

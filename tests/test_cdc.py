@@ -1,0 +1,181 @@
+"""Discovery side: anchored content-defined chunking, chunk content
+hash, registry.  CPU tests pin the oracle (oracle/cdc_oracle.c) to published generator vectors, to the Gear-hash
+window identity, to a list-based re-implementation of the boundary rule and to the property the paper relies on
+(content behind an anchor chunks identically wherever it sits, so a registry hit returns the edit's Delta).
+GPU tests compare the CUDA chunker / registry with the oracle bit for bit.
+"""
+import numpy as np
+import pytest
+
+from helpers import golden
+from oracle import cdc as OC
+
+V = golden("published_hash_vectors.txt")
+M64 = (1 << 64) - 1
+SEED, MIN, MAX, BITS = 0x5EED, 16, 256, 6
+ANCHORS = [100000, 100001, 100002]            # stand-ins for chat-template special tokens (PAPER.md:389 (iii))
+
+
+def random_prompt(rng, n, vocab=50000, anchor_every=None):
+    t = rng.integers(0, vocab, size=n).astype(np.int32)
+    if anchor_every:
+        pos = np.cumsum(rng.integers(anchor_every // 2, anchor_every * 2, size=2 * n // anchor_every + 1))
+        pos = pos[pos < n]
+        t[pos] = rng.choice(ANCHORS, size=len(pos))
+    return t
+
+
+# ----------------------------------------------------------------------------- generators: published vectors
+
+def test_d1_gear_is_splitmix64():
+    assert OC.gear(0, 0) == V["splitmix64_seed0_out1"]
+    assert OC.gear(0, 1) == V["splitmix64_seed0_out2"]
+    assert OC.gear(0, 2) == V["splitmix64_seed0_out3"]
+    # the seed is the generator's starting state: seed = one increment shifts the stream by one
+    assert OC.gear(0x9E3779B97F4A7C15, 0) == V["splitmix64_seed0_out2"]
+
+
+def test_d4_content_hash_is_fnv1a64_over_le_bytes():
+    p = V["fnv1a64_prime"]
+    # "a" then three zero bytes: x ^= 0 leaves x, so the hash is FNV("a") * prime^3
+    assert OC.content_hash([0x61], 0, 1) == (V["fnv1a64_a"] * p ** 3) & M64
+    # "foob" + "ar\0\0" as two little-endian words
+    w0 = int.from_bytes(b"foob", "little")
+    w1 = int.from_bytes(b"ar\0\0", "little")
+    assert OC.content_hash([w0, w1], 0, 2) == (V["fnv1a64_foobar"] * p ** 2) & M64
+    # empty range: the offset basis; sub-ranges hash their own tokens only
+    assert OC.content_hash([5, 6, 7], 1, 1) == V["fnv1a64_offset_basis"]
+    assert OC.content_hash([9, w0, w1, 9], 1, 3) == OC.content_hash([w0, w1], 0, 2)
+
+
+# ----------------------------------------------------------------------------- D2: the Gear window
+
+def test_d2_signature_is_a_64_token_window_sum():
+    """h_i = (h_{i-1} << 1) + G(t_i) mod 2^64  ==  sum_{j < 64} G(t_{i-j}) << j, cut at the last anchor / sequence start
+    (bit k of h_i depends on the last k+1 tokens only: the Gear hash's defining property, Xia et al.)."""
+    rng = np.random.default_rng(0)
+    t = random_prompt(rng, 700, anchor_every=90)
+    so = [0, 300, 300, 700]                      # an empty sequence in the middle
+    sig = OC.signature(SEED, t, so, ANCHORS)
+    for i in range(len(t)):
+        seq_start = 0 if i < 300 else 300
+        acc, j = 0, 0
+        while j < 64 and i - j >= seq_start and not (j > 0 and int(t[i - j]) in ANCHORS):
+            acc += OC.gear(SEED, int(t[i - j])) << j
+            j += 1
+        assert int(sig[i]) == acc & M64, i
+
+
+# ----------------------------------------------------------------------------- D3: the boundary rule, brute force
+
+def chunk_by_lists(tokens, seq_offsets, anchors, seed, mn, mx, bits):
+    """Independent restatement of D3 with Python lists and the window-sum form of the signature."""
+    out = []
+    for s in range(len(seq_offsets) - 1):
+        seq = [int(x) for x in tokens[seq_offsets[s]:seq_offsets[s + 1]]]
+        cur, run = [], []                        # cur: tokens of the open chunk; run: tokens since the last anchor
+        for k, tok in enumerate(seq):
+            cur.append(tok)
+            run.append(tok)
+            h = sum(OC.gear(seed, x) << j for j, x in enumerate(reversed(run[-64:]))) & M64
+            if tok in anchors:
+                kind = OC.KIND_ANCHOR
+            elif k == len(seq) - 1:
+                kind = OC.KIND_SEQ_END
+            elif len(cur) == mx:
+                kind = OC.KIND_MAX
+            elif len(cur) >= mn and (bits == 0 or h >> (64 - bits) == 0):
+                kind = OC.KIND_HASH
+            else:
+                continue
+            if kind == OC.KIND_ANCHOR:
+                run = []
+            out.append((seq_offsets[s] + k + 1, tuple(cur), kind))
+            cur = []
+    return out
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_d3_boundaries_match_list_restatement(seed):
+    rng = np.random.default_rng(seed)
+    n = int(rng.integers(1, 1500))
+    t = random_prompt(rng, n, vocab=int(rng.choice([3, 50, 50000])), anchor_every=int(rng.choice([0, 40, 200])) or None)
+    cuts = np.sort(rng.integers(0, n + 1, size=int(rng.integers(0, 4))))
+    so = [0, *[int(c) for c in cuts], n]
+    mn, mx, bits = int(rng.choice([1, 4, 16])), int(rng.choice([16, 64, 256])), int(rng.choice([0, 2, 4, 6]))
+    end, hsh, kind = OC.chunk(SEED + seed, mn, mx, bits, t, so, ANCHORS)
+    want = chunk_by_lists(t, so, ANCHORS, SEED + seed, mn, mx, bits)
+    assert [int(e) for e in end] == [w[0] for w in want]
+    assert [int(k) for k in kind] == [w[2] for w in want]
+    for h, w in zip(hsh, want):
+        assert int(h) == OC.content_hash(list(w[1]), 0, len(w[1]))
+
+
+def test_d3_invariants_and_chunk_length_law():
+    rng = np.random.default_rng(11)
+    n = 400000
+    t = random_prompt(rng, n)
+    end, hsh, kind = OC.chunk(SEED, MIN, MAX, BITS, t, None, ANCHORS)
+    start = np.concatenate([[0], end[:-1]])
+    ln = end - start
+    assert end[-1] == n and (ln >= 1).all() and (ln <= MAX).all()               # chunks tile the sequence
+    assert (ln[kind == OC.KIND_HASH] >= MIN).all() and (ln[kind == OC.KIND_MAX] == MAX).all()
+    assert (kind[:-1] != OC.KIND_SEQ_END).all() and kind[-1] == OC.KIND_SEQ_END
+    # random tokens: past min_size every position is a boundary with probability 2^-bits, truncated at max_size:
+    # E[len] = (MIN - 1) + sum_{k=1..MAX-MIN+1} P(len >= MIN-1+k), a geometric law
+    q = 1.0 - 2.0 ** -BITS
+    expect = (MIN - 1) + sum(q ** (k - 1) for k in range(1, MAX - MIN + 2))
+    assert abs(ln[:-1].mean() - expect) / expect < 0.03, (ln.mean(), expect)
+    assert abs((kind == OC.KIND_MAX).mean() - q ** (MAX - MIN + 1)) < 0.01
+
+
+# ----------------------------------------------------------------------------- the property the paper relies on
+
+def build_and_replay(rng, edit_at_turn=2, n_turns=8, turn_len=700, stub_len=11):
+    """BUILD prompt = turns separated by anchor tokens; REPLAY prompt = the same with one turn's body replaced by a
+    short stub (a summarisation edit).  Returns (build, replay, edit_start, edit_end, stub_len)."""
+    turns = [rng.integers(0, 50000, size=turn_len + int(rng.integers(0, 50))).astype(np.int32) for _ in range(n_turns)]
+    sep = np.array([ANCHORS[0]], np.int32)
+    build = np.concatenate([np.concatenate([tr, sep]) for tr in turns])
+    s = sum(len(tr) + 1 for tr in turns[:edit_at_turn])
+    e = s + len(turns[edit_at_turn])
+    stub = rng.integers(0, 50000, size=stub_len).astype(np.int32)
+    replay = np.concatenate([build[:s], stub, build[e:]])
+    return build, replay, s, e, stub_len
+
+
+def test_anchored_chunks_behind_an_edit_are_found_with_the_edits_delta():
+    """PAPER.md:389 (iii), :397: with the anchored chunker every chunk that lies wholly behind the edited turn is
+    re-discovered in the edited prompt, at its old position + Delta, Delta = |R| - |span|."""
+    rng = np.random.default_rng(5)
+    build, replay, s, e, r = build_and_replay(rng)
+    delta = r - (e - s)
+    b_end, b_hash, _ = OC.chunk(SEED, MIN, MAX, BITS, build, None, ANCHORS)
+    r_end, r_hash, _ = OC.chunk(SEED, MIN, MAX, BITS, replay, None, ANCHORS)
+    b_start = np.concatenate([[0], b_end[:-1]])
+    r_start = np.concatenate([[0], r_end[:-1]])
+    reg = OC.Registry()
+    reg.insert(b_hash, b_start)
+    src = reg.lookup(r_hash)
+    behind = r_start >= s + r + 1                     # chunks after the edited turn's closing anchor
+    assert behind.sum() > 20
+    assert (src[behind] >= 0).all()                   # every one of them is found ...
+    assert ((r_start[behind] - src[behind]) == delta).all()   # ... at exactly the directive's Delta
+    before = r_end <= s
+    assert ((r_start[before] - src[before]) == 0).all()       # the untouched prefix maps to itself
+
+
+def test_unanchored_chunker_resynchronises_only_after_a_window():
+    """Without anchors (the paper's 'legacy purely-Gear-hash chunker') boundaries behind an edit depend
+    on where the previous boundary fell (min / max sizes), so the first chunks behind the edit may differ; content
+    64 tokens past a COMMON boundary chunks identically again."""
+    rng = np.random.default_rng(6)
+    build, replay, s, e, r = build_and_replay(rng)
+    delta = r - (e - s)
+    b_end, b_hash, _ = OC.chunk(SEED, MIN, MAX, BITS, build, None, [])
+    r_end, r_hash, _ = OC.chunk(SEED, MIN, MAX, BITS, replay, None, [])
+    common = np.intersect1d(b_end[b_end > e] + delta, r_end[r_end > s + r])
+    common = common[common >= s + r + 64]              # the window no longer sees the edit: signatures agree from here
+    assert len(common) > 0                             # the two chunkings do meet again ...
+    first = common[0]
+    assert set(r_end[r_end >= first]) == set(b_end[b_end >= first - delta] + delta)   # ... and stay together
