@@ -58,6 +58,11 @@ class Tuning(C.Structure):
                 ("stages", C.c_int32), ("layer_group", C.c_int32), ("consumer_warps", C.c_int32)]
 
 
+class CdcParams(C.Structure):
+    _fields_ = [("seed", C.c_uint64), ("min_size", C.c_int32), ("max_size", C.c_int32), ("mask_bits", C.c_int32),
+                ("reserved_", C.c_int32)]
+
+
 class LeylineError(RuntimeError):
     def __init__(self, status: int, where: str, detail: str = ""):
         self.status = status
@@ -99,6 +104,15 @@ def _load() -> C.CDLL:
     L.leyline_get_tuning.restype = C.c_int
     L.leyline_get_tuning.argtypes = [C.POINTER(Tuning)]
     L.leyline_version.restype = C.c_char_p
+    # discovery side (include/leyline_cdc.h)
+    L.leyline_cdc_chunk.restype = C.c_int
+    L.leyline_cdc_chunk.argtypes = [C.POINTER(CdcParams), vp, i64, vp, i32, vp, i32, vp, vp, vp, i64, vp, vp]
+    L.leyline_registry_clear.restype = C.c_int
+    L.leyline_registry_clear.argtypes = [vp, vp, i64, vp]
+    L.leyline_registry_insert.restype = C.c_int
+    L.leyline_registry_insert.argtypes = [vp, vp, i64, vp, vp, i64, vp, vp]
+    L.leyline_registry_lookup.restype = C.c_int
+    L.leyline_registry_lookup.argtypes = [vp, vp, i64, vp, i64, vp, vp]
     return L
 
 
@@ -302,3 +316,33 @@ def leyline_rotate_inplace(plan: Plan, layers, layer_repl=None, slot_idx_out=Non
     c, _k3 = _ptr_array(layer_repl, n, "layer_repl")
     st = _lib.leyline_rotate_inplace(plan._h, a, c, _dev_ptr(slot_idx_out), _stream_handle(stream))
     _check(st, "leyline_rotate_inplace")
+
+
+# ----------------------------------------------------------------------------- discovery side (leyline_cdc.h)
+
+CDC_HASH, CDC_ANCHOR, CDC_MAX, CDC_SEQ_END = range(4)
+
+
+def leyline_cdc_chunk(params: CdcParams, tokens, n_tokens: int, seq_offsets, n_seqs: int, anchor_ids, n_anchor_ids: int,
+                      chunk_end, chunk_hash, chunk_kind, capacity: int, n_chunks, stream=None):
+    """leyline_cdc.h: leyline_cdc_chunk.  Every array argument is a device tensor (or raw device pointer, or None
+    where the header allows NULL); outputs are written in place."""
+    st = _lib.leyline_cdc_chunk(C.byref(params), _dev_ptr(tokens), n_tokens, _dev_ptr(seq_offsets), n_seqs,
+                                _dev_ptr(anchor_ids), n_anchor_ids, _dev_ptr(chunk_end), _dev_ptr(chunk_hash),
+                                _dev_ptr(chunk_kind), capacity, _dev_ptr(n_chunks), _stream_handle(stream))
+    _check(st, "leyline_cdc_chunk")
+
+
+def leyline_registry_clear(keys, vals, capacity: int, stream=None):
+    _check(_lib.leyline_registry_clear(_dev_ptr(keys), _dev_ptr(vals), capacity, _stream_handle(stream)),
+           "leyline_registry_clear")
+
+
+def leyline_registry_insert(keys, vals, capacity: int, hashes, values, n: int, n_dropped=None, stream=None):
+    _check(_lib.leyline_registry_insert(_dev_ptr(keys), _dev_ptr(vals), capacity, _dev_ptr(hashes), _dev_ptr(values), n,
+                                        _dev_ptr(n_dropped), _stream_handle(stream)), "leyline_registry_insert")
+
+
+def leyline_registry_lookup(keys, vals, capacity: int, hashes, n: int, out, stream=None):
+    _check(_lib.leyline_registry_lookup(_dev_ptr(keys), _dev_ptr(vals), capacity, _dev_ptr(hashes), n, _dev_ptr(out),
+                                        _stream_handle(stream)), "leyline_registry_lookup")

@@ -179,3 +179,139 @@ def test_unanchored_chunker_resynchronises_only_after_a_window():
     assert len(common) > 0                             # the two chunkings do meet again ...
     first = common[0]
     assert set(r_end[r_end >= first]) == set(b_end[b_end >= first - delta] + delta)   # ... and stay together
+
+
+# ----------------------------------------------------------------------------- GPU parity (bit-exact: integer work)
+
+def gpu_chunk(tokens, seq_offsets, anchors, seed, mn, mx, bits, capacity=None):
+    import torch
+    from paper_2606_01065_b200 import binding as B
+    dev = torch.device("cuda:0")
+    n = len(tokens)
+    so = [0, n] if seq_offsets is None else seq_offsets
+    t = torch.from_numpy(np.ascontiguousarray(tokens, np.int32)).to(dev)
+    off = torch.tensor(so, dtype=torch.int64, device=dev)
+    an = torch.tensor(sorted(anchors), dtype=torch.int32, device=dev) if anchors else None
+    cap = n if capacity is None else capacity
+    end = torch.full((max(cap, 1),), -7, dtype=torch.int64, device=dev)
+    hsh = torch.zeros(max(cap, 1), dtype=torch.int64, device=dev)        # uint64 bit patterns
+    kind = torch.full((max(cap, 1),), -7, dtype=torch.int32, device=dev)
+    cnt = torch.full((1,), -7, dtype=torch.int64, device=dev)
+    B.leyline_cdc_chunk(B.CdcParams(seed, mn, mx, bits, 0), t, n, off, len(so) - 1, an, len(anchors) if anchors else 0,
+                        end, hsh, kind, cap, cnt)
+    torch.cuda.synchronize()
+    c = int(cnt.item())
+    m = min(c, cap)
+    return c, end.cpu().numpy()[:m], hsh.cpu().numpy().view(np.uint64)[:m], kind.cpu().numpy()[:m], (end, kind)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed", range(8))
+def test_gpu_chunker_matches_oracle_small(seed):
+    rng = np.random.default_rng(100 + seed)
+    n = int(rng.integers(1, 6000))
+    t = random_prompt(rng, n, vocab=int(rng.choice([3, 50, 50000])), anchor_every=int(rng.choice([0, 40, 200])) or None)
+    cuts = np.sort(rng.integers(0, n + 1, size=int(rng.integers(0, 5))))
+    so = [0, *[int(c) for c in cuts], n]
+    mn, mx, bits = int(rng.choice([1, 4, 16])), int(rng.choice([16, 64, 256])), int(rng.choice([0, 2, 4, 6]))
+    c, end, hsh, kind, _ = gpu_chunk(t, so, ANCHORS, SEED + seed, mn, mx, bits)
+    o_end, o_hash, o_kind = OC.chunk(SEED + seed, mn, mx, bits, t, so, ANCHORS)
+    assert c == len(o_end)
+    np.testing.assert_array_equal(end, o_end)
+    np.testing.assert_array_equal(kind, o_kind)
+    np.testing.assert_array_equal(hsh, o_hash)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("anchored", [True, False])
+def test_gpu_chunker_matches_oracle_long_batch(anchored):
+    """16 sessions x ~17K-token prompts (the paper's microbenchmark shape) in one call, plus a
+    128K-token sequence; several compaction blocks, a ragged tail, empty sequences."""
+    rng = np.random.default_rng(17)
+    lens = [int(rng.integers(16000, 18000)) for _ in range(16)] + [0, 131072, 0, 1]
+    t = random_prompt(rng, sum(lens), anchor_every=600 if anchored else None)
+    so = [0, *np.cumsum(lens).tolist()]
+    anchors = ANCHORS if anchored else []
+    c, end, hsh, kind, _ = gpu_chunk(t, so, anchors, SEED, MIN, MAX, BITS)
+    o_end, o_hash, o_kind = OC.chunk(SEED, MIN, MAX, BITS, t, so, anchors)
+    assert c == len(o_end)
+    np.testing.assert_array_equal(end, o_end)
+    np.testing.assert_array_equal(kind, o_kind)
+    np.testing.assert_array_equal(hsh, o_hash)
+
+
+@pytest.mark.gpu
+def test_gpu_chunker_edge_cases():
+    import torch
+    from paper_2606_01065_b200 import binding as B
+    # empty input: zero chunks, nothing written
+    c, end, hsh, kind, _ = gpu_chunk(np.zeros(0, np.int32), [0, 0], ANCHORS, SEED, MIN, MAX, BITS)
+    assert c == 0
+    # every token an anchor: one chunk per token
+    t = np.full(300, ANCHORS[1], np.int32)
+    c, end, hsh, kind, _ = gpu_chunk(t, None, ANCHORS, SEED, MIN, MAX, BITS)
+    assert c == 300 and (end == np.arange(1, 301)).all() and (kind[:-1] == B.CDC_ANCHOR).all()
+    # one repeated token, mask never satisfied or always satisfied: max-size / min-size chunks
+    t = np.full(1000, 7, np.int32)
+    c, end, hsh, kind, _ = gpu_chunk(t, None, [], SEED, 4, 64, 0)
+    o_end, o_hash, o_kind = OC.chunk(SEED, 4, 64, 0, t, None, [])
+    np.testing.assert_array_equal(end, o_end)
+    assert (np.diff(np.concatenate([[0], end]))[:-1] == 4).all()
+    # capacity smaller than the number of chunks: the count is still reported, only `capacity` entries are written
+    rng = np.random.default_rng(3)
+    t = random_prompt(rng, 20000)
+    full_c, full_end, full_hash, full_kind, _ = gpu_chunk(t, None, [], SEED, MIN, MAX, BITS)
+    c, end, hsh, kind, (end_t, kind_t) = gpu_chunk(t, None, [], SEED, MIN, MAX, BITS, capacity=10)
+    assert c == full_c and len(end) == 10
+    np.testing.assert_array_equal(end, full_end[:10])
+    np.testing.assert_array_equal(hsh, full_hash[:10])
+    # bad arguments are refused before any launch
+    with pytest.raises(B.LeylineError):
+        gpu_chunk(t, None, [], SEED, 0, MAX, BITS)
+    with pytest.raises(B.LeylineError):
+        gpu_chunk(t, None, [], SEED, 32, 16, BITS)
+
+
+@pytest.mark.gpu
+def test_gpu_registry_and_discovery_returns_the_edits_delta():
+    """BUILD registers its chunks, REPLAY looks its own up: every chunk behind the edited turn is found at
+    old position + Delta -- on the device, against the oracle's registry (D5: smallest value wins)."""
+    import torch
+    from paper_2606_01065_b200 import binding as B
+    rng = np.random.default_rng(5)
+    build, replay, s, e, r = build_and_replay(rng)
+    delta = r - (e - s)
+    dev = torch.device("cuda:0")
+    cap = 1 << 12
+    keys = torch.empty(cap, dtype=torch.int64, device=dev)
+    vals = torch.empty(cap, dtype=torch.int64, device=dev)
+    B.leyline_registry_clear(keys, vals, cap)
+    bc, b_end, b_hash, _, _ = gpu_chunk(build, None, ANCHORS, SEED, MIN, MAX, BITS)
+    rc, r_end, r_hash, _, _ = gpu_chunk(replay, None, ANCHORS, SEED, MIN, MAX, BITS)
+    b_start = np.concatenate([[0], b_end[:-1]])
+    r_start = np.concatenate([[0], r_end[:-1]])
+    # duplicates on purpose: the build prompt registered twice, the second time with larger values
+    ins_h = np.concatenate([b_hash, b_hash]).view(np.int64)
+    ins_v = np.concatenate([b_start + 100000, b_start]).astype(np.int64)
+    dropped = torch.full((1,), -1, dtype=torch.int64, device=dev)
+    B.leyline_registry_insert(keys, vals, cap, torch.from_numpy(ins_h).to(dev), torch.from_numpy(ins_v).to(dev), len(ins_h),
+                              dropped)
+    out = torch.empty(rc, dtype=torch.int64, device=dev)
+    B.leyline_registry_lookup(keys, vals, cap, torch.from_numpy(r_hash.view(np.int64).copy()).to(dev), rc, out)
+    torch.cuda.synchronize()
+    assert int(dropped.item()) == 0
+    reg = OC.Registry()
+    reg.insert(np.concatenate([b_hash, b_hash]), ins_v)
+    src = out.cpu().numpy()
+    np.testing.assert_array_equal(src, reg.lookup(r_hash))
+    behind = r_start >= s + r + 1
+    assert behind.sum() > 20 and (src[behind] >= 0).all()
+    assert ((r_start[behind] - src[behind]) == delta).all()
+    # a table that is too small reports what it could not store
+    tiny_k = torch.empty(8, dtype=torch.int64, device=dev)
+    tiny_v = torch.empty(8, dtype=torch.int64, device=dev)
+    B.leyline_registry_clear(tiny_k, tiny_v, 8)
+    B.leyline_registry_insert(tiny_k, tiny_v, 8, torch.from_numpy(b_hash.view(np.int64).copy()).to(dev),
+                              torch.from_numpy(b_start.astype(np.int64)).to(dev), bc, dropped)
+    torch.cuda.synchronize()
+    assert int(dropped.item()) == len(set(b_hash.tolist())) - 8

@@ -21,10 +21,12 @@ MODES = [B.FRESH, B.INPLACE_MOVE, B.ROTATE_ONLY]
 
 
 def test_abi_exports_every_declared_symbol():
-    text = open(os.path.join(ROOT, "include", "leyline.h")).read()
+    inc = os.path.join(ROOT, "include")
+    text = "".join(open(os.path.join(inc, f)).read() for f in sorted(os.listdir(inc)) if f.endswith(".h"))
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     names = set(re.findall(r"\b(leyline_[a-z_0-9]+)\s*\(", text))
-    assert {"leyline_plan", "leyline_splice", "leyline_rotate_inplace", "leyline_plan_destroy"} <= names
+    assert {"leyline_plan", "leyline_splice", "leyline_rotate_inplace", "leyline_plan_destroy", "leyline_plan_prefetch",
+            "leyline_cdc_chunk", "leyline_registry_insert", "leyline_registry_lookup"} <= names
     lib = ctypes.CDLL(B.LIB_PATH)
     for n in sorted(names):
         assert hasattr(lib, n), f"{n} declared in leyline.h but not exported"
