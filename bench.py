@@ -203,6 +203,51 @@ def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1):
             "mover": int(info.mover), "tile_rows": int(info.tile_rows)}
 
 
+def time_discovery(dev, n_sessions: int = 16, prompt_len: int = 17000, reps: int = 20):
+    """Supplementary line: the discovery side (leyline_cdc_chunk) on the shape of the paper's
+    microbenchmark -- 16 sessions x ~17 K-token prompts, anchors every ~600 tokens -- against
+    the oracle's sequential chunker on the host."""
+    import torch
+    from oracle import cdc as OC
+    from paper_2606_01065_b200 import binding as B
+    rng = np.random.default_rng(17)
+    n = n_sessions * prompt_len
+    anchors = [100000, 100001, 100002]
+    t = rng.integers(0, 50000, size=n).astype(np.int32)
+    pos = np.cumsum(rng.integers(300, 1200, size=2 * n // 600))
+    t[pos[pos < n]] = anchors[0]
+    so = [i * prompt_len for i in range(n_sessions + 1)]
+    td = torch.from_numpy(t).to(dev)
+    off = torch.tensor(so, dtype=torch.int64, device=dev)
+    an = torch.tensor(anchors, dtype=torch.int32, device=dev)
+    end = torch.empty(n, dtype=torch.int64, device=dev)
+    hsh = torch.empty(n, dtype=torch.int64, device=dev)
+    kind = torch.empty(n, dtype=torch.int32, device=dev)
+    cnt = torch.zeros(1, dtype=torch.int64, device=dev)
+    prm = B.CdcParams(0x5EED, 16, 256, 6, 0)
+
+    def run():
+        B.leyline_cdc_chunk(prm, td, n, off, n_sessions, an, len(anchors), end, hsh, kind, n, cnt)
+
+    for _ in range(3):
+        run()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        run()
+    e1.record()
+    torch.cuda.synchronize()
+    gpu_ms = e0.elapsed_time(e1) / reps
+    t0 = time.perf_counter()
+    o_end, o_hash, o_kind = OC.chunk(0x5EED, 16, 256, 6, t, so, anchors)
+    cpu_ms = (time.perf_counter() - t0) * 1e3
+    c = int(cnt.item())
+    same = c == len(o_end) and bool((end[:c].cpu().numpy() == o_end).all()) and \
+        bool((hsh[:c].cpu().numpy().view(np.uint64) == o_hash).all())
+    return {"tokens": n, "chunks": c, "gpu_ms": gpu_ms, "gpu_Mtok_per_s": n / gpu_ms / 1e3, "oracle_ms": cpu_ms,
+            "oracle_Mtok_per_s": n / cpu_ms / 1e3, "matches_oracle": same}
+
+
 def cpu_baseline(pools, repls, scales, w, mode: int, bytes_per_layer: int, budget_s: float = 15.0, max_layers: int = 1 << 30):
     """The oracle as it stands (one thread, explicit per-token loops, fp64 libm trig) on whole layers of the same
     workload, on this host, until about `budget_s` seconds of oracle time are spent (a bounded sample: whole layers,
@@ -342,6 +387,7 @@ def run_ours(args):
                 extras[name] = {"ms_per_step": x["ms_per_step"], "GBps": x["bytes"] / x["ms_per_step"] / 1e6,
                                 "kernel_GBps": x["bytes"] / x["kernel_ms"] / 1e6, "bytes": x["bytes"]}
             cache.w = w
+            extras["discovery_cdc"] = time_discovery(cache.device)
             out["extras"] = extras
         if not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(lambda l: cache.pools[l].cpu().numpy(), lambda l: cache.repl[l].cpu().numpy(),
