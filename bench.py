@@ -248,6 +248,29 @@ def time_discovery(dev, n_sessions: int = 16, prompt_len: int = 17000, reps: int
             "oracle_Mtok_per_s": n / cpu_ms / 1e3, "matches_oracle": same}
 
 
+def cpu_baseline_all_cores(pools, repls, scales, w, mode: int, bytes_per_layer: int, n_layers: int = 48):
+    """the same oracle with a thread per layer (layers are independent given the plan; the C
+    oracle runs outside the GIL), on all host cores.  A reported baseline, not a target."""
+    import oracle as O
+    from concurrent.futures import ThreadPoolExecutor
+    cores = os.cpu_count() or 1
+    n_layers = min(n_layers, w.n_layers)
+    free = w.free_slots() if mode == O.ROTATE_ONLY else w.free_pages
+    inputs = [(pools(l), repls(l)) for l in range(n_layers)]
+    t0 = time.perf_counter()
+    bm = O.plan_batch(mode, w.page_size, w.seq_lens, w.pt_offsets, w.pages, w.directives, free)
+
+    def one(l):
+        O.splice_layer(w.dtype, w.pairing_of(l), w.latent_dim, w.rope_dim, w.row_bytes, w.inv_freq, scales[l], inputs[l][0],
+                       inputs[l][1], bm, n_heads=w.rope_heads)
+
+    with ThreadPoolExecutor(max_workers=cores) as ex:
+        list(ex.map(one, range(n_layers)))
+    dt = time.perf_counter() - t0
+    return {"value": n_layers * bytes_per_layer / dt / 1e9, "unit": UNIT, "cores": min(cores, n_layers), "kind": "oracle, one thread per layer",
+            "sample": f"{n_layers} of {w.n_layers} layers of {w.name}, {dt:.1f} s", "host_cpus": cores}
+
+
 def cpu_baseline(pools, repls, scales, w, mode: int, bytes_per_layer: int, budget_s: float = 15.0, max_layers: int = 1 << 30):
     """The oracle as it stands (one thread, explicit per-token loops, fp64 libm trig) on whole layers of the same
     workload, on this host, until about `budget_s` seconds of oracle time are spent (a bounded sample: whole layers,
@@ -392,6 +415,9 @@ def run_ours(args):
         if not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(lambda l: cache.pools[l].cpu().numpy(), lambda l: cache.repl[l].cpu().numpy(),
                                                cache.scales, w, mode, bytes_per_layer)
+            out["cpu_baseline_all_cores"] = cpu_baseline_all_cores(lambda l: cache.pools[l].cpu().numpy(),
+                                                                   lambda l: cache.repl[l].cpu().numpy(), cache.scales, w, mode,
+                                                                   bytes_per_layer)
         if not args.no_e2e and mode == B.FRESH:
             try:
                 out["e2e"] = run_e2e(cache, w, steps=min(args.steps, 3))

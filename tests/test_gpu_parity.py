@@ -238,3 +238,17 @@ def test_full_width_small_pages(mode, page):
 def test_full_width_full_size(cfg, mode):
     w = synth.config(cfg, pool_factor=2.0)
     run_and_compare(w, mode, check_layers=[0, w.n_layers - 1])
+
+
+@pytest.mark.parametrize("mode,mover", [(O.FRESH, 1), (O.FRESH, 2), (O.INPLACE_MOVE, 1), (O.INPLACE_MOVE, 2), (O.ROTATE_ONLY, 0)])
+def test_byte_offsets_beyond_2_to_the_31(mode, mover):
+    """SURVEY.md section 7 "64-bit addressing" (G17): slot ids fit int32, byte offsets do not.  One layer whose pool is
+    4.6 GiB (4 M slots x 1152 B) with the request's pages scattered over all of it by the seeded permutation, so about
+    half of the rows every kernel touches sit beyond byte 2^31 and a quarter beyond 2^32.  Whole-pool comparison."""
+    w = synth.Workload("big_pool", 1, [8192 + 37], 64, inv_freq=synth.yarn_inv_freq(),
+                       directives=[(0, 700, 1900, 333, 0, 0), (0, 4000, 4001, 0, 0, 0), (0, 6000, 6000, 77, 0, 0)],
+                       seed=31, pool_factor=1.0, extra_pages=(1 << 16) - 129).finalize()
+    assert w.layer_bytes > (1 << 32)
+    slots = w.pages.astype(np.int64) * 64
+    assert (slots * w.row_bytes > (1 << 31)).mean() > 0.3 and (slots * w.row_bytes > (1 << 32)).any()
+    run_and_compare(w, mode, tuning={"kernel": mover})
