@@ -206,7 +206,10 @@ leyline_status leyline_plan_trig_table(const leyline_plan_t* plan, float* out);
 /*
  * leyline_splice -- execute a FRESH or INPLACE_MOVE plan on `cuda_stream` (steps a2-a4).
  *
- *   layer_src   HOST array of n_layers DEVICE pointers to the pools read (16-byte aligned).
+ *   layer_src   HOST array of n_layers DEVICE pointers to the pools read (16-byte aligned).  "Device pointer" means any
+ *               address the device can dereference: device memory, or pinned (page-locked, mapped) host memory --
+ *               a host-resident cache is then spliced over PCIe by the same kernels, moving only the rows the plan
+ *               touches.
  *   layer_dst   HOST array of n_layers DEVICE pointers to the pools written.  May equal layer_src (fresh pages of
  *               the same pool); MUST equal it for INPLACE_MOVE.
  *   layer_repl  HOST array of n_layers DEVICE pointers to the replacement KV rows, [rows x row_stride_bytes] per

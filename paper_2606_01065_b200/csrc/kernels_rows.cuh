@@ -97,7 +97,15 @@ __global__ void __launch_bounds__(kThreads, 3) k_move_rows(const __grid_constant
         if (t.trig >= 0) band = rotate_band_chunk<DT, PAIRING>(band, bj, NB, p.trig + (int64_t)t.trig * 2 * p.H, p.H, has_band);
 
         if (HAZARD) {
-            /* rule M2: publish "loaded", then wait for the tiles whose source rows this tile overwrites */
+            /* rule M2: publish "loaded", then wait for the tiles whose source rows this tile overwrites.
+             * "Loaded" must mean the data has ARRIVED: the fence below orders the accesses, but when the pool sits in
+             * pinned host memory a posted PCIe write may pass an earlier read request, so every loaded register is
+             * consumed first (the xor chain cannot issue before the loads have returned). */
+            uint32_t landed = (uint32_t)(band.x ^ band.y ^ band.z ^ band.w);
+#pragma unroll
+            for (int k = 0; k < kLatPerThread; ++k)
+                if (tid + k * kThreads < n_lat) landed ^= (uint32_t)(lat[k].x ^ lat[k].y ^ lat[k].z ^ lat[k].w);
+            asm volatile("" :: "r"(landed) : "memory");
             __threadfence();
             __syncthreads();
             int32_t* flags = p.flags + p.layer0 + layer;

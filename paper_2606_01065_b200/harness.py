@@ -14,15 +14,17 @@ class DeviceCache:
     """Per-layer pools ``[n_slots * row_bytes]`` uint8 on `device`, plus per-layer replacement rows.
     `layers` restricts which layers of the workload are materialised (layers are independent buffers)."""
 
-    def __init__(self, w: synth.Workload, device="cuda:0", layers=None, fill=True, with_dst=False):
+    def __init__(self, w: synth.Workload, device="cuda:0", layers=None, fill=True, with_dst=False, host_resident=False):
         self.w = w
         self.device = torch.device(device)
         self.layer_ids = list(range(w.n_layers)) if layers is None else list(layers)
         self.pools, self.repl, self.scales = [], [], []
+        # host_resident: pools and replacement rows in pinned host memory; the library takes those pointers as they are
+        where = dict(device="cpu", pin_memory=True) if host_resident else dict(device=self.device)
         for l in self.layer_ids:
-            buf = torch.empty(w.layer_bytes, dtype=torch.uint8, device=self.device)
+            buf = torch.empty(w.layer_bytes, dtype=torch.uint8, **where)
             scale = synth.fill_layer_(buf, w, l) if fill else 1.0
-            rp = torch.empty(max(w.n_repl_rows, 1) * w.row_bytes, dtype=torch.uint8, device=self.device)
+            rp = torch.empty(max(w.n_repl_rows, 1) * w.row_bytes, dtype=torch.uint8, **where)
             if fill:
                 synth.fill_repl_(rp[: w.n_repl_rows * w.row_bytes], w, l, scale)
             self.pools.append(buf)

@@ -20,15 +20,16 @@ MODE_NAME = {O.FRESH: "fresh", O.INPLACE_MOVE: "inplace", O.ROTATE_ONLY: "rotate
 MOVERS = [1, 2]
 
 
-def run_and_compare(w, mode, check_layers=None, tuning=None, **launch):
+def run_and_compare(w, mode, check_layers=None, tuning=None, host_resident=False, **launch):
     from paper_2606_01065_b200 import binding as B
     from paper_2606_01065_b200 import harness
     if tuning:
         B.leyline_set_tuning(**tuning)
     try:
-        cache = harness.DeviceCache(w, "cuda:0")
+        cache = harness.DeviceCache(w, "cuda:0", host_resident=host_resident)
         check_layers = list(range(w.n_layers)) if check_layers is None else check_layers
-        old = {l: cache.pools[l].cpu().numpy() for l in check_layers}
+        # a pinned host pool IS a cpu tensor: .cpu() would alias it, and the splice then overwrites the snapshot
+        old = {l: (cache.pools[l].clone() if host_resident else cache.pools[l].cpu()).numpy() for l in check_layers}
         plan, pt, idx = harness.run_workload(cache, mode, **launch)
         torch.cuda.synchronize()
     finally:
@@ -252,3 +253,15 @@ def test_byte_offsets_beyond_2_to_the_31(mode, mover):
     slots = w.pages.astype(np.int64) * 64
     assert (slots * w.row_bytes > (1 << 31)).mean() > 0.3 and (slots * w.row_bytes > (1 << 32)).any()
     run_and_compare(w, mode, tuning={"kernel": mover})
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("mover", MOVERS)
+def test_host_resident_cache_is_spliced_over_pcie(mode, mover):
+    """include/leyline.h: layer pointers may be pinned host memory.  The same kernels gather from and scatter to the
+    host-resident pools (bench.py's e2e leg); results and untouched bytes must match the oracle exactly as on device."""
+    rng = np.random.default_rng(909)
+    w = tiny_workload(rng, P=16, n_req=3)
+    run_and_compare(w, mode, tuning={"kernel": mover}, host_resident=True)
+    if mode != O.INPLACE_MOVE:
+        run_and_compare(synth.config(1, pool_factor=2.5), mode, tuning={"kernel": mover}, host_resident=True)
