@@ -265,3 +265,45 @@ def test_host_resident_cache_is_spliced_over_pcie(mode, mover):
     run_and_compare(w, mode, tuning={"kernel": mover}, host_resident=True)
     if mode != O.INPLACE_MOVE:
         run_and_compare(synth.config(1, pool_factor=2.5), mode, tuning={"kernel": mover}, host_resident=True)
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_forget_directives_truncate_on_device_too(mode):
+    """a FORGET directive routes to a prefix-trimmed re-prefill -- the request is cut at the directive's
+    start (new coordinates), everything behind it is released and no kernel touches it.  Mixed with AMORTIZE edits."""
+    rng = np.random.default_rng(4242)
+    done = 0
+    while done < 6:
+        w = tiny_workload(rng, forget=True)
+        if not any(d[5] == synth.FORGET for d in w.directives):
+            continue
+        run_and_compare(w, mode)
+        done += 1
+
+
+def test_two_plans_in_flight_on_two_streams():
+    """Plans own their tables, tickets and hazard flags, so independent splices may overlap on different streams
+    (a server splices several requests' caches concurrently); each result must equal its own oracle."""
+    from paper_2606_01065_b200 import binding as B
+    from paper_2606_01065_b200 import harness
+    ws = [synth.config(2, pool_factor=2.2, n_layers=3), synth.config("3m", pool_factor=2.0, n_layers=2)]
+    modes = [O.INPLACE_MOVE, O.FRESH]
+    caches = [harness.DeviceCache(w, "cuda:0") for w in ws]
+    olds = [[p.cpu().numpy() for p in c.pools] for c in caches]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    outs = []
+    for rep in range(2):                      # second round: FRESH again on stream 1 while a rotate runs on stream 0
+        for c, m, s in zip(caches, modes, streams):
+            if rep == 1 and m != O.FRESH:
+                continue
+            outs.append((c, m, harness.run_workload(c, m, stream=s, prefetch=(rep == 0))))
+    torch.cuda.synchronize()
+    for (c, m, (plan, pt, idx)), old in zip(outs[:2], olds):
+        bm = oracle_plan(c.w, m)
+        assert_plan_equal(plan, bm, m)
+        np.testing.assert_array_equal(idx.cpu().numpy()[:int(plan.info.total_new_tokens)], oracle_slot_list(bm))
+        for l in range(c.w.n_layers):
+            compare_layer(c.w, bm, m, old[l], c.pools[l].cpu().numpy(), c.repl[l].cpu().numpy(), c.scales[l], layer=l)
+    for _, _, (plan, _, _) in outs:
+        plan.close()
