@@ -28,7 +28,8 @@ struct BulkStageInfo {
     int32_t tile;
     int32_t layer;
     int32_t dep_lo, dep_hi;
-    int32_t pad_[2];
+    int32_t from_repl;             /* replacement rows: nobody waits for this tile, so "loaded" is not published */
+    int32_t pad_;
 };
 
 /* ---- PTX wrappers (sm_90+ async-proxy bulk copies, mbarrier) ---- */
@@ -171,7 +172,7 @@ k_move_bulk(const __grid_constant__ MoveParams p, const int n_stages, const int 
                     if (half * 32 + lane < t.n_rows) info.dst_off[half * 32 + lane] = d_off[half];
                 if (lane == 0) {
                     info.n_rows = t.n_rows; info.trig = t.trig; info.tile = tile_i; info.layer = layer;
-                    info.dep_lo = t.dep_lo; info.dep_hi = t.dep_hi;
+                    info.dep_lo = t.dep_lo; info.dep_hi = t.dep_hi; info.from_repl = from_repl ? 1 : 0;
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive_expect_tx(&s_full[stage], (uint32_t)(t.n_rows * row_bytes));
@@ -218,7 +219,7 @@ k_move_bulk(const __grid_constant__ MoveParams p, const int n_stages, const int 
             const BulkStageInfo& info = s_info[stage];
             if (info.n_rows == 0) break;
             int32_t* flags = p.flags + p.layer0 + info.layer;
-            if (lane == 0) st_release(flags + (int64_t)info.tile * p.n_layers_total, 1);
+            if (lane == 0 && !info.from_repl) st_release(flags + (int64_t)info.tile * p.n_layers_total, 1);
             for (int d = info.dep_lo + lane; d <= info.dep_hi; d += 32)
                 while (ld_acquire(flags + (int64_t)d * p.n_layers_total) == 0) __nanosleep(32);
             __syncwarp();

@@ -106,10 +106,10 @@ __global__ void __launch_bounds__(kThreads, 3) k_move_rows(const __grid_constant
             for (int k = 0; k < kLatPerThread; ++k)
                 if (tid + k * kThreads < n_lat) landed ^= (uint32_t)(lat[k].x ^ lat[k].y ^ lat[k].z ^ lat[k].w);
             asm volatile("" :: "r"(landed) : "memory");
-            __threadfence();
+            if (!from_repl) __threadfence(); /* nobody waits for a replacement tile: it publishes nothing */
             __syncthreads();
             int32_t* flags = p.flags + p.layer0 + layer;
-            if (tid == 0) st_release(flags + (int64_t)tile_i * p.n_layers_total, 1);
+            if (tid == 0 && !from_repl) st_release(flags + (int64_t)tile_i * p.n_layers_total, 1);
             for (int d = t.dep_lo + tid; d <= t.dep_hi; d += kThreads)
                 while (ld_acquire(flags + (int64_t)d * p.n_layers_total) == 0) __nanosleep(64);
             __syncthreads();

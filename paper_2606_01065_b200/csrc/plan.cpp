@@ -366,6 +366,7 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
             }
         } else { /* INPLACE_MOVE, rule M2 */
             std::vector<DevTile> left, right;
+            const size_t first_insert = insert_tiles.size();
             for (const Seg& s : w.segs) {
                 if (s.kind == 1) {
                     split_tiles(s.src, s.dst, s.len, s.dst, TR, [&](int64_t a, int64_t b, int32_t n) {
@@ -404,6 +405,24 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
                 t.dep_lo = base_r + (int32_t)lo;
                 t.dep_hi = base_r + (int32_t)hi - 1;
                 move_tiles.push_back(t);
+            }
+            /* inserts run in the same launch, after every move in ticket order: a replacement row may land on a row
+             * some move tile of this request still has to read, so it waits for the hull of those tiles (a superset
+             * is safe: all of them hold smaller tickets) */
+            for (size_t q = first_insert; q < insert_tiles.size(); ++q) {
+                DevTile& t = insert_tiles[q];
+                const int64_t d0 = t.dst_pos, d1 = t.dst_pos + t.n_rows;
+                /* within the left-shifters (and within the right-shifters) sources are monotone in ticket order, so
+                 * the overlapping tiles of one group are a contiguous, exact range; only an insert that lands on
+                 * sources of BOTH groups gets the hull across them */
+                int32_t lo = INT32_MAX, hi = -1;
+                for (int32_t m = base_l; m < (int32_t)move_tiles.size(); ++m)
+                    if (move_tiles[m].src_pos < d1 && move_tiles[m].src_pos + move_tiles[m].n_rows > d0) {
+                        lo = std::min(lo, m);
+                        hi = std::max(hi, m);
+                    }
+                t.dep_lo = hi >= 0 ? lo : 0;
+                t.dep_hi = hi;
             }
         }
     }

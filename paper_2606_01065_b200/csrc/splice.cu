@@ -134,7 +134,7 @@ leyline_status upload_tables(leyline_plan_s* pl, int dev, cudaStream_t stream) {
     pl->off_slot_runs = place((int64_t)pl->slot_runs.size() * sizeof(IdxRun));
     pl->off_page_runs = place((int64_t)pl->page_runs.size() * sizeof(IdxRun));
     pl->blob_bytes = off > 0 ? off : 256;
-    const int64_t n_flags = pl->mode == LEYLINE_INPLACE_MOVE ? pl->info.n_move_tiles * pl->desc.n_layers : 0;
+    const int64_t n_flags = pl->mode == LEYLINE_INPLACE_MOVE ? pl->info.n_tiles * pl->desc.n_layers : 0;
     pl->scratch_bytes = 256 + align_up(n_flags * (int64_t)sizeof(int32_t), 256);
     PinnedBuf pin = pin_acquire((size_t)pl->blob_bytes, dev);
     std::string pageable;
@@ -458,20 +458,16 @@ extern "C" leyline_status leyline_splice(leyline_plan_t* pl, void* const* layer_
     int slot = 0;
     const int cps = pl->tuning.ctas_per_sm;
     if (pl->use_bulk) {
-        /* bulk kernel (TMA 1-D copies through shared memory); inserts after the moves for INPLACE_MOVE */
+        /* bulk kernel (TMA 1-D copies through shared memory) */
         if (inplace) {
-            st = run_tiles_bulk(pl, true, 0, n_move, layer_src, layer_dst, layer_repl, stream, &slot);
-            if (st != LEYLINE_OK) return st;
-            st = run_tiles_bulk(pl, false, (int32_t)n_move, n_ins, layer_src, layer_dst, layer_repl, stream, &slot);
+            /* one launch: the insert tiles hold the last tickets and wait for the move tiles that read their rows */
+            st = run_tiles_bulk(pl, true, 0, n_move + n_ins, layer_src, layer_dst, layer_repl, stream, &slot);
         } else {
             st = run_tiles_bulk(pl, false, 0, n_move + n_ins, layer_src, layer_dst, layer_repl, stream, &slot);
         }
     } else if (inplace) {
-        /* a3 under rule M2 ordering, then a4 once every move has landed (stream order) */
-        st = run_tiles(pl, true, 0, cps, 0, n_move, layer_src, layer_dst, layer_repl, stream, &slot);
-        if (st != LEYLINE_OK) return st;
-        st = run_tiles(pl, false, 0, cps, (int32_t)n_move, n_ins, layer_src, layer_dst, layer_repl,
-                       stream, &slot);
+        /* a3 under rule M2 ordering and a4 in one launch: insert tiles wait for the move tiles that read their rows */
+        st = run_tiles(pl, true, 0, cps, 0, n_move + n_ins, layer_src, layer_dst, layer_repl, stream, &slot);
     } else {
         /* a3 + a4 in one launch: fresh pages alias nothing */
         st = run_tiles(pl, false, 0, cps, 0, n_move + n_ins, layer_src, layer_dst, layer_repl, stream,

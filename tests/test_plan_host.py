@@ -234,7 +234,8 @@ def test_error_codes_follow_rule_v():
 
 def simulate_inplace(plan, w, rng):
     """Execute the plan's tiles on integer row labels: a tile's LOAD may happen at any time, its STORE only after
-    its own load and the loads of tiles [dep_lo, dep_hi]; inserts run after every move.  The interleaving is a
+    its own load and the loads of tiles [dep_lo, dep_hi]; insert tiles are part of the same schedule (they read the
+    replacement buffer and wait for the move tiles that still read their destination rows).  The interleaving is a
     random legal one.  Returns the pool of labels."""
     P = w.page_size
     pool = np.full(w.n_slots, -1, np.int64)
@@ -257,8 +258,8 @@ def simulate_inplace(plan, w, rng):
         return row[p // P].astype(np.int64) * P + p % P
 
     loaded, stored, regs = set(), set(), {}
-    pending = list(range(n_move))
-    while len(stored) < n_move:
+    pending = list(range(len(tiles)))
+    while len(stored) < len(tiles):
         ready = []
         for i in pending:
             if i not in loaded:
@@ -269,14 +270,16 @@ def simulate_inplace(plan, w, rng):
         stores = [x for x in ready if x[0] == "S"]
         op, i = stores[int(rng.integers(len(stores)))] if stores and rng.random() < 0.7 else ready[int(rng.integers(len(ready)))]
         if op == "L":
-            regs[i] = pool[src_slots(tiles[i])].copy()
+            t = tiles[i]
+            if i >= n_move:      # label = -(req, repl row) - 2
+                regs[i] = -(t.request * 10 ** 6 + t.src_pos + np.arange(t.n_rows)) - 2
+            else:
+                regs[i] = pool[src_slots(t)].copy()
             loaded.add(i)
         else:
             pool[dst_slots(tiles[i])] = regs.pop(i)
             stored.add(i)
             pending.remove(i)
-    for t in tiles[n_move:]:
-        pool[dst_slots(t)] = -(t.request * 10 ** 6 + t.src_pos + np.arange(t.n_rows)) - 2   # label = -(req, repl row) - 2
     return pool
 
 
