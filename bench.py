@@ -158,9 +158,9 @@ def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1):
     pt = torch.empty(max(int(info.total_new_pages), 1), dtype=torch.int32, device=dev)
     idx = torch.empty(max(int(info.total_new_tokens), 1), dtype=torch.int32, device=dev)
     nbytes = int(info.bytes_read + info.bytes_written)
-    # k_index (page table + slot list, one launch) + the movers: FRESH one k_move_bulk; INPLACE_MOVE moves then
-    # inserts; ROTATE_ONLY k_rotate_band then the insert tiles
-    launches = 1 + (1 if mode == B.FRESH else 2)
+    # per step: k_index (page table + slot list, one launch) + ONE data kernel: k_move_bulk (FRESH; INPLACE_MOVE with the
+    # inserts as its last tickets) or k_rotate_band (ROTATE_ONLY, inserts as trailing copy items)
+    launches = 2
     plan0.close()
     plans, host_us = [], []
 

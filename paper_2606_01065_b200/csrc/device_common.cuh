@@ -30,6 +30,9 @@ struct MoveParams {
     unsigned long long* ticket;   /* work counter, zeroed before the launch */
     int32_t* flags;               /* INPLACE_MOVE "loaded" flags [move tile][layer], zeroed before the launch */
     long long n_items;            /* tiles in this launch * layers in this launch */
+    long long n_copy_items;       /* k_rotate_band only: replacement-insert tiles * layers, handled after the rotations */
+    int32_t copy_tile_begin;      /* k_rotate_band only: first insert tile */
+    int32_t pad0_;
     int64_t stride;               /* row stride in bytes */
     int32_t tile_begin;           /* first tile of this launch in the plan's list */
     int32_t n_layers;             /* layers in this launch */

@@ -172,10 +172,9 @@ __global__ void __launch_bounds__(kThreads, DT == LEYLINE_FP8_E4M3 ? 2 : 3) k_ro
             it.slot[k] = rk[k] < t.n_rows ? (int32_t)slot_of(p.tabs, t.src_tab, t.src_pos + rk[k], p.page_shift) : -1;
     };
     long long item = blockIdx.x;
-    if (item >= p.n_items) return;
     Item cur, nxt;
-    resolve(item, cur);
-    for (;;) {
+    if (item < p.n_items) resolve(item, cur);
+    while (item < p.n_items) {
         uint8_t* __restrict__ base = p.dst[cur.layer];
         int4 lo[kRotUnroll], hi[kRotUnroll];
         uint8_t* addr[kRotUnroll];
@@ -206,6 +205,35 @@ __global__ void __launch_bounds__(kThreads, DT == LEYLINE_FP8_E4M3 ? 2 : 3) k_ro
         if (!more) break;
         cur = nxt;
         item = next;
+    }
+
+    /* a4 in the same launch: replacement rows are byte-copied into the free slots the plan consumed (disjoint from
+     * every rotated row).  16-byte chunks, four loads in flight per thread. */
+    const int row_chunks = p.lat_chunks + p.band_chunks;
+    for (long long ci = blockIdx.x; ci < p.n_copy_items; ci += gridDim.x) {
+        const DevTile t = p.tiles[p.copy_tile_begin + (int)(ci / p.n_layers)];
+        const int layer = (int)(ci % p.n_layers);
+        const uint8_t* __restrict__ src = p.repl[layer] + t.src_pos * p.stride;
+        uint8_t* __restrict__ dst = p.dst[layer];
+        const int shift = (t.flags & TILE_DST_TOKEN) ? 0 : p.page_shift;
+        const int n_chunks = t.n_rows * row_chunks;
+        for (int c0 = tid; c0 < n_chunks; c0 += kThreads * 4) {
+            int4 v[4];
+            uint8_t* out[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int c = c0 + k * kThreads;
+                out[k] = nullptr;
+                if (c < n_chunks) {
+                    const int r = c / row_chunks, col = c - r * row_chunks;
+                    v[k] = ld_stream(src + (int64_t)r * p.stride + col * 16);
+                    out[k] = dst + slot_of(p.tabs, t.dst_tab, t.dst_pos + r, shift) * p.stride + col * 16;
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (out[k]) st_stream(out[k], v[k]);
+        }
     }
 }
 

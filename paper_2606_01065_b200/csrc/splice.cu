@@ -349,16 +349,19 @@ leyline_status run_tiles(leyline_plan_s* pl, bool hazard, int smem, int max_ctas
 }
 
 /* a5: k_rotate_band takes its (tile, layer) items round-robin; enough blocks that the hardware scheduler balances. */
-leyline_status run_rotate(leyline_plan_s* pl, int32_t tile_begin, int64_t tile_count, void* const* layer_ptrs,
-                          cudaStream_t stream, int* ticket_slot) {
-    if (tile_count <= 0) return LEYLINE_OK;
+leyline_status run_rotate(leyline_plan_s* pl, int32_t tile_begin, int64_t tile_count, int64_t insert_count,
+                          void* const* layer_ptrs, const void* const* layer_repl, cudaStream_t stream, int* ticket_slot) {
+    if (tile_count + insert_count <= 0) return LEYLINE_OK;
     for (const LayerChunk& lc : layer_chunks(pl)) {
         MoveKernel fn = pick_rotate(pl, lc.pairing);
         MoveParams mp;
-        fill_params(pl, mp, tile_begin, tile_count, lc, nullptr, layer_ptrs, nullptr, *ticket_slot);
+        fill_params(pl, mp, tile_begin, tile_count, lc, nullptr, layer_ptrs, layer_repl, *ticket_slot);
+        mp.n_copy_items = insert_count * (long long)lc.layers.size();   /* a4 rides in the same launch */
+        mp.copy_tile_begin = tile_begin + (int32_t)tile_count;
         const int per_sm = occupancy(reinterpret_cast<const void*>(fn), 0);
         long long grid = (long long)g_dev.sms * per_sm * 8;
-        if (grid > mp.n_items) grid = mp.n_items;
+        const long long most = mp.n_items > mp.n_copy_items ? mp.n_items : mp.n_copy_items;
+        if (grid > most) grid = most;
         fn<<<(unsigned)grid, kThreads, 0, stream>>>(mp);
         CU(cudaGetLastError());
     }
@@ -497,13 +500,7 @@ extern "C" leyline_status leyline_rotate_inplace(leyline_plan_t* pl, void* const
     if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_start), stream));
     int slot = 0;
     /* a5: rotate where the rows sit; a4: replacement rows go to the consumed free slots (disjoint from a5's) */
-    st = run_rotate(pl, 0, n_rot, layer_ptrs, stream, &slot);
-    if (st != LEYLINE_OK) return st;
-    if (pl->use_bulk)
-        st = run_tiles_bulk(pl, false, (int32_t)n_rot, n_ins, layer_ptrs, layer_ptrs, layer_repl, stream, &slot);
-    else
-        st = run_tiles(pl, false, 0, pl->tuning.ctas_per_sm, (int32_t)n_rot, n_ins, layer_ptrs, layer_ptrs,
-                       layer_repl, stream, &slot);
+    st = run_rotate(pl, 0, n_rot, n_ins, layer_ptrs, layer_repl, stream, &slot);
     if (st != LEYLINE_OK) return st;
     if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_stop), stream));
     return LEYLINE_OK;
