@@ -213,7 +213,10 @@ leyline_status leyline_plan_trig_table(const leyline_plan_t* plan, float* out);
  *   layer_dst   HOST array of n_layers DEVICE pointers to the pools written.  May equal layer_src (fresh pages of
  *               the same pool); MUST equal it for INPLACE_MOVE.
  *   layer_repl  HOST array of n_layers DEVICE pointers to the replacement KV rows, [rows x row_stride_bytes] per
- *               layer, K_pe already roped at its FINAL position (G12).  May be NULL iff the plan inserts no row.
+ *               layer, K_pe already roped at its FINAL position (G12).  NULL = the caller fills the replacement
+ *               slots itself -- the paper's own flow, where step (b) is the model's prefill of R into the new
+ *               slots (PAPER.md:405(b)): the slots are allocated in the new page table / slot list and their bytes
+ *               are left untouched.
  *   dev_page_table_out  DEVICE int32 [total_new_pages] or NULL: receives the new page-table rows (concatenated,
  *               leyline_plan_new_pt_offsets).
  *   dev_slot_idx_out    DEVICE int32 [total_new_tokens] or NULL: receives the token-level slot of every new position.

@@ -439,7 +439,8 @@ extern "C" leyline_status leyline_splice(leyline_plan_t* pl, void* const* layer_
     if (!pl || pl->mode == LEYLINE_ROTATE_ONLY) return LEYLINE_E_INVALID;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     const bool inplace = pl->mode == LEYLINE_INPLACE_MOVE;
-    const int64_t n_move = pl->info.n_move_tiles, n_ins = pl->info.n_tiles - n_move;
+    /* layer_repl == NULL: the caller prefills the replacement slots itself (PAPER.md:405(b)); insert tiles are skipped */
+    const int64_t n_move = pl->info.n_move_tiles, n_ins = layer_repl ? pl->info.n_tiles - n_move : 0;
     if (n_move + n_ins > 0) {
         leyline_status st = check_layers(pl, layer_dst, "layer_dst");
         if (st == LEYLINE_OK && n_move > 0) st = check_layers(pl, layer_src, "layer_src");

@@ -76,15 +76,25 @@ def rotated_rows(w: synth.Workload, bm: O.BatchMap, mode: int):
 
 
 def compare_layer(w: synth.Workload, bm: O.BatchMap, mode: int, old_pool: np.ndarray, gpu_pool: np.ndarray,
-                  repl: np.ndarray, scale: float = 1.0, layer: int = 0) -> dict:
+                  repl: np.ndarray, scale: float = 1.0, layer: int = 0, inserts_prefilled: bool = False) -> dict:
     """One layer, whole pool.  old_pool / gpu_pool / repl: flat uint8.  Asserts the bar and returns statistics."""
     stride = w.row_bytes
     E = w.elem_bytes
     pairing = w.pairing_of(layer)
+    if repl is None:                      # the oracle always copies the replacement rows; they are masked out below
+        repl = np.zeros(max(w.n_repl_rows, 1) * stride, np.uint8)
     want = O.splice_layer(w.dtype, pairing, w.latent_dim, w.rope_dim, stride, w.inv_freq, scale, old_pool, repl, bm,
                           n_heads=w.rope_heads)
     g = gpu_pool.reshape(-1, stride)
     o = want.reshape(-1, stride)
+    if inserts_prefilled:
+        # layer_repl = NULL: the replacement slots belong to the caller's prefill and must not have been written
+        oo = old_pool.reshape(-1, stride)
+        for rm in bm.requests:
+            for (kind, src, dst, ln, sh) in rm.segs.as_tuples():
+                if kind == O.INSERT:
+                    s_ins = rm.slot_new[dst:dst + ln].astype(np.int64)
+                    o[s_ins] = oo[s_ins]
     new_s, old_s = rotated_rows(w, bm, mode)
     band0 = w.latent_dim * E
     # 1. everything outside rotated bands: bit-exact over the whole pool

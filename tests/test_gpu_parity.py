@@ -20,7 +20,7 @@ MODE_NAME = {O.FRESH: "fresh", O.INPLACE_MOVE: "inplace", O.ROTATE_ONLY: "rotate
 MOVERS = [1, 2]
 
 
-def run_and_compare(w, mode, check_layers=None, tuning=None, host_resident=False, **launch):
+def run_and_compare(w, mode, check_layers=None, tuning=None, host_resident=False, inserts_prefilled=False, **launch):
     from paper_2606_01065_b200 import binding as B
     from paper_2606_01065_b200 import harness
     if tuning:
@@ -30,6 +30,8 @@ def run_and_compare(w, mode, check_layers=None, tuning=None, host_resident=False
         check_layers = list(range(w.n_layers)) if check_layers is None else check_layers
         # a pinned host pool IS a cpu tensor: .cpu() would alias it, and the splice then overwrites the snapshot
         old = {l: (cache.pools[l].clone() if host_resident else cache.pools[l].cpu()).numpy() for l in check_layers}
+        if inserts_prefilled:
+            cache.repl = None                 # layer_repl = NULL: the caller prefills the replacement slots
         plan, pt, idx = harness.run_workload(cache, mode, **launch)
         torch.cuda.synchronize()
     finally:
@@ -45,8 +47,9 @@ def run_and_compare(w, mode, check_layers=None, tuning=None, host_resident=False
         np.testing.assert_array_equal(pt.cpu().numpy()[:n_pg], want)
     stats = []
     for l in check_layers:
-        stats.append(compare_layer(w, bm, mode, old[l], cache.pools[l].cpu().numpy(), cache.repl[l].cpu().numpy(),
-                                   cache.scales[l], layer=l))
+        stats.append(compare_layer(w, bm, mode, old[l], cache.pools[l].cpu().numpy(),
+                                   None if inserts_prefilled else cache.repl[l].cpu().numpy(),
+                                   cache.scales[l], layer=l, inserts_prefilled=inserts_prefilled))
     plan.close()
     tot = sum(s["rotated_elems"] for s in stats)
     if tot:
@@ -307,3 +310,14 @@ def test_two_plans_in_flight_on_two_streams():
             compare_layer(c.w, bm, m, old[l], c.pools[l].cpu().numpy(), c.repl[l].cpu().numpy(), c.scales[l], layer=l)
     for _, _, (plan, _, _) in outs:
         plan.close()
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("mover", MOVERS)
+def test_caller_prefills_replacement_slots(mode, mover):
+    """PAPER.md:405(b): in the paper step (b) is the model's prefill of R into the new slots.  With layer_repl = NULL
+    the library allocates those slots in the new maps and never writes their bytes; everything else is as usual."""
+    rng = np.random.default_rng(405)
+    for _ in range(4):
+        run_and_compare(tiny_workload(rng, P=int(rng.choice([1, 16]))), mode, tuning={"kernel": mover}, inserts_prefilled=True)
+    run_and_compare(synth.config(1, pool_factor=2.5), mode, tuning={"kernel": mover}, inserts_prefilled=True)
