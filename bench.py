@@ -36,7 +36,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="3", help="BASELINE.json config: 2, 3, 3m, 4, 5; full-width K: gqa, mha96")
+    ap.add_argument("--workload", default="3", help="BASELINE.json config: 2, 3, 3m, 4, 5; full-width K: gqa, mha96; appB: the paper's App. B counters' shape")
     ap.add_argument("--mode", default="fresh", choices=list(MODES))
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

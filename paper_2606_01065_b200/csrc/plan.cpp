@@ -234,8 +234,14 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
         int32_t g = (int32_t)pl->trig_shifts.size();
         trig_of.emplace(C, g);
         pl->trig_shifts.push_back(C);
-        for (int i = 0; i < H; ++i) pl->trig.push_back((float)std::cos((double)C * (double)pl->inv_freq[i]));
-        for (int i = 0; i < H; ++i) pl->trig.push_back((float)std::sin((double)C * (double)pl->inv_freq[i]));
+        const size_t at = pl->trig.size();
+        pl->trig.resize(at + 2 * (size_t)H);
+        for (int i = 0; i < H; ++i) { /* fp64 product, fp64 libm (one sincos call), rounded once to fp32 */
+            double sn, cs;
+            ::sincos((double)C * (double)pl->inv_freq[i], &sn, &cs);
+            pl->trig[at + (size_t)i] = (float)cs;
+            pl->trig[at + (size_t)H + (size_t)i] = (float)sn;
+        }
         return g;
     };
 

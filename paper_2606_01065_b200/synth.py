@@ -222,6 +222,20 @@ def config(n: int, **over) -> Workload:
                      directives=[(0, L // 16, L // 16 + 2048, 67, 0, AMORTIZE),
                                  (0, L // 4, L // 4 + 4096, 3, 0, AMORTIZE),
                                  (0, 3 * L // 4, 3 * L // 4 + 512, 251, 0, AMORTIZE)], seed=7)
+    elif n == "appB":
+        # The shape of the paper's own splice counters (App. B): DeepSeek-V2-Lite (27 layers, bf16,
+        # token-level slots as in SGLang's pool), one run = 167-203 chunks spliced and ">= 740 MB rotated", i.e. ~129
+        # tokens of 31,104 B per chunk.  Here: 185 chunk copies in ONE call.  Request k holds the d_k tokens in front of
+        # a matched chunk plus its n_k tokens; the directive drops the d_k tokens, so the chunk lands in fresh slots
+        # d_k positions earlier, rotated by -d_k (the paper's copy-to-dst_slots path).  n_k ~ U[66,194],
+        # d_k ~ U[1,512] (the delta range of App. F); slots are a random permutation (worst case).
+        rng = np.random.default_rng(383)
+        n_req = 185
+        n_k = rng.integers(66, 195, size=n_req)
+        d_k = rng.integers(1, 513, size=n_req)
+        w = Workload("appB_dsv2lite_185_chunks", 27, [int(a + b) for a, b in zip(d_k, n_k)], 1,
+                     inv_freq=rope_inv_freq(64, 10000.0),
+                     directives=[(r, 0, int(d_k[r]), 0, 0, AMORTIZE) for r in range(n_req)], seed=383)
     else:
         raise ValueError(n)
     for k, v in over.items():

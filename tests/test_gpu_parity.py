@@ -321,3 +321,10 @@ def test_caller_prefills_replacement_slots(mode, mover):
     for _ in range(4):
         run_and_compare(tiny_workload(rng, P=int(rng.choice([1, 16]))), mode, tuning={"kernel": mover}, inserts_prefilled=True)
     run_and_compare(synth.config(1, pool_factor=2.5), mode, tuning={"kernel": mover}, inserts_prefilled=True)
+
+
+@pytest.mark.parametrize("mode", [O.FRESH, O.ROTATE_ONLY])
+def test_paper_appendix_b_shape(mode):
+    """185 matched chunks of ~130 tokens copied to fresh token-level slots and rotated in one call (the shape of the
+    paper's bytes_rotated / kernel-time counters), and the same rotated where they sit."""
+    run_and_compare(synth.config("appB", pool_factor=2.0), mode, check_layers=[0, 13, 26])
