@@ -265,6 +265,16 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
         if (id < 0 || id >= free_limit) badfree = true;
         return id;
     };
+    /* the next `count` free ids appended to `dst` in one go (front to back, as take_free would) */
+    auto take_free_range = [&](std::vector<int32_t>& dst, int64_t count) {
+        if (count <= 0) return;
+        if (consumed + count > n_free) { nofree = true; return; }
+        const int32_t* ids = free_ids + consumed;
+        for (int64_t q = 0; q < count; ++q)
+            if (ids[q] < 0 || ids[q] >= free_limit) badfree = true;
+        dst.insert(dst.end(), ids, ids + count);
+        consumed += count;
+    };
 
     /* pass 1: segments, maps, released lists (requests ascending, free ids front to back) */
     for (int32_t r = 0; r < n_requests && !nofree; ++r) {
@@ -290,13 +300,14 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
             } else {
                 w.k0 = directives[d0].start / P;
                 pl->new_pages.insert(pl->new_pages.end(), old_row, old_row + w.k0);
-                for (int64_t p = w.k0; p < n_new && !nofree; ++p) pl->new_pages.push_back(take_free());
-                for (int64_t p = w.k0; p < n_old; ++p) pl->released.push_back(old_row[p]);
+                take_free_range(pl->new_pages, n_new - w.k0);
+                if (n_old > w.k0) pl->released.insert(pl->released.end(), old_row + w.k0, old_row + n_old);
             }
         } else if (mode == LEYLINE_INPLACE_MOVE) {
             /* M2: identity on the common pages, growth appends, shrink releases the tail */
-            for (int64_t p = 0; p < n_new && !nofree; ++p) pl->new_pages.push_back(p < n_old ? old_row[p] : take_free());
-            for (int64_t p = n_new; p < n_old; ++p) pl->released.push_back(old_row[p]);
+            pl->new_pages.insert(pl->new_pages.end(), old_row, old_row + std::min(n_old, n_new));
+            take_free_range(pl->new_pages, n_new - n_old);
+            if (n_old > n_new) pl->released.insert(pl->released.end(), old_row + n_new, old_row + n_old);
         } else {
             /* M3: no row moves; removed positions' slots are released in order */
             int64_t pos = 0;
