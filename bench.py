@@ -203,6 +203,40 @@ def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1):
             "mover": int(info.mover), "tile_rows": int(info.tile_rows)}
 
 
+def time_single_calls(cache, w, mode: int, reps: int = 10):
+    """Latency of ONE call on an idle GPU (nothing to hide the table upload behind): host wall clock from leyline_plan
+    to the stream being drained, median of `reps`.  The throughput figure above pipelines back-to-back steps."""
+    import torch
+    from paper_2606_01065_b200 import binding as B
+    desc, keep = cache.desc()
+    pools, repl = B.layer_pointers(cache.pools), B.layer_pointers(cache.repl)
+    free = w.free_slots() if mode == B.ROTATE_ONLY else w.free_pages
+    dirs = B.pack_directives(w.directives)
+    pt = idx = None
+    out = []
+    for i in range(reps + 2):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        plan = B.leyline_plan(desc, mode, w.seq_lens, w.pt_offsets, w.pages, dirs, free)
+        plan.prefetch()
+        if pt is None:
+            pt = torch.empty(max(int(plan.info.total_new_pages), 1), dtype=torch.int32, device=cache.device)
+            idx = torch.empty(max(int(plan.info.total_new_tokens), 1), dtype=torch.int32, device=cache.device)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+        if mode == B.ROTATE_ONLY:
+            B.leyline_rotate_inplace(plan, pools, repl, idx)
+        else:
+            B.leyline_splice(plan, pools, pools, repl, pt, idx)
+        torch.cuda.synchronize()
+        if i >= 2:
+            out.append((time.perf_counter() - t0) * 1e6)
+        plan.close()
+    del keep
+    return {"median_us": float(np.median(out)), "min_us": float(np.min(out)), "calls": reps,
+            "us_per_directive": float(np.median(out)) / max(1, len(w.directives))}
+
+
 def time_discovery(dev, n_sessions: int = 16, prompt_len: int = 17000, reps: int = 20):
     """Supplementary line: the discovery side (leyline_cdc_chunk) on the shape of the paper's
     microbenchmark -- 16 sessions x ~17 K-token prompts, anchors every ~600 tokens -- against
@@ -404,6 +438,7 @@ def run_ours(args):
                 extras[name] = {"ms_per_step": x["ms_per_step"], "GBps": x["bytes"] / x["ms_per_step"] / 1e6,
                                 "kernel_GBps": x["bytes"] / x["kernel_ms"] / 1e6, "bytes": x["bytes"]}
             cache.w = w
+            extras["single_call_idle_gpu"] = time_single_calls(cache, w, mode)
             extras["discovery_cdc"] = time_discovery(cache.device)
             out["extras"] = extras
         if not args.no_cpu_baseline:
