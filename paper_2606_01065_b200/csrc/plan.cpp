@@ -472,6 +472,15 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
     in.mover = pl->use_bulk ? 2 : 1;
     if (mode == LEYLINE_ROTATE_ONLY) pl->new_pages.clear();
 
+    if (mode == LEYLINE_INPLACE_MOVE) { /* how far back (in tiles) a waiting tile's dependencies sit: a launch hint */
+        std::vector<int32_t> dist;
+        for (size_t i = 0; i < move_tiles.size(); ++i)
+            if (move_tiles[i].dep_hi >= move_tiles[i].dep_lo) dist.push_back((int32_t)i - move_tiles[i].dep_hi);
+        if (!dist.empty()) {
+            std::nth_element(dist.begin(), dist.begin() + (long)(dist.size() / 2), dist.end());
+            pl->dep_distance_median = dist[dist.size() / 2];
+        }
+    }
     pl->tiles = std::move(move_tiles);
     pl->tiles.insert(pl->tiles.end(), insert_tiles.begin(), insert_tiles.end());
     *out = pl;

@@ -62,6 +62,7 @@ struct leyline_plan_s {
     int32_t rot_tile_rows = 0;          /* ROTATE_ONLY: rows per k_rotate_band work item */
     int32_t n_heads = 1;                /* heads in the rotated band (desc.rope_heads, 0 read as 1) */
     int32_t head_chunks = 8;            /* 16-byte chunks per head */
+    int32_t dep_distance_median = -1;   /* INPLACE_MOVE: median of (tile index - dep_hi) over tiles that wait, -1 if none */
     bool use_bulk = false;              /* a3/a4 run on k_move_bulk (TMA bulk copies) instead of k_move_rows */
     leyline_tuning tuning{};
 
