@@ -254,7 +254,7 @@ const char* leyline_last_cuda_error(void);
 
 /* Process-wide tuning knobs (benchmarking; defaults are what bench.py reports).  Read by leyline_plan. */
 typedef struct {
-    int32_t kernel;        /* a3/a4 mover: 0 = auto (bulk when pages hold >= 16 unpadded rows, or when the band is not a
+    int32_t kernel;        /* a3/a4 mover: 0 = auto (bulk for unpadded rows in pages of >= 16 rows or of >= 1 KB each, or when the band is not a
                               single head of 2^k <= 32 chunks), 1 = row kernel (LDG/STG through registers; single-head
                               bands of 2^k chunks only, else LEYLINE_E_UNSUPPORTED), 2 = bulk kernel (TMA 1-D bulk
                               copies through shared memory) */

@@ -109,14 +109,16 @@ leyline_status check_directives(int32_t n_req, const int64_t* seq_lens, int32_t 
 }
 
 /* Which mover runs a3/a4 (and ROTATE_ONLY's inserts).  The bulk kernel moves contiguous runs of rows with TMA 1-D
- * copies, so it pays with runs: pages of >= 16 rows and unpadded rows (padding must never be written); otherwise the
+ * copies, so it pays with runs: unpadded rows (padding must never be written) in pages of >= 16 rows, or rows of >= 1 KB; otherwise the
  * register-staged row kernel is used where it covers the band geometry.  tuning.kernel = 1 / 2 forces one of them. */
 bool choose_bulk(const leyline_cache_desc& c, int E, const leyline_tuning& t, int mode) {
     if (!row_kernel_ok(c, E)) return true;
     if (mode == LEYLINE_ROTATE_ONLY) return false;
     if (t.kernel == 1) return false;
     if (t.kernel == 2) return true;
-    return c.page_size >= 16 && c.row_stride_bytes == row_elems(c) * E;
+    /* unpadded rows; pages of >= 16 rows give multi-row runs, and even row-by-row (token-level pools) the bulk copies
+     * win once a row is >= 1 KB (measured on the scattered rows of the appB workload: 4.79 -> 5.38 TB/s) */
+    return c.row_stride_bytes == row_elems(c) * E && (c.page_size >= 16 || row_elems(c) * E >= 1024);
 }
 
 int choose_tile_rows(const leyline_cache_desc& c, int E, const leyline_tuning& t, bool bulk) {

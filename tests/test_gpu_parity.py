@@ -16,7 +16,7 @@ pytestmark = pytest.mark.gpu
 MODES = [O.FRESH, O.INPLACE_MOVE, O.ROTATE_ONLY]
 MODE_NAME = {O.FRESH: "fresh", O.INPLACE_MOVE: "inplace", O.ROTATE_ONLY: "rotate_only"}
 # leyline_tuning.kernel: the a3/a4 mover.  1 = k_move_rows (register-staged), 2 = k_move_bulk (TMA bulk copies through
-# shared memory); 0 = the planner's choice (bulk when pages hold >= 16 unpadded rows), which is what bench.py times.
+# shared memory); 0 = the planner's choice (bulk for unpadded rows in pages of >= 16 rows or of >= 1 KB each), which is what bench.py times.
 MOVERS = [1, 2]
 
 
