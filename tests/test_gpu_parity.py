@@ -328,3 +328,45 @@ def test_paper_appendix_b_shape(mode):
     """185 matched chunks of ~130 tokens copied to fresh token-level slots and rotated in one call (the shape of the
     paper's bytes_rotated / kernel-time counters), and the same rotated where they sit."""
     run_and_compare(synth.config("appB", pool_factor=2.0), mode, check_layers=[0, 13, 26])
+
+
+def test_launch_argument_errors_are_refused_before_any_launch():
+    """leyline.h: the launch entry points return only argument / launch errors -- and nothing is written when they do."""
+    from paper_2606_01065_b200 import binding as B
+    from paper_2606_01065_b200 import harness
+    w = synth.config(1, pool_factor=2.5)
+    cache = harness.DeviceCache(w, "cuda:0")
+    before = [p.clone() for p in cache.pools]
+    desc, keep = cache.desc()
+    idx = torch.full((8192,), -5, dtype=torch.int32, device="cuda:0")
+
+    def status_of(fn):
+        with pytest.raises(B.LeylineError) as ei:
+            fn()
+        return ei.value.status
+
+    rot = harness.plan_workload(w, B.ROTATE_ONLY, desc)
+    fresh = harness.plan_workload(w, B.FRESH, desc)
+    inpl = harness.plan_workload(w, B.INPLACE_MOVE, desc)
+    other = [torch.empty_like(p) for p in cache.pools]
+    # a plan of the wrong mode
+    assert status_of(lambda: B.leyline_splice(rot, cache.pools, cache.pools, cache.repl, None, idx)) == B.E_INVALID
+    assert status_of(lambda: B.leyline_rotate_inplace(fresh, cache.pools, cache.repl, idx)) == B.E_INVALID
+    # INPLACE_MOVE must read and write the same buffers
+    assert status_of(lambda: B.leyline_splice(inpl, cache.pools, other, cache.repl, None, idx)) == B.E_INVALID
+    # a NULL or misaligned layer pointer
+    bad = [cache.pools[0].data_ptr() + 8, cache.pools[1].data_ptr()]
+    assert status_of(lambda: B.leyline_splice(fresh, bad, bad, cache.repl, None, idx)) == B.E_INVALID
+    assert status_of(lambda: B.leyline_splice(fresh, [0, 0], [0, 0], cache.repl, None, idx)) == B.E_INVALID
+    # wrong number of layers is caught by the binding itself
+    with pytest.raises(ValueError):
+        B.leyline_splice(fresh, cache.pools[:1], cache.pools, cache.repl, None, idx)
+    torch.cuda.synchronize()
+    assert all(bool((a == b).all()) for a, b in zip(before, cache.pools)) and bool((idx == -5).all())
+    # and the plans are still usable afterwards
+    B.leyline_splice(fresh, cache.pools, cache.pools, cache.repl, None, idx)
+    torch.cuda.synchronize()
+    assert int(idx[0].item()) != -5
+    for p in (rot, fresh, inpl):
+        p.close()
+    del keep
