@@ -31,7 +31,7 @@ bool cuda_ok(cudaError_t e, const char* what) {
 inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
 struct DeviceInfo { int device = -1; int sms = 0; int smem_optin = 0; };
-DeviceInfo g_dev;
+thread_local DeviceInfo g_dev; /* per host thread: callers may drive different devices from different threads */
 
 /* ---- pinned staging for the plan upload ----
  * A pageable source makes the runtime stage the tables itself (an extra host copy, and a DMA that cannot start
@@ -113,11 +113,12 @@ leyline_status device_info(int* dev_out) {
     int dev = 0;
     CU(cudaGetDevice(&dev));
     if (g_dev.device != dev) {
-        cudaDeviceProp prop;
-        CU(cudaGetDeviceProperties(&prop, dev));
+        int sms = 0, optin = 0;
+        CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        CU(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
         g_dev.device = dev;
-        g_dev.sms = prop.multiProcessorCount;
-        g_dev.smem_optin = (int)prop.sharedMemPerBlockOptin;
+        g_dev.sms = sms;
+        g_dev.smem_optin = optin;
     }
     *dev_out = dev;
     return LEYLINE_OK;
@@ -264,8 +265,8 @@ MoveKernel pick_rotate(const leyline_plan_s* pl, int pairing) {
 namespace {
 
 struct OccCache { const void* fn; int smem; int blocks; };
-OccCache g_occ[64];
-int g_occ_n = 0;
+thread_local OccCache g_occ[64];
+thread_local int g_occ_n = 0;
 
 int occupancy(const void* fn, int smem) {
     for (int i = 0; i < g_occ_n; ++i)

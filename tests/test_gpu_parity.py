@@ -370,3 +370,45 @@ def test_launch_argument_errors_are_refused_before_any_launch():
     for p in (rot, fresh, inpl):
         p.close()
     del keep
+
+
+def test_two_host_threads_drive_the_library_at_once():
+    """ctypes releases the GIL, so two Python threads really are inside libleyline.so together: planning, pinned
+    staging, the table pool and the launches are shared state that must hold up (each thread on its own stream)."""
+    import threading
+    from paper_2606_01065_b200 import harness
+    ws = [synth.config(2, pool_factor=2.2, n_layers=2), synth.config(1, pool_factor=2.5)]
+    modes = [O.FRESH, O.ROTATE_ONLY]
+    caches = [harness.DeviceCache(w, "cuda:0") for w in ws]
+    olds = [[p.cpu().numpy() for p in c.pools] for c in caches]
+    torch.cuda.synchronize()
+    results, errors = [None, None], []
+
+    def work(i):
+        try:
+            s = torch.cuda.Stream()
+            last = None
+            for rep in range(20 if modes[i] == O.FRESH else 1):      # FRESH is idempotent: hammer it
+                if last is not None:
+                    last[0].close()
+                last = harness.run_workload(caches[i], modes[i], stream=s, prefetch=bool(rep % 2))
+            s.synchronize()
+            results[i] = last
+        except Exception as ex:        # surfaced in the main thread
+            errors.append(ex)
+
+    threads = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    torch.cuda.synchronize()
+    for i, (c, m) in enumerate(zip(caches, modes)):
+        plan, pt, idx = results[i]
+        bm = oracle_plan(c.w, m)
+        assert_plan_equal(plan, bm, m)
+        np.testing.assert_array_equal(idx.cpu().numpy()[:int(plan.info.total_new_tokens)], oracle_slot_list(bm))
+        for l in range(c.w.n_layers):
+            compare_layer(c.w, bm, m, olds[i][l], c.pools[l].cpu().numpy(), c.repl[l].cpu().numpy(), c.scales[l], layer=l)
+        plan.close()
