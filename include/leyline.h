@@ -237,6 +237,21 @@ leyline_status leyline_rotate_inplace(leyline_plan_t* plan, void* const* layer_p
                                       int32_t* dev_slot_idx_out, void* cuda_stream);
 
 /*
+ * leyline_rotate_inplace_master -- leyline_rotate_inplace with the RE-ANCHOR option: besides
+ * the pools the caller keeps, per layer, an fp32 MASTER copy of the rotated band,
+ *   layer_master[l]: DEVICE float [pool_slots][rope_heads * rope_dim]  (dense rows, 16-byte aligned).
+ * Chained splices round a bf16 K_pe once per turn and the error random-walks (Table 6: rel-L2
+ * 4.3e-3 at N=2 -> 2.6e-2 at N=100; the paper's remedy is periodic re-prefill).  Here every rotation is applied to
+ * the master in fp32 (fma, error ~2^-24 per turn) and the stored band is re-derived from the master by ONE
+ * round-to-nearest-even, so K_pe never carries more than one rounding however often its slot is re-rotated.
+ * Rows of C = 0 segments are untouched (band and master).  Replacement rows (layer_repl != NULL) are copied into the
+ * pool and their band widened exactly into the master; with layer_repl == NULL the caller fills both.
+ * bf16 caches and ROTATE_ONLY plans only (else LEYLINE_E_UNSUPPORTED / LEYLINE_E_INVALID).
+ */
+leyline_status leyline_rotate_inplace_master(leyline_plan_t* plan, void* const* layer_ptrs, void* const* layer_master,
+                                             const void* const* layer_repl, int32_t* dev_slot_idx_out, void* cuda_stream);
+
+/*
  * leyline_plan_prefetch -- OPTIONAL: start uploading the plan's device tables (tiles, cos/sin table, page tables,
  * index runs; SURVEY.md section 3(3) "one small H2D copy") on a library-owned copy stream of the CURRENT device and
  * return at once.  The first leyline_splice / leyline_rotate_inplace of the plan then only waits for that copy's

@@ -63,7 +63,7 @@ def lib():
         L.ora_rerope_pair.restype = None
         L.ora_rerope_pair.argtypes = [C.c_double] * 5 + [C.POINTER(C.c_double), C.POINTER(C.c_double)]
         for name in ("ora_validate", "ora_segments", "ora_map_fresh", "ora_map_inplace", "ora_map_rotate_only",
-                     "ora_apply_layer"):
+                     "ora_apply_layer", "ora_rotate_master_layer"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -293,3 +293,18 @@ def splice_layer(dtype: int, pairing: int, Dc: int, Dr: int, stride: int, inv_fr
         st = apply_layer(dtype, pairing, Dc, Dr, stride, inv_freq, scale, old_pool, new_pool, repl, rm, n_heads)
         assert st == OK, st
     return new_pool
+
+
+def rotate_master_layer(pairing: int, Dc: int, Dr: int, stride: int, inv_freq: np.ndarray, pool: np.ndarray,
+                        master: np.ndarray, repl: np.ndarray | None, bm: BatchMap, n_heads: int = 1):
+    """DESIGN.md reading R1 (fp32 master band), one layer, ROTATE_ONLY maps, bf16 pool.  `pool` (uint8) and `master`
+    (float32 [n_slots, n_heads*Dr]) are updated IN PLACE (rows do not move in this mode)."""
+    assert pool.dtype == np.uint8 and master.dtype == np.float32 and pool.flags.c_contiguous and master.flags.c_contiguous
+    inv = np.ascontiguousarray(inv_freq, dtype=np.float32)
+    rp = _p(np.ascontiguousarray(repl)) if repl is not None else None
+    for rm in bm.requests:
+        s = rm.segs
+        st = lib().ora_rotate_master_layer(C.c_int(pairing), C.c_int32(Dc), C.c_int32(Dr), C.c_int32(n_heads), C.c_int64(stride),
+                                           _p(inv), _p(pool), _p(master), rp, C.c_int32(len(s)), _p(s.kind), _p(s.src),
+                                           _p(s.dst), _p(s.len), _p(s.shift), _p(_i64(rm.slot_new)))
+        assert st == OK, st

@@ -340,3 +340,52 @@ int ora_apply_layer(int dtype, int pairing, int32_t Dc, int32_t Dr, int32_t n_he
     }
     return ORA_OK;
 }
+
+/* The RE-ANCHOR option of the in-place path (chained bf16 rotations drift,
+ * "periodic re-prefill of the affected slots" is the paper's remedy).  DESIGN.md reading R1: next to the bf16 pool the
+ * caller keeps an fp32 master of the rotated band, master[slot][n_heads*Dr]; a ROTATE_ONLY splice
+ *   - rotates the master of every downstream token (shift C != 0): exact fp32 inputs, fp64 rotation with fresh libm
+ *     sin/cos, ONE rounding to fp32 (the C cast, round-to-nearest-even);
+ *   - re-derives the stored band from the NEW master: bf16 = RNE(fp32 value) -- the decision is taken on the fp32
+ *     value, the precision both sides hold;
+ *   - copies replacement rows into the pool and widens their band exactly into the master;
+ *   - leaves C = 0 rows alone.
+ * Rows do not move in this mode: slot_new[dst + q] == slot_old[src + q]. */
+int ora_rotate_master_layer(int pairing, int32_t Dc, int32_t Dr, int32_t n_heads, int64_t stride, const float* inv_freq,
+                            uint8_t* pool, float* master, const uint8_t* repl, int32_t n_seg, const int32_t* kind,
+                            const int64_t* src, const int64_t* dst, const int64_t* len, const int64_t* shift,
+                            const int64_t* slot_new) {
+    int32_t H = Dr / 2;
+    int64_t band = (int64_t)n_heads * Dr;
+    if (Dr % 2 != 0 || n_heads < 1) return ORA_E_UNSUPPORTED;
+    for (int32_t g = 0; g < n_seg; ++g) {
+        for (int64_t q = 0; q < len[g]; ++q) {
+            int64_t slot = slot_new[dst[g] + q];
+            uint8_t* row = pool + slot * stride;
+            float* m = master + slot * band;
+            if (kind[g] == ORA_INSERT) {
+                if (!repl) continue; /* the caller prefills pool and master */
+                memcpy(row, repl + (src[g] + q) * stride, (size_t)(Dc + band) * 2);
+                for (int64_t e = 0; e < band; ++e) m[e] = (float)load_elem(ORA_BF16, row + (int64_t)Dc * 2, e, 1.0);
+                continue;
+            }
+            if (shift[g] == 0) continue;
+            for (int32_t h = 0; h < n_heads; ++h) {
+                float* mh = m + (int64_t)h * Dr;
+                uint8_t* kout = row + ((int64_t)Dc + (int64_t)h * Dr) * 2;
+                for (int32_t i = 0; i < H; ++i) {
+                    int64_t ia = (pairing == ORA_NEOX) ? i : 2 * i;
+                    int64_t ib = (pairing == ORA_NEOX) ? i + H : 2 * i + 1;
+                    double phi = (double)shift[g] * (double)inv_freq[i];
+                    double a2, b2;
+                    ora_rotate_pair((double)mh[ia], (double)mh[ib], phi, &a2, &b2);
+                    mh[ia] = (float)a2;
+                    mh[ib] = (float)b2;
+                    store_elem(ORA_BF16, kout, ia, (double)mh[ia], 1.0);
+                    store_elem(ORA_BF16, kout, ib, (double)mh[ib], 1.0);
+                }
+            }
+        }
+    }
+    return ORA_OK;
+}

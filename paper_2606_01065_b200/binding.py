@@ -90,6 +90,8 @@ def _load() -> C.CDLL:
     L.leyline_splice.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     L.leyline_rotate_inplace.restype = C.c_int
     L.leyline_rotate_inplace.argtypes = [vp, vp, vp, vp, vp]
+    L.leyline_rotate_inplace_master.restype = C.c_int
+    L.leyline_rotate_inplace_master.argtypes = [vp, vp, vp, vp, vp, vp]
     L.leyline_plan_kernel_ms.restype = C.c_int
     L.leyline_plan_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.leyline_plan_prefetch.restype = C.c_int
@@ -316,6 +318,16 @@ def leyline_rotate_inplace(plan: Plan, layers, layer_repl=None, slot_idx_out=Non
     c, _k3 = _ptr_array(layer_repl, n, "layer_repl")
     st = _lib.leyline_rotate_inplace(plan._h, a, c, _dev_ptr(slot_idx_out), _stream_handle(stream))
     _check(st, "leyline_rotate_inplace")
+
+
+def leyline_rotate_inplace_master(plan: Plan, layers, layer_master, layer_repl=None, slot_idx_out=None, stream=None):
+    """leyline.h: leyline_rotate_inplace_master (fp32 master band per layer, float32 tensors [pool_slots, band])."""
+    n = layers.n if isinstance(layers, LayerPointers) else len(layers)
+    a, _k1 = _ptr_array(layers, n, "layer_ptrs")
+    m, _k2 = _ptr_array(layer_master, n, "layer_master")
+    c, _k3 = _ptr_array(layer_repl, n, "layer_repl")
+    st = _lib.leyline_rotate_inplace_master(plan._h, a, m, c, _dev_ptr(slot_idx_out), _stream_handle(stream))
+    _check(st, "leyline_rotate_inplace_master")
 
 
 # ----------------------------------------------------------------------------- discovery side (leyline_cdc.h)

@@ -198,12 +198,9 @@ __device__ __forceinline__ int4 rotate_chunk_interleaved(const int4& mine, const
  * Interleaved: `lo` = chunk q of the head, `hi` = chunk q + half; each holds N/2 whole pairs;
  *       c[0..N/2) / s[0..N/2) belong to lo (pairs q*N/2 ..), c[N/2..N) / s[N/2..N) to hi (pairs (q+half)*N/2 ..).
  * Same fp32 expressions as rotate_chunk_neox / rotate_chunk_interleaved: a' = fma(b, -s, a*c), b' = fma(a, s, b*c). */
-template <int DT, int PAIRING>
-__device__ __forceinline__ void rotate_chunk_pair(int4& lo, int4& hi, const float* c, const float* s) {
-    constexpr int N = Codec<DT>::kElems;
-    float a[N], b[N];
-    Codec<DT>::unpack(lo, a);
-    Codec<DT>::unpack(hi, b);
+/* The fp32 arithmetic of one (lo, hi) chunk pair: N elements each, cos / sin as described above. */
+template <int PAIRING, int N>
+__device__ __forceinline__ void rotate_pair_f32(float* a, float* b, const float* c, const float* s) {
     if (PAIRING == LEYLINE_ROPE_NEOX) {
 #pragma unroll
         for (int e = 0; e < N; ++e) {
@@ -221,6 +218,15 @@ __device__ __forceinline__ void rotate_chunk_pair(int4& lo, int4& hi, const floa
             b[2 * q + 1] = __fmaf_rn(x1, s[N / 2 + q], y1 * c[N / 2 + q]);
         }
     }
+}
+
+template <int DT, int PAIRING>
+__device__ __forceinline__ void rotate_chunk_pair(int4& lo, int4& hi, const float* c, const float* s) {
+    constexpr int N = Codec<DT>::kElems;
+    float a[N], b[N];
+    Codec<DT>::unpack(lo, a);
+    Codec<DT>::unpack(hi, b);
+    rotate_pair_f32<PAIRING, N>(a, b, c, s);
     lo = Codec<DT>::pack(a);
     hi = Codec<DT>::pack(b);
 }

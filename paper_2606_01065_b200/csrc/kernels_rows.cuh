@@ -237,6 +237,80 @@ __global__ void __launch_bounds__(kThreads, DT == LEYLINE_FP8_E4M3 ? 2 : 3) k_ro
     }
 }
 
+/* ------------------------------------------------------------------ a5 with an fp32 master band ---- */
+
+/* Chained splices round the bf16 K_pe once per turn and the error random-walks (Table 6; the paper's
+ * remedy is "periodic re-prefill of the affected slots").  The re-anchor option keeps an fp32 MASTER copy of the band
+ * per slot ([pool_slots][rope_heads * rope_dim] floats per layer, caller-owned): the rotation is applied to the master
+ * in fp32 (error ~2^-24 per turn instead of 2^-9) and the bf16 band is re-derived from it by one RNE, so the stored
+ * K_pe never carries more than one rounding however often its slot is re-rotated.  bf16 caches, ROTATE_ONLY plans.
+ * p.src[layer] carries the master pointers.  Same unit as k_rotate_band: (row, pair column), both partner chunks in one
+ * thread.  Replacement rows (trailing copy items) are copied into the pool and widened into the master. */
+template <int PAIRING>
+__global__ void __launch_bounds__(kThreads) k_rotate_master(const __grid_constant__ MoveParams p) {
+    constexpr int N = Codec<LEYLINE_BF16>::kElems; /* 8 elements per 16-byte chunk */
+    const int tid = threadIdx.x;
+    const int half = p.head_chunks >> 1, cols = p.n_heads * half;
+    const int64_t band0 = (int64_t)p.lat_chunks * 16;
+    const int64_t band_elems = (int64_t)p.band_chunks * N;
+    for (long long item = blockIdx.x; item < p.n_items; item += gridDim.x) {
+        const DevTile t = p.tiles[p.tile_begin + (int)(item / p.n_layers)];
+        const int layer = (int)(item % p.n_layers);
+        uint8_t* __restrict__ pool = p.dst[layer];
+        float* __restrict__ master = reinterpret_cast<float*>(const_cast<uint8_t*>(p.src[layer]));
+        const float* __restrict__ trig_row = p.trig + (int64_t)t.trig * 2 * p.H;
+        const int total = t.n_rows * cols;
+        for (int u = tid; u < total; u += kThreads) {
+            const int r = u / cols, col = u - r * cols;
+            const int head = col / half, q = col - head * half;
+            const int chunk = head * p.head_chunks + q;
+            const int64_t slot = slot_of(p.tabs, t.src_tab, t.src_pos + r, p.page_shift);
+            float4* mlo = reinterpret_cast<float4*>(master + slot * band_elems + (int64_t)chunk * N);
+            float4* mhi = mlo + half * (N / 4);
+            float a[N], b[N], c[N], s[N];
+#pragma unroll
+            for (int k = 0; k < N / 4; ++k) {
+                const float4 x = mlo[k], y = mhi[k];
+                a[4 * k] = x.x; a[4 * k + 1] = x.y; a[4 * k + 2] = x.z; a[4 * k + 3] = x.w;
+                b[4 * k] = y.x; b[4 * k + 1] = y.y; b[4 * k + 2] = y.z; b[4 * k + 3] = y.w;
+            }
+            load_pair_trig<LEYLINE_BF16, PAIRING>(trig_row, p.H, q, half, c, s);
+            rotate_pair_f32<PAIRING, N>(a, b, c, s);
+#pragma unroll
+            for (int k = 0; k < N / 4; ++k) {
+                mlo[k] = make_float4(a[4 * k], a[4 * k + 1], a[4 * k + 2], a[4 * k + 3]);
+                mhi[k] = make_float4(b[4 * k], b[4 * k + 1], b[4 * k + 2], b[4 * k + 3]);
+            }
+            uint8_t* band = pool + slot * p.stride + band0 + (int64_t)chunk * 16;
+            st_stream(band, Codec<LEYLINE_BF16>::pack(a));              /* one RNE from the fp32 master */
+            st_stream(band + half * 16, Codec<LEYLINE_BF16>::pack(b));
+        }
+    }
+    const int row_chunks = p.lat_chunks + p.band_chunks;
+    for (long long ci = blockIdx.x; ci < p.n_copy_items; ci += gridDim.x) {
+        const DevTile t = p.tiles[p.copy_tile_begin + (int)(ci / p.n_layers)];
+        const int layer = (int)(ci % p.n_layers);
+        const uint8_t* __restrict__ src = p.repl[layer] + t.src_pos * p.stride;
+        uint8_t* __restrict__ pool = p.dst[layer];
+        float* __restrict__ master = reinterpret_cast<float*>(const_cast<uint8_t*>(p.src[layer]));
+        const int shift = (t.flags & TILE_DST_TOKEN) ? 0 : p.page_shift;
+        const int n_chunks = t.n_rows * row_chunks;
+        for (int c0 = tid; c0 < n_chunks; c0 += kThreads) {
+            const int r = c0 / row_chunks, col = c0 - r * row_chunks;
+            const int4 v = ld_stream(src + (int64_t)r * p.stride + col * 16);
+            const int64_t slot = slot_of(p.tabs, t.dst_tab, t.dst_pos + r, shift);
+            st_stream(pool + slot * p.stride + col * 16, v);
+            if (col >= p.lat_chunks) { /* the replacement's K_pe is the new master, widened exactly */
+                float f[N];
+                Codec<LEYLINE_BF16>::unpack(v, f);
+                float4* m = reinterpret_cast<float4*>(master + slot * band_elems + (int64_t)(col - p.lat_chunks) * N);
+                m[0] = make_float4(f[0], f[1], f[2], f[3]);
+                m[1] = make_float4(f[4], f[5], f[6], f[7]);
+            }
+        }
+    }
+}
+
 }  // namespace leyline
 
 #endif /* LEYLINE_KERNELS_ROWS_CUH_ */

@@ -515,6 +515,45 @@ extern "C" leyline_status leyline_rotate_inplace(leyline_plan_t* pl, void* const
     return LEYLINE_OK;
 }
 
+extern "C" leyline_status leyline_rotate_inplace_master(leyline_plan_t* pl, void* const* layer_ptrs, void* const* layer_master,
+                                                        const void* const* layer_repl, int32_t* dev_slot_idx_out,
+                                                        void* cuda_stream) {
+    g_last_error.clear();
+    if (!pl || pl->mode != LEYLINE_ROTATE_ONLY) return LEYLINE_E_INVALID;
+    if (pl->desc.dtype != LEYLINE_BF16) { g_last_error = "the fp32 master option covers bf16 caches"; return LEYLINE_E_UNSUPPORTED; }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const int64_t n_rot = pl->info.n_move_tiles, n_ins = layer_repl ? pl->info.n_tiles - n_rot : 0;
+    if (n_rot + n_ins > 0) {
+        leyline_status st = check_layers(pl, layer_ptrs, "layer_ptrs");
+        if (st == LEYLINE_OK) st = check_layers(pl, layer_master, "layer_master");
+        if (st == LEYLINE_OK && n_ins > 0) st = check_layers(pl, layer_repl, "layer_repl");
+        if (st != LEYLINE_OK) return st;
+    }
+    leyline_status st = begin_call(pl, stream);
+    if (st != LEYLINE_OK) return st;
+    st = launch_index(pl, nullptr, dev_slot_idx_out, stream);
+    if (st != LEYLINE_OK) return st;
+    if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_start), stream));
+    if (n_rot + n_ins > 0) {
+        for (const LayerChunk& lc : layer_chunks(pl)) {
+            MoveKernel fn = lc.pairing == LEYLINE_ROPE_NEOX ? k_rotate_master<LEYLINE_ROPE_NEOX> : k_rotate_master<LEYLINE_ROPE_INTERLEAVED>;
+            MoveParams mp;
+            /* the master pointers travel in the (otherwise unused) source slots of the parameter block */
+            fill_params(pl, mp, 0, n_rot, lc, layer_master, layer_ptrs, layer_repl, 0);
+            mp.n_copy_items = n_ins * (long long)lc.layers.size();
+            mp.copy_tile_begin = (int32_t)n_rot;
+            const int per_sm = occupancy(reinterpret_cast<const void*>(fn), 0);
+            long long grid = (long long)g_dev.sms * per_sm * 8;
+            const long long most = mp.n_items > mp.n_copy_items ? mp.n_items : mp.n_copy_items;
+            if (grid > most) grid = most;
+            fn<<<(unsigned)grid, kThreads, 0, stream>>>(mp);
+            CU(cudaGetLastError());
+        }
+    }
+    if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_stop), stream));
+    return LEYLINE_OK;
+}
+
 extern "C" leyline_status leyline_plan_prefetch(leyline_plan_t* pl) {
     g_last_error.clear();
     if (!pl) return LEYLINE_E_INVALID;

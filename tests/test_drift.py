@@ -19,6 +19,7 @@ import pytest
 
 import oracle as O
 from helpers import from_storage, golden, rope_complex, to_storage
+from parity import _bf16_ord
 from paper_2606_01065_b200 import synth
 
 T6 = golden("paper_table6.txt")
@@ -195,3 +196,152 @@ def test_gpu_chain_matches_oracle_chain(n):
     assert abs(rg - ro) <= 0.05 * ro                                # same random walk, statistically
     # the chains differ only where a rounding decision differed (<= 1 ulp per turn, < 1 % of elements per turn)
     assert rel_l2(got_g, got_o) <= 0.5 * ro
+
+
+# ----------------------------------------------------------------------------- the re-anchor option: fp32 master band
+
+def bf16_bits_of_f32(x: np.ndarray) -> np.ndarray:
+    """float32 -> bf16 bit patterns through torch's converter (round-to-nearest-even; a library routine, not the oracle's)."""
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x, np.float32)).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+
+
+class MasterChain(OracleChain):
+    """OracleChain plus the fp32 master of the band per slot (reading R1), initialised from the un-rounded
+    fp32 K_pe -- what a prefill holds before it rounds to the cache's bf16."""
+
+    def __init__(self, rows, n_slots, seed):
+        super().__init__(O.BF16, rows, n_slots, seed)
+        self.masters = []
+        for l in range(N_LAYERS):
+            m = np.zeros((n_slots, DR), np.float32)
+            m[self.idx] = rows[l][:, DC:].astype(np.float32)
+            self.masters.append(m)
+
+    def step(self, S, delta, repl):
+        seq, pto, pages, dirs, free = self.step_inputs(S, delta)
+        bm = O.plan_batch(O.ROTATE_ONLY, 1, seq, pto, pages, dirs, free)
+        assert bm.status == O.OK
+        for l in range(N_LAYERS):
+            O.rotate_master_layer(O.NEOX, DC, DR, self.stride, H64, self.pools[l], self.masters[l], repl[l], bm)
+        self.idx = bm.requests[0].slot_new.astype(np.int32)
+        return bm
+
+    def tracked_master(self):
+        return np.stack([m[self.idx[-N_TRACKED:]] for m in self.masters]).astype(np.float64)
+
+
+def finite_repl(rng):
+    """Replacement rows as a prefill would write them: N(0,1) in bf16 (random BYTES would contain NaN patterns, whose
+    widened master could not be compared by value)."""
+    return [to_storage(rng.standard_normal((CACHE, DC + DR)), O.BF16).reshape(-1) for _ in range(N_LAYERS)]
+
+
+def run_master_chain(n, seed):
+    rng = np.random.default_rng(1000 + seed)
+    s0 = int(rng.integers(1024, 4096))
+    deltas = chain_deltas(rng, n, s0)
+    raw, rows = initial_rows(rng, s0)
+    ch = MasterChain(rows, 2 * CACHE, seed)
+    repl = finite_repl(rng)
+    S = s0
+    for d in deltas:
+        ch.step(S, d, repl)
+        S += d
+    return ch, raw, s0, deltas, repl
+
+
+def test_master_band_keeps_the_drift_at_one_rounding():
+    lo, hi = 2.0 ** -8 / np.sqrt(12.0), 2.0 ** -7 / np.sqrt(12.0)        # one RNE to bf16, see above
+    rels = {}
+    for n in (2, 100):
+        ch, raw, s0, deltas, _ = run_master_chain(n, 3)
+        ref = fresh_reference(raw, s0, deltas)
+        band, master = ch.tracked(), ch.tracked_master()
+        # the master is fresh RoPE to fp32 accuracy: n rotations of ~2^-24 relative error each
+        assert np.abs(master - ref).max() <= (n + 2) * 2.0 ** -23 * np.abs(ref).max()
+        # the stored band IS the master rounded once, by torch's converter
+        stored = np.stack([p.reshape(-1, ch.stride)[ch.idx[-N_TRACKED:], DC * 2:] for p in ch.pools]).view(np.uint16)
+        np.testing.assert_array_equal(stored, bf16_bits_of_f32(master.astype(np.float32)))
+        rels[n] = rel_l2(band, ref)
+        assert lo <= rels[n] <= hi, (n, rels[n])
+        assert rels[n] < T6["rel_l2"][0]                                   # under Table 6's N = 2 row for ANY n
+    assert abs(rels[100] - rels[2]) / rels[2] < 0.05                       # no growth with the number of turns
+
+
+def test_master_replacement_rows_are_widened_exactly():
+    ch, raw, s0, deltas, repl = run_master_chain(1, 4)
+    S = s0 + deltas[0]                               # the replacement rows sit at new positions [0, S)
+    for l in (0, N_LAYERS - 1):
+        rows = ch.pools[l].reshape(-1, ch.stride)[ch.idx[:S]]
+        np.testing.assert_array_equal(rows, repl[l].reshape(-1, ch.stride)[:S])                 # byte copy
+        np.testing.assert_array_equal(ch.masters[l][ch.idx[:S]].astype(np.float64), from_storage(rows, O.BF16)[:, DC:])
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n", [1, 20, 100])
+def test_gpu_master_chain_matches_oracle(n):
+    import torch
+    from paper_2606_01065_b200 import binding as B
+    seed = 9
+    rng = np.random.default_rng(1000 + seed)
+    s0 = int(rng.integers(1024, 4096))
+    deltas = chain_deltas(rng, n, s0)
+    raw, rows = initial_rows(rng, s0)
+    ch = MasterChain(rows, 2 * CACHE, seed)
+    repl = finite_repl(rng)
+    dev = torch.device("cuda:0")
+    pools = [torch.from_numpy(p.copy()).to(dev) for p in ch.pools]
+    masters = [torch.from_numpy(m.copy()).to(dev) for m in ch.masters]
+    repl_d = [torch.from_numpy(r).to(dev) for r in repl]
+    desc, keep = B.make_desc(N_LAYERS, DC, DR, 1, B.BF16, B.NEOX, ch.stride, ch.n_slots, H64)
+    idx = ch.idx.copy()
+    out = torch.empty(CACHE, dtype=torch.int32, device=dev)
+    S = s0
+    for step, d in enumerate(deltas):
+        seq, pto, pages, dirs, free = ch.step_inputs(S, d)
+        plan = B.leyline_plan(desc, B.ROTATE_ONLY, seq, pto, idx, dirs, free)
+        if step == 0:
+            # single-step parity from identical state: master within a few fp32 roundings, band within 1 bf16 code
+            B.leyline_rotate_inplace_master(plan, pools, masters, repl_d, out)
+            ch.step(S, d, repl)
+            L_new = int(plan.new_seq_lens[0])
+            idx = out[:L_new].cpu().numpy()
+            np.testing.assert_array_equal(idx, ch.idx)
+            for l in range(N_LAYERS):
+                g_m, o_m = masters[l].cpu().numpy().astype(np.float64), ch.masters[l].astype(np.float64)
+                rho = np.sqrt(o_m[:, :DR // 2] ** 2 + o_m[:, DR // 2:] ** 2)
+                assert (np.abs(g_m - o_m) <= 4 * 2.0 ** -24 * np.concatenate([rho, rho], axis=1) + 1e-30).all()
+                g_p, o_p = pools[l].cpu().numpy().reshape(-1, ch.stride), ch.pools[l].reshape(-1, ch.stride)
+                np.testing.assert_array_equal(g_p[:, :DC * 2], o_p[:, :DC * 2])                     # latent untouched
+                # tolerance T of DESIGN.md: 1 bf16 code, or the cancellation floor 2^-20 * rho where the result is tiny
+                far = np.abs(_bf16_ord(g_p[:, DC * 2:].copy().view(np.uint16)) - _bf16_ord(o_p[:, DC * 2:].copy().view(np.uint16))) > 1
+                gv, ov = from_storage(g_p, O.BF16)[:, DC:], from_storage(o_p, O.BF16)[:, DC:]
+                assert (np.abs(gv - ov)[far] <= (2.0 ** -20 * np.concatenate([rho, rho], axis=1))[far]).all()
+        else:
+            B.leyline_rotate_inplace_master(plan, pools, masters, repl_d, out)
+            ch.step(S, d, repl)
+            L_new = int(plan.new_seq_lens[0])
+            idx = out[:L_new].cpu().numpy()
+            np.testing.assert_array_equal(idx, ch.idx)
+        plan.close()
+        S += d
+    del keep
+    torch.cuda.synchronize()
+    ref = fresh_reference(raw, s0, deltas)
+    tr = idx[-N_TRACKED:]
+    g_master = np.stack([m.cpu().numpy()[tr] for m in masters])
+    g_band_bits = np.stack([p.cpu().numpy().reshape(-1, ch.stride)[tr, DC * 2:].copy().view(np.uint16) for p in pools])
+    np.testing.assert_array_equal(g_band_bits, bf16_bits_of_f32(g_master))          # band = one RNE of the master
+    assert np.abs(g_master - ref).max() <= (n + 2) * 2.0 ** -23 * np.abs(ref).max()
+    g_band = np.stack([from_storage(p.cpu().numpy().reshape(-1, ch.stride)[tr], O.BF16)[:, DC:] for p in pools])
+    rg, ro = rel_l2(g_band, ref), rel_l2(ch.tracked(), ref)
+    print(f"[drift, fp32 master] N={n}: rel-L2 vs fresh  gpu {rg:.3e}  oracle {ro:.3e}  (no master, Table 6 N=2: {T6['rel_l2'][0]:.1e})")
+    assert rg <= 2.0 ** -7 / np.sqrt(12.0) and abs(rg - ro) <= 0.05 * ro
+    # a cache of another dtype, or a plan of another mode, is refused
+    w8, keep8 = B.make_desc(N_LAYERS, 16, DR, 1, B.FP8_E4M3, B.NEOX, 80, ch.n_slots, H64)
+    p8 = B.leyline_plan(w8, B.ROTATE_ONLY, [4], [0, 4], [0, 1, 2, 3], [], [9])
+    with pytest.raises(B.LeylineError) as ei:
+        B.leyline_rotate_inplace_master(p8, pools, masters, None, out)
+    assert ei.value.status == B.E_UNSUPPORTED
+    p8.close()
