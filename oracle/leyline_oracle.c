@@ -21,13 +21,15 @@
  *                                                        :650 fp32-or-better trig, downcast on store)
  *   O4' ora_rerope_pair     brute-force re-RoPE R(p+C) R(-p) k, the second independent path
  *                                                       (PAPER.md:110 K_pe[i]=R(i)K_raw[i]; :509)
+ *   O5  ora_rotate_master_layer  the re-anchor option: fp32 master of the band, rotated in fp64 and rounded once to
+ *                                                       fp32, band = RNE_bf16(master) (reading R1)
  *   codecs                  bf16 / e4m3 <-> fp64, direct round-to-nearest-even from fp64.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): paper's worked example 5+57+9 / stub 11,
  * closure, fresh-RoPE equality, logit preservation, O4 vs O4', 2*pi periods, hand 2x2 rotation,
  * codec sweeps against torch's converters, brute-force list slicing for the maps.
- * Unpinned by the paper (pinned only by the rules in DESIGN.md + brute force): page rules M1-M3
- * and the fp8 cache semantics ("parity unpinned" by the paper).
+ * Unpinned by the paper (pinned only by the rules in DESIGN.md + brute force): page rules M1-M3,
+ * the fp8 cache semantics and the master-band reading R1 ("parity unpinned" by the paper).
  */
 #include <math.h>
 #include <stdint.h>
