@@ -237,12 +237,11 @@ def time_single_calls(cache, w, mode: int, reps: int = 10):
             "us_per_directive": float(np.median(out)) / max(1, len(w.directives))}
 
 
-def time_discovery(dev, n_sessions: int = 16, prompt_len: int = 17000, reps: int = 20):
+def time_discovery(dev, with_oracle: bool, n_sessions: int = 16, prompt_len: int = 17000, reps: int = 20):
     """Supplementary line: the discovery side (leyline_cdc_chunk) on the shape of the paper's
     microbenchmark -- 16 sessions x ~17 K-token prompts, anchors every ~600 tokens -- against
     the oracle's sequential chunker on the host."""
     import torch
-    from oracle import cdc as OC
     from paper_2606_01065_b200 import binding as B
     rng = np.random.default_rng(17)
     n = n_sessions * prompt_len
@@ -272,14 +271,17 @@ def time_discovery(dev, n_sessions: int = 16, prompt_len: int = 17000, reps: int
     e1.record()
     torch.cuda.synchronize()
     gpu_ms = e0.elapsed_time(e1) / reps
-    t0 = time.perf_counter()
-    o_end, o_hash, o_kind = OC.chunk(0x5EED, 16, 256, 6, t, so, anchors)
-    cpu_ms = (time.perf_counter() - t0) * 1e3
     c = int(cnt.item())
-    same = c == len(o_end) and bool((end[:c].cpu().numpy() == o_end).all()) and \
-        bool((hsh[:c].cpu().numpy().view(np.uint64) == o_hash).all())
-    return {"tokens": n, "chunks": c, "gpu_ms": gpu_ms, "gpu_Mtok_per_s": n / gpu_ms / 1e3, "oracle_ms": cpu_ms,
-            "oracle_Mtok_per_s": n / cpu_ms / 1e3, "matches_oracle": same}
+    out = {"tokens": n, "chunks": c, "gpu_ms": gpu_ms, "gpu_Mtok_per_s": n / gpu_ms / 1e3}
+    if with_oracle:      # part of the cpu_baseline leg: the oracle's sequential chunker timed on the host beside it
+        from oracle import cdc as OC
+        t0 = time.perf_counter()
+        o_end, o_hash, o_kind = OC.chunk(0x5EED, 16, 256, 6, t, so, anchors)
+        cpu_ms = (time.perf_counter() - t0) * 1e3
+        same = c == len(o_end) and bool((end[:c].cpu().numpy() == o_end).all()) and \
+            bool((hsh[:c].cpu().numpy().view(np.uint64) == o_hash).all())
+        out.update(oracle_ms=cpu_ms, oracle_Mtok_per_s=n / cpu_ms / 1e3, matches_oracle=same)
+    return out
 
 
 def cpu_baseline_all_cores(pools, repls, scales, w, mode: int, bytes_per_layer: int, n_layers: int = 48):
@@ -439,7 +441,7 @@ def run_ours(args):
                                 "kernel_GBps": x["bytes"] / x["kernel_ms"] / 1e6, "bytes": x["bytes"]}
             cache.w = w
             extras["single_call_idle_gpu"] = time_single_calls(cache, w, mode)
-            extras["discovery_cdc"] = time_discovery(cache.device)
+            extras["discovery_cdc"] = time_discovery(cache.device, with_oracle=not args.no_cpu_baseline)
             out["extras"] = extras
         if not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(lambda l: cache.pools[l].cpu().numpy(), lambda l: cache.repl[l].cpu().numpy(),
