@@ -345,3 +345,47 @@ def test_gpu_master_chain_matches_oracle(n):
         B.leyline_rotate_inplace_master(p8, pools, masters, None, out)
     assert ei.value.status == B.E_UNSUPPORTED
     p8.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("pairing", [synth.NEOX, synth.INTERLEAVED])
+@pytest.mark.parametrize("page", [1, 16])
+def test_gpu_master_single_step_paged_multi_request(pairing, page):
+    """The master option on paged pools, several requests, several directives, both pairings: one call against the
+    oracle from identical state (pool bytes outside rotated bands bit-exact, master and band within tolerance)."""
+    import torch
+    from paper_2606_01065_b200 import binding as B
+    from paper_2606_01065_b200 import harness
+    from parity import oracle_plan, oracle_slot_list
+    from test_plan_host import tiny_workload
+    rng = np.random.default_rng(700 + page + pairing)
+    for _ in range(4):
+        w = tiny_workload(rng, P=page, n_req=3)
+        w.pairing = pairing
+        cache = harness.DeviceCache(w, "cuda:0")
+        band0 = w.latent_dim * 2
+        masters = [p.view(torch.bfloat16).view(w.n_slots, -1)[:, w.latent_dim:].float().contiguous() for p in cache.pools]
+        pools_o = [p.cpu().numpy().copy() for p in cache.pools]
+        masters_o = [m.cpu().numpy().copy() for m in masters]
+        desc, keep = cache.desc()
+        plan = harness.plan_workload(w, B.ROTATE_ONLY, desc)
+        idx = torch.empty(max(int(plan.info.total_new_tokens), 1), dtype=torch.int32, device="cuda:0")
+        B.leyline_rotate_inplace_master(plan, cache.pools, masters, cache.repl, idx)
+        torch.cuda.synchronize()
+        bm = oracle_plan(w, O.ROTATE_ONLY)
+        np.testing.assert_array_equal(idx.cpu().numpy()[:int(plan.info.total_new_tokens)], oracle_slot_list(bm))
+        for l in range(w.n_layers):
+            O.rotate_master_layer(pairing, w.latent_dim, w.rope_dim, w.row_bytes, w.inv_freq, pools_o[l], masters_o[l],
+                                  cache.repl[l].cpu().numpy(), bm)
+            g_p = cache.pools[l].cpu().numpy().reshape(-1, w.row_bytes)
+            o_p = pools_o[l].reshape(-1, w.row_bytes)
+            np.testing.assert_array_equal(g_p[:, :band0], o_p[:, :band0])
+            g_m, o_m = masters[l].cpu().numpy().astype(np.float64), masters_o[l].astype(np.float64)
+            finite = np.isfinite(o_m) & np.isfinite(g_m)
+            assert (np.isfinite(o_m) == np.isfinite(g_m)).all()
+            scale = np.abs(np.where(finite, o_m, 0)).max(axis=1, keepdims=True) * np.sqrt(2.0) + 1e-30
+            assert (np.abs(np.where(finite, g_m - o_m, 0)) <= 4 * 2.0 ** -24 * scale).all()
+            # band = one RNE of the (GPU) master, bit for bit
+            np.testing.assert_array_equal(g_p[:, band0:].copy().view(np.uint16)[finite], bf16_bits_of_f32(g_m.astype(np.float32))[finite])
+        plan.close()
+        del keep
