@@ -12,6 +12,7 @@
 #include <cmath>
 #include <cstring>
 #include <map>
+#include <mutex>
 #include <new>
 
 #include "plan_internal.h"
@@ -147,6 +148,54 @@ int choose_rot_tile_rows(const leyline_cache_desc& c, int E, const leyline_tunin
     return (int)std::max<int64_t>(1, std::min(want, cap));
 }
 
+/* A plan per turn is the steady state of a server: the large tables of a destroyed plan (tiles, page tables, released
+ * list, ...) are handed to the next plan instead of going back to the allocator, which would return them to the OS
+ * and make the next plan fault every page in again (measured: 130 of the 140 us of a config-3 plan). */
+struct PlanBuffers {
+    std::vector<DevTile> tiles;
+    std::vector<int32_t> tabs, released, new_pages;
+    std::vector<float> trig;
+    std::vector<leyline_segment> segments;
+    std::vector<IdxRun> slot_runs, page_runs;
+};
+std::mutex g_recycle_mu;
+std::vector<PlanBuffers> g_recycled;
+constexpr size_t kMaxRecycled = 8;
+
+void take_buffers(leyline_plan_s* pl) {
+    std::lock_guard<std::mutex> lk(g_recycle_mu);
+    if (g_recycled.empty()) return;
+    PlanBuffers b = std::move(g_recycled.back());
+    g_recycled.pop_back();
+    pl->tiles = std::move(b.tiles);         pl->tiles.clear();
+    pl->tabs = std::move(b.tabs);           pl->tabs.clear();
+    pl->released = std::move(b.released);   pl->released.clear();
+    pl->new_pages = std::move(b.new_pages); pl->new_pages.clear();
+    pl->trig = std::move(b.trig);           pl->trig.clear();
+    pl->segments = std::move(b.segments);   pl->segments.clear();
+    pl->slot_runs = std::move(b.slot_runs); pl->slot_runs.clear();
+    pl->page_runs = std::move(b.page_runs); pl->page_runs.clear();
+}
+
+void give_buffers(leyline_plan_s* pl) {
+    PlanBuffers b;
+    b.tiles = std::move(pl->tiles);
+    b.tabs = std::move(pl->tabs);
+    b.released = std::move(pl->released);
+    b.new_pages = std::move(pl->new_pages);
+    b.trig = std::move(pl->trig);
+    b.segments = std::move(pl->segments);
+    b.slot_runs = std::move(pl->slot_runs);
+    b.page_runs = std::move(pl->page_runs);
+    std::lock_guard<std::mutex> lk(g_recycle_mu);
+    if (g_recycled.size() < kMaxRecycled) g_recycled.push_back(std::move(b));
+}
+
+void discard(leyline_plan_s* pl) { /* a plan abandoned half-built: its buffers are still worth keeping */
+    give_buffers(pl);
+    delete pl;
+}
+
 /* split [dst0, dst0+len) into tiles whose boundaries are multiples of tile_rows in `align_pos` space */
 template <class F>
 void split_tiles(int64_t src0, int64_t dst0, int64_t len, int64_t align0, int tile_rows, F&& emit) {
@@ -193,6 +242,7 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
 
     leyline_plan_s* pl = new (std::nothrow) leyline_plan_s();
     if (!pl) return LEYLINE_E_INVALID;
+    take_buffers(pl);
     pl->desc = *desc;
     const int H = desc->rope_dim / 2;
     pl->inv_freq.assign(desc->inv_freq, desc->inv_freq + H);
@@ -210,7 +260,7 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
     pl->n_heads = heads_of(*desc);
     pl->head_chunks = desc->rope_dim * E / 16;
     if (g_tuning.kernel == 1 && !row_kernel_ok(*desc, E)) { /* forced row kernel on a band it does not cover */
-        delete pl;
+        discard(pl);
         return LEYLINE_E_UNSUPPORTED;
     }
     pl->use_bulk = choose_bulk(*desc, E, g_tuning, mode);
@@ -256,7 +306,8 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
     struct ReqWork { std::vector<Seg> segs; int64_t k0; int32_t new_tab; };
     std::vector<ReqWork> work(n_requests);
     std::vector<int32_t> token_lists;               /* ROTATE_ONLY: consumed free slots, in consumption order */
-    std::vector<DevTile> move_tiles, insert_tiles;
+    std::vector<DevTile> move_tiles = std::move(pl->tiles), insert_tiles; /* the recycled capacity, if any */
+    move_tiles.clear();
     int64_t consumed = 0;
     int32_t di = 0;
     bool nofree = false, badfree = false;
@@ -327,7 +378,7 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
         pl->new_pt_offsets[r + 1] = (int64_t)pl->new_pages.size();
     }
     if (nofree || badfree) {
-        delete pl;
+        discard(pl);
         return nofree ? LEYLINE_E_NOFREE : LEYLINE_E_RANGE;
     }
 
@@ -384,7 +435,10 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
                             });
             }
         } else { /* INPLACE_MOVE, rule M2 */
-            std::vector<DevTile> left, right;
+            /* per-thread scratch that keeps its capacity from plan to plan (same reason as PlanBuffers) */
+            static thread_local std::vector<DevTile> left, right;
+            left.clear();
+            right.clear();
             const size_t first_insert = insert_tiles.size();
             for (const Seg& s : w.segs) {
                 if (s.kind == 1) {
@@ -548,6 +602,7 @@ extern "C" leyline_status leyline_plan_trig_table(const leyline_plan_t* plan, fl
 extern "C" void leyline_plan_destroy(leyline_plan_t* plan) {
     if (!plan) return;
     leyline_plan_release_device_(plan);
+    give_buffers(plan);
     delete plan;
 }
 
