@@ -173,6 +173,28 @@ __global__ void __launch_bounds__(kThreads, DT == LEYLINE_FP8_E4M3 ? 2 : 3) k_ro
     };
     long long item = blockIdx.x;
     Item cur, nxt;
+    if (cols > kThreads * kRotUnroll) {
+        /* a row with more pair columns than one block pass holds (e.g. 128 heads x 256: 2048 columns; the planner
+         * then makes one-row items): plain strided loop over the row's units, no pipelining */
+        for (; item < p.n_items; item += gridDim.x) {
+            const DevTile t = p.tiles[p.tile_begin + (int)(item / p.n_layers)];
+            uint8_t* __restrict__ base = p.dst[(int)(item % p.n_layers)];
+            const float* __restrict__ trig_row = p.trig + (int64_t)t.trig * 2 * p.H;
+            const int total = t.n_rows * cols;
+            for (int u = tid; u < total; u += kThreads) {
+                const int r = u / cols, col = u - r * cols;
+                const int head = col / half, q = col - head * half;
+                uint8_t* a = base + slot_of(p.tabs, t.src_tab, t.src_pos + r, p.page_shift) * p.stride + band0 +
+                             (int64_t)(head * p.head_chunks + q) * 16;
+                int4 lo = ld_coherent(a), hi = ld_coherent(a + half * 16);
+                float c[N], s[N];
+                load_pair_trig<DT, PAIRING>(trig_row, p.H, q, half, c, s);
+                rotate_chunk_pair<DT, PAIRING>(lo, hi, c, s);
+                st_stream(a, lo);
+                st_stream(a + half * 16, hi);
+            }
+        }
+    }
     if (item < p.n_items) resolve(item, cur);
     while (item < p.n_items) {
         uint8_t* __restrict__ base = p.dst[cur.layer];

@@ -412,3 +412,31 @@ def test_two_host_threads_drive_the_library_at_once():
         for l in range(c.w.n_layers):
             compare_layer(c.w, bm, m, olds[i][l], c.pools[l].cpu().numpy(), c.repl[l].cpu().numpy(), c.scales[l], layer=l)
         plan.close()
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("heads,d,latent,dtype", [
+    (128, 256, 0, synth.DT_BF16),      # the largest row the library takes: 128 heads x 256 = 65,536 B (one row per tile)
+    (2, 512, 0, synth.DT_BF16),        # the widest head: 64 chunks
+    (128, 32, 2048, synth.DT_FP8),     # most heads of the narrowest kind (one chunk per half) behind a wide latent
+    (1, 32, 32736, synth.DT_BF16),     # a 64 KB row that is nearly all latent, with a small bf16 band
+])
+def test_maximum_geometries(mode, heads, d, latent, dtype):
+    """leyline.h limits: head <= 64 chunks, <= 128 heads, rows <= 64 KB."""
+    w = synth.Workload("max_geom", 2, [300, 41], 16, dtype=dtype, latent_dim=latent, rope_dim=d, rope_heads=heads,
+                       inv_freq=synth.rope_inv_freq(d, 1.0e4),
+                       directives=[(0, 10, 50, 7, 0, 0), (0, 200, 201, 30, 0, 0), (1, 0, 3, 0, 0, 0)],
+                       seed=64, pool_factor=3.0, extra_pages=8).finalize()
+    assert w.row_bytes <= 65536
+    run_and_compare(w, mode)
+
+
+def test_geometries_beyond_the_limits_are_refused():
+    from paper_2606_01065_b200 import binding as B
+    for heads, d, latent in ((129, 16, 0), (1, 1024, 0), (128, 256, 16), (1, 24, 0)):
+        w = synth.Workload("too_big", 1, [16], 16, latent_dim=latent, rope_dim=d, rope_heads=heads,
+                           inv_freq=synth.rope_inv_freq(d, 1.0e4), directives=[], seed=1, pool_factor=2.0).finalize()
+        desc, keep = B.make_desc(1, latent, d, 16, B.BF16, B.NEOX, w.row_bytes, w.n_slots, w.inv_freq, rope_heads=heads)
+        with pytest.raises(B.LeylineError) as ei:
+            B.leyline_plan(desc, B.FRESH, w.seq_lens, w.pt_offsets, w.pages, [], w.free_pages)
+        assert ei.value.status == B.E_UNSUPPORTED, (heads, d, latent)
