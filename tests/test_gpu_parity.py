@@ -440,3 +440,28 @@ def test_geometries_beyond_the_limits_are_refused():
         with pytest.raises(B.LeylineError) as ei:
             B.leyline_plan(desc, B.FRESH, w.seq_lens, w.pt_offsets, w.pages, [], w.free_pages)
         assert ei.value.status == B.E_UNSUPPORTED, (heads, d, latent)
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("page", [256, 1024])
+def test_large_pages(mode, page):
+    """Pages larger than a tile and larger than the requests' edits: tiles never straddle more than two pages, runs are
+    capped by the tile, the boundary page of FRESH is copied from its head."""
+    w = synth.Workload("large_pages", 2, [5000, 1300], page, inv_freq=synth.yarn_inv_freq(),
+                       directives=[(0, 300, 1100, 77, 0, 0), (0, 3000, 3001, 600, 0, 0), (1, 1290, 1300, 0, 0, 0)],
+                       seed=256, pool_factor=3.0, extra_pages=4).finalize()
+    for mover in MOVERS:
+        run_and_compare(w, mode, tuning={"kernel": mover})
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("mixed", [False, True])
+def test_more_layers_than_one_launch_holds(mode, mixed):
+    """LEYLINE_MAX_LAYERS_PER_LAUNCH = 128: 130 layers (two conventions mixed) take several launches per mover; hazard
+    flags are numbered per launch."""
+    rng = np.random.default_rng(130)
+    w = tiny_workload(rng, P=4, n_req=2)
+    w.n_layers = 130
+    w.layer_pairing = [int(x) for x in rng.integers(0, 2, size=130)] if mixed else None     # one convention: 128 + 2 layers
+    for mover in MOVERS:
+        run_and_compare(w, mode, tuning={"kernel": mover}, check_layers=[0, 1, 64, 127, 128, 129])
