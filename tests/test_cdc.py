@@ -315,3 +315,20 @@ def test_gpu_registry_and_discovery_returns_the_edits_delta():
                               torch.from_numpy(b_start.astype(np.int64)).to(dev), bc, dropped)
     torch.cuda.synchronize()
     assert int(dropped.item()) == len(set(b_hash.tolist())) - 8
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("mn,mx,bits", [(1, 1, 0), (1, 1, 6), (7, 7, 3), (4096, 4096, 0), (1, 4096, 32), (64, 4096, 12), (1, 2, 1)])
+def test_gpu_chunker_parameter_extremes(mn, mx, bits):
+    """Every token its own chunk, fixed-size chunks, the largest chunk size, a mask that never / always fires; thousands
+    of tiny sequences next to long ones (more sequences than one grid pass of k_cdc_seq_ends)."""
+    rng = np.random.default_rng(mn * 31 + mx * 7 + bits)
+    lens = [int(x) for x in rng.integers(0, 4, size=70000)] + [50000, 0, 9000] + [int(x) for x in rng.integers(0, 3, size=5000)]
+    t = random_prompt(rng, sum(lens), vocab=1000, anchor_every=500)
+    so = [0, *np.cumsum(lens).tolist()]
+    c, end, hsh, kind, _ = gpu_chunk(t, so, ANCHORS, SEED, mn, mx, bits)
+    o_end, o_hash, o_kind = OC.chunk(SEED, mn, mx, bits, t, so, ANCHORS)
+    assert c == len(o_end)
+    np.testing.assert_array_equal(end, o_end)
+    np.testing.assert_array_equal(kind, o_kind)
+    np.testing.assert_array_equal(hsh, o_hash)

@@ -132,6 +132,14 @@ def test_prefetched_tables(mode, mover):
     """leyline_plan_prefetch: tables uploaded on the library's copy stream, the launch only waits on the event."""
     rng = np.random.default_rng(77)
     run_and_compare(tiny_workload(rng, P=16, n_req=3), mode, tuning={"kernel": mover}, prefetch=True)
+    # a prefetched plan that is never launched gives its tables back on the copy stream
+    from paper_2606_01065_b200 import harness
+    w = tiny_workload(rng, P=16, n_req=2)
+    d, keep = harness.DeviceCache(w, "cuda:0", fill=False).desc()
+    for _ in range(3):
+        harness.plan_workload(w, mode, d).prefetch().close()
+    torch.cuda.synchronize()
+    del keep
 
 
 @pytest.mark.parametrize("prefetch", [False, True])
