@@ -473,3 +473,41 @@ def test_more_layers_than_one_launch_holds(mode, mixed):
     w.layer_pairing = [int(x) for x in rng.integers(0, 2, size=130)] if mixed else None     # one convention: 128 + 2 layers
     for mover in MOVERS:
         run_and_compare(w, mode, tuning={"kernel": mover}, check_layers=[0, 1, 64, 127, 128, 129])
+
+
+def fuzz_workload(rng):
+    """Several requests of up to a few thousand tokens, up to 6 directives each with the edit shapes of the paper's
+    randomised suites (spans U[8,200] or long, |R| in [0, 2|span|], both signs), random page size,
+    storage type, pairing and band geometry."""
+    P = int(rng.choice([1, 2, 8, 16, 64, 128]))
+    n_req = int(rng.integers(1, 7))
+    seq_lens = [int(rng.integers(0, 6000)) for _ in range(n_req)]
+    dirs = []
+    for r, L in enumerate(seq_lens):
+        k = int(rng.integers(0, 7))
+        cuts = np.sort(rng.integers(0, L + 1, size=2 * k))
+        for j in range(k):
+            s, e = int(cuts[2 * j]), int(cuts[2 * j + 1])
+            if rng.random() < 0.6:
+                e = min(e, s + int(rng.integers(8, 201)))
+            n = int(rng.integers(0, 2 * (e - s) + 3)) if rng.random() < 0.85 else 0
+            dirs.append((r, s, e, min(n, 700), 0, 0))
+    geom = [(512, 64, 1), (0, 128, 2), (64, 96, 3), (16, 32, 1)][int(rng.integers(0, 4))]
+    w = synth.Workload("fuzz", 2, seq_lens, P, dtype=int(rng.integers(0, 2)), pairing=int(rng.integers(0, 2)),
+                       latent_dim=geom[0], rope_dim=geom[1], rope_heads=geom[2],
+                       inv_freq=synth.rope_inv_freq(geom[1], float(rng.choice([1.0e4, 5.0e5]))), directives=dirs,
+                       seed=int(rng.integers(1 << 30)), pool_factor=2.5, extra_pages=sum(d[3] for d in dirs) // P + 16)
+    return w.finalize()
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("seed", range(4))
+def test_fuzz_medium(mode, seed):
+    rng = np.random.default_rng(31337 + 17 * seed + mode)
+    for _ in range(6):
+        w = fuzz_workload(rng)
+        tuning = {"kernel": int(rng.choice([0, 2])), "tile_rows": int(rng.choice([0, 0, 5, 16, 64])),
+                  "stages": int(rng.choice([0, 3, 5])), "layer_group": int(rng.choice([0, 1, 2]))}
+        if w.rope_heads == 1 and w.rope_dim in (32, 64) and rng.random() < 0.4:
+            tuning = {"kernel": 1, "tile_rows": int(rng.choice([0, 3, 32]))}
+        run_and_compare(w, mode, tuning=tuning, prefetch=bool(rng.integers(0, 2)))
