@@ -22,11 +22,15 @@
  * (bf16, or fp8 e4m3 with one fp32 scale per layer).  Page p of a layer is rows [p*page_size, (p+1)*page_size).
  * A request's logical position t lives at slot  table[t / page_size] * page_size + t % page_size.
  *
- * Threading / streams: leyline_plan is pure host code (no CUDA call, no device needed).  leyline_splice and
- * leyline_rotate_inplace upload the plan's tables on first use (stream-ordered), launch on the caller's
- * stream and return without synchronising.  A plan may be in flight on one stream at a time.
+ * Threading / streams: leyline_plan is pure host code (no CUDA call, no device needed).  leyline_splice,
+ * leyline_rotate_inplace and leyline_rotate_inplace_master upload the plan's tables on first use (stream-ordered; or
+ * earlier, on the library's copy stream, after leyline_plan_prefetch), launch one index kernel and one data kernel on
+ * the caller's stream and return without synchronising.  A plan may be in flight on one stream at a time; different
+ * plans may be in flight on different streams and may be driven from different host threads.
+ * leyline_set_tuning is a process-wide benchmarking knob and is not synchronised with concurrent leyline_plan calls.
  * Nothing is thrown across the ABI: every entry point returns a leyline_status.
- * There is no CPU fallback: without a CUDA device the two launch entry points return LEYLINE_E_CUDA.
+ * There is no CPU fallback: without a CUDA device the launch entry points return LEYLINE_E_CUDA.
+ * The discovery side (chunker, registry) is declared in leyline_cdc.h.
  */
 #ifndef LEYLINE_H_
 #define LEYLINE_H_
