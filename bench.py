@@ -406,7 +406,7 @@ def run_ours(args):
     value = world * r["bytes"] / (ms * 1e-3) / 1e9
     peak, peak_src = peaks()
     kernel_gbs = r["bytes"] / (r["kernel_ms"] * 1e-3) / 1e9
-    kname = "k_rotate_band" if mode == B.ROTATE_ONLY else ("k_move_bulk" if r["mover"] == 2 else "k_move_rows")
+    kname = "k_move_bulk" if r["mover"] == 2 else ("k_rotate_band" if mode == B.ROTATE_ONLY else "k_move_rows")
     traffic, traffic_src = ncu_traffic(args.workload, args.mode, kname)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

@@ -135,7 +135,10 @@ typedef struct {
     int64_t bytes_index;       /* 4 B per new token + 4 B per new page-table entry (once, not per layer) */
     int64_t tile_rows;         /* rows per device work item of the a3/a4 mover chosen for this plan */
     int64_t rot_tile_rows;     /* ROTATE_ONLY: rows per in-place rotation work item (a5), else 0 */
-    int64_t mover;             /* a3/a4 kernel this plan launches: 1 = k_move_rows, 2 = k_move_bulk (see leyline_tuning) */
+    int64_t mover;             /* a3/a4 kernel this plan launches: 1 = k_move_rows, 2 = k_move_bulk (see leyline_tuning).
+                                  ROTATE_ONLY: 1 = k_rotate_band (strided band kernel), 2 = the band is at least half of
+                                  the row (full-width K), so whole rows stream through k_move_bulk and are written back
+                                  to the slots they were read from */
 } leyline_plan_info;
 
 typedef struct leyline_plan_s leyline_plan_t;

@@ -150,7 +150,8 @@ k_move_bulk(const __grid_constant__ MoveParams p, const int n_stages, const int 
                 int64_t s_slot = 0, d_slot = 0;
                 if (valid) {
                     s_slot = from_repl ? t.src_pos + r : slot_of(p.tabs, t.src_tab, t.src_pos + r, p.page_shift);
-                    d_slot = slot_of(p.tabs, t.dst_tab, t.dst_pos + r, (t.flags & TILE_DST_TOKEN) ? 0 : p.page_shift);
+                    d_slot = (t.flags & TILE_DST_IS_SRC) ? s_slot /* in-place rotation: back where it came from */
+                                                         : slot_of(p.tabs, t.dst_tab, t.dst_pos + r, (t.flags & TILE_DST_TOKEN) ? 0 : p.page_shift);
                 }
                 s_off[half] = s_slot * p.stride;
                 d_off[half] = d_slot * p.stride;

@@ -266,6 +266,17 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
     pl->use_bulk = choose_bulk(*desc, E, g_tuning, mode);
     pl->tile_rows = choose_tile_rows(*desc, E, g_tuning, pl->use_bulk);
     pl->rot_tile_rows = mode == LEYLINE_ROTATE_ONLY ? choose_rot_tile_rows(*desc, E, g_tuning) : 0;
+    /* ROTATE_ONLY on a full-width K pool rewrites most of every row anyway: whole rows then
+     * stream through the bulk mover and come back to the slots they were read from (measured: GQA 6.42 -> 6.7 TB/s,
+     * head_dim 96 5.86 -> 6.5), instead of the strided band kernel that MLA's 1/9 band needs */
+    pl->rotate_with_bulk = mode == LEYLINE_ROTATE_ONLY && g_tuning.kernel != 1 &&
+                           2 * (int64_t)heads_of(*desc) * desc->rope_dim >= row_elems(*desc) &&
+                           desc->row_stride_bytes == row_elems(*desc) * E;
+    if (pl->rotate_with_bulk) {
+        pl->use_bulk = true;
+        pl->tile_rows = choose_tile_rows(*desc, E, g_tuning, true);
+        pl->rot_tile_rows = pl->tile_rows;
+    }
     const int TR = pl->tile_rows;
     const int TR_ROT = pl->rot_tile_rows;
 
@@ -401,7 +412,8 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
                     int32_t g = trig_index(s.shift);
                     if (g < 0) continue;
                     split_tiles(s.src, s.dst, s.len, s.src, TR_ROT, [&](int64_t a, int64_t b, int32_t n) {
-                        move_tiles.push_back({a, b, src_tab, src_tab, n, g, 0, 0, -1, r});
+                        move_tiles.push_back({a, b, src_tab, src_tab, n, g, pl->rotate_with_bulk ? leyline::TILE_DST_IS_SRC : 0,
+                                              0, -1, r});
                     });
                 } else {
                     int32_t list = token_base + (int32_t)token_cursor;
@@ -525,7 +537,8 @@ extern "C" leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t m
     in.bytes_index = 4 * in.total_new_tokens + 4 * in.total_new_pages;
     in.tile_rows = pl->tile_rows;
     in.rot_tile_rows = pl->rot_tile_rows;
-    in.mover = pl->use_bulk ? 2 : 1;
+    in.mover = pl->use_bulk ? 2 : 1; /* ROTATE_ONLY: 2 = the rotation itself runs on the bulk mover (wide bands) */
+    if (mode == LEYLINE_ROTATE_ONLY && !pl->rotate_with_bulk) in.mover = 1;
     if (mode == LEYLINE_ROTATE_ONLY) pl->new_pages.clear();
 
     if (mode == LEYLINE_INPLACE_MOVE) { /* how far back (in tiles) a waiting tile's dependencies sit: a launch hint */

@@ -31,7 +31,8 @@ struct DevTile {
 };
 static_assert(sizeof(DevTile) == 48, "DevTile layout");
 
-enum : int32_t { TILE_SRC_REPL = 1, TILE_DST_TOKEN = 2 };
+enum : int32_t { TILE_SRC_REPL = 1, TILE_DST_TOKEN = 2,
+                 TILE_DST_IS_SRC = 4 /* rows are written back to the slots they were read from (in-place rotation) */ };
 
 /* k_rotate_band (a5): (row, pair column) units one block handles = 256 threads x 4; ROTATE_ONLY tiles hold at most
  * this many units, i.e. rot_tile_rows = kRotUnitsPerItem / (rope_heads * head_chunks / 2) rows. */
@@ -63,6 +64,7 @@ struct leyline_plan_s {
     int32_t n_heads = 1;                /* heads in the rotated band (desc.rope_heads, 0 read as 1) */
     int32_t head_chunks = 8;            /* 16-byte chunks per head */
     int32_t dep_distance_median = -1;   /* INPLACE_MOVE: median of (tile index - dep_hi) over tiles that wait, -1 if none */
+    bool rotate_with_bulk = false;      /* ROTATE_ONLY on a band that is most of the row: the rotation runs on k_move_bulk, in place */
     bool use_bulk = false;              /* a3/a4 run on k_move_bulk (TMA bulk copies) instead of k_move_rows */
     leyline_tuning tuning{};
 

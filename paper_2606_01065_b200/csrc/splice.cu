@@ -509,7 +509,10 @@ extern "C" leyline_status leyline_rotate_inplace(leyline_plan_t* pl, void* const
     if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_start), stream));
     int slot = 0;
     /* a5: rotate where the rows sit; a4: replacement rows go to the consumed free slots (disjoint from a5's) */
-    st = run_rotate(pl, 0, n_rot, n_ins, layer_ptrs, layer_repl, stream, &slot);
+    if (pl->rotate_with_bulk) /* wide band: whole rows through the bulk mover, written back in place; inserts as usual */
+        st = run_tiles_bulk(pl, false, 0, n_rot + n_ins, layer_ptrs, layer_ptrs, layer_repl, stream, &slot);
+    else
+        st = run_rotate(pl, 0, n_rot, n_ins, layer_ptrs, layer_repl, stream, &slot);
     if (st != LEYLINE_OK) return st;
     if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_stop), stream));
     return LEYLINE_OK;

@@ -138,7 +138,8 @@ def check_tiles_cover(plan, bm, w, mode):
         is_repl = bool(t.flags & B.TILE_SRC_REPL)
         if mode == B.ROTATE_ONLY and not is_repl:     # a5 work items: <= 1024 (row, pair column) units per block
             assert 1 <= t.n_rows <= plan.info.rot_tile_rows
-            assert plan.info.rot_tile_rows * w.rope_heads * (w.rope_dim * w.elem_bytes // 32) <= 1024 or plan.info.rot_tile_rows == 1
+            assert (plan.info.rot_tile_rows * w.rope_heads * (w.rope_dim * w.elem_bytes // 32) <= 1024 or plan.info.rot_tile_rows == 1
+                    or plan.info.mover == 2)
         else:
             assert 1 <= t.n_rows <= plan.info.tile_rows <= 64
         assert is_repl == (t_i >= n_move)
@@ -320,7 +321,7 @@ def test_heads_descriptor_rules():
             row = 8 * 128 * 2
             if mode == B.ROTATE_ONLY:
                 assert i.bytes_read == (i.rows_rotated * row + i.rows_inserted * row) * w.n_layers
-                assert i.rot_tile_rows == 1024 // (8 * 8)
+                assert i.rot_tile_rows == i.tile_rows == 24   # full-width K: the rotation runs on the bulk mover, 48 KB tiles
             else:
                 assert i.bytes_read == (i.rows_moved + i.rows_inserted) * row * w.n_layers
     inv = synth.rope_inv_freq(128, 5e5)
