@@ -218,7 +218,9 @@ leyline_status leyline_plan_trig_table(const leyline_plan_t* plan, float* out);
  *               a host-resident cache is then spliced over PCIe by the same kernels, moving only the rows the plan
  *               touches.
  *   layer_dst   HOST array of n_layers DEVICE pointers to the pools written.  May equal layer_src (fresh pages of
- *               the same pool); MUST equal it for INPLACE_MOVE.
+ *               the same pool); MUST equal it for INPLACE_MOVE.  When it differs (FRESH), page ids mean the same
+ *               pages in both pools and only the fresh pages are written, into layer_dst: e.g. a swapped-out,
+ *               host-resident source spliced straight into the device pool.  The kept prefix pages are not copied.
  *   layer_repl  HOST array of n_layers DEVICE pointers to the replacement KV rows, [rows x row_stride_bytes] per
  *               layer, K_pe already roped at its FINAL position (G12).  NULL = the caller fills the replacement
  *               slots itself -- the paper's own flow, where step (b) is the model's prefill of R into the new

@@ -511,3 +511,57 @@ def test_fuzz_medium(mode, seed):
         if w.rope_heads == 1 and w.rope_dim in (32, 64) and rng.random() < 0.4:
             tuning = {"kernel": 1, "tile_rows": int(rng.choice([0, 3, 32]))}
         run_and_compare(w, mode, tuning=tuning, prefetch=bool(rng.integers(0, 2)))
+
+
+@pytest.mark.parametrize("mover", MOVERS)
+@pytest.mark.parametrize("src_on_host", [False, True])
+def test_fresh_into_a_separate_pool(mover, src_on_host):
+    """leyline.h: for FRESH, layer_dst may differ from layer_src.  Only the fresh pages are written, into layer_dst
+    (page ids are the same in both pools); the source pool -- here optionally a host-resident, swapped-out copy -- is
+    never written, and nothing else of the destination is touched."""
+    from paper_2606_01065_b200 import binding as B
+    from paper_2606_01065_b200 import harness
+    rng = np.random.default_rng(606 + mover)
+    for w in (tiny_workload(rng, P=16, n_req=3), synth.config(1, pool_factor=2.5)):
+        B.leyline_set_tuning(kernel=mover)
+        try:
+            cache = harness.DeviceCache(w, "cuda:0", host_resident=src_on_host)
+            old = [p.clone().numpy() if src_on_host else p.cpu().numpy() for p in cache.pools]
+            dst = [torch.full((w.layer_bytes,), 0xA5, dtype=torch.uint8, device="cuda:0") for _ in cache.pools]
+            desc, keep = cache.desc()
+            plan = harness.plan_workload(w, B.FRESH, desc)
+            B.leyline_splice(plan, cache.pools, dst, cache.repl, None, None)
+            torch.cuda.synchronize()
+        finally:
+            B.leyline_set_tuning()
+        bm = oracle_plan(w, O.FRESH)
+        assert_plan_equal(plan, bm, O.FRESH)
+        fresh_pages = plan.new_pages[~np.isin(plan.new_pages, w.pages)]        # ids taken from the free list
+        rows = (fresh_pages.astype(np.int64)[:, None] * w.page_size + np.arange(w.page_size)[None, :]).reshape(-1)
+        for l in range(w.n_layers):
+            src_now = cache.pools[l].numpy() if src_on_host else cache.pools[l].cpu().numpy()
+            np.testing.assert_array_equal(src_now, old[l])                      # the source is never written
+            want = O.splice_layer(w.dtype, w.pairing, w.latent_dim, w.rope_dim, w.row_bytes, w.inv_freq, cache.scales[l],
+                                  old[l], cache.repl[l].cpu().numpy(), bm).reshape(-1, w.row_bytes)
+            got = dst[l].cpu().numpy().reshape(-1, w.row_bytes)
+            mask = np.zeros(len(got), bool)
+            mask[rows] = True
+            assert (got[~mask] == 0xA5).all()                                   # nothing outside the fresh pages
+            # inside the fresh pages: rows the plan wrote equal the oracle's; slots past L_new in a last page stay canary
+            live = np.zeros(len(got), bool)
+            for rm in bm.requests:
+                live[rm.slot_new.astype(np.int64)] = True
+            live &= mask
+            assert (got[mask & ~live] == 0xA5).all()
+            gl, wl = got[live], want[live]
+            band0 = w.latent_dim * w.elem_bytes
+            np.testing.assert_array_equal(gl[:, :band0], wl[:, :band0])
+            d = np.abs(_ord16(gl[:, band0:]) - _ord16(wl[:, band0:]))
+            assert d.max() <= 2
+        plan.close()
+        del keep
+
+
+def _ord16(b):
+    v = np.ascontiguousarray(b).view(np.uint16).astype(np.int32)
+    return np.where(v & 0x8000, -(v & 0x7FFF), v & 0x7FFF)
