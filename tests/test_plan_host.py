@@ -348,3 +348,50 @@ def test_heads_descriptor_rules():
     d, k = B.make_desc(1, 512, 64, 16, 0, 0, 1152, w.n_slots, synth.rope_inv_freq(64), rope_heads=0)
     with B.leyline_plan(d, B.FRESH, w.seq_lens, w.pt_offsets, w.pages, w.directives, w.free_pages) as plan:
         assert plan.info.bytes_read == (plan.info.rows_moved + plan.info.rows_inserted) * 1152
+
+
+def test_headers_are_plain_c_and_the_abi_links_from_c(tmp_path):
+    """The boundary is a C ABI: both headers compile as C99 with -Wall -Werror -pedantic, and a C program linked
+    against libleyline.so plans the paper's worked example (5 + 57 + 9 tokens, 11-token stub: Delta = -46, L 71 -> 25;
+    PAPER.md:155) and prints what the getters return.  Host only; no device call is made."""
+    import subprocess
+    src = tmp_path / "abi.c"
+    src.write_text(r'''
+#include <stdio.h>
+#include "leyline.h"
+#include "leyline_cdc.h"
+int main(void) {
+    float inv_freq[32];
+    int i;
+    for (i = 0; i < 32; ++i) inv_freq[i] = 1.0f / (float)(i + 1);
+    leyline_cache_desc c = {0};
+    c.n_layers = 2; c.latent_dim = 512; c.rope_dim = 64; c.page_size = 1; c.dtype = LEYLINE_BF16;
+    c.pairing = LEYLINE_ROPE_NEOX; c.rope_heads = 1; c.row_stride_bytes = 1152; c.pool_slots = 256; c.inv_freq = inv_freq;
+    int64_t seq_lens[1] = {71}, pt_offsets[2] = {0, 71}, new_len[1] = {0};
+    int32_t pages[71], free_ids[64];
+    for (i = 0; i < 71; ++i) pages[i] = i;
+    for (i = 0; i < 64; ++i) free_ids[i] = 100 + i;
+    leyline_directive d = {0};
+    d.request = 0; d.start = 5; d.end = 62; d.repl_len = 11; d.repl_row = 0; d.semantic = LEYLINE_AMORTIZE;
+    leyline_plan_t* plan = 0;
+    leyline_status st = leyline_plan(&c, LEYLINE_FRESH, 1, seq_lens, pt_offsets, pages, 1, &d, free_ids, 64, &plan);
+    if (st != LEYLINE_OK) { printf("plan failed: %s\n", leyline_strerror(st)); return 1; }
+    leyline_plan_info info;
+    leyline_plan_get_info(plan, &info);
+    leyline_plan_new_seq_lens(plan, new_len);
+    printf("L_new=%lld consumed=%lld released=%lld rows_moved=%lld rows_inserted=%lld version=%s\n", (long long)new_len[0],
+           (long long)info.n_free_consumed, (long long)info.n_released, (long long)info.rows_moved,
+           (long long)info.rows_inserted, leyline_version());
+    leyline_plan_destroy(plan);
+    return 0;
+}
+''')
+    exe = tmp_path / "abi"
+    inc = os.path.join(ROOT, "include")
+    libdir = os.path.dirname(B.LIB_PATH)
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Wextra", "-Werror", "-pedantic", "-I", inc, str(src), "-o", str(exe),
+                    "-L", libdir, "-lleyline", f"-Wl,-rpath,{libdir}"], check=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout
+    # tokens 5..61 removed, 11 inserted, 9 downstream tokens moved by -46; token-level FRESH keeps slots [0, 5)
+    assert "L_new=25 consumed=20 released=66 rows_moved=9 rows_inserted=11" in out, out
+    assert "sm_100a" in out
