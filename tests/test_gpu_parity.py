@@ -565,3 +565,19 @@ def test_fresh_into_a_separate_pool(mover, src_on_host):
 def _ord16(b):
     v = np.ascontiguousarray(b).view(np.uint16).astype(np.int32)
     return np.where(v & 0x8000, -(v & 0x7FFF), v & 0x7FFF)
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_paper_section_4_1_layout(mode):
+    """The paper's constructed prompt: 5 prefix tokens, a 57-token chunk replaced by an 11-token stub,
+    9 post tokens -- Delta = -46, L 71 -> 25, post tokens 62..70 -> 16..24 -- on the DeepSeek-V2-Lite shape (27 layers,
+    token-level slots, NeoX and interleaved)."""
+    g = __import__("helpers").golden("paper_worked_example.txt")
+    pre, chunk, post, stub = int(g["pre_tokens"]), int(g["chunk_tokens"]), int(g["post_tokens"]), int(g["stub_tokens"])
+    for pairing in (synth.NEOX, synth.INTERLEAVED):
+        w = synth.Workload("sec4_1", 27, [pre + chunk + post], 1, pairing=pairing, inv_freq=synth.rope_inv_freq(64, 10000.0),
+                           directives=[(0, pre, pre + chunk, stub, 0, 0)], seed=41, pool_factor=3.0, extra_pages=16).finalize()
+        stats = run_and_compare(w, mode)
+        bm = oracle_plan(w, mode)
+        assert bm.requests[0].L_new == pre + chunk + post + int(g["delta"]) == 25
+        assert sum(s["rotated_elems"] for s in stats) == post * 64 * 27
