@@ -581,3 +581,59 @@ def test_paper_section_4_1_layout(mode):
         bm = oracle_plan(w, mode)
         assert bm.requests[0].L_new == pre + chunk + post + int(g["delta"]) == 25
         assert sum(s["rotated_elems"] for s in stats) == post * 64 * 27
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_attention_logits_are_preserved_on_the_device(mode):
+    """The property the method exists for (north_star "q.k logits are preserved for every query
+    position"): after a three-directive splice executed by the CUDA path, (R(m) q) . K_pe_new[n] equals the
+    relative-position logit computed from the RAW keys, for every query position m and every key n -- to the accuracy
+    the bf16 cache allows (two roundings: the stored input, the stored output)."""
+    from helpers import list_splice, rope_complex, to_storage, from_storage
+    from paper_2606_01065_b200 import harness
+    rng = np.random.default_rng(123)
+    L, P, Dr, Dc = 700, 16, 64, 512
+    inv = synth.yarn_inv_freq()
+    dirs3 = [(40, 150, 9), (300, 301, 120), (600, 640, 0)]
+    w = synth.Workload("logits", 2, [L], P, inv_freq=inv, directives=[(0, s, e, n, 0, 0) for s, e, n in dirs3], seed=5,
+                       pool_factor=3.0, extra_pages=16).finalize()
+    seq = list_splice(L, [(s, e, n, row) for (_, s, e, n, row, _) in w.directives])
+    cache = harness.DeviceCache(w, "cuda:0", fill=False)
+    slot_old = w.pages.astype(np.int64)[np.arange(L) // P] * P + np.arange(L) % P
+    raws, raw_rs = [], []
+    for l in range(w.n_layers):
+        raw = rng.standard_normal((L, Dr))
+        raw_r = rng.standard_normal((w.n_repl_rows, Dr))
+        final_pos = np.array([n for n, tok in enumerate(seq) if tok[0] == "r"])          # replacement K_pe: roped at its
+        order = np.array([tok[1] for tok in seq if tok[0] == "r"])                        # FINAL position (G12)
+        pos_of_row = np.empty(w.n_repl_rows, np.int64)
+        pos_of_row[order] = final_pos
+        pool = np.zeros((w.n_slots, w.row_bytes), np.uint8)
+        pool[slot_old] = to_storage(np.concatenate([rng.standard_normal((L, Dc)), rope_complex(raw, np.arange(L), inv)], axis=1), O.BF16)
+        repl = to_storage(np.concatenate([rng.standard_normal((w.n_repl_rows, Dc)), rope_complex(raw_r, pos_of_row, inv)], axis=1), O.BF16)
+        cache.pools[l].copy_(torch.from_numpy(pool.reshape(-1)))
+        cache.repl[l].copy_(torch.from_numpy(repl.reshape(-1)))
+        raws.append(raw)
+        raw_rs.append(raw_r)
+    plan, pt, idx = harness.run_workload(cache, mode)
+    torch.cuda.synchronize()
+    slots = idx.cpu().numpy()[:len(seq)].astype(np.int64)
+    H = Dr // 2
+    th = inv.astype(np.float64)
+    worst = 0.0
+    for l in range(w.n_layers):
+        k_new = from_storage(cache.pools[l].cpu().numpy().reshape(-1, w.row_bytes)[slots], O.BF16)[:, Dc:]
+        k_raw = np.stack([raws[l][tok[1]] if tok[0] == "o" else raw_rs[l][tok[1]] for tok in seq])
+        kc = k_raw[:, :H] + 1j * k_raw[:, H:]
+        q_raw = rng.standard_normal(Dr)
+        qc = q_raw[:H] + 1j * q_raw[H:]
+        for m in range(0, len(seq), 7):
+            q_m = rope_complex(q_raw, m, inv)
+            got = k_new @ q_m
+            want = np.real(np.sum(qc[None, :] * np.conj(kc) * np.exp(1j * (m - np.arange(len(seq)))[:, None] * th[None, :]), axis=1))
+            # bf16 K (two roundings, 2^-8 relative each at most) against an exact q: |err| <= 2^-7 * |q| * |k|
+            bound = 2.0 ** -7 * np.linalg.norm(q_raw) * np.linalg.norm(k_raw, axis=1)
+            assert (np.abs(got - want) <= bound).all()
+            worst = max(worst, float((np.abs(got - want) / bound).max()))
+    print(f"[logits] mode {mode}: worst |logit error| / (2^-7 |q||k|) = {worst:.3f}")
+    plan.close()
