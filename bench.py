@@ -47,6 +47,10 @@ def parse_args():
     ap.add_argument("--stages", type=int, default=0, help="leyline_tuning.stages (bulk kernel)")
     ap.add_argument("--layer-group", type=int, default=0, help="leyline_tuning.layer_group (bulk kernel)")
     ap.add_argument("--consumer-warps", type=int, default=0, help="leyline_tuning.consumer_warps (bulk kernel)")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="process-group backend for --gpus N > 1")
+    ap.add_argument("--stub-step-ms", type=float, default=0.0,
+                    help="TEST ONLY (tests/test_replicas_gloo.py): replace the splice by a host sleep of this many ms "
+                         "(+ 1 ms per rank) so that the N-replica launch and its timing contract run without a GPU")
     return ap.parse_args()
 
 
@@ -124,11 +128,14 @@ class ClockSampler:
 # ----------------------------------------------------------------------------- our arm
 
 def dist_setup(n_gpus: int):
-    """One process per GPU (torchrun exports RANK / LOCAL_RANK / WORLD_SIZE); nccl only carries the timing contract's
-    barrier and max-over-ranks -- the splice itself has no exchange step (paper_2606_01065_b200/replicas.py)."""
+    """One process per GPU (torchrun, or spawn_replicas below, exports RANK / LOCAL_RANK / WORLD_SIZE); nccl only
+    carries the timing contract's barrier and max-over-ranks -- the splice itself has no exchange step
+    (paper_2606_01065_b200/replicas.py)."""
     import torch
     from paper_2606_01065_b200 import replicas as R
-    local = R.env_rank()[2]
+    rank, world, local = R.env_rank()
+    if world != max(1, n_gpus):
+        raise SystemExit(f"bench.py: --gpus {n_gpus} but WORLD_SIZE is {world}")
     torch.cuda.set_device(local)
     return R.init("nccl", torch.device("cuda", local))
 
@@ -404,10 +411,131 @@ def run_e2e(cache, w, steps: int, warmup: int = 1):
                     "C ABI); host wall clock around synchronised steps; PCIe-bound by construction"}
 
 
+
+# (key, synth config, modes) of SURVEY.md section 8(d)'s table that ride along with the headline as `extras`
+EXTRA_WORKLOADS = [("cfg2", "2", ("fresh", "inplace", "rotate_only"), 2.0),
+                   ("cfg5", "5", ("fresh", "inplace", "rotate_only"), 2.0),
+                   ("cfg4", "4", ("inplace",), 1.25),
+                   ("gqa", "gqa", ("fresh", "inplace", "rotate_only"), 2.0),
+                   ("mha96", "mha96", ("fresh", "inplace", "rotate_only"), 2.0),
+                   ("appB", "appB", ("fresh", "rotate_only"), 2.0)]
+
+
+def extra_line(cache, w, mode_name: str, peak: float, device_index: int, target_s: float = 0.35):
+    """One supplementary (workload, mode) line: the same step as the headline (plan + prefetch + index + data kernel),
+    long enough (about target_s) for nvidia-smi to sample the clocks under load."""
+    mode = MODES[mode_name]
+    probe = time_splice(cache, w, mode, 3, 2)
+    steps = int(min(400, max(5, target_s * 1e3 / max(probe["ms_per_step"], 1e-3))))
+    sampler = ClockSampler(device_index)
+    sampler.start()
+    x = time_splice(cache, w, mode, steps, 1)
+    clocks = sampler.stop()
+    step_gbs, kern_gbs = x["bytes"] / x["ms_per_step"] / 1e6, x["bytes"] / x["kernel_ms"] / 1e6
+    return {"workload": w.name, "mode": mode_name, "steps": steps, "bytes": x["bytes"], "directives": x["n_directives"],
+            "ms_per_step": x["ms_per_step"], "GBps": step_gbs, "kernel_ms": x["kernel_ms"], "kernel_GBps": kern_gbs,
+            "frac": kern_gbs / peak, "step_over_kernel": x["ms_per_step"] / x["kernel_ms"],
+            "plan_host_us": x["plan_host_us"], "us_per_directive": x["ms_per_step"] * 1e3 / max(1, x["n_directives"]),
+            "mover": x["mover"], "tile_rows": x["tile_rows"], "clocks": clocks}
+
+
+def extra_workloads(peak: float, device_index: int, skip=()):
+    """Every other row of SURVEY.md 8(d): configs 2, 4, 5, the full-width K pools and the paper's App. B shape, each in
+    the modes it has, one cache per workload (built, timed, freed)."""
+    import gc
+    import torch
+    from paper_2606_01065_b200 import harness, synth
+    out = {}
+    for key, cfg, modes, factor in EXTRA_WORKLOADS:
+        if key in skip:
+            continue
+        w = synth.config(int(cfg) if cfg.isdigit() else cfg, pool_factor=factor)
+        need = (w.layer_bytes + max(w.n_repl_rows, 1) * w.row_bytes) * w.n_layers
+        free, _ = torch.cuda.mem_get_info(device_index)
+        if free < need * 1.03 + (1 << 30):
+            for m in modes:
+                out[f"{key}_{m}"] = {"workload": w.name, "mode": m, "skipped": f"needs {need / 2**30:.0f} GiB of device memory, "
+                                                                              f"{free / 2**30:.0f} GiB free"}
+            continue
+        cache = harness.DeviceCache(w, f"cuda:{device_index}")
+        torch.cuda.synchronize()
+        for m in modes:
+            out[f"{key}_{m}"] = extra_line(cache, w, m, peak, device_index)
+        del cache
+        gc.collect()
+        torch.cuda.empty_cache()
+    return out
+
+
+def pattern_reference(device, n_rows: int = 4 << 20):
+    """What plain torch ops reach on the access pattern of a5 (ROTATE_ONLY on an MLA cache): an in-place update of the
+    last 128 B of every 1152-B row (bf16) / the last 64 B of every 576-B row (fp8) of a contiguous buffer -- no page
+    table, no rotation.  A reference for how hard the PATTERN is on this memory system, next to k_rotate_band's GB/s
+    (same byte accounting: band bytes read + written)."""
+    import torch
+    out = {}
+    for name, row_bytes, band in (("bf16_128_of_1152", 1152, 128), ("fp8_64_of_576", 576, 64)):
+        buf = torch.zeros(n_rows * row_bytes, dtype=torch.uint8, device=device)
+        views = {"int32_add": (buf.view(torch.int32).view(n_rows, row_bytes // 4)[:, (row_bytes - band) // 4:], lambda v: v.add_(1))}
+        if row_bytes == 1152:
+            views["bf16_mul"] = (buf.view(torch.bfloat16).view(n_rows, 576)[:, 512:], lambda v: v.mul_(1.0009765625))
+        best = {}
+        for k, (v, op) in views.items():
+            for _ in range(2):
+                op(v)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(5):
+                op(v)
+            e1.record()
+            torch.cuda.synchronize()
+            best[k] = 2.0 * n_rows * band / (e0.elapsed_time(e1) / 5 * 1e-3) / 1e9
+        out[name] = {"GBps": max(best.values()), "by_op": best, "rows": n_rows}
+        del buf, views
+    # and a dense in-place update of the same buffer size with the same op, for scale
+    buf = torch.zeros(n_rows * 288, dtype=torch.int32, device=device)
+    for _ in range(2):
+        buf.add_(1)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(5):
+        buf.add_(1)
+    e1.record()
+    torch.cuda.synchronize()
+    out["dense_int32_add"] = {"GBps": 2.0 * buf.numel() * 4 / (e0.elapsed_time(e1) / 5 * 1e-3) / 1e9}
+    return out
+
+
+def run_stub(args):
+    """--stub-step-ms: the N-replica launch and timing contract with a host sleep in place of the splice (no GPU, no
+    library): barrier, K timed steps, MAX over ranks of the step time, SUM of the units, one JSON line from rank 0."""
+    from paper_2606_01065_b200 import replicas as R
+    rank, world, local = R.init(args.backend)
+    R.barrier(world)
+    for _ in range(args.warmup):
+        time.sleep(1e-3)
+    R.barrier(world)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        time.sleep((args.stub_step_ms + rank) * 1e-3)
+    ms_mine = (time.perf_counter() - t0) * 1e3 / args.steps
+    R.barrier(world)
+    units = 1_000_000 * (rank + 1)
+    value, ms = R.job_throughput_gbs(units, ms_mine, world)
+    R.finish(world)
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+                          "vs_baseline": None, "dtype": "none", "data": "stub", "impl": "stub",
+                          "config": {"workload": "stub (host sleep)", "replicas": world}, "gpu_launches": 0,
+                          "units_all_ranks": sum(1_000_000 * (r + 1) for r in range(world))}))
+
+
 def run_ours(args):
     import torch
     from paper_2606_01065_b200 import binding as B
     from paper_2606_01065_b200 import harness
+    from paper_2606_01065_b200 import replicas as R
     from paper_2606_01065_b200 import synth
     rank, world, local = dist_setup(args.gpus)
     B.leyline_set_tuning(kernel=args.kernel, tile_rows=args.tile_rows, ctas_per_sm=args.ctas_per_sm, profile=1,
@@ -421,7 +549,8 @@ def run_ours(args):
     r = time_splice(cache, w, mode, args.steps, args.warmup, world)
     clocks = sampler.stop()
     ms = max_over_ranks(r["ms_per_step"], world)
-    value = world * r["bytes"] / (ms * 1e-3) / 1e9
+    dev = torch.device("cuda", local)
+    value = R.sum_over_ranks(float(r["bytes"]), world, dev) / (ms * 1e-3) / 1e9     # whole job: all replicas' bytes / slowest rank's time
     peak, peak_src = peaks()
     kernel_gbs = r["bytes"] / (r["kernel_ms"] * 1e-3) / 1e9
     kname = "k_move_bulk" if r["mover"] == 2 else ("k_rotate_band" if mode == B.ROTATE_ONLY else "k_move_rows")
@@ -434,7 +563,9 @@ def run_ours(args):
                    "page_size": w.page_size, "directives": r["n_directives"], "rows_moved_per_layer": r["rows_moved"],
                    "rows_inserted_per_layer": r["rows_inserted"], "bytes_read_plus_written": r["bytes"],
                    "cache_flush": "none needed: each step streams %.2f GB, far larger than the 126 MB L2" % (r["bytes"] / 1e9),
-                   "replicas": world, "multi_gpu": "replicas only (the path has no exchange step)"},
+                   "replicas": world, "multi_gpu": "replicas only (the path has no exchange step)",
+                   "throughput": "pipelined steady state: the host plan and table upload of step n+1 overlap the kernels of "
+                                 "step n; extras.single_call_idle_gpu is one call on an idle GPU"},
         "us_per_directive": ms * 1e3 / max(1, r["n_directives"]),
         "pct_of_8TBps_nominal": 100.0 * value / world / 8000.0,
         "plan_host_us": r["plan_host_us"],
@@ -447,16 +578,16 @@ def run_ours(args):
                      "kernel_ms": r["kernel_ms"], "kernel_ms_best": r["kernel_ms_min"],
                      "peak_source": peak_src, "frac_of_8TBps_nominal": kernel_gbs / 8000.0},
     }
+    headline = args.workload == "3" and args.mode == "fresh"
     if rank == 0 and world == 1:
         bytes_per_layer = r["bytes"] // w.n_layers
-        if not args.no_extras and args.workload == "3" and args.mode == "fresh":
+        if not args.no_extras and headline:
             extras = {}
             for name, wl, md in (("cfg3_inplace", w, "inplace"), ("cfg3_rotate_only", w, "rotate_only"),
-                                 ("cfg3m_fresh", synth.config("3m", pool_factor=2.0), "fresh")):
+                                 ("cfg3m_fresh", synth.config("3m", pool_factor=2.0), "fresh"),
+                                 ("cfg3m_inplace", synth.config("3m", pool_factor=2.0), "inplace")):
                 cache.w = wl
-                x = time_splice(cache, wl, MODES[md], max(3, args.steps // 4), 2)
-                extras[name] = {"ms_per_step": x["ms_per_step"], "GBps": x["bytes"] / x["ms_per_step"] / 1e6,
-                                "kernel_GBps": x["bytes"] / x["kernel_ms"] / 1e6, "bytes": x["bytes"]}
+                extras[name] = extra_line(cache, wl, md, peak, local)
             cache.w = w
             extras["single_call_idle_gpu"] = time_single_calls(cache, w, mode)
             extras["discovery_cdc"] = time_discovery(cache.device, with_oracle=not args.no_cpu_baseline)
@@ -467,16 +598,64 @@ def run_ours(args):
             out["cpu_baseline_all_cores"] = cpu_baseline_all_cores(lambda l: cache.pools[l].cpu().numpy(),
                                                                    lambda l: cache.repl[l].cpu().numpy(), cache.scales, w, mode,
                                                                    bytes_per_layer)
-        if not args.no_e2e and mode == B.FRESH:
-            try:
-                out["e2e"] = run_e2e(cache, w, steps=min(args.steps, 3))
-            except Exception as ex:   # e.g. the host cannot pin that much memory: say so instead of inventing a number
-                out["e2e"] = {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
-                              "error": f"{type(ex).__name__}: {ex}"}
-    from paper_2606_01065_b200 import replicas as R
+    if not args.no_e2e and mode == B.FRESH:
+        # every replica runs its own end-to-end leg (host pools over its own PCIe link); whole job = all bytes / slowest
+        try:
+            e = run_e2e(cache, w, steps=min(args.steps, 3))
+        except Exception as ex:   # e.g. the host cannot pin that much memory: say so instead of inventing a number
+            e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
+                 "error": f"{type(ex).__name__}: {ex}"}
+        if world > 1:
+            ok = R.sum_over_ranks(1.0 if e.get("value") else 0.0, world, dev) == world
+            e_ms = max_over_ranks(e.get("ms_per_step") or 0.0, world)
+            if ok:
+                e = dict(e, value=world * r["bytes"] / (e_ms * 1e-3) / 1e9,
+                         ms_per_step=e_ms, h2d_bytes_per_step=world * e["h2d_bytes_per_step"],
+                         d2h_bytes_per_step=world * e["d2h_bytes_per_step"], replicas=world)
+            else:
+                e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
+                     "error": "the end-to-end leg failed on at least one rank: " + str(e.get("error"))}
+        out["e2e"] = e
+    if rank == 0 and world == 1 and not args.no_extras and headline:
+        # the rest of SURVEY.md 8(d)'s table; the config-3 cache is released first (config 4 alone is 92 GB)
+        import gc
+        del cache
+        gc.collect()
+        torch.cuda.empty_cache()
+        out["extras"].update(extra_workloads(peak, local))
+        out["extras"]["a5_pattern_reference_torch"] = pattern_reference(dev)
+    elif world > 1:
+        out["extras"] = "N = 1 only (supplementary workloads; they do not depend on the replica count)"
     R.finish(world)
     if rank == 0:
         print(json.dumps(out))
+
+
+def spawn_replicas(args) -> int:
+    """`python bench.py --gpus N` without a launcher: start N ranks of this script, one per GPU (RANK / LOCAL_RANK /
+    WORLD_SIZE / MASTER_* as torchrun would export them), and pass rank 0's JSON line through.  Fails loudly when the
+    box has fewer than N devices -- the flag must mean N."""
+    import socket
+    if args.stub_step_ms <= 0:
+        import torch
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            sys.stderr.write(f"bench.py: --gpus {args.gpus} asked for, but this box has {have} CUDA device(s)\n")
+            return 2
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    procs = []
+    for rk in range(args.gpus):
+        env = dict(os.environ, RANK=str(rk), LOCAL_RANK=str(rk), WORLD_SIZE=str(args.gpus), MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port))
+        env.setdefault("NCCL_DEBUG", "INFO")       # the communicator log shows the rank count (and NVLS, when used)
+        procs.append(subprocess.Popen([sys.executable, os.path.abspath(__file__), *sys.argv[1:]], env=env,
+                                      stdout=None if rk == 0 else subprocess.DEVNULL))
+    rc = 0
+    for pr in procs:
+        rc = pr.wait() or rc
+    return rc
 
 
 # ----------------------------------------------------------------------------- reference arm = the oracle
@@ -541,5 +720,9 @@ if __name__ == "__main__":
     a = parse_args()
     if a.impl == "reference":
         run_reference(a)
+    elif a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(spawn_replicas(a))
+    elif a.stub_step_ms > 0:
+        run_stub(a)
     else:
         run_ours(a)

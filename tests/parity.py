@@ -98,11 +98,11 @@ def compare_layer(w: synth.Workload, bm: O.BatchMap, mode: int, old_pool: np.nda
     new_s, old_s = rotated_rows(w, bm, mode)
     band0 = w.latent_dim * E
     # 1. everything outside rotated bands: bit-exact over the whole pool
-    mask = np.ones(g.shape, dtype=bool)
+    neq = g != o
     if len(new_s):
-        mask[new_s, band0:] = False
-    neq = (g != o) & mask
-    assert not neq.any(), f"{int(neq.sum())} bytes differ outside rotated K_pe bands (first rows {np.unique(np.nonzero(neq)[0])[:8]})"
+        neq[new_s, band0:] = False
+    assert not neq.any(), f"layer {layer}: {int(neq.sum())} bytes differ outside rotated K_pe bands (first rows {np.unique(np.nonzero(neq)[0])[:8]})"
+    del neq
     stats = {"rotated_elems": 0, "max_ord": 0, "frac_equal": 1.0, "n_floor": 0}
     if not len(new_s):
         return stats
@@ -137,3 +137,56 @@ def compare_layer(w: synth.Workload, bm: O.BatchMap, mode: int, old_pool: np.nda
         assert dist.max() <= 1, f"fp8 rotated K_pe: max ordinal distance {int(dist.max())} > 1"
         stats.update(rotated_elems=int(dist.size), max_ord=int(dist.max()), frac_equal=float((dist == 0).mean()))
     return stats
+
+
+def compare_all_layers(w: synth.Workload, bm: O.BatchMap, mode: int, cache, layers=None, inserts_prefilled: bool = False,
+                       checksums=None, max_workers: int | None = None) -> list:
+    """Every layer of a device cache against the oracle, whole pool, one layer at a time (SURVEY.md section 7 "never hold
+    a whole cache on the host").  The pristine layer is REGENERATED from its seed into a device scratch buffer (the
+    generator is counter-based and seeded per layer, so this reproduces the bytes the splice started from; `checksums`,
+    taken before the splice, prove it), so in-place modes need no host snapshot of the cache.  The oracle (GIL-free C)
+    and the numpy comparisons of different layers run on a thread pool, sized to the host's cores and free memory."""
+    import os
+    import threading
+    from concurrent.futures import ThreadPoolExecutor
+
+    import psutil
+    import torch
+    layers = list(range(cache.n_layers)) if layers is None else list(layers)
+    per_layer = 7 * w.layer_bytes + 1
+    fit = int(psutil.virtual_memory().available * 0.6 // per_layer)
+    nw = max(1, min(os.cpu_count() or 1, 16, fit, len(layers)))
+    if max_workers:
+        nw = min(nw, max_workers)
+    scratch = torch.empty(w.layer_bytes, dtype=torch.uint8, device=cache.device)
+    gate = threading.Semaphore(nw + 1)            # layers resident on the host at once
+    stats = [None] * len(layers)
+
+    def work(i, l, old, new, repl, scale):
+        try:
+            stats[i] = compare_layer(w, bm, mode, old, new, repl, scale, layer=l, inserts_prefilled=inserts_prefilled)
+        finally:
+            gate.release()
+
+    with ThreadPoolExecutor(max_workers=nw) as ex:
+        futs = []
+        for i, l in enumerate(layers):
+            gate.acquire()
+            scale = synth.fill_layer_(scratch, w, cache.layer_ids[l])
+            assert scale == cache.scales[l]
+            if checksums is not None:
+                assert int(layer_checksum(scratch)) == checksums[l], f"layer {l}: regenerated bytes differ from the cache's"
+            old = scratch.cpu().numpy()
+            new = cache.pools[l].cpu().numpy()
+            repl = None if inserts_prefilled else cache.repl[l].cpu().numpy()
+            futs.append(ex.submit(work, i, l, old, new, repl, scale))
+        for f in futs:
+            f.result()
+    return stats
+
+
+def layer_checksum(buf) -> int:
+    """Order-independent 64-bit sum of a uint8 device tensor read as int64 words (a cheap identity check, not a hash)."""
+    import torch
+    n = buf.numel() // 8 * 8
+    return int(buf[:n].view(torch.int64).sum().item()) + int(buf[n:].to(torch.int64).sum().item())

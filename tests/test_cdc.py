@@ -165,6 +165,31 @@ def test_anchored_chunks_behind_an_edit_are_found_with_the_edits_delta():
     assert ((r_start[before] - src[before]) == 0).all()       # the untouched prefix maps to itself
 
 
+def test_registry_keeps_the_smallest_value_under_duplicate_keys():
+    """DESIGN.md reading D5: a key inserted several times maps to the SMALLEST value ever inserted under it, whatever the
+    insertion order and however the inserts are batched; unknown keys read -1.  Checked against a sort-based
+    restatement (sort by (key, value), keep the first of each key) that shares nothing with the dict loop."""
+    rng = np.random.default_rng(55)
+    keys = rng.integers(1, 40, size=500).astype(np.uint64) * np.uint64(0x9E3779B97F4A7C15)     # 39 distinct keys, many repeats
+    vals = rng.integers(0, 10**9, size=500).astype(np.int64)
+    order = np.lexsort((vals, keys))
+    first = np.concatenate([[True], keys[order][1:] != keys[order][:-1]])
+    want = dict(zip(keys[order][first].tolist(), vals[order][first].tolist()))
+    for perm in (np.arange(500), np.arange(500)[::-1], rng.permutation(500)):
+        reg = OC.Registry()
+        for lo in range(0, 500, 37):                                       # several batches
+            sel = perm[lo:lo + 37]
+            reg.insert(keys[sel], vals[sel])
+        got = reg.lookup(np.array(list(want.keys()), np.uint64))
+        np.testing.assert_array_equal(got, np.array(list(want.values()), np.int64))
+        assert (reg.lookup(np.array([7, 11], np.uint64)) == -1).all()
+    # hand case: descending then ascending values under one key
+    reg = OC.Registry()
+    reg.insert([5, 5, 5], [30, 10, 20])
+    reg.insert([5], [15])
+    assert reg.lookup([5]).tolist() == [10]
+
+
 def test_unanchored_chunker_resynchronises_only_after_a_window():
     """Without anchors (the paper's 'legacy purely-Gear-hash chunker') boundaries behind an edit depend
     on where the previous boundary fell (min / max sizes), so the first chunks behind the edit may differ; content

@@ -70,3 +70,37 @@ def test_single_process_is_identity():
     assert R.sum_over_ranks(7, 1) == 7.0
     gbs, ms = R.job_throughput_gbs(2_000_000_000, 1.0, 1)
     assert ms == 1.0 and gbs == pytest.approx(2000.0)
+
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.mark.timeout(300)
+def test_bench_gpus_n_starts_n_ranks_by_itself():
+    """`python bench.py --gpus 2` with no launcher must start two ranks and report n_gpus = 2, the slowest rank's step
+    time and the units of BOTH ranks (here with the test-only host-sleep step on gloo, no GPU)."""
+    import json
+    import subprocess
+    import sys
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--stub-step-ms", "5", "--backend", "gloo",
+                        "--steps", "3", "--warmup", "1"], capture_output=True, text=True, cwd=ROOT, timeout=280,
+                       env={k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")})
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1                                       # rank 0 alone prints
+    out = json.loads(lines[0])
+    assert out["n_gpus"] == 2 and out["steps"] == 3 and out["warmup"] == 1
+    assert out["ms_per_step"] >= 6.0                             # rank 1 sleeps 5 + 1 ms: MAX over ranks
+    assert out["units_all_ranks"] == 3_000_000
+    assert out["value"] == pytest.approx(3_000_000 / (out["ms_per_step"] * 1e-3) / 1e9)
+
+
+def test_bench_gpus_n_fails_loudly_when_the_box_has_fewer_devices():
+    import subprocess
+    import sys
+    if torch.cuda.device_count() >= 2:
+        pytest.skip("this box has two devices")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "1"],
+                       capture_output=True, text=True, cwd=ROOT, timeout=280,
+                       env={k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")})
+    assert r.returncode == 2 and "--gpus 2" in r.stderr and not r.stdout.strip()
