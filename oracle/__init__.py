@@ -58,6 +58,7 @@ def lib():
         L.ora_e4m3_encode.restype = C.c_uint8
         L.ora_e4m3_encode.argtypes = [C.c_double]
         L.ora_slot_of.restype = C.c_int64
+        L.ora_first_edit.restype = C.c_int64
         L.ora_rotate_pair.restype = None
         L.ora_rotate_pair.argtypes = [C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.ora_rerope_pair.restype = None
@@ -202,7 +203,9 @@ def map_request(mode: int, P: int, L_old: int, old_pages, directives, free_ids) 
     slot_old = _slots_of_fast(P, old_pages, L_old)
     if mode == FRESH:
         released = np.zeros(n_old + 1, np.int32)
-        s0 = directives[0][0] if len(directives) else -1
+        d = list(directives)
+        s0 = lib().ora_first_edit(C.c_int32(len(d)), _p(_i64([x[0] for x in d])), _p(_i64([x[1] for x in d])),
+                                  _p(_i64([x[2] for x in d])), _p(_i32([x[4] for x in d])))
         st = lib().ora_map_fresh(C.c_int64(P), C.c_int64(L_old), C.c_int64(L_new), C.c_int64(s0), _p(old_pages),
                                  _p(free_ids), C.c_int64(len(free_ids)), _p(new_pages), C.byref(nn), C.byref(nc),
                                  _p(released), C.byref(nr))

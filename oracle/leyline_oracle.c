@@ -200,18 +200,35 @@ int32_t ora_segments(int64_t L_old, int32_t k, const int64_t* start, const int64
 
 static int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
-/* M1 FRESH (the paper's dst_slots path): k0 = floor(s_0 / P); new table = old pages
- * [0,k0) by identity, then ceil(L_new/P) - k0 ids taken from the free list front to back; old pages
- * [k0, ceil(L_old/P)) are released in ascending logical order and never written.  A request without
- * directives (s0 < 0) keeps its table.  Returns ORA_E_NOFREE when the free list is too short. */
+/* First directive of a request, in order, that changes a byte or the running shift: AMORTIZE with a non-empty
+ * span or a non-empty replacement.  No-op directives (start == end, |R| = 0) are skipped; a FORGET directive ends
+ * the search (everything from its start on is dropped, nothing is rewritten in front of it).
+ * Returns that directive's start, or -1 when there is none (DESIGN.md rule M1). */
+int64_t ora_first_edit(int32_t k, const int64_t* start, const int64_t* end, const int64_t* repl_len,
+                       const int32_t* semantic) {
+    for (int32_t j = 0; j < k; ++j) {
+        if (semantic[j] == ORA_FORGET) return -1;
+        if (end[j] > start[j] || repl_len[j] > 0) return start[j];
+    }
+    return -1;
+}
+
+/* M1 FRESH (the paper's dst_slots path): s0 = ora_first_edit(...); k0 = floor(s0 / P); new
+ * table = old pages [0,k0) by identity, then ceil(L_new/P) - k0 ids taken from the free list front to back; old
+ * pages [k0, ceil(L_old/P)) are released in ascending logical order and never written.  A request that no directive
+ * edits (s0 < 0: no directives, no-ops only, or a FORGET before any edit) keeps its first ceil(L_new/P) pages --
+ * all of them unless a FORGET truncated it -- releases the rest, and consumes nothing.
+ * Returns ORA_E_NOFREE when the free list is too short. */
 int ora_map_fresh(int64_t P, int64_t L_old, int64_t L_new, int64_t s0, const int32_t* old_pages,
                   const int32_t* free_ids, int64_t n_free, int32_t* new_pages, int64_t* n_new_pages,
                   int64_t* n_consumed, int32_t* released, int64_t* n_released) {
     int64_t n_old = ceil_div(L_old, P);
     *n_consumed = 0; *n_released = 0;
     if (s0 < 0) {
-        for (int64_t p = 0; p < n_old; ++p) new_pages[p] = old_pages[p];
-        *n_new_pages = n_old;
+        int64_t n_keep = ceil_div(L_new, P); /* L_new <= L_old here: nothing was inserted */
+        for (int64_t p = 0; p < n_keep; ++p) new_pages[p] = old_pages[p];
+        for (int64_t p = n_keep; p < n_old; ++p) released[(*n_released)++] = old_pages[p];
+        *n_new_pages = n_keep;
         return ORA_OK;
     }
     int64_t k0 = s0 / P, n_new = ceil_div(L_new, P);

@@ -176,10 +176,12 @@ def test_p11_maps_brute_force(mode, seed):
         else:
             n_old, n_new = n_pages[r], -(-rm.L_new // P)
             if mode == O.FRESH:
-                keep = n_old if not per_req[r] else per_req[r][0][0] // P
-                want_pages = list(row_old[:keep]) + [int(x) for x in free[used_free:used_free + (0 if not per_req[r] else n_new - keep)]]
-                want_rel = [] if not per_req[r] else list(row_old[keep:])
-                used_free += 0 if not per_req[r] else n_new - keep
+                # rule M1: pages in front of the first directive that changes anything are kept; no-ops do not count
+                edits = [d for d in per_req[r] if d[1] > d[0] or d[2] > 0]
+                keep = n_old if not edits else edits[0][0] // P
+                want_pages = list(row_old[:keep]) + [int(x) for x in free[used_free:used_free + (0 if not edits else n_new - keep)]]
+                want_rel = [] if not edits else list(row_old[keep:])
+                used_free += 0 if not edits else n_new - keep
             else:
                 keep = min(n_old, n_new)
                 want_pages = list(row_old[:keep]) + [int(x) for x in free[used_free:used_free + max(0, n_new - n_old)]]
@@ -226,6 +228,34 @@ def test_forget_truncates():
     segs = O.segments(100, [(10, 20, 4, 0, O.AMORTIZE), (50, 60, 3, 4, O.FORGET), (70, 80, 1, 7, O.AMORTIZE)])
     assert segs.forget_trim == 50 - 6 and segs.L_new == 44
     assert segs.as_tuples() == [(O.KEEP, 0, 0, 10, 0), (O.INSERT, 0, 10, 4, 0), (O.KEEP, 20, 14, 30, -6)]
+
+
+def test_m1_fresh_rewrites_nothing_in_front_of_the_first_real_edit():
+    """Rule M1: FRESH keeps every page in front of the first directive that changes a byte or the shift.
+    No-op directives (start == end, |R| = 0) and a FORGET before any edit therefore consume no free page and copy
+    nothing ("prefix-trimmed": a FORGET only drops the tail); hand-computed tables."""
+    P, L = 4, 22                                   # pages 0..5 hold positions [0,4) .. [20,22)
+    pages = np.array([10, 11, 12, 13, 14, 15], np.int32)
+    free = np.array([20, 21, 22, 23, 24, 25, 26], np.int32)
+
+    def fresh(dirs):
+        bm = O.plan_batch(O.FRESH, P, [L], [0, 6], pages, [(0, *d) for d in dirs], free)
+        assert bm.status == O.OK
+        rm = bm.requests[0]
+        return rm.L_new, list(rm.new_pages), list(rm.released), bm.n_consumed
+
+    # no-ops only: the table is kept as it is
+    assert fresh([(3, 3, 0, 0, O.AMORTIZE), (9, 9, 0, 0, O.AMORTIZE)]) == (22, [10, 11, 12, 13, 14, 15], [], 0)
+    # a no-op in page 0, then a real edit in page 3: pages 0..2 are kept (the no-op does not pull k0 forward)
+    assert fresh([(1, 1, 0, 0, O.AMORTIZE), (13, 15, 0, 0, O.AMORTIZE)]) == (20, [10, 11, 12, 20, 21], [13, 14, 15], 2)
+    # FORGET only: truncation at 9 -> 3 pages kept, the rest released, nothing consumed
+    assert fresh([(9, 9, 0, 0, O.FORGET)]) == (9, [10, 11, 12], [13, 14, 15], 0)
+    assert fresh([(8, 12, 5, 0, O.FORGET)]) == (8, [10, 11], [12, 13, 14, 15], 0)
+    assert fresh([(0, 0, 0, 0, O.FORGET)]) == (0, [], [10, 11, 12, 13, 14, 15], 0)
+    # an edit in page 1, then a FORGET at 17 (new coordinate 17 + 2 = 19): compaction from page 1, 5 pages in all
+    assert fresh([(5, 6, 3, 0, O.AMORTIZE), (17, 20, 0, 3, O.FORGET)]) == (19, [10, 20, 21, 22, 23], [11, 12, 13, 14, 15], 4)
+    # a pure insert counts as an edit
+    assert fresh([(6, 6, 1, 0, O.AMORTIZE)]) == (23, [10, 20, 21, 22, 23, 24], [11, 12, 13, 14, 15], 5)
 
 
 # ----------------------------------------------------------------------------- P2: identity
