@@ -47,6 +47,7 @@ def parse_args():
     ap.add_argument("--stages", type=int, default=0, help="leyline_tuning.stages (bulk kernel)")
     ap.add_argument("--layer-group", type=int, default=0, help="leyline_tuning.layer_group (bulk kernel)")
     ap.add_argument("--consumer-warps", type=int, default=0, help="leyline_tuning.consumer_warps (bulk kernel)")
+    ap.add_argument("--rotate-kernel", type=int, default=0, help="leyline_tuning.rotate_kernel (0 auto, 1 strided registers, 2 TMA boxes)")
     ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="process-group backend for --gpus N > 1")
     ap.add_argument("--stub-step-ms", type=float, default=0.0,
                     help="TEST ONLY (tests/test_replicas_gloo.py): replace the splice by a host sleep of this many ms "
@@ -174,10 +175,11 @@ def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1):
     pools, repl = B.layer_pointers(cache.pools), B.layer_pointers(cache.repl)   # marshalled once, as a server would
     free = w.free_slots() if mode == B.ROTATE_ONLY else w.free_pages
     dirs = B.pack_directives(w.directives)
+    seq_lens = np.asarray(w.seq_lens, np.int64)          # a server holds these as arrays already
 
     def step():
         t0 = time.perf_counter()
-        plan = B.leyline_plan(desc, mode, w.seq_lens, w.pt_offsets, w.pages, dirs, free)
+        plan = B.leyline_plan(desc, mode, seq_lens, w.pt_offsets, w.pages, dirs, free)
         host_us.append((time.perf_counter() - t0) * 1e6)
         plan.prefetch()          # table upload on the library's copy stream; the launch below only waits on its event
         if mode == B.ROTATE_ONLY:
@@ -539,7 +541,8 @@ def run_ours(args):
     from paper_2606_01065_b200 import synth
     rank, world, local = dist_setup(args.gpus)
     B.leyline_set_tuning(kernel=args.kernel, tile_rows=args.tile_rows, ctas_per_sm=args.ctas_per_sm, profile=1,
-                         stages=args.stages, layer_group=args.layer_group, consumer_warps=args.consumer_warps)
+                         stages=args.stages, layer_group=args.layer_group, consumer_warps=args.consumer_warps,
+                         rotate_kernel=args.rotate_kernel)
     mode = MODES[args.mode]
     w = workload_of(args.workload, args.mode)
     cache = harness.DeviceCache(w, f"cuda:{local}")
@@ -690,8 +693,15 @@ def run_reference(args):
         if not nbytes:
             rows = 0
             for r, rm in enumerate(bm.requests):
-                mine = [d for d in w.directives if d[0] == r]
-                k0P = (mine[0][1] // w.page_size) * w.page_size if mine else rm.L_new
+                # rule M1: FRESH rewrites from the page of the first directive that changes anything (FORGET ends the search)
+                first = None
+                for d in (d for d in w.directives if d[0] == r):
+                    if d[5] != 0:
+                        break
+                    if d[2] > d[1] or d[3] > 0:
+                        first = d[1]
+                        break
+                k0P = (first // w.page_size) * w.page_size if first is not None else rm.L_new
                 for (k, s, d, n, c) in rm.segs.as_tuples():
                     if k == O.INSERT:
                         rows += n

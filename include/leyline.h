@@ -27,8 +27,11 @@
  * earlier, on the library's copy stream, after leyline_plan_prefetch), launch one index kernel and one data kernel on
  * the caller's stream and return without synchronising.  A plan may be in flight on one stream at a time; different
  * plans may be in flight on different streams and may be driven from different host threads.
- * leyline_set_tuning is a process-wide benchmarking knob and is not synchronised with concurrent leyline_plan calls.
- * Nothing is thrown across the ABI: every entry point returns a leyline_status.
+ * leyline_set_tuning is a process-wide benchmarking default read (under a lock) by leyline_plan only; leyline_plan_ex
+ * takes its tuning as an argument and never looks at the process-wide one.
+ * Nothing is thrown across the ABI: every entry point returns a leyline_status (a C++ exception inside the library,
+ * e.g. std::bad_alloc while planning a very large batch, comes back as LEYLINE_E_NOMEM / LEYLINE_E_INVALID).
+ * Only the functions declared in include/ are exported from libleyline.so (-fvisibility=hidden + LEYLINE_API).
  * There is no CPU fallback: without a CUDA device the launch entry points return LEYLINE_E_CUDA.
  * The discovery side (chunker, registry) is declared in leyline_cdc.h.
  */
@@ -36,6 +39,12 @@
 #define LEYLINE_H_
 
 #include <stdint.h>
+
+#if defined(__GNUC__)
+#define LEYLINE_API __attribute__((visibility("default")))
+#else
+#define LEYLINE_API
+#endif
 
 #ifdef __cplusplus
 extern "C" {
@@ -49,7 +58,11 @@ typedef enum {
     LEYLINE_E_RANGE = 4,       /* request id or span outside the request */
     LEYLINE_E_NOFREE = 5,      /* free list too short for the pages / slots the plan must consume */
     LEYLINE_E_UNSUPPORTED = 6, /* geometry the kernels do not cover (see leyline_cache_desc) */
-    LEYLINE_E_CUDA = 7         /* CUDA runtime error (message via leyline_last_cuda_error) */
+    LEYLINE_E_CUDA = 7,        /* CUDA runtime error (message via leyline_last_cuda_error) */
+    LEYLINE_E_NOMEM = 8,       /* host allocation failed inside the library (nothing was produced) */
+    LEYLINE_E_ALIAS = 9        /* a consumed free id is a live page / slot or appears twice, or (INPLACE_MOVE,
+                                  ROTATE_ONLY) a page is listed by two requests of which one is edited: executing the
+                                  plan would overwrite live KV */
 } leyline_status;
 
 typedef enum { LEYLINE_BF16 = 0, LEYLINE_FP8_E4M3 = 1 } leyline_dtype;
@@ -62,7 +75,8 @@ typedef enum { LEYLINE_ROPE_NEOX = 0, LEYLINE_ROPE_INTERLEAVED = 1 } leyline_pai
  * ROTATE_ONLY  : the paper's in-place path: no row moves, K_pe rotated where it sits, the
  *                token-level slot index list is rewritten (M3). */
 typedef enum { LEYLINE_FRESH = 0, LEYLINE_INPLACE_MOVE = 1, LEYLINE_ROTATE_ONLY = 2 } leyline_mode;
-/* PAPER.md:98, :102.  FORGET truncates the request at the directive's start; no kernel work. */
+/* PAPER.md:98, :102.  FORGET truncates the request at the directive's start: everything from there on is released and
+ * no kernel touches it (a request whose first effective directive is a FORGET launches nothing at all). */
 typedef enum { LEYLINE_AMORTIZE = 0, LEYLINE_FORGET = 1 } leyline_semantic;
 
 #define LEYLINE_MAX_LAYERS_PER_LAUNCH 128
@@ -138,10 +152,29 @@ typedef struct {
     int64_t mover;             /* a3/a4 kernel this plan launches: 1 = k_move_rows, 2 = k_move_bulk (see leyline_tuning).
                                   ROTATE_ONLY: 1 = k_rotate_band (strided band kernel), 2 = the band is at least half of
                                   the row (full-width K), so whole rows stream through k_move_bulk and are written back
-                                  to the slots they were read from */
+                                  to the slots they were read from, 3 = k_rotate_band_tma (2-D TMA boxes of the band) */
 } leyline_plan_info;
 
 typedef struct leyline_plan_s leyline_plan_t;
+
+/* Tuning knobs of a plan (defaults = all zero = what bench.py reports).  leyline_plan_ex takes them per call;
+ * leyline_plan reads the process-wide default set by leyline_set_tuning. */
+typedef struct leyline_tuning_s {
+    int32_t kernel;        /* a3/a4 mover: 0 = auto (bulk for unpadded rows in pages of >= 16 rows or of >= 1 KB each, or when the band is not a
+                              single head of 2^k <= 32 chunks), 1 = row kernel (LDG/STG through registers; single-head
+                              bands of 2^k chunks only, else LEYLINE_E_UNSUPPORTED), 2 = bulk kernel (TMA 1-D bulk
+                              copies through shared memory) */
+    int32_t tile_rows;     /* rows per tile of the move/insert kernels, 0 = default (row kernel <= 32, bulk <= 64) */
+    int32_t ctas_per_sm;   /* row kernel only, 0 = default */
+    int32_t profile;       /* 1: record CUDA events around the data-moving kernels (leyline_plan_kernel_ms) */
+    int32_t stages;        /* bulk / TMA-band kernels: shared-memory stages per CTA, 0 = as many as fit (bulk: at most 8) */
+    int32_t layer_group;   /* bulk / TMA-band kernels: layers per work item (one stage each), 0 = default */
+    int32_t consumer_warps;/* bulk kernel only: warps that rotate the band in shared memory, 0 = default (4 for MLA's
+                              narrow band, more when the band is most of the row), at most 16 */
+    int32_t rotate_kernel; /* a5 on a narrow band (MLA): 0 = auto, 1 = k_rotate_band (strided 16-byte loads / stores through
+                              registers), 2 = k_rotate_band_tma (the band of a page as one 2-D TMA box staged through shared
+                              memory; pages of >= 16 rows, else falls back to 1) */
+} leyline_tuning;
 
 /*
  * leyline_plan -- the host planner (step a1).
@@ -149,7 +182,8 @@ typedef struct leyline_plan_s leyline_plan_t;
  *   desc          cache geometry (copied).
  *   n_requests    number of requests; seq_lens[r] = cached tokens of request r (HOST).
  *   pt_offsets    HOST [n_requests+1]: row r of the page table is pages[pt_offsets[r] .. pt_offsets[r+1]),
- *                 at least ceil(seq_lens[r]/page_size) entries.
+ *                 EXACTLY ceil(seq_lens[r]/page_size) entries (a longer row is refused with LEYLINE_E_INVALID: pages
+ *                 behind the last token would be neither kept nor released).
  *   pages         HOST int32 page ids.
  *   directives    HOST, sorted by (request, start), spans of one request non-overlapping (adjacent allowed).
  *   free_ids      HOST int32: free PAGE ids (FRESH, INPLACE_MOVE) or free SLOT ids (ROTATE_ONLY); consumed front to
@@ -160,29 +194,39 @@ typedef struct leyline_plan_s leyline_plan_t;
  * on error *out is NULL.  Validation order is rule V of DESIGN.md (first failure wins, directives in order):
  * request out of range -> RANGE; start<0 | end<start | repl_len<0 | repl_row<0 | bad semantic -> INVALID;
  * end > seq_len -> RANGE; request or start decreasing -> UNSORTED; start < previous end -> OVERLAP;
- * then free list too short -> NOFREE.  Accepted: start==end (pure insert), repl_len==0 (pure delete,
- * PAPER.md:605), both (no-op), adjacent spans, start==0, requests without directives (untouched).
+ * then free list too short -> NOFREE; a consumed free id outside the pool -> RANGE; then the alias rule -> ALIAS:
+ * a consumed free id that is a live page (a slot of a live page, ROTATE_ONLY) or is consumed twice, and -- for the
+ * modes that write a request's own pages, INPLACE_MOVE and ROTATE_ONLY -- a page listed twice when one of its owners
+ * has directives (FRESH never writes a request's own pages, so requests may share prefix pages there).
+ * Accepted: start==end (pure insert), repl_len==0 (pure delete), both (no-op: changes nothing, in any
+ * mode), adjacent spans, start==0, requests without directives (untouched).  directive.reserved_ must be 0.
+ * leyline_plan uses the process-wide tuning (leyline_set_tuning); leyline_plan_ex takes `tuning` (NULL = defaults).
  */
-leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t mode, int32_t n_requests,
+LEYLINE_API leyline_status leyline_plan_ex(const leyline_cache_desc* desc, int32_t mode, int32_t n_requests,
+                                           const int64_t* seq_lens, const int64_t* pt_offsets, const int32_t* pages,
+                                           int32_t n_directives, const leyline_directive* directives,
+                                           const int32_t* free_ids, int64_t n_free, const leyline_tuning* tuning,
+                                           leyline_plan_t** out);
+LEYLINE_API leyline_status leyline_plan(const leyline_cache_desc* desc, int32_t mode, int32_t n_requests,
                             const int64_t* seq_lens, const int64_t* pt_offsets, const int32_t* pages,
                             int32_t n_directives, const leyline_directive* directives, const int32_t* free_ids,
                             int64_t n_free, leyline_plan_t** out);
 
 /* Plan queries (all HOST output buffers, sized from leyline_plan_info). */
-leyline_status leyline_plan_get_info(const leyline_plan_t* plan, leyline_plan_info* out);
-leyline_status leyline_plan_new_seq_lens(const leyline_plan_t* plan, int64_t* out /*[n_requests]*/);
+LEYLINE_API leyline_status leyline_plan_get_info(const leyline_plan_t* plan, leyline_plan_info* out);
+LEYLINE_API leyline_status leyline_plan_new_seq_lens(const leyline_plan_t* plan, int64_t* out /*[n_requests]*/);
 /* First FORGET directive's start in new coordinates per request, -1 if none. */
-leyline_status leyline_plan_forget_trim(const leyline_plan_t* plan, int64_t* out /*[n_requests]*/);
+LEYLINE_API leyline_status leyline_plan_forget_trim(const leyline_plan_t* plan, int64_t* out /*[n_requests]*/);
 /* Offsets of each request inside the token-level index list: [n_requests+1], prefix sums of new_seq_lens. */
-leyline_status leyline_plan_slot_offsets(const leyline_plan_t* plan, int64_t* out);
+LEYLINE_API leyline_status leyline_plan_slot_offsets(const leyline_plan_t* plan, int64_t* out);
 /* New page tables (FRESH / INPLACE_MOVE; LEYLINE_E_INVALID for ROTATE_ONLY): offsets [n_requests+1] and ids. */
-leyline_status leyline_plan_new_pt_offsets(const leyline_plan_t* plan, int64_t* out);
-leyline_status leyline_plan_new_pages(const leyline_plan_t* plan, int32_t* out /*[total_new_pages]*/);
+LEYLINE_API leyline_status leyline_plan_new_pt_offsets(const leyline_plan_t* plan, int64_t* out);
+LEYLINE_API leyline_status leyline_plan_new_pages(const leyline_plan_t* plan, int32_t* out /*[total_new_pages]*/);
 /* Released ids, requests ascending: pages in ascending logical order (FRESH: old pages from the first edited
  * page on; INPLACE_MOVE: tail pages) or, for ROTATE_ONLY, the slots of every removed old position in order.
  * Their bytes are never written (PAPER.md:405(a); G14). */
-leyline_status leyline_plan_released(const leyline_plan_t* plan, int32_t* out /*[n_released]*/);
-leyline_status leyline_plan_segments(const leyline_plan_t* plan, leyline_segment* out /*[n_segments]*/);
+LEYLINE_API leyline_status leyline_plan_released(const leyline_plan_t* plan, int32_t* out /*[n_released]*/);
+LEYLINE_API leyline_status leyline_plan_segments(const leyline_plan_t* plan, leyline_segment* out /*[n_segments]*/);
 
 /* One device work item per layer (query result, for tests and tooling): `n_rows` rows that are consecutive in
  * NEW logical position, `dst_pos .. dst_pos+n_rows` of `request`, read from OLD logical positions
@@ -204,11 +248,17 @@ typedef struct {
     int32_t dep_lo, dep_hi;
     int32_t request;
 } leyline_tile;
-leyline_status leyline_plan_tiles(const leyline_plan_t* plan, leyline_tile* out /*[n_tiles]*/);
+LEYLINE_API leyline_status leyline_plan_tiles(const leyline_plan_t* plan, leyline_tile* out /*[n_tiles]*/);
 /* Shifts C of the cos/sin table rows: row g holds cos/sin(C_g * theta_i), i in [0, rope_dim/2). */
-leyline_status leyline_plan_trig_shifts(const leyline_plan_t* plan, int64_t* out /*[n_trig]*/);
-/* The table itself, [n_trig][2][rope_dim/2] fp32: cos then sin of C_g * theta_i (fp64 product and trig, rounded once). */
-leyline_status leyline_plan_trig_table(const leyline_plan_t* plan, float* out);
+LEYLINE_API leyline_status leyline_plan_trig_shifts(const leyline_plan_t* plan, int64_t* out /*[n_trig]*/);
+/* The table itself, [n_trig][2][rope_dim/2] fp32: cos then sin of C_g * theta_i (fp64 product and trig, rounded once),
+ * evaluated on the HOST by this call (libm).  The launches never upload it: the index kernel of every launch evaluates
+ * the same expression in fp64 on the device (CUDA's sincos, <= 2 ulp of fp64 before the one rounding to fp32), which
+ * takes the 32 fp64 sincos per distinct shift off the host's critical path (hundreds of shifts per call in the paper's
+ * chunk workload).  leyline_plan_trig_table_device copies the device's table back (after the plan has
+ * been launched and its stream synchronised; LEYLINE_E_INVALID before that) so that the two can be compared. */
+LEYLINE_API leyline_status leyline_plan_trig_table(const leyline_plan_t* plan, float* out);
+LEYLINE_API leyline_status leyline_plan_trig_table_device(const leyline_plan_t* plan, float* out);
 
 /*
  * leyline_splice -- execute a FRESH or INPLACE_MOVE plan on `cuda_stream` (steps a2-a4).
@@ -233,7 +283,7 @@ leyline_status leyline_plan_trig_table(const leyline_plan_t* plan, float* out);
  * Kernels: index / page-table rewrite, then the fused gather -> rotate -> scatter (+ replacement insert).
  * Asynchronous; only launch errors are returned.  Bytes the mode says are never written are never written.
  */
-leyline_status leyline_splice(leyline_plan_t* plan, void* const* layer_src, void* const* layer_dst,
+LEYLINE_API leyline_status leyline_splice(leyline_plan_t* plan, void* const* layer_src, void* const* layer_dst,
                               const void* const* layer_repl, int32_t* dev_page_table_out, int32_t* dev_slot_idx_out,
                               void* cuda_stream);
 
@@ -242,7 +292,7 @@ leyline_status leyline_splice(leyline_plan_t* plan, void* const* layer_src, void
  * token where it sits (128 B of every 1152 B bf16 MLA row; the whole row of a full-width K pool), optionally copy the replacement rows into the consumed
  * free slots (layer_repl == NULL: the caller already prefilled them), and write the new token-level index list.
  */
-leyline_status leyline_rotate_inplace(leyline_plan_t* plan, void* const* layer_ptrs, const void* const* layer_repl,
+LEYLINE_API leyline_status leyline_rotate_inplace(leyline_plan_t* plan, void* const* layer_ptrs, const void* const* layer_repl,
                                       int32_t* dev_slot_idx_out, void* cuda_stream);
 
 /*
@@ -257,7 +307,7 @@ leyline_status leyline_rotate_inplace(leyline_plan_t* plan, void* const* layer_p
  * pool and their band widened exactly into the master; with layer_repl == NULL the caller fills both.
  * bf16 caches and ROTATE_ONLY plans only (else LEYLINE_E_UNSUPPORTED / LEYLINE_E_INVALID).
  */
-leyline_status leyline_rotate_inplace_master(leyline_plan_t* plan, void* const* layer_ptrs, void* const* layer_master,
+LEYLINE_API leyline_status leyline_rotate_inplace_master(leyline_plan_t* plan, void* const* layer_ptrs, void* const* layer_master,
                                              const void* const* layer_repl, int32_t* dev_slot_idx_out, void* cuda_stream);
 
 /*
@@ -269,36 +319,23 @@ leyline_status leyline_rotate_inplace_master(leyline_plan_t* plan, void* const* 
  * first launch, in order on its stream.  Idempotent; a no-op once the tables are on the device.
  * Returns LEYLINE_E_CUDA without a device (the plan itself stays valid and usable for queries).
  */
-leyline_status leyline_plan_prefetch(leyline_plan_t* plan);
+LEYLINE_API leyline_status leyline_plan_prefetch(leyline_plan_t* plan);
 
-void leyline_plan_destroy(leyline_plan_t* plan);
-const char* leyline_strerror(leyline_status s);
+LEYLINE_API void leyline_plan_destroy(leyline_plan_t* plan);
+LEYLINE_API const char* leyline_strerror(leyline_status s);
 /* Text of the last CUDA error seen by this thread's calls into the library ("" if none). */
-const char* leyline_last_cuda_error(void);
+LEYLINE_API const char* leyline_last_cuda_error(void);
 
-/* Process-wide tuning knobs (benchmarking; defaults are what bench.py reports).  Read by leyline_plan. */
-typedef struct {
-    int32_t kernel;        /* a3/a4 mover: 0 = auto (bulk for unpadded rows in pages of >= 16 rows or of >= 1 KB each, or when the band is not a
-                              single head of 2^k <= 32 chunks), 1 = row kernel (LDG/STG through registers; single-head
-                              bands of 2^k chunks only, else LEYLINE_E_UNSUPPORTED), 2 = bulk kernel (TMA 1-D bulk
-                              copies through shared memory) */
-    int32_t tile_rows;     /* rows per tile of the move/insert kernels, 0 = default (row kernel <= 32, bulk <= 64) */
-    int32_t ctas_per_sm;   /* row kernel only, 0 = default */
-    int32_t profile;       /* 1: record CUDA events around the data-moving kernels (leyline_plan_kernel_ms) */
-    int32_t stages;        /* bulk kernel only: shared-memory stages per CTA, 0 = as many as fit (at most 8) */
-    int32_t layer_group;   /* bulk kernel only: layers per work item (one stage each), 0 = default */
-    int32_t consumer_warps;/* bulk kernel only: warps that rotate the band in shared memory, 0 = default (4 for MLA's
-                              narrow band, more when the band is most of the row), at most 16 */
-} leyline_tuning;
-leyline_status leyline_set_tuning(const leyline_tuning* t);
-leyline_status leyline_get_tuning(leyline_tuning* t);
+/* Process-wide default tuning, read by leyline_plan (benchmarking; leyline_plan_ex takes its own). */
+LEYLINE_API leyline_status leyline_set_tuning(const leyline_tuning* t);
+LEYLINE_API leyline_status leyline_get_tuning(leyline_tuning* t);
 
 /* Device time of the data-moving kernels (a3+a4 / a5) of the plan's last launch, from CUDA events recorded on
  * the launching stream when the plan was created with tuning.profile = 1.  Call after synchronising the stream. */
-leyline_status leyline_plan_kernel_ms(const leyline_plan_t* plan, float* ms);
+LEYLINE_API leyline_status leyline_plan_kernel_ms(const leyline_plan_t* plan, float* ms);
 
 /* Library / build description, e.g. "leyline-b200 0.1 sm_100a". */
-const char* leyline_version(void);
+LEYLINE_API const char* leyline_version(void);
 
 #ifdef __cplusplus
 }

@@ -58,7 +58,7 @@ typedef enum { LEYLINE_CDC_HASH = 0, LEYLINE_CDC_ANCHOR = 1, LEYLINE_CDC_MAX = 2
  *
  * Scratch memory is allocated and freed stream-ordered by the call itself (about 30 B per token).
  */
-leyline_status leyline_cdc_chunk(const leyline_cdc_params* params, const int32_t* dev_tokens, int64_t n_tokens,
+LEYLINE_API leyline_status leyline_cdc_chunk(const leyline_cdc_params* params, const int32_t* dev_tokens, int64_t n_tokens,
                                  const int64_t* dev_seq_offsets, int32_t n_seqs, const int32_t* dev_anchor_ids,
                                  int32_t n_anchor_ids, int64_t* dev_chunk_end, uint64_t* dev_chunk_hash,
                                  int32_t* dev_chunk_kind, int64_t capacity, int64_t* dev_n_chunks, void* cuda_stream);
@@ -72,11 +72,11 @@ leyline_status leyline_cdc_chunk(const leyline_cdc_params* params, const int32_t
  *   lookup  out[i] = the value stored under hashes[i], or -1.
  * Hash 0 is never a valid key (D4 remaps it).
  */
-leyline_status leyline_registry_clear(uint64_t* dev_keys, int64_t* dev_vals, int64_t capacity, void* cuda_stream);
-leyline_status leyline_registry_insert(uint64_t* dev_keys, int64_t* dev_vals, int64_t capacity,
+LEYLINE_API leyline_status leyline_registry_clear(uint64_t* dev_keys, int64_t* dev_vals, int64_t capacity, void* cuda_stream);
+LEYLINE_API leyline_status leyline_registry_insert(uint64_t* dev_keys, int64_t* dev_vals, int64_t capacity,
                                        const uint64_t* dev_hashes, const int64_t* dev_values, int64_t n,
                                        int64_t* dev_n_dropped, void* cuda_stream);
-leyline_status leyline_registry_lookup(const uint64_t* dev_keys, const int64_t* dev_vals, int64_t capacity,
+LEYLINE_API leyline_status leyline_registry_lookup(const uint64_t* dev_keys, const int64_t* dev_vals, int64_t capacity,
                                        const uint64_t* dev_hashes, int64_t n, int64_t* dev_out, void* cuda_stream);
 
 #ifdef __cplusplus

@@ -15,7 +15,7 @@ import numpy as np
 
 from . import build as _build
 
-OK, E_INVALID, E_UNSORTED, E_OVERLAP, E_RANGE, E_NOFREE, E_UNSUPPORTED, E_CUDA = range(8)
+OK, E_INVALID, E_UNSORTED, E_OVERLAP, E_RANGE, E_NOFREE, E_UNSUPPORTED, E_CUDA, E_NOMEM, E_ALIAS = range(10)
 BF16, FP8_E4M3 = 0, 1
 NEOX, INTERLEAVED = 0, 1
 FRESH, INPLACE_MOVE, ROTATE_ONLY = 0, 1, 2
@@ -55,7 +55,8 @@ class Tile(C.Structure):
 
 class Tuning(C.Structure):
     _fields_ = [("kernel", C.c_int32), ("tile_rows", C.c_int32), ("ctas_per_sm", C.c_int32), ("profile", C.c_int32),
-                ("stages", C.c_int32), ("layer_group", C.c_int32), ("consumer_warps", C.c_int32)]
+                ("stages", C.c_int32), ("layer_group", C.c_int32), ("consumer_warps", C.c_int32),
+                ("rotate_kernel", C.c_int32)]
 
 
 class CdcParams(C.Structure):
@@ -78,7 +79,9 @@ def _load() -> C.CDLL:
     vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
     L.leyline_plan.restype = C.c_int
     L.leyline_plan.argtypes = [C.POINTER(CacheDesc), i32, i32, vp, vp, vp, i32, vp, vp, i64, C.POINTER(vp)]
-    for name in ("leyline_plan_new_seq_lens", "leyline_plan_forget_trim", "leyline_plan_slot_offsets",
+    L.leyline_plan_ex.restype = C.c_int
+    L.leyline_plan_ex.argtypes = [C.POINTER(CacheDesc), i32, i32, vp, vp, vp, i32, vp, vp, i64, C.POINTER(Tuning), C.POINTER(vp)]
+    for name in ("leyline_plan_trig_table_device", "leyline_plan_new_seq_lens", "leyline_plan_forget_trim", "leyline_plan_slot_offsets",
                  "leyline_plan_new_pt_offsets", "leyline_plan_new_pages", "leyline_plan_released",
                  "leyline_plan_segments", "leyline_plan_tiles", "leyline_plan_trig_shifts", "leyline_plan_trig_table"):
         f = getattr(L, name)
@@ -132,8 +135,8 @@ def leyline_version() -> str:
 
 
 def leyline_set_tuning(kernel: int = 0, tile_rows: int = 0, ctas_per_sm: int = 0, profile: int = 0, stages: int = 0,
-                       layer_group: int = 0, consumer_warps: int = 0):
-    t = Tuning(kernel, tile_rows, ctas_per_sm, profile, stages, layer_group, consumer_warps)
+                       layer_group: int = 0, consumer_warps: int = 0, rotate_kernel: int = 0):
+    t = Tuning(kernel, tile_rows, ctas_per_sm, profile, stages, layer_group, consumer_warps, rotate_kernel)
     _check(_lib.leyline_set_tuning(C.byref(t)), "leyline_set_tuning")
 
 
@@ -142,7 +145,7 @@ def leyline_get_tuning() -> dict:
     _check(_lib.leyline_get_tuning(C.byref(t)), "leyline_get_tuning")
     return {"kernel": t.kernel, "tile_rows": t.tile_rows, "ctas_per_sm": t.ctas_per_sm, "profile": t.profile,
             "stages": t.stages, "layer_group": t.layer_group,
-            "consumer_warps": t.consumer_warps}
+            "consumer_warps": t.consumer_warps, "rotate_kernel": t.rotate_kernel}
 
 
 def _arr(x, dtype):
@@ -204,6 +207,11 @@ class Plan:
         return self._get("leyline_plan_trig_table", self.info.n_trig * 2 * self._H, np.float32).reshape(-1, 2, self._H)
 
     @property
+    def trig_table_device(self):
+        """The table the launches use (evaluated in fp64 on the device); valid after a launch."""
+        return self._get("leyline_plan_trig_table_device", self.info.n_trig * 2 * self._H, np.float32).reshape(-1, 2, self._H)
+
+    @property
     def segments(self):
         buf = (Segment * int(self.info.n_segments))()
         _check(_lib.leyline_plan_segments(self._h, C.cast(buf, C.c_void_p)), "leyline_plan_segments")
@@ -260,6 +268,18 @@ def leyline_plan(desc: CacheDesc, mode: int, seq_lens, pt_offsets, pages, direct
     st = _lib.leyline_plan(C.byref(desc), mode, len(sl), _ptr(sl), _ptr(po), _ptr(pg), len(d), _ptr(d), _ptr(fr),
                            len(fr), C.byref(h))
     _check(st, "leyline_plan")
+    return Plan(h.value, len(sl), desc.rope_dim)
+
+
+def leyline_plan_ex(desc: CacheDesc, mode: int, seq_lens, pt_offsets, pages, directives, free_ids, tuning: Tuning | None = None) -> Plan:
+    """leyline.h: leyline_plan_ex -- the planner with its tuning passed per call (None = defaults); the process-wide
+    tuning of leyline_set_tuning is not consulted."""
+    sl, po, pg, fr = _arr(seq_lens, np.int64), _arr(pt_offsets, np.int64), _arr(pages, np.int32), _arr(free_ids, np.int32)
+    d = directives if isinstance(directives, np.ndarray) else pack_directives(directives)
+    h = C.c_void_p()
+    st = _lib.leyline_plan_ex(C.byref(desc), mode, len(sl), _ptr(sl), _ptr(po), _ptr(pg), len(d), _ptr(d), _ptr(fr),
+                              len(fr), C.byref(tuning) if tuning is not None else None, C.byref(h))
+    _check(st, "leyline_plan_ex")
     return Plan(h.value, len(sl), desc.rope_dim)
 
 

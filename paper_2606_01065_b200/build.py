@@ -16,7 +16,7 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libleyline.so")
 SOURCES = ["plan.cpp", "splice.cu", "cdc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler",
-              "-fPIC,-Wall,-Wextra", "-Xptxas", "-v", "--shared", "-cudart", "static"]
+              "-fPIC,-Wall,-Wextra,-fvisibility=hidden", "-Xptxas", "-v", "--shared", "-cudart", "static"]
 
 
 def _stale() -> bool:

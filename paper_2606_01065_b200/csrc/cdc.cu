@@ -18,6 +18,7 @@
 #include <string>
 
 #include "leyline_cdc.h"
+#include "plan_internal.h" /* LEYLINE_CATCH_STATUS */
 
 namespace {
 
@@ -274,11 +275,11 @@ unsigned grid_for(int64_t n, int per_block = kT) {
 
 }  // namespace
 
-extern "C" leyline_status leyline_cdc_chunk(const leyline_cdc_params* p, const int32_t* dev_tokens, int64_t n,
+extern "C" LEYLINE_API leyline_status leyline_cdc_chunk(const leyline_cdc_params* p, const int32_t* dev_tokens, int64_t n,
                                             const int64_t* dev_seq_offsets, int32_t n_seqs, const int32_t* dev_anchor_ids,
                                             int32_t n_anchor_ids, int64_t* dev_chunk_end, uint64_t* dev_chunk_hash,
                                             int32_t* dev_chunk_kind, int64_t capacity, int64_t* dev_n_chunks,
-                                            void* cuda_stream) {
+                                            void* cuda_stream) try {
     g_cdc_error.clear();
     if (!p || p->reserved_ != 0 || p->min_size < 1 || p->max_size < p->min_size || p->max_size > 4096 ||
         p->mask_bits < 0 || p->mask_bits > 32)
@@ -333,21 +334,21 @@ extern "C" leyline_status leyline_cdc_chunk(const leyline_cdc_params* p, const i
     if (!ok(cudaGetLastError())) st = LEYLINE_E_CUDA;
     if (!ok(cudaFreeAsync(ws, stream))) st = LEYLINE_E_CUDA;
     return st;
-}
+} LEYLINE_CATCH_STATUS
 
 static bool pow2(int64_t x) { return x > 0 && (x & (x - 1)) == 0; }
 
-extern "C" leyline_status leyline_registry_clear(uint64_t* dev_keys, int64_t* dev_vals, int64_t capacity, void* cuda_stream) {
+extern "C" LEYLINE_API leyline_status leyline_registry_clear(uint64_t* dev_keys, int64_t* dev_vals, int64_t capacity, void* cuda_stream) try {
     g_cdc_error.clear();
     if (!dev_keys || !dev_vals || !pow2(capacity)) return LEYLINE_E_INVALID;
     k_reg_clear<<<grid_for(capacity), kT, 0, static_cast<cudaStream_t>(cuda_stream)>>>(dev_keys, dev_vals, capacity);
     CU(cudaGetLastError());
     return LEYLINE_OK;
-}
+} LEYLINE_CATCH_STATUS
 
-extern "C" leyline_status leyline_registry_insert(uint64_t* dev_keys, int64_t* dev_vals, int64_t capacity,
+extern "C" LEYLINE_API leyline_status leyline_registry_insert(uint64_t* dev_keys, int64_t* dev_vals, int64_t capacity,
                                                   const uint64_t* dev_hashes, const int64_t* dev_values, int64_t n,
-                                                  int64_t* dev_n_dropped, void* cuda_stream) {
+                                                  int64_t* dev_n_dropped, void* cuda_stream) try {
     g_cdc_error.clear();
     if (!dev_keys || !dev_vals || !pow2(capacity) || n < 0 || (n > 0 && (!dev_hashes || !dev_values))) return LEYLINE_E_INVALID;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
@@ -356,14 +357,14 @@ extern "C" leyline_status leyline_registry_insert(uint64_t* dev_keys, int64_t* d
     k_reg_insert<<<grid_for(n), kT, 0, stream>>>(dev_keys, dev_vals, capacity, dev_hashes, dev_values, n, dev_n_dropped);
     CU(cudaGetLastError());
     return LEYLINE_OK;
-}
+} LEYLINE_CATCH_STATUS
 
-extern "C" leyline_status leyline_registry_lookup(const uint64_t* dev_keys, const int64_t* dev_vals, int64_t capacity,
-                                                  const uint64_t* dev_hashes, int64_t n, int64_t* dev_out, void* cuda_stream) {
+extern "C" LEYLINE_API leyline_status leyline_registry_lookup(const uint64_t* dev_keys, const int64_t* dev_vals, int64_t capacity,
+                                                  const uint64_t* dev_hashes, int64_t n, int64_t* dev_out, void* cuda_stream) try {
     g_cdc_error.clear();
     if (!dev_keys || !dev_vals || !pow2(capacity) || n < 0 || (n > 0 && (!dev_hashes || !dev_out))) return LEYLINE_E_INVALID;
     if (n == 0) return LEYLINE_OK;
     k_reg_lookup<<<grid_for(n), kT, 0, static_cast<cudaStream_t>(cuda_stream)>>>(dev_keys, dev_vals, capacity, dev_hashes, n, dev_out);
     CU(cudaGetLastError());
     return LEYLINE_OK;
-}
+} LEYLINE_CATCH_STATUS

@@ -58,6 +58,18 @@ struct IndexParams {
     int32_t page_shift;
 };
 
+/* The cos/sin table of the launch, evaluated on the device by the index kernel: row g = cos then sin of
+ * shifts[g] * inv_freq[i], i in [0, H) -- fp64 product of the exact integer shift and the fp32 theta_i promoted exactly,
+ * fp64 sincos (CUDA math library, <= 2 ulp of fp64, exact argument reduction for |x| up to ~1.3e5 rad here), rounded
+ * once to fp32. */
+struct TrigParams {
+    const int64_t* shifts;
+    const float* inv_freq;
+    float* out;
+    int32_t n_trig;
+    int32_t H;
+};
+
 /* ---- global memory access ---- */
 
 __device__ __forceinline__ int4 ld_stream(const void* p) { /* read-only for the whole kernel, read once */

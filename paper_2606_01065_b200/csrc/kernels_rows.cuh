@@ -1,7 +1,8 @@
 /*
  * kernels_rows.cuh -- the register-staged ("row") kernels: steps a2, a3, a4, a5 of DESIGN.md.
  *
- *   k_index        a2  slot-index list / page-table rewrite (PAPER.md:135, :405(c) "re-keyed")
+ *   k_index        a2  slot-index list / page-table rewrite (PAPER.md:135, :405(c) "re-keyed"), and the cos/sin table
+ *                  of the plan's shifts (fp64 on the device)
  *   k_move_rows    a3+a4  gather -> rotate -> scatter of whole rows, replacement insert as extra tiles
  *                  (PAPER.md:118-127, :405(b)(c)); with HAZARD = true it is the in-place mover of rule M2
  *   k_rotate_band  a5  in-place rotation of the K_pe band only
@@ -37,9 +38,25 @@ __device__ __forceinline__ void index_body(const IndexParams& p, long long block
     }
 }
 
-__global__ void __launch_bounds__(kThreads) k_index(const IndexParams a, const IndexParams b, const int blocks_a) {
-    if ((int)blockIdx.x < blocks_a) index_body(a, blockIdx.x, blocks_a);
-    else index_body(b, blockIdx.x - blocks_a, gridDim.x - blocks_a);
+/* blocks [0, blocks_a): page-table rows; [blocks_a, blocks_a + blocks_b): token-level slot list; the rest: the cos/sin
+ * table of the plan's distinct shifts, one (shift, frequency) per thread, in fp64 (see TrigParams).  The data kernel
+ * that consumes the table is launched behind this one on the same stream. */
+__global__ void __launch_bounds__(kThreads) k_index(const IndexParams a, const IndexParams b, const TrigParams tp,
+                                                     const int blocks_a, const int blocks_b) {
+    if ((int)blockIdx.x < blocks_a) {
+        index_body(a, blockIdx.x, blocks_a);
+    } else if ((int)blockIdx.x < blocks_a + blocks_b) {
+        index_body(b, blockIdx.x - blocks_a, blocks_b);
+    } else {
+        const int u = ((int)blockIdx.x - blocks_a - blocks_b) * kThreads + (int)threadIdx.x;
+        if (u < tp.n_trig * tp.H) {
+            const int g = u / tp.H, i = u - g * tp.H;
+            double sn, cs;
+            sincos((double)tp.shifts[g] * (double)tp.inv_freq[i], &sn, &cs);
+            tp.out[(int64_t)g * 2 * tp.H + i] = (float)cs;
+            tp.out[(int64_t)g * 2 * tp.H + tp.H + i] = (float)sn;
+        }
+    }
 }
 
 /* ------------------------------------------------------------------ a3 + a4 ---- */

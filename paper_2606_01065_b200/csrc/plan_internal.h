@@ -6,6 +6,7 @@
 #define LEYLINE_PLAN_INTERNAL_H_
 
 #include <cstdint>
+#include <new>
 #include <vector>
 
 #include "leyline.h"
@@ -38,6 +39,17 @@ enum : int32_t { TILE_SRC_REPL = 1, TILE_DST_TOKEN = 2,
  * this many units, i.e. rot_tile_rows = kRotUnitsPerItem / (rope_heads * head_chunks / 2) rows. */
 constexpr int kRotUnitsPerItem = 1024;
 
+/* k_rotate_band_tma (a5 on paged pools): the band of up to kRotTmaBoxRows consecutive slots is one 2-D TMA box. */
+constexpr int kRotTmaBoxRows = 64;
+constexpr bool kRotateTmaByDefault = false; /* decided by measurement */
+
+/* ROTATE_ONLY: `count` removed old positions pos0.. of the request whose old page table starts at tabs[tab]; their slots
+ * are the released list (expanded by leyline_plan_released). */
+struct ReleasedRun {
+    int32_t tab;
+    int64_t pos0, count;
+};
+
 /* One run of the token-level index list / page-table output (step a2). */
 struct IdxRun {
     int64_t out_begin; /* first output element */
@@ -65,24 +77,29 @@ struct leyline_plan_s {
     int32_t head_chunks = 8;            /* 16-byte chunks per head */
     int32_t dep_distance_median = -1;   /* INPLACE_MOVE: median of (tile index - dep_hi) over tiles that wait, -1 if none */
     bool rotate_with_bulk = false;      /* ROTATE_ONLY on a band that is most of the row: the rotation runs on k_move_bulk, in place */
+    bool rotate_with_tma = false;       /* ROTATE_ONLY on a narrow band in pages of >= 16 rows: k_rotate_band_tma (2-D TMA boxes) */
     bool use_bulk = false;              /* a3/a4 run on k_move_bulk (TMA bulk copies) instead of k_move_rows */
     leyline_tuning tuning{};
 
     std::vector<int64_t> old_seq_lens, new_seq_lens, forget_trim, slot_offsets, new_pt_offsets, old_pt_offsets;
     std::vector<int32_t> new_pages;     /* concatenated new page-table rows (FRESH / INPLACE_MOVE) */
-    std::vector<int32_t> released;
+    std::vector<int32_t> released;      /* page modes: released page ids */
+    std::vector<leyline::ReleasedRun> released_runs; /* ROTATE_ONLY: released slots as runs of removed old positions */
+    std::vector<int64_t> seg_begin;     /* segments of request r: [seg_begin[r], seg_begin[r+1]) */
     std::vector<leyline_segment> segments;
     std::vector<leyline::DevTile> tiles;   /* move tiles first, then insert tiles; ticket order */
     std::vector<int64_t> trig_shifts;
-    std::vector<float> trig;            /* [n_trig][2][H]: cos then sin of C * theta_i, fp64 libm rounded to fp32 */
+                                        /* the cos/sin table [n_trig][2][H] of C * theta_i is evaluated in fp64 on the
+                                           device by the launch's index kernel (and by the host only for the query) */
     std::vector<int32_t> tabs;          /* old page tables ++ new page tables ++ token-level lists */
     std::vector<leyline::IdxRun> slot_runs;  /* produce dev_slot_idx_out */
     std::vector<leyline::IdxRun> page_runs;  /* produce dev_page_table_out */
     leyline_plan_info info{};
 
     /* device side (owned by splice.cu; created on first launch, freed by leyline_plan_destroy) */
-    void* d_blob = nullptr;             /* tiles | trig | tabs | slot_runs | page_runs */
-    int64_t off_tiles = 0, off_trig = 0, off_tabs = 0, off_slot_runs = 0, off_page_runs = 0, blob_bytes = 0;
+    void* d_blob = nullptr;             /* tiles | trig (device-computed) | shifts | inv_freq | tabs | slot_runs | page_runs */
+    int64_t off_tiles = 0, off_trig = 0, off_shifts = 0, off_inv_freq = 0, off_tabs = 0, off_slot_runs = 0, off_page_runs = 0,
+            blob_bytes = 0;
     void* d_scratch = nullptr;          /* tail of d_blob: [0,256) ticket counters; then hazard flags [n_move_tiles * n_layers] int32 */
     int64_t scratch_bytes = 0;
     int device = -1;
@@ -91,9 +108,17 @@ struct leyline_plan_s {
     void* last_stream = nullptr;        /* stream of the last launch: the device tables are freed on it */
     void* ev_uploaded = nullptr;        /* leyline_plan_prefetch: cudaEvent_t recorded after the upload on the copy stream */
     bool scratch_clean = false;         /* the upload path already zeroed d_scratch; the first launch skips its memset */
+    bool trig_ready = false;            /* the device cos/sin table has been written by a launch's index kernel */
 };
 
-/* implemented in splice.cu; plan.cpp calls it from leyline_plan_destroy */
-extern "C" void leyline_plan_release_device_(leyline_plan_s* plan);
+/* closes a function-try-block of an extern "C" entry point: nothing is thrown across the ABI */
+#define LEYLINE_CATCH_STATUS                                     \
+    catch (const std::bad_alloc&) { return LEYLINE_E_NOMEM; }    \
+    catch (...) { return LEYLINE_E_INVALID; }
+
+namespace leyline {
+/* implemented in splice.cu; plan.cpp calls it from leyline_plan_destroy (not part of the ABI, not exported) */
+void plan_release_device(leyline_plan_s* plan);
+}  // namespace leyline
 
 #endif /* LEYLINE_PLAN_INTERNAL_H_ */

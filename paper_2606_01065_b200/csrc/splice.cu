@@ -126,24 +126,29 @@ leyline_status device_info(int* dev_out) {
 
 /* Allocate tables + scratch, copy the tables and zero the scratch, all stream-ordered on `stream`. */
 leyline_status upload_tables(leyline_plan_s* pl, int dev, cudaStream_t stream) {
-    /* one allocation: tiles | trig | tabs | slot_runs | page_runs | scratch, each 256-byte aligned */
+    /* one allocation: shifts | inv_freq | tiles | tabs | slot_runs | page_runs (uploaded) | trig (written by k_index) |
+     * scratch, each 256-byte aligned */
     int64_t off = 0;
     auto place = [&](int64_t bytes) { int64_t o = off; off = align_up(off + bytes, 256); return o; };
+    pl->off_shifts = place((int64_t)pl->trig_shifts.size() * sizeof(int64_t));
+    pl->off_inv_freq = place((int64_t)pl->inv_freq.size() * sizeof(float));
     pl->off_tiles = place((int64_t)pl->tiles.size() * sizeof(DevTile));
-    pl->off_trig = place((int64_t)pl->trig.size() * sizeof(float));
     pl->off_tabs = place((int64_t)pl->tabs.size() * sizeof(int32_t));
     pl->off_slot_runs = place((int64_t)pl->slot_runs.size() * sizeof(IdxRun));
     pl->off_page_runs = place((int64_t)pl->page_runs.size() * sizeof(IdxRun));
+    const int64_t upload_bytes = off > 0 ? off : 256;
+    pl->off_trig = place((int64_t)pl->trig_shifts.size() * 2 * (int64_t)pl->inv_freq.size() * sizeof(float));
     pl->blob_bytes = off > 0 ? off : 256;
     const int64_t n_flags = pl->mode == LEYLINE_INPLACE_MOVE ? pl->info.n_tiles * pl->desc.n_layers : 0;
     pl->scratch_bytes = 256 + align_up(n_flags * (int64_t)sizeof(int32_t), 256);
-    PinnedBuf pin = pin_acquire((size_t)pl->blob_bytes, dev);
+    PinnedBuf pin = pin_acquire((size_t)upload_bytes, dev);
     std::string pageable;
-    if (!pin.p) pageable.resize((size_t)pl->blob_bytes);
+    if (!pin.p) pageable.resize((size_t)upload_bytes);
     uint8_t* host = pin.p ? static_cast<uint8_t*>(pin.p) : reinterpret_cast<uint8_t*>(&pageable[0]);
     auto put = [&](int64_t o, const void* src, size_t bytes) { if (bytes) std::memcpy(host + o, src, bytes); };
+    put(pl->off_shifts, pl->trig_shifts.data(), pl->trig_shifts.size() * sizeof(int64_t));
+    put(pl->off_inv_freq, pl->inv_freq.data(), pl->inv_freq.size() * sizeof(float));
     put(pl->off_tiles, pl->tiles.data(), pl->tiles.size() * sizeof(DevTile));
-    put(pl->off_trig, pl->trig.data(), pl->trig.size() * sizeof(float));
     put(pl->off_tabs, pl->tabs.data(), pl->tabs.size() * sizeof(int32_t));
     put(pl->off_slot_runs, pl->slot_runs.data(), pl->slot_runs.size() * sizeof(IdxRun));
     put(pl->off_page_runs, pl->page_runs.data(), pl->page_runs.size() * sizeof(IdxRun));
@@ -157,7 +162,7 @@ leyline_status upload_tables(leyline_plan_s* pl, int dev, cudaStream_t stream) {
     }
     pl->d_scratch = static_cast<uint8_t*>(pl->d_blob) + pl->blob_bytes;
     /* pinned source: a plain stream-ordered DMA; pageable fallback: the runtime stages it before returning */
-    bool ok = cuda_ok(cudaMemcpyAsync(pl->d_blob, host, (size_t)pl->blob_bytes, cudaMemcpyHostToDevice, stream),
+    bool ok = cuda_ok(cudaMemcpyAsync(pl->d_blob, host, (size_t)upload_bytes, cudaMemcpyHostToDevice, stream),
                       "cudaMemcpyAsync(plan tables)");
     if (pin.p) pin_release(pin, stream);
     ok = ok && cuda_ok(cudaMemsetAsync(pl->d_scratch, 0, (size_t)pl->scratch_bytes, stream), "cudaMemsetAsync(scratch)");
@@ -198,18 +203,26 @@ IndexParams index_params(const leyline_plan_s* pl, const std::vector<IdxRun>& ru
     return ip;
 }
 
-/* a2: page-table rows and token-level slot list in ONE launch (either output may be NULL). */
-leyline_status launch_index(const leyline_plan_s* pl, int32_t* page_table_out, int32_t* slot_idx_out, cudaStream_t stream) {
+/* a2: page-table rows and token-level slot list (either output may be NULL), and the cos/sin table the data kernel
+ * behind it reads, in ONE launch. */
+leyline_status launch_index(leyline_plan_s* pl, int32_t* page_table_out, int32_t* slot_idx_out, cudaStream_t stream) {
     const IndexParams a = index_params(pl, pl->page_runs, pl->off_page_runs, page_table_out);
     const IndexParams b = index_params(pl, pl->slot_runs, pl->off_slot_runs, slot_idx_out);
+    TrigParams tp;
+    tp.shifts = blob_at<int64_t>(pl, pl->off_shifts);
+    tp.inv_freq = blob_at<float>(pl, pl->off_inv_freq);
+    tp.out = const_cast<float*>(blob_at<float>(pl, pl->off_trig));
+    tp.n_trig = pl->trig_ready ? 0 : (int32_t)pl->trig_shifts.size(); /* a relaunched plan keeps its table */
+    tp.H = (int32_t)pl->inv_freq.size();
     auto blocks_of = [](const IndexParams& ip) {
         long long n = (ip.total + kThreads - 1) / kThreads;
         return n > 4LL * g_dev.sms ? 4LL * g_dev.sms : n;
     };
-    const long long na = blocks_of(a), nb = blocks_of(b);
-    if (na + nb == 0) return LEYLINE_OK;
-    k_index<<<(unsigned)(na + nb), kThreads, 0, stream>>>(a, b, (int)na);
+    const long long na = blocks_of(a), nb = blocks_of(b), nt = ((long long)tp.n_trig * tp.H + kThreads - 1) / kThreads;
+    if (na + nb + nt == 0) return LEYLINE_OK;
+    k_index<<<(unsigned)(na + nb + nt), kThreads, 0, stream>>>(a, b, tp, (int)na, (int)nb);
     CU(cudaGetLastError());
+    pl->trig_ready = true;
     return LEYLINE_OK;
 }
 
@@ -440,9 +453,9 @@ leyline_status begin_call(leyline_plan_s* pl, cudaStream_t stream) {
 
 }  // namespace
 
-extern "C" leyline_status leyline_splice(leyline_plan_t* pl, void* const* layer_src, void* const* layer_dst,
+extern "C" LEYLINE_API leyline_status leyline_splice(leyline_plan_t* pl, void* const* layer_src, void* const* layer_dst,
                                          const void* const* layer_repl, int32_t* dev_page_table_out,
-                                         int32_t* dev_slot_idx_out, void* cuda_stream) {
+                                         int32_t* dev_slot_idx_out, void* cuda_stream) try {
     g_last_error.clear();
     if (!pl || pl->mode == LEYLINE_ROTATE_ONLY) return LEYLINE_E_INVALID;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
@@ -488,11 +501,11 @@ extern "C" leyline_status leyline_splice(leyline_plan_t* pl, void* const* layer_
     if (st != LEYLINE_OK) return st;
     if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_stop), stream));
     return LEYLINE_OK;
-}
+} LEYLINE_CATCH_STATUS
 
-extern "C" leyline_status leyline_rotate_inplace(leyline_plan_t* pl, void* const* layer_ptrs,
+extern "C" LEYLINE_API leyline_status leyline_rotate_inplace(leyline_plan_t* pl, void* const* layer_ptrs,
                                                  const void* const* layer_repl, int32_t* dev_slot_idx_out,
-                                                 void* cuda_stream) {
+                                                 void* cuda_stream) try {
     g_last_error.clear();
     if (!pl || pl->mode != LEYLINE_ROTATE_ONLY) return LEYLINE_E_INVALID;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
@@ -516,11 +529,11 @@ extern "C" leyline_status leyline_rotate_inplace(leyline_plan_t* pl, void* const
     if (st != LEYLINE_OK) return st;
     if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_stop), stream));
     return LEYLINE_OK;
-}
+} LEYLINE_CATCH_STATUS
 
-extern "C" leyline_status leyline_rotate_inplace_master(leyline_plan_t* pl, void* const* layer_ptrs, void* const* layer_master,
+extern "C" LEYLINE_API leyline_status leyline_rotate_inplace_master(leyline_plan_t* pl, void* const* layer_ptrs, void* const* layer_master,
                                                         const void* const* layer_repl, int32_t* dev_slot_idx_out,
-                                                        void* cuda_stream) {
+                                                        void* cuda_stream) try {
     g_last_error.clear();
     if (!pl || pl->mode != LEYLINE_ROTATE_ONLY) return LEYLINE_E_INVALID;
     if (pl->desc.dtype != LEYLINE_BF16) { g_last_error = "the fp32 master option covers bf16 caches"; return LEYLINE_E_UNSUPPORTED; }
@@ -555,9 +568,9 @@ extern "C" leyline_status leyline_rotate_inplace_master(leyline_plan_t* pl, void
     }
     if (pl->tuning.profile) CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_stop), stream));
     return LEYLINE_OK;
-}
+} LEYLINE_CATCH_STATUS
 
-extern "C" leyline_status leyline_plan_prefetch(leyline_plan_t* pl) {
+extern "C" LEYLINE_API leyline_status leyline_plan_prefetch(leyline_plan_t* pl) try {
     g_last_error.clear();
     if (!pl) return LEYLINE_E_INVALID;
     if (pl->d_blob || pl->device >= 0) return LEYLINE_OK;
@@ -572,16 +585,28 @@ extern "C" leyline_status leyline_plan_prefetch(leyline_plan_t* pl) {
     CU(cudaEventRecord(static_cast<cudaEvent_t>(pl->ev_uploaded), pp->copy_stream));
     pl->last_stream = pp->copy_stream; /* until a launch replaces it: a never-launched plan frees its tables there */
     return LEYLINE_OK;
-}
+} LEYLINE_CATCH_STATUS
 
-extern "C" leyline_status leyline_plan_kernel_ms(const leyline_plan_t* pl, float* ms) {
+extern "C" LEYLINE_API leyline_status leyline_plan_kernel_ms(const leyline_plan_t* pl, float* ms) try {
     g_last_error.clear();
     if (!pl || !ms || !pl->ev_start) return LEYLINE_E_INVALID;
     CU(cudaEventElapsedTime(ms, static_cast<cudaEvent_t>(pl->ev_start), static_cast<cudaEvent_t>(pl->ev_stop)));
     return LEYLINE_OK;
-}
+} LEYLINE_CATCH_STATUS
 
-extern "C" void leyline_plan_release_device_(leyline_plan_s* pl) {
+/* The device's own cos/sin table, for comparison with the host evaluation (tests / tooling). */
+extern "C" LEYLINE_API leyline_status leyline_plan_trig_table_device(const leyline_plan_t* pl, float* out) try {
+    g_last_error.clear();
+    if (!pl || (!out && !pl->trig_shifts.empty()) || !pl->trig_ready || !pl->d_blob) return LEYLINE_E_INVALID;
+    if (pl->trig_shifts.empty()) return LEYLINE_OK;
+    const size_t bytes = pl->trig_shifts.size() * 2 * pl->inv_freq.size() * sizeof(float);
+    cudaStream_t stream = static_cast<cudaStream_t>(pl->last_stream);
+    CU(cudaMemcpyAsync(out, blob_at<float>(pl, pl->off_trig), bytes, cudaMemcpyDeviceToHost, stream));
+    CU(cudaStreamSynchronize(stream));
+    return LEYLINE_OK;
+} LEYLINE_CATCH_STATUS
+
+void leyline::plan_release_device(leyline_plan_s* pl) {
     if (pl->ev_start) cudaEventDestroy(static_cast<cudaEvent_t>(pl->ev_start));
     if (pl->ev_stop) cudaEventDestroy(static_cast<cudaEvent_t>(pl->ev_stop));
     if (pl->ev_uploaded) cudaEventDestroy(static_cast<cudaEvent_t>(pl->ev_uploaded));
@@ -593,4 +618,4 @@ extern "C" void leyline_plan_release_device_(leyline_plan_s* pl) {
     if (pl->device >= 0) (void)cudaGetLastError();
 }
 
-extern "C" const char* leyline_last_cuda_error(void) { return g_last_error.c_str(); }
+extern "C" LEYLINE_API const char* leyline_last_cuda_error(void) { return g_last_error.c_str(); }

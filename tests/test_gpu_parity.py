@@ -655,3 +655,29 @@ def test_attention_logits_are_preserved_on_the_device(mode):
             worst = max(worst, float((np.abs(got - want) / bound).max()))
     print(f"[logits] mode {mode}: worst |logit error| / (2^-7 |q||k|) = {worst:.3f}")
     plan.close()
+
+
+def test_device_trig_table_matches_the_host_evaluation():
+    """the cos/sin table of a launch is evaluated in fp64 ON THE DEVICE (k_index) -- fp64 product of
+    the integer shift and theta_i, fp64 sincos, one rounding to fp32.  Against numpy's fp64 trig rounded once (an
+    independent evaluation) it must agree to the last fp32 bit almost everywhere and never differ by more than one fp32
+    ulp; the host query leyline_plan_trig_table must equal numpy exactly."""
+    from paper_2606_01065_b200 import binding as B
+    from paper_2606_01065_b200 import harness
+    for cfg, mode in (("appB", B.ROTATE_ONLY), (4, B.ROTATE_ONLY), ("3m", B.FRESH)):
+        w = synth.config(cfg, pool_factor=2.0, n_layers=1)
+        cache = harness.DeviceCache(w, "cuda:0", fill=False)
+        for p in cache.pools + cache.repl:
+            p.zero_()
+        plan, pt, idx = harness.run_workload(cache, mode)
+        torch.cuda.synchronize()
+        dev, host, shifts = plan.trig_table_device, plan.trig_table, plan.trig_shifts
+        assert len(shifts) >= 3
+        phi = shifts.astype(np.float64)[:, None] * w.inv_freq.astype(np.float64)[None, :]
+        want = np.stack([np.cos(phi), np.sin(phi)], axis=1).astype(np.float32)
+        np.testing.assert_array_equal(host, want)
+        d = np.abs(dev.view(np.int32).astype(np.int64) - want.view(np.int32).astype(np.int64))
+        same_sign = np.signbit(dev) == np.signbit(want)
+        assert ((d <= 1) & same_sign | (np.abs(dev.astype(np.float64) - want) < 1e-45)).all()
+        assert (d == 0).mean() > 0.9999, (cfg, float((d == 0).mean()))
+        plan.close()

@@ -31,6 +31,12 @@ def test_abi_exports_every_declared_symbol():
     for n in sorted(names):
         assert hasattr(lib, n), f"{n} declared in leyline.h but not exported"
     assert "sm_100a" in B.leyline_version()
+    # ... and nothing else: the library is built with -fvisibility=hidden, only LEYLINE_API declarations are exported
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", B.LIB_PATH], check=True, capture_output=True, text=True).stdout
+    exported = {ln.split()[-1] for ln in out.splitlines() if " T " in ln}
+    assert {e for e in exported if e.startswith("leyline")} == names, sorted(exported ^ names)
+    assert not [e for e in exported if not e.startswith("leyline") and not e.startswith("_")], exported
 
 
 def test_enum_values_match_oracle_contract():
@@ -155,8 +161,16 @@ def check_tiles_cover(plan, bm, w, mode):
         segs = rm.segs.as_tuples()
         k0P = 0
         if mode == B.FRESH:
-            mine = [d for d in w.directives if d[0] == r]
-            k0P = (mine[0][1] // w.page_size) * w.page_size if mine else rm.L_new
+            # rule M1: everything in front of the first directive that changes anything stays where it is; a FORGET
+            # ends the search, no-ops do not count
+            first = None
+            for d in (d for d in w.directives if d[0] == r):
+                if d[5] == B.FORGET:
+                    break
+                if d[2] > d[1] or d[3] > 0:
+                    first = d[1]
+                    break
+            k0P = (first // w.page_size) * w.page_size if first is not None else rm.L_new
         ins_cursor = 0
         for (kind, src, dst, ln, sh) in segs:
             for q in range(ln):
@@ -229,6 +243,111 @@ def test_error_codes_follow_rule_v():
     assert status([], desc=bad) == B.E_UNSUPPORTED
     bad, k5 = B.make_desc(2, 512, 64, 4, 0, 0, 1152, 8, w.inv_freq)                # page ids beyond the pool
     assert status([]) == B.OK and status([], desc=bad) == B.E_RANGE
+    # directive.reserved_ must be 0 (leyline.h)
+    packed = B.pack_directives([(0, 5, 6, 0, 0, A)])
+    packed["reserved_"] = 7
+    assert status(packed) == B.E_INVALID
+    # a free id outside the pool is RANGE and wins over the alias rule; NOFREE wins over both
+    assert status([(1, 28, 28, 5, 0, A)], free=np.array([w.pool_pages + 3, w.pages[0]], np.int32)) == B.E_RANGE   # consumes 2
+    assert status([(1, 28, 28, 5, 0, A)], free=np.array([w.free_pages[0], w.pages[0]], np.int32)) == B.E_ALIAS
+    assert status([(0, 0, 0, 400, 0, A)], free=np.array([w.pages[0]], np.int32)) == B.E_NOFREE
+
+
+def test_alias_rule_refuses_plans_that_would_overwrite_live_kv():
+    """leyline.h, LEYLINE_E_ALIAS: a consumed free id that is live or handed out twice, and -- for the modes that write
+    a request's own pages -- a page listed by two requests of which one is edited.  Hand-built tables, P = 4."""
+    inv = synth.rope_inv_freq(64)
+    d, keep = B.make_desc(1, 512, 64, 4, 0, 0, 1152, 64 * 4, inv)
+    seq, pto, pages = [10, 6], [0, 3, 5], np.array([0, 1, 2, 3, 4], np.int32)
+    A = B.AMORTIZE
+
+    def status(mode, dirs, free, pages=pages, pto=pto, seq=seq):
+        try:
+            B.leyline_plan(d, mode, seq, pto, pages, dirs, np.asarray(free, np.int32)).close()
+            return B.OK
+        except B.LeylineError as e:
+            return e.status
+
+    grow = [(0, 2, 2, 9, 0, A)]                                   # request 0 grows by 9 rows: FRESH consumes 4 pages
+    assert status(B.FRESH, grow, [10, 11, 12, 13, 14]) == B.OK
+    assert status(B.FRESH, grow, [10, 1, 12, 13, 14]) == B.E_ALIAS        # page 1 is a live page of request 0
+    assert status(B.FRESH, grow, [10, 4, 12, 13, 14]) == B.E_ALIAS        # page 4 is a live page of request 1
+    assert status(B.FRESH, grow, [10, 11, 11, 13, 14]) == B.E_ALIAS       # handed out twice
+    assert status(B.FRESH, grow, [10, 11, 12, 13, 1]) == B.E_ALIAS        # every CONSUMED id is checked (5 are) ...
+    assert status(B.FRESH, grow, [10, 11, 12, 13, 14, 1]) == B.OK         # ... ids that are not consumed are not
+    assert status(B.INPLACE_MOVE, grow, [10, 3]) == B.E_ALIAS            # growth by 2 pages: the 2nd is request 1's
+    assert status(B.INPLACE_MOVE, grow, [10, 11]) == B.OK
+    # ROTATE_ONLY consumes free SLOTS: slot 13 sits in live page 3
+    assert status(B.ROTATE_ONLY, grow, [40, 41, 42, 43, 44, 45, 46, 47, 13]) == B.E_ALIAS
+    assert status(B.ROTATE_ONLY, grow, [40, 41, 42, 43, 44, 45, 46, 47, 40]) == B.E_ALIAS
+    assert status(B.ROTATE_ONLY, grow, [40, 41, 42, 43, 44, 45, 46, 47, 48]) == B.OK
+    # a page shared by two requests (a common prefix): fine for FRESH, which never writes a request's own pages ...
+    shared = np.array([0, 1, 2, 0, 4], np.int32)
+    edit1 = [(1, 5, 6, 0, 0, A)]
+    assert status(B.FRESH, edit1, [10, 11], pages=shared) == B.OK
+    # ... refused for the in-place modes when either owner is edited, accepted when nobody is
+    assert status(B.INPLACE_MOVE, edit1, [10], pages=shared) == B.E_ALIAS
+    assert status(B.ROTATE_ONLY, edit1, [40], pages=shared) == B.E_ALIAS
+    assert status(B.INPLACE_MOVE, [(0, 9, 10, 0, 0, A)], [10], pages=shared) == B.E_ALIAS
+    assert status(B.INPLACE_MOVE, [], [10], pages=shared) == B.OK
+    assert status(B.INPLACE_MOVE, edit1, [10], pages=np.array([0, 1, 2, 3, 3], np.int32)) == B.E_ALIAS   # twice in one request
+    del keep
+
+
+def test_page_table_rows_must_be_exactly_as_long_as_the_request():
+    """leyline.h: a row longer than ceil(L/P) is refused -- its surplus pages would be neither kept nor released."""
+    inv = synth.rope_inv_freq(64)
+    d, keep = B.make_desc(1, 512, 64, 4, 0, 0, 1152, 64 * 4, inv)
+    for mode in MODES:
+        with pytest.raises(B.LeylineError) as ei:
+            B.leyline_plan(d, mode, [10], [0, 5], [0, 1, 2, 3, 4], [], [9])
+        assert ei.value.status == B.E_INVALID
+        with pytest.raises(B.LeylineError) as ei:
+            B.leyline_plan(d, mode, [10], [0, 2], [0, 1], [], [9])
+        assert ei.value.status == B.E_INVALID
+        B.leyline_plan(d, mode, [10], [0, 3], [0, 1, 2], [], [9]).close()
+    del keep
+
+
+def test_noop_and_forget_only_requests_launch_nothing():
+    """PAPER.md:102 and rule M1: a request whose directives change nothing (no-ops) or only truncate it (FORGET before any
+    edit) produces no tile in any mode, consumes no free id, and FRESH keeps its pages."""
+    inv = synth.rope_inv_freq(64)
+    d, keep = B.make_desc(1, 512, 64, 4, 0, 0, 1152, 64 * 4, inv)
+    pages = np.arange(6, dtype=np.int32) + 10
+    for mode in MODES:
+        free = np.arange(40, 60, dtype=np.int32)
+        for dirs, L_new, n_pages in (([(0, 3, 3, 0, 0, B.AMORTIZE), (0, 9, 9, 0, 0, B.AMORTIZE)], 22, 6),
+                                     ([(0, 9, 9, 0, 0, B.FORGET)], 9, 3), ([(0, 1, 1, 0, 0, B.AMORTIZE), (0, 8, 12, 5, 0, B.FORGET)], 8, 2)):
+            with B.leyline_plan(d, mode, [22], [0, 6], pages, dirs, free) as plan:
+                i = plan.info
+                assert (i.n_tiles, i.n_free_consumed, i.rows_moved, i.rows_inserted, i.rows_rotated) == (0, 0, 0, 0, 0)
+                assert plan.new_seq_lens[0] == L_new
+                if mode != B.ROTATE_ONLY:
+                    assert list(plan.new_pages) == list(pages[:n_pages]) and list(plan.released) == list(pages[n_pages:])
+                else:
+                    assert list(plan.released) == [int(pages[t // 4]) * 4 + t % 4 for t in range(L_new, 22)]
+    del keep
+
+
+def test_plan_ex_takes_its_tuning_per_call():
+    """leyline.h: leyline_plan_ex never looks at the process-wide tuning of leyline_set_tuning, and the other way round."""
+    w = synth.config(2, pool_factor=2.2)
+    d, keep = B.make_desc(w.n_layers, w.latent_dim, w.rope_dim, w.page_size, w.dtype, w.pairing, w.row_bytes, w.n_slots, w.inv_freq)
+    args = (d, B.FRESH, w.seq_lens, w.pt_offsets, w.pages, w.directives, w.free_pages)
+    with B.leyline_plan_ex(*args) as p0, B.leyline_plan_ex(*args, B.Tuning(1, 7, 0, 0, 0, 0, 0, 0)) as p1:
+        assert (p0.info.mover, p0.info.tile_rows) == (2, 32) and (p1.info.mover, p1.info.tile_rows) == (1, 7)
+    B.leyline_set_tuning(kernel=1, tile_rows=5)
+    try:
+        with B.leyline_plan_ex(*args) as p0, B.leyline_plan(*args[:7]) as p2:
+            assert (p0.info.mover, p0.info.tile_rows) == (2, 32)           # plan_ex: defaults, whatever the global says
+            assert (p2.info.mover, p2.info.tile_rows) == (1, 5)            # leyline_plan: the process-wide default
+    finally:
+        B.leyline_set_tuning()
+    with pytest.raises(B.LeylineError) as ei:
+        B.leyline_plan_ex(*args, B.Tuning(9, 0, 0, 0, 0, 0, 0, 0))
+    assert ei.value.status == B.E_INVALID
+    del keep
 
 
 # ----------------------------------------------------------------------------- rule M2 as a schedule
