@@ -177,6 +177,16 @@ def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1):
     dirs = B.pack_directives(w.directives)
     seq_lens = np.asarray(w.seq_lens, np.int64)          # a server holds these as arrays already
 
+    kms = []
+
+    def retire(keep_in_flight):
+        # a server destroys a plan once its launch has finished (its host tables are then recycled by the next plan);
+        # the plan of 3 steps ago has long finished, so reading its kernel time does not stall the pipeline
+        while len(plans) > keep_in_flight:
+            p = plans.pop(0)
+            kms.append(p.kernel_ms())
+            p.close()
+
     def step():
         t0 = time.perf_counter()
         plan = B.leyline_plan(desc, mode, seq_lens, w.pt_offsets, w.pages, dirs, free)
@@ -187,14 +197,14 @@ def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1):
         else:
             B.leyline_splice(plan, pools, pools, repl, pt, idx)
         plans.append(plan)
+        retire(3)
 
     for _ in range(warmup):
         step()
     barrier(world)
-    for p in plans:
-        p.close()
-    plans.clear()
+    retire(0)
     host_us.clear()
+    kms.clear()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(steps):
@@ -202,9 +212,7 @@ def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1):
     e1.record()
     barrier(world)
     ms = e0.elapsed_time(e1) / steps
-    kms = [p.kernel_ms() for p in plans]
-    for p in plans:
-        p.close()
+    retire(0)
     del keep
     return {"ms_per_step": ms, "kernel_ms": float(np.mean(kms)), "kernel_ms_min": float(np.min(kms)), "bytes": nbytes,
             "plan_host_us": float(np.median(host_us)), "launches_per_step": launches,
@@ -249,7 +257,9 @@ def time_single_calls(cache, w, mode: int, reps: int = 10):
 def time_discovery(dev, with_oracle: bool, n_sessions: int = 16, prompt_len: int = 17000, reps: int = 20):
     """Supplementary line: the discovery side (leyline_cdc_chunk) on the shape of the paper's
     microbenchmark -- 16 sessions x ~17 K-token prompts, anchors every ~600 tokens -- against
-    the oracle's sequential chunker on the host."""
+    the oracle's sequential chunker on the host, for the default chunk parameters (16, 256, 6) and for long chunks
+    (64, 4096, 12).  The input is 1 MB, so the call is bound by its chain of dependent small launches, not by bytes:
+    `launch_bound_ms` = launches x the measured cost of one tiny dependent launch on this stream."""
     import torch
     from paper_2606_01065_b200 import binding as B
     rng = np.random.default_rng(17)
@@ -266,30 +276,38 @@ def time_discovery(dev, with_oracle: bool, n_sessions: int = 16, prompt_len: int
     hsh = torch.empty(n, dtype=torch.int64, device=dev)
     kind = torch.empty(n, dtype=torch.int32, device=dev)
     cnt = torch.zeros(1, dtype=torch.int64, device=dev)
-    prm = B.CdcParams(0x5EED, 16, 256, 6, 0)
 
-    def run():
-        B.leyline_cdc_chunk(prm, td, n, off, n_sessions, an, len(anchors), end, hsh, kind, n, cnt)
+    def timed(fn, reps):
+        for _ in range(3):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
 
-    for _ in range(3):
-        run()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(reps):
-        run()
-    e1.record()
-    torch.cuda.synchronize()
-    gpu_ms = e0.elapsed_time(e1) / reps
-    c = int(cnt.item())
-    out = {"tokens": n, "chunks": c, "gpu_ms": gpu_ms, "gpu_Mtok_per_s": n / gpu_ms / 1e3}
-    if with_oracle:      # part of the cpu_baseline leg: the oracle's sequential chunker timed on the host beside it
-        from oracle import cdc as OC
-        t0 = time.perf_counter()
-        o_end, o_hash, o_kind = OC.chunk(0x5EED, 16, 256, 6, t, so, anchors)
-        cpu_ms = (time.perf_counter() - t0) * 1e3
-        same = c == len(o_end) and bool((end[:c].cpu().numpy() == o_end).all()) and \
-            bool((hsh[:c].cpu().numpy().view(np.uint64) == o_hash).all())
-        out.update(oracle_ms=cpu_ms, oracle_Mtok_per_s=n / cpu_ms / 1e3, matches_oracle=same)
+    keys, vals = torch.zeros(1, dtype=torch.int64, device=dev), torch.zeros(1, dtype=torch.int64, device=dev)
+    launch_ms = timed(lambda: B.leyline_registry_clear(keys, vals, 1), 200)      # one tiny kernel per call, back to back
+    rounds = int(np.ceil(np.log2(n + 1)))
+    launches = 1 + 5 + rounds + 4          # memset; flags, seq_ends, signature, level1, next; doubling; count, scan, emit, hash
+    out = {"tokens": n, "tiny_launch_us": launch_ms * 1e3, "launches_per_call": launches,
+           "launch_bound_ms": launches * launch_ms}
+    for name, (mn, mx, bits) in (("min16_max256_bits6", (16, 256, 6)), ("min64_max4096_bits12", (64, 4096, 12))):
+        prm = B.CdcParams(0x5EED, mn, mx, bits, 0)
+        gpu_ms = timed(lambda: B.leyline_cdc_chunk(prm, td, n, off, n_sessions, an, len(anchors), end, hsh, kind, n, cnt), reps)
+        c = int(cnt.item())
+        line = {"chunks": c, "gpu_ms": gpu_ms, "gpu_Mtok_per_s": n / gpu_ms / 1e3, "over_launch_bound": gpu_ms / (launches * launch_ms)}
+        if with_oracle:      # part of the cpu_baseline leg: the oracle's sequential chunker timed on the host beside it
+            from oracle import cdc as OC
+            t0 = time.perf_counter()
+            o_end, o_hash, o_kind = OC.chunk(0x5EED, mn, mx, bits, t, so, anchors)
+            cpu_ms = (time.perf_counter() - t0) * 1e3
+            same = c == len(o_end) and bool((end[:c].cpu().numpy() == o_end).all()) and \
+                bool((hsh[:c].cpu().numpy().view(np.uint64) == o_hash).all())
+            line.update(oracle_ms=cpu_ms, oracle_Mtok_per_s=n / cpu_ms / 1e3, matches_oracle=same)
+        out[name] = line
     return out
 
 
@@ -429,6 +447,7 @@ def extra_line(cache, w, mode_name: str, peak: float, device_index: int, target_
     mode = MODES[mode_name]
     probe = time_splice(cache, w, mode, 3, 2)
     steps = int(min(400, max(5, target_s * 1e3 / max(probe["ms_per_step"], 1e-3))))
+    time.sleep(0.5)              # let the power average settle: these lines run back to back behind cache fills
     sampler = ClockSampler(device_index)
     sampler.start()
     x = time_splice(cache, w, mode, steps, 1)
@@ -466,6 +485,31 @@ def extra_workloads(peak: float, device_index: int, skip=()):
         del cache
         gc.collect()
         torch.cuda.empty_cache()
+    return out
+
+
+def pattern_probe(device, n_rows: int = 8 << 20):
+    """The library's own probe of the a5 access pattern (leyline_probe_band_update: contiguous rows, no page table, no
+    rotation, full-line accesses): what the memory system allows on 128 B of every 1152-B row / 64 B of every 576-B row,
+    read + written in place.  k_rotate_band's GB/s is to be read against this, not against a dense copy."""
+    import torch
+    from paper_2606_01065_b200 import binding as B
+    out = {}
+    for name, row_bytes, band in (("bf16_128_of_1152", 1152, 128), ("fp8_64_of_576", 576, 64), ("dense_1152_of_1152", 1152, 1152)):
+        buf = torch.zeros(n_rows * row_bytes, dtype=torch.uint8, device=device)
+        best = {}
+        for per_sm in (4, 8, 16):
+            for _ in range(2):
+                B.leyline_probe_band_update(buf, n_rows, row_bytes, row_bytes - band, band, per_sm)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(5):
+                B.leyline_probe_band_update(buf, n_rows, row_bytes, row_bytes - band, band, per_sm)
+            e1.record()
+            torch.cuda.synchronize()
+            best[f"ctas_per_sm_{per_sm}"] = 2.0 * n_rows * band / (e0.elapsed_time(e1) / 5 * 1e-3) / 1e9
+        out[name] = {"GBps": max(best.values()), "by_grid": best, "rows": n_rows}
+        del buf
     return out
 
 
@@ -626,6 +670,7 @@ def run_ours(args):
         gc.collect()
         torch.cuda.empty_cache()
         out["extras"].update(extra_workloads(peak, local))
+        out["extras"]["a5_pattern_probe"] = pattern_probe(dev)
         out["extras"]["a5_pattern_reference_torch"] = pattern_reference(dev)
     elif world > 1:
         out["extras"] = "N = 1 only (supplementary workloads; they do not depend on the replica count)"

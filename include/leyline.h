@@ -174,6 +174,9 @@ typedef struct leyline_tuning_s {
     int32_t rotate_kernel; /* a5 on a narrow band (MLA): 0 = auto, 1 = k_rotate_band (strided 16-byte loads / stores through
                               registers), 2 = k_rotate_band_tma (the band of a page as one 2-D TMA box staged through shared
                               memory; pages of >= 16 rows, else falls back to 1) */
+    int32_t skip_alias_check; /* 1: the caller guarantees what the alias rule checks (free ids disjoint from live pages and
+                              from each other, no page shared with a request edited in place); LEYLINE_E_ALIAS is then
+                              never returned and the planner skips its pass over every live page */
 } leyline_tuning;
 
 /*
@@ -331,10 +334,23 @@ LEYLINE_API leyline_status leyline_set_tuning(const leyline_tuning* t);
 LEYLINE_API leyline_status leyline_get_tuning(leyline_tuning* t);
 
 /* Device time of the data-moving kernels (a3+a4 / a5) of the plan's last launch, from CUDA events recorded on
- * the launching stream when the plan was created with tuning.profile = 1.  Call after synchronising the stream. */
+ * the launching stream when the plan was created with tuning.profile = 1.  Waits for that launch to finish (only for
+ * it: later work on the stream keeps running). */
 LEYLINE_API leyline_status leyline_plan_kernel_ms(const leyline_plan_t* plan, float* ms);
 
-/* Library / build description, e.g. "leyline-b200 0.1 sm_100a". */
+/*
+ * leyline_probe_band_update -- MEASUREMENT AID, not part of the method: the memory access pattern of step a5 with
+ * everything else taken away.  `band_bytes` at byte `band_offset_bytes` of every `row_stride_bytes`-byte row of one
+ * contiguous device buffer of n_rows rows are read, changed (an integer add) and written back in place: no page table,
+ * no plan, no rotation, full-line 16-byte accesses, 8 independent loads per thread, ctas_per_sm x SM count blocks
+ * (0 = 8).  Timing it gives the rate the memory system allows ANY kernel on "128 B of every 1152-B row" (bf16 MLA) or
+ * "64 B of every 576-B row" (fp8); bench.py reports it next to k_rotate_band as extras.a5_pattern_probe.  Asynchronous.
+ */
+LEYLINE_API leyline_status leyline_probe_band_update(void* dev_buf, int64_t n_rows, int64_t row_stride_bytes,
+                                                     int32_t band_offset_bytes, int32_t band_bytes, int32_t ctas_per_sm,
+                                                     void* cuda_stream);
+
+/* Library / build description, e.g. "leyline-b200 0.2 sm_100a". */
 LEYLINE_API const char* leyline_version(void);
 
 #ifdef __cplusplus

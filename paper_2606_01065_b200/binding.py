@@ -56,7 +56,7 @@ class Tile(C.Structure):
 class Tuning(C.Structure):
     _fields_ = [("kernel", C.c_int32), ("tile_rows", C.c_int32), ("ctas_per_sm", C.c_int32), ("profile", C.c_int32),
                 ("stages", C.c_int32), ("layer_group", C.c_int32), ("consumer_warps", C.c_int32),
-                ("rotate_kernel", C.c_int32)]
+                ("rotate_kernel", C.c_int32), ("skip_alias_check", C.c_int32)]
 
 
 class CdcParams(C.Structure):
@@ -99,6 +99,8 @@ def _load() -> C.CDLL:
     L.leyline_plan_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.leyline_plan_prefetch.restype = C.c_int
     L.leyline_plan_prefetch.argtypes = [vp]
+    L.leyline_probe_band_update.restype = C.c_int
+    L.leyline_probe_band_update.argtypes = [vp, i64, i64, i32, i32, i32, vp]
     L.leyline_plan_destroy.restype = None
     L.leyline_plan_destroy.argtypes = [vp]
     L.leyline_strerror.restype = C.c_char_p
@@ -135,8 +137,8 @@ def leyline_version() -> str:
 
 
 def leyline_set_tuning(kernel: int = 0, tile_rows: int = 0, ctas_per_sm: int = 0, profile: int = 0, stages: int = 0,
-                       layer_group: int = 0, consumer_warps: int = 0, rotate_kernel: int = 0):
-    t = Tuning(kernel, tile_rows, ctas_per_sm, profile, stages, layer_group, consumer_warps, rotate_kernel)
+                       layer_group: int = 0, consumer_warps: int = 0, rotate_kernel: int = 0, skip_alias_check: int = 0):
+    t = Tuning(kernel, tile_rows, ctas_per_sm, profile, stages, layer_group, consumer_warps, rotate_kernel, skip_alias_check)
     _check(_lib.leyline_set_tuning(C.byref(t)), "leyline_set_tuning")
 
 
@@ -145,7 +147,7 @@ def leyline_get_tuning() -> dict:
     _check(_lib.leyline_get_tuning(C.byref(t)), "leyline_get_tuning")
     return {"kernel": t.kernel, "tile_rows": t.tile_rows, "ctas_per_sm": t.ctas_per_sm, "profile": t.profile,
             "stages": t.stages, "layer_group": t.layer_group,
-            "consumer_warps": t.consumer_warps, "rotate_kernel": t.rotate_kernel}
+            "consumer_warps": t.consumer_warps, "rotate_kernel": t.rotate_kernel, "skip_alias_check": t.skip_alias_check}
 
 
 def _arr(x, dtype):
@@ -348,6 +350,13 @@ def leyline_rotate_inplace_master(plan: Plan, layers, layer_master, layer_repl=N
     c, _k3 = _ptr_array(layer_repl, n, "layer_repl")
     st = _lib.leyline_rotate_inplace_master(plan._h, a, m, c, _dev_ptr(slot_idx_out), _stream_handle(stream))
     _check(st, "leyline_rotate_inplace_master")
+
+
+def leyline_probe_band_update(buf, n_rows: int, row_stride_bytes: int, band_offset_bytes: int, band_bytes: int,
+                              ctas_per_sm: int = 0, stream=None):
+    """leyline.h: leyline_probe_band_update (measurement aid: the a5 access pattern on a contiguous buffer)."""
+    _check(_lib.leyline_probe_band_update(_dev_ptr(buf), n_rows, row_stride_bytes, band_offset_bytes, band_bytes, ctas_per_sm,
+                                          _stream_handle(stream)), "leyline_probe_band_update")
 
 
 # ----------------------------------------------------------------------------- discovery side (leyline_cdc.h)

@@ -6,10 +6,19 @@
  * The sequential definition (one rolling hash, one open chunk) is restated so that every step is data-parallel:
  *   k_cdc_flags      per token: gear value G(t) (D1), "anchor" and "last token of its sequence" flags
  *   k_cdc_signature  per position: h_i as the 64-term window sum  sum_j G(t_{i-j}) << j  cut at the last reset (D2
- *                    in closed form: the shift drops a token out of the 64-bit word after 64 steps), candidate flag
- *   k_cdc_next       per position s: where a chunk that STARTS at s would end (D3), scanning <= max_size flags
- *   k_cdc_reach      pointer doubling over s -> next(s): marks the starts actually reached from the sequence starts
- *   k_cdc_count / k_cdc_scan / k_cdc_emit   ordered compaction of the marked starts, content hash per chunk (D4)
+ *                    in closed form: the shift drops a token out of the 64-bit word after 64 steps); the "hash
+ *                    candidate" and "hard stop" (anchor / sequence end) predicates go into two BITMAPS, one ballot per
+ *                    32 positions, with a second level (one bit per non-empty word) built by k_cdc_level1
+ *   k_cdc_next       per position s: where a chunk that STARTS at s would end (D3) = min(next hard stop >= s,
+ *                    s + max_size - 1, next candidate >= s + min_size - 1); "next set bit at or after i" is a
+ *                    find-first-set in the position's word, else in the level-1 word: O(1) loads per position for
+ *                    every legal (min_size, max_size, mask_bits), so the pass is linear in n
+ *   k_cdc_reach      pointer doubling over s -> next(s): marks the starts actually reached from the sequence starts;
+ *                    a round that sets no new mark proves the longest per-sequence chain is covered, and every later
+ *                    round returns at once (ceil(log2(longest chain)) working rounds, not ceil(log2 n))
+ *   k_cdc_count / k_cdc_scan / k_cdc_emit   ordered compaction of the marked starts
+ *   k_cdc_hash       content hash per chunk (D4).  FNV-1a is a serial recurrence (x = (x ^ byte) * prime), so its
+ *                    floor is the LONGEST chunk: 4 dependent 64-bit multiplies per token, <= 4 * max_size in a row
  * Integer work throughout; results are bit-exact against the CPU oracle.
  */
 #include <cuda_runtime.h>
@@ -23,7 +32,7 @@
 namespace {
 
 constexpr int kT = 256;
-constexpr uint8_t F_ANCHOR = 1, F_SEQ_END = 2, F_CAND = 4;
+constexpr uint8_t F_ANCHOR = 1, F_SEQ_END = 2;
 
 thread_local std::string g_cdc_error;
 bool ok(cudaError_t e) {
@@ -55,46 +64,96 @@ __global__ void __launch_bounds__(kT) k_cdc_flags(const int32_t* __restrict__ to
     }
 }
 
-/* the last token of every non-empty sequence (runs after k_cdc_flags on the same stream) */
-__global__ void __launch_bounds__(kT) k_cdc_seq_ends(const int64_t* __restrict__ seq_offsets, int n_seqs, uint8_t* __restrict__ flags,
-                                                     uint8_t* __restrict__ mark) {
+/* the last token of every non-empty sequence (runs after k_cdc_flags on the same stream).  Offsets live on the device
+ * and cannot be validated by the host: anything outside [0, n] is ignored here rather than followed. */
+__global__ void __launch_bounds__(kT) k_cdc_seq_ends(const int64_t* __restrict__ seq_offsets, int n_seqs, int64_t n,
+                                                     uint8_t* __restrict__ flags, uint8_t* __restrict__ mark) {
     for (int s = blockIdx.x * kT + threadIdx.x; s < n_seqs; s += gridDim.x * kT) {
         const int64_t b = seq_offsets[s], e = seq_offsets[s + 1];
-        if (e > b) {
+        if (e > b && b >= 0 && e <= n) {
             flags[e - 1] |= F_SEQ_END; /* one writer per byte: sequences do not share tokens */
             mark[b] = 1;               /* a chunk starts at every sequence start */
         }
     }
 }
 
-__global__ void __launch_bounds__(kT) k_cdc_signature(const uint64_t* __restrict__ gear, int64_t n, int mask_bits,
-                                                      uint8_t* __restrict__ flags) {
-    for (int64_t i = blockIdx.x * (int64_t)kT + threadIdx.x; i < n; i += (int64_t)gridDim.x * kT) {
-        uint64_t h = gear[i];
-        for (int j = 1; j < 64; ++j) {
-            const int64_t k = i - j;
-            if (k < 0 || (flags[k] & (F_ANCHOR | F_SEQ_END))) break; /* the signature was reset after token k */
-            h += gear[k] << j;
+/* D2 + the two predicates of D3 as bitmaps.  Word w of hard0 / cand0 covers positions [32w, 32w + 32): a warp handles 32
+ * consecutive positions and lane 0 stores the ballot, so every word (also the tail, where positions >= n read as 0) is
+ * written exactly once and nothing is modified in place. */
+__global__ void __launch_bounds__(kT) k_cdc_signature(const uint64_t* __restrict__ gear, const uint8_t* __restrict__ flags, int64_t n,
+                                                      int64_t n_padded, int mask_bits, uint32_t* __restrict__ hard0,
+                                                      uint32_t* __restrict__ cand0) {
+    for (int64_t i = blockIdx.x * (int64_t)kT + threadIdx.x; i < n_padded; i += (int64_t)gridDim.x * kT) {
+        bool hard = false, cand = false;
+        if (i < n) {
+            uint64_t h = gear[i];
+            for (int j = 1; j < 64; ++j) {
+                const int64_t k = i - j;
+                if (k < 0 || flags[k]) break; /* the signature was reset after token k (anchor or end of a sequence) */
+                h += gear[k] << j;
+            }
+            hard = flags[i] != 0;
+            cand = mask_bits == 0 || (h >> (64 - mask_bits)) == 0;
         }
-        /* only bit 2 changes here and only this thread writes flags[i]; neighbours read bits 0-1, which are final */
-        if (mask_bits == 0 || (h >> (64 - mask_bits)) == 0) flags[i] |= F_CAND;
+        const unsigned hb = __ballot_sync(0xFFFFFFFFu, hard), cb = __ballot_sync(0xFFFFFFFFu, cand);
+        if ((threadIdx.x & 31) == 0) { hard0[i >> 5] = hb; cand0[i >> 5] = cb; }
     }
 }
 
-/* D3 for a chunk starting at s: nxt[s] = exclusive end, kind[s] = why. */
-__global__ void __launch_bounds__(kT) k_cdc_next(const uint8_t* __restrict__ flags, int64_t n, int min_size, int max_size,
+/* level 1: bit b of word v <=> level-0 word 32v + b is non-zero (both bitmaps in one pass) */
+__global__ void __launch_bounds__(kT) k_cdc_level1(const uint32_t* __restrict__ hard0, const uint32_t* __restrict__ cand0, int64_t n_words,
+                                                   int64_t n_words_padded, uint32_t* __restrict__ hard1, uint32_t* __restrict__ cand1) {
+    for (int64_t w = blockIdx.x * (int64_t)kT + threadIdx.x; w < n_words_padded; w += (int64_t)gridDim.x * kT) {
+        const unsigned hb = __ballot_sync(0xFFFFFFFFu, w < n_words && hard0[w] != 0);
+        const unsigned cb = __ballot_sync(0xFFFFFFFFu, w < n_words && cand0[w] != 0);
+        if ((threadIdx.x & 31) == 0) { hard1[w >> 5] = hb; cand1[w >> 5] = cb; }
+    }
+}
+
+/* first set position >= i and <= last in a two-level bitmap, or INT64_MAX.  At most 2 + (last - i) / 1024 word loads. */
+__device__ __forceinline__ int64_t next_set(const uint32_t* __restrict__ l0, const uint32_t* __restrict__ l1, int64_t i, int64_t last) {
+    if (i > last) return INT64_MAX;
+    int64_t w = i >> 5;
+    uint32_t m = __ldg(l0 + w) & (0xFFFFFFFFu << (i & 31));
+    if (!m) {
+        int64_t v = w >> 5;
+        const int b = (int)(w & 31);
+        uint32_t m1 = b == 31 ? 0u : (__ldg(l1 + v) & (0xFFFFFFFFu << (b + 1)));
+        const int64_t v_last = last >> 10;
+        while (!m1) {
+            if (++v > v_last) return INT64_MAX;
+            m1 = __ldg(l1 + v);
+        }
+        w = (v << 5) + (__ffs((int)m1) - 1);
+        m = __ldg(l0 + w);
+    }
+    const int64_t pos = (w << 5) + (__ffs((int)m) - 1);
+    return pos <= last ? pos : INT64_MAX;
+}
+
+/* D3 for a chunk starting at s: nxt[s] = exclusive end, kind[s] = why.  The first of: an anchor or the end of the
+ * sequence at or after s, the max_size-th token, a hash candidate from the min_size-th token on (D3's order decides
+ * ties).  Never reads or reports anything past n, whatever the device-side offsets say. */
+__global__ void __launch_bounds__(kT) k_cdc_next(const uint8_t* __restrict__ flags, const uint32_t* __restrict__ hard0,
+                                                 const uint32_t* __restrict__ hard1, const uint32_t* __restrict__ cand0,
+                                                 const uint32_t* __restrict__ cand1, int64_t n, int min_size, int max_size,
                                                  int32_t* __restrict__ nxt, uint8_t* __restrict__ kind) {
     for (int64_t s = blockIdx.x * (int64_t)kT + threadIdx.x; s <= n; s += (int64_t)gridDim.x * kT) {
         if (s == n) { nxt[s] = (int32_t)n; break; } /* terminal: the chain stops here */
-        int64_t i = s;
+        const int64_t i_max = min(s + max_size - 1, n - 1); /* the last token of the pool ends a chunk in any case */
+        const int64_t i_hard = next_set(hard0, hard1, s, i_max);
+        const int64_t i_cand = next_set(cand0, cand1, s + min_size - 1, i_max);
+        int64_t i;
         int why;
-        for (;; ++i) {
-            const uint8_t f = flags[i];
-            const int64_t len = i - s + 1;
-            if (f & F_ANCHOR) { why = LEYLINE_CDC_ANCHOR; break; }
-            if (f & F_SEQ_END) { why = LEYLINE_CDC_SEQ_END; break; }
-            if (len == max_size) { why = LEYLINE_CDC_MAX; break; }
-            if (len >= min_size && (f & F_CAND)) { why = LEYLINE_CDC_HASH; break; }
+        if (i_hard <= i_cand && i_hard != INT64_MAX) {
+            i = i_hard;
+            why = (flags[i] & F_ANCHOR) ? LEYLINE_CDC_ANCHOR : LEYLINE_CDC_SEQ_END;
+        } else if (i_cand != INT64_MAX && i_cand < s + max_size - 1) {
+            i = i_cand;
+            why = LEYLINE_CDC_HASH;
+        } else {
+            i = i_max;
+            why = i_max == s + max_size - 1 ? LEYLINE_CDC_MAX : LEYLINE_CDC_SEQ_END;
         }
         nxt[s] = (int32_t)(i + 1);
         kind[s] = (uint8_t)why;
@@ -102,14 +161,20 @@ __global__ void __launch_bounds__(kT) k_cdc_next(const uint8_t* __restrict__ fla
 }
 
 /* One round of pointer doubling: jump_in = next applied 2^k times.  Every marked start marks the start 2^k chunks
- * ahead; marks only ever land on starts of the true chain, so reading a mark set in this same round is harmless. */
+ * ahead; marks only ever land on starts of the true chain, so reading a mark set in this same round is harmless.
+ * progress[0] (the previous round's) == 0: that round set no new mark, so every chain is complete (a sequence's k-th
+ * round is the only one that can mark its chunks 2^k .. 2^(k+1) - 1) and this round has nothing to do. */
 __global__ void __launch_bounds__(kT) k_cdc_reach(const int32_t* __restrict__ jump_in, int32_t* __restrict__ jump_out, int64_t n,
-                                                  uint8_t* __restrict__ mark) {
+                                                  uint8_t* __restrict__ mark, const int32_t* __restrict__ progress_prev,
+                                                  int32_t* __restrict__ progress) {
+    if (progress_prev && *progress_prev == 0) return;
+    bool any = false;
     for (int64_t s = blockIdx.x * (int64_t)kT + threadIdx.x; s <= n; s += (int64_t)gridDim.x * kT) {
         const int32_t j = jump_in[s];
-        if (s < n && j < n && mark[s]) mark[j] = 1;
+        if (s < n && j < n && mark[s] && !mark[j]) { mark[j] = 1; any = true; }
         jump_out[s] = jump_in[j];
     }
+    if (__any_sync(0xFFFFFFFFu, any) && (threadIdx.x & 31) == 0) *progress = 1;
 }
 
 /* ---- ordered compaction of the marked starts ---- */
@@ -293,12 +358,18 @@ extern "C" LEYLINE_API leyline_status leyline_cdc_chunk(const leyline_cdc_params
         CU(cudaMemsetAsync(dev_n_chunks, 0, sizeof(int64_t), stream));
         return LEYLINE_OK;
     }
-    /* scratch: gear u64[n] | jumpA i32[n+1] | jumpB i32[n+1] | nxt i32[n+1] | start i32[n] | blocks i32 | flags, kind, mark */
+    /* scratch: gear u64[n] | jumpA i32[n+1] | jumpB i32[n+1] | nxt i32[n+1] | start i32[n] | blocks i32 | bitmaps (two
+     * levels x two predicates) | progress i32[rounds] | flags, kind, mark */
     auto up = [](int64_t x) { return (x + 255) / 256 * 256; };
     const int64_t n_blocks = (n + kBlockSpan - 1) / kBlockSpan;
+    const int64_t n_words = (n + 31) / 32, n_words_padded = (n_words + 31) / 32 * 32, n_words1 = n_words_padded / 32;
+    int rounds = 0; /* the chain has at most n links: ceil(log2(n + 1)) doubling rounds reach all of it */
+    for (int64_t reach = 1; reach <= n; reach <<= 1) ++rounds;
     const int64_t o_gear = 0, o_ja = o_gear + up(n * 8), o_jb = o_ja + up((n + 1) * 4), o_nxt = o_jb + up((n + 1) * 4),
-                  o_start = o_nxt + up((n + 1) * 4), o_blk = o_start + up(n * 4), o_flags = o_blk + up(n_blocks * 4),
-                  o_kind = o_flags + up(n + 1), o_mark = o_kind + up(n + 1), total = o_mark + up(n + 1);
+                  o_start = o_nxt + up((n + 1) * 4), o_blk = o_start + up(n * 4), o_h0 = o_blk + up(n_blocks * 4),
+                  o_c0 = o_h0 + up(n_words_padded * 4), o_h1 = o_c0 + up(n_words_padded * 4), o_c1 = o_h1 + up((n_words1 + 1) * 4),
+                  o_prog = o_c1 + up((n_words1 + 1) * 4), o_flags = o_prog + up((rounds + 1) * 4), o_kind = o_flags + up(n + 1),
+                  o_mark = o_kind + up(n + 1), total = o_mark + up(n + 1);
     uint8_t* ws = nullptr;
     CU(cudaMallocAsync(reinterpret_cast<void**>(&ws), (size_t)total, stream));
     uint64_t* gear = reinterpret_cast<uint64_t*>(ws + o_gear);
@@ -307,19 +378,23 @@ extern "C" LEYLINE_API leyline_status leyline_cdc_chunk(const leyline_cdc_params
     int32_t* nxt = reinterpret_cast<int32_t*>(ws + o_nxt);
     int32_t* start = reinterpret_cast<int32_t*>(ws + o_start);
     int32_t* blk = reinterpret_cast<int32_t*>(ws + o_blk);
+    uint32_t *hard0 = reinterpret_cast<uint32_t*>(ws + o_h0), *cand0 = reinterpret_cast<uint32_t*>(ws + o_c0),
+             *hard1 = reinterpret_cast<uint32_t*>(ws + o_h1), *cand1 = reinterpret_cast<uint32_t*>(ws + o_c1);
+    int32_t* progress = reinterpret_cast<int32_t*>(ws + o_prog);
     uint8_t *flags = ws + o_flags, *kind = ws + o_kind, *mark = ws + o_mark;
     leyline_status st = LEYLINE_OK;
     auto fail = [&]() { cudaFreeAsync(ws, stream); return LEYLINE_E_CUDA; };
-    if (!ok(cudaMemsetAsync(mark, 0, (size_t)(n + 1), stream))) return fail();
+    /* progress | flags | kind | mark are contiguous: one memset (flags must be 0 where k_cdc_flags does not write) */
+    if (!ok(cudaMemsetAsync(progress, 0, (size_t)(total - o_prog), stream))) return fail();
     k_cdc_flags<<<grid_for(n), kT, 0, stream>>>(dev_tokens, n, dev_anchor_ids, n_anchor_ids, p->seed, gear, flags);
-    k_cdc_seq_ends<<<grid_for(n_seqs), kT, 0, stream>>>(dev_seq_offsets, n_seqs, flags, mark);
-    k_cdc_signature<<<grid_for(n), kT, 0, stream>>>(gear, n, p->mask_bits, flags);
-    k_cdc_next<<<grid_for(n + 1), kT, 0, stream>>>(flags, n, p->min_size, p->max_size, nxt, kind);
-    /* the chain has at most n links: ceil(log2(n + 1)) doubling rounds reach all of it */
+    k_cdc_seq_ends<<<grid_for(n_seqs), kT, 0, stream>>>(dev_seq_offsets, n_seqs, n, flags, mark);
+    k_cdc_signature<<<grid_for(n_words * 32), kT, 0, stream>>>(gear, flags, n, n_words * 32, p->mask_bits, hard0, cand0);
+    k_cdc_level1<<<grid_for(n_words_padded), kT, 0, stream>>>(hard0, cand0, n_words, n_words_padded, hard1, cand1);
+    k_cdc_next<<<grid_for(n + 1), kT, 0, stream>>>(flags, hard0, hard1, cand0, cand1, n, p->min_size, p->max_size, nxt, kind);
     const int32_t* jin = nxt;
     int32_t* jout = ja;
-    for (int64_t reach = 1; reach <= n; reach <<= 1) {
-        k_cdc_reach<<<grid_for(n + 1), kT, 0, stream>>>(jin, jout, n, mark);
+    for (int r = 0; r < rounds; ++r) {
+        k_cdc_reach<<<grid_for(n + 1), kT, 0, stream>>>(jin, jout, n, mark, r ? progress + r - 1 : nullptr, progress + r);
         jin = jout;
         jout = (jout == ja) ? jb : ja;
     }

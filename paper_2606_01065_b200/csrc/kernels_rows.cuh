@@ -350,6 +350,37 @@ __global__ void __launch_bounds__(kThreads) k_rotate_master(const __grid_constan
     }
 }
 
+/* ------------------------------------------------------------------ measurement aid ---- */
+
+/* The access pattern of a5 with everything else taken away (leyline_probe_band_update): `band_chunks` 16-byte chunks at
+ * byte `band0` of every `stride`-byte row of ONE contiguous buffer are read, changed (one integer add) and written back
+ * in place.  No page table, no tiles, no rotation; consecutive lanes take consecutive chunks of a row (full-line
+ * requests), U independent loads per thread are issued before the first store.  What this reaches is what the memory
+ * system gives ANY kernel on that pattern; bench.py reports it next to k_rotate_band. */
+template <int U>
+__global__ void __launch_bounds__(kThreads) k_probe_band_update(uint8_t* __restrict__ base, const long long n_rows, const long long stride,
+                                                                const int band0, const int band_chunks) {
+    const long long total = n_rows * band_chunks;
+    const long long n_threads = (long long)gridDim.x * blockDim.x;
+    for (long long u0 = blockIdx.x * (long long)blockDim.x + threadIdx.x; u0 < total; u0 += n_threads * U) {
+        int4 v[U];
+        uint8_t* a[U];
+#pragma unroll
+        for (int k = 0; k < U; ++k) {
+            const long long u = u0 + k * n_threads;
+            a[k] = nullptr;
+            if (u < total) {
+                const long long r = u / band_chunks;
+                a[k] = base + r * stride + band0 + (int)(u - r * band_chunks) * 16;
+                v[k] = ld_coherent(a[k]);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < U; ++k)
+            if (a[k]) { v[k].x += 1; st_stream(a[k], v[k]); }
+    }
+}
+
 }  // namespace leyline
 
 #endif /* LEYLINE_KERNELS_ROWS_CUH_ */

@@ -49,7 +49,7 @@ struct PhaseClock {
 namespace {
 
 std::mutex g_tuning_mu;
-leyline_tuning g_tuning = {0, 0, 0, 0, 0, 0, 0, 0};
+leyline_tuning g_tuning = {0, 0, 0, 0, 0, 0, 0, 0, 0};
 
 inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
@@ -100,7 +100,7 @@ leyline_status check_tuning(const leyline_tuning* t) {
     if (t->kernel < 0 || t->kernel > 2 || t->tile_rows < 0 || t->tile_rows > 64 || t->ctas_per_sm < 0 ||
         t->ctas_per_sm > 32 || t->stages < 0 || t->stages > 32 || t->layer_group < 0 ||
         t->layer_group > LEYLINE_MAX_LAYERS_PER_LAUNCH || t->consumer_warps < 0 || t->consumer_warps > 16 ||
-        t->rotate_kernel < 0 || t->rotate_kernel > 2)
+        t->rotate_kernel < 0 || t->rotate_kernel > 2 || t->skip_alias_check < 0 || t->skip_alias_check > 1)
         return LEYLINE_E_INVALID;
     return LEYLINE_OK;
 }
@@ -363,7 +363,7 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
      * aligned to the page in OLD position space.  tuning.rotate_kernel: 0 auto, 1 strided register kernel, 2 TMA boxes. */
     {
         const int64_t band_bytes = (int64_t)heads_of(*desc) * desc->rope_dim * E;
-        const bool tma_ok = mode == LEYLINE_ROTATE_ONLY && !pl->rotate_with_bulk && P >= 16 && band_bytes <= 1024 &&
+        const bool tma_ok = mode == LEYLINE_ROTATE_ONLY && !pl->rotate_with_bulk && P >= 16 && band_bytes <= 256 &&
                             tuning.tile_rows == 0;
         pl->rotate_with_tma = tma_ok && (tuning.rotate_kernel == 2 || (tuning.rotate_kernel == 0 && leyline::kRotateTmaByDefault));
         if (pl->rotate_with_tma) pl->rot_tile_rows = (int32_t)std::min<int64_t>(P, leyline::kRotTmaBoxRows);
@@ -406,8 +406,9 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
     const uint8_t gen = S.gen;
     uint8_t* const stamp = S.stamp.data();
     const bool inplace_mode = mode != LEYLINE_FRESH;
+    const bool check_alias = tuning.skip_alias_check == 0;
     bool alias = false;
-    for (int32_t r = 0; r < n_requests; ++r) {
+    for (int32_t r = 0; r < n_requests && check_alias; ++r) {
         const int32_t* row = pl->tabs.data() + S.old_tab_off[(size_t)r];
         const int64_t need = S.old_tab_off[(size_t)r + 1] - S.old_tab_off[(size_t)r];
         if (!inplace_mode) {
@@ -443,6 +444,7 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
         const int32_t* ids = free_ids + consumed;
         for (int64_t q = 0; q < count; ++q) {
             if (ids[q] < 0 || ids[q] >= free_limit) { badfree = true; continue; }
+            if (!check_alias) continue;
             alias = alias || stamp[ids[q]] >= gen; /* live, or consumed before */
             stamp[ids[q]] = gen;
         }
@@ -514,7 +516,7 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
                     const int32_t* ids = free_ids + consumed;
                     for (int64_t q = 0; q < s.length; ++q) {
                         if (ids[q] < 0 || ids[q] >= free_limit) { badfree = true; continue; }
-                        alias = alias || stamp[ids[q] >> pshift] >= gen; /* a slot of a live page */
+                        alias = alias || (check_alias && stamp[ids[q] >> pshift] >= gen); /* a slot of a live page */
                     }
                     S.token_lists.insert(S.token_lists.end(), ids, ids + s.length);
                     consumed += s.length;
@@ -527,7 +529,7 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
     PHASE(3); /* pass 1 */
     if (nofree) return LEYLINE_E_NOFREE;
     if (badfree) return LEYLINE_E_RANGE;
-    if (mode == LEYLINE_ROTATE_ONLY && !alias && S.token_lists.size() > 1) { /* the same free slot handed out twice */
+    if (mode == LEYLINE_ROTATE_ONLY && check_alias && !alias && S.token_lists.size() > 1) { /* the same free slot handed out twice */
         S.slot_ids = S.token_lists;
         std::sort(S.slot_ids.begin(), S.slot_ids.end());
         alias = std::adjacent_find(S.slot_ids.begin(), S.slot_ids.end()) != S.slot_ids.end();
@@ -741,7 +743,7 @@ extern "C" LEYLINE_API leyline_status leyline_plan_ex(const leyline_cache_desc* 
     if (!out) return LEYLINE_E_INVALID;
     *out = nullptr;
     LEYLINE_GUARDED(
-        leyline_tuning t = {0, 0, 0, 0, 0, 0, 0, 0};
+        leyline_tuning t = {0, 0, 0, 0, 0, 0, 0, 0, 0};
         if (tuning) {
             if (check_tuning(tuning) != LEYLINE_OK) return LEYLINE_E_INVALID;
             t = *tuning;

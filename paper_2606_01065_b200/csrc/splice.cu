@@ -11,6 +11,9 @@
 #include <string>
 #include <vector>
 
+#include <cudaTypedefs.h> /* PFN_cuTensorMapEncodeTiled */
+
+#include "kernels_band_tma.cuh"
 #include "kernels_bulk.cuh"
 #include "kernels_rows.cuh"
 
@@ -297,7 +300,7 @@ int occupancy(const void* fn, int smem) {
  * `flag_base` numbers the launch's layers uniquely inside the call (hazard-flag column). */
 struct LayerChunk { int pairing; int flag_base; std::vector<int> layers; };
 
-std::vector<LayerChunk> layer_chunks(const leyline_plan_s* pl) {
+std::vector<LayerChunk> layer_chunks(const leyline_plan_s* pl, size_t kMaxLayers = leyline::kMaxLayers) {
     std::vector<LayerChunk> out;
     const int L = pl->desc.n_layers;
     int base = 0;
@@ -377,6 +380,101 @@ leyline_status run_rotate(leyline_plan_s* pl, int32_t tile_begin, int64_t tile_c
         const long long most = mp.n_items > mp.n_copy_items ? mp.n_items : mp.n_copy_items;
         if (grid > most) grid = most;
         fn<<<(unsigned)grid, kThreads, 0, stream>>>(mp);
+        CU(cudaGetLastError());
+    }
+    return LEYLINE_OK;
+}
+
+/* ---- a5 with 2-D TMA boxes (k_rotate_band_tma) ----
+ * One tensor map per layer pool: a [pool_slots x band] view of the pool (pitch = row stride, base = pool + latent bytes),
+ * box = box_rows x band.  cuTensorMapEncodeTiled is host-only arithmetic (no driver call into the device); it is fetched
+ * from the driver once, and encoded maps are kept per (pointer, geometry) since a serving pool's layer pointers are
+ * stable. */
+PFN_cuTensorMapEncodeTiled g_encode_tiled = nullptr;
+std::once_flag g_encode_once;
+
+struct MapKey {
+    const void* base; int64_t stride, slots; int32_t band_bytes, box_rows;
+    bool operator==(const MapKey& o) const {
+        return base == o.base && stride == o.stride && slots == o.slots && band_bytes == o.band_bytes && box_rows == o.box_rows;
+    }
+};
+struct MapEntry { MapKey key; CUtensorMap map; };
+thread_local std::vector<MapEntry> g_maps; /* small: layers x pools in use by this thread */
+
+leyline_status band_map(const leyline_plan_s* pl, void* pool, int box_rows, CUtensorMap* out) {
+    const int64_t band0 = (int64_t)pl->desc.latent_dim * pl->elem_bytes;
+    const int32_t band_bytes = pl->n_heads * pl->desc.rope_dim * pl->elem_bytes;
+    const MapKey key{static_cast<uint8_t*>(pool) + band0, pl->desc.row_stride_bytes, pl->desc.pool_slots, band_bytes, box_rows};
+    for (const MapEntry& e : g_maps)
+        if (e.key == key) { *out = e.map; return LEYLINE_OK; }
+    std::call_once(g_encode_once, [] {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            g_encode_tiled = reinterpret_cast<PFN_cuTensorMapEncodeTiled>(fn);
+        (void)cudaGetLastError();
+    });
+    if (!g_encode_tiled) { g_last_error = "cuTensorMapEncodeTiled is not available from this driver"; return LEYLINE_E_CUDA; }
+    /* elements are 32-bit words: the band is a multiple of 32 bytes, and a box edge holds at most 256 elements */
+    const cuuint64_t dims[2] = {(cuuint64_t)(band_bytes / 4), (cuuint64_t)pl->desc.pool_slots};
+    const cuuint64_t strides[1] = {(cuuint64_t)pl->desc.row_stride_bytes};
+    const cuuint32_t box[2] = {(cuuint32_t)(band_bytes / 4), (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    MapEntry e;
+    e.key = key;
+    const CUresult r = g_encode_tiled(&e.map, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, const_cast<void*>(key.base), dims, strides, box, estr,
+                                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { g_last_error = "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")"; return LEYLINE_E_CUDA; }
+    if (g_maps.size() >= 4096) g_maps.clear();
+    g_maps.push_back(e);
+    *out = e.map;
+    return LEYLINE_OK;
+}
+
+using BandKernel = void (*)(const MoveParams, const BandMaps, int, int, int, int, int);
+
+template <int DT>
+BandKernel pick_band_dt(int pairing) {
+    return pairing == LEYLINE_ROPE_NEOX ? k_rotate_band_tma<DT, LEYLINE_ROPE_NEOX> : k_rotate_band_tma<DT, LEYLINE_ROPE_INTERLEAVED>;
+}
+
+leyline_status run_rotate_tma(leyline_plan_s* pl, int64_t tile_count, int64_t insert_count, void* const* layer_ptrs,
+                              const void* const* layer_repl, cudaStream_t stream, int* ticket_slot) {
+    if (tile_count + insert_count <= 0) return LEYLINE_OK;
+    const int band_bytes = pl->n_heads * pl->desc.rope_dim * pl->elem_bytes;
+    const int box_rows = pl->rot_tile_rows;
+    const int stage_bytes = (int)align_up((int64_t)box_rows * band_bytes, 128);
+    for (const LayerChunk& lc : layer_chunks(pl, kBandTmaLayers)) {
+        const int nl = (int)lc.layers.size();
+        BandKernel fn = pl->desc.dtype == LEYLINE_BF16 ? pick_band_dt<LEYLINE_BF16>(lc.pairing) : pick_band_dt<LEYLINE_FP8_E4M3>(lc.pairing);
+        cudaFuncAttributes fa;
+        CU(cudaFuncGetAttributes(&fa, reinterpret_cast<const void*>(fn)));
+        int stages = (g_dev.smem_optin - (int)fa.sharedSizeBytes - 1024) / stage_bytes;
+        if (pl->tuning.stages > 0 && stages > pl->tuning.stages) stages = pl->tuning.stages;
+        if (stages > kBandMaxStages) stages = kBandMaxStages;
+        if (stages < kBandStoresInFlight + 2) { g_last_error = "TMA band kernel: too few shared-memory stages"; return LEYLINE_E_UNSUPPORTED; }
+        const int smem = stages * stage_bytes;
+        CU(cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        if (*ticket_slot >= 32) { g_last_error = "too many launches for one plan"; return LEYLINE_E_UNSUPPORTED; }
+        MoveParams mp;
+        fill_params(pl, mp, 0, tile_count, lc, nullptr, layer_ptrs, layer_repl, (*ticket_slot)++);
+        BandMaps maps;
+        std::memset(&maps, 0, sizeof(maps));
+        for (int l = 0; l < nl; ++l) {
+            leyline_status st = band_map(pl, layer_ptrs[lc.layers[l]], box_rows, &maps.m[l]);
+            if (st != LEYLINE_OK) return st;
+        }
+        int group = pl->tuning.layer_group > 0 ? pl->tuning.layer_group : 8;
+        if (group > nl) group = nl;
+        mp.n_items = tile_count * ((nl + group - 1) / group);
+        mp.n_copy_items = insert_count * (long long)nl;   /* a4 rides in the same launch */
+        mp.copy_tile_begin = (int32_t)tile_count;
+        long long grid = g_dev.sms;
+        const long long most = mp.n_items > mp.n_copy_items ? mp.n_items : mp.n_copy_items;
+        if (grid > most) grid = most;
+        fn<<<(unsigned)grid, kBandThreads, (size_t)smem, stream>>>(mp, maps, stages, stage_bytes, box_rows, band_bytes, group);
         CU(cudaGetLastError());
     }
     return LEYLINE_OK;
@@ -524,6 +622,8 @@ extern "C" LEYLINE_API leyline_status leyline_rotate_inplace(leyline_plan_t* pl,
     /* a5: rotate where the rows sit; a4: replacement rows go to the consumed free slots (disjoint from a5's) */
     if (pl->rotate_with_bulk) /* wide band: whole rows through the bulk mover, written back in place; inserts as usual */
         st = run_tiles_bulk(pl, false, 0, n_rot + n_ins, layer_ptrs, layer_ptrs, layer_repl, stream, &slot);
+    else if (pl->rotate_with_tma) /* narrow band in pages: one 2-D TMA box per page and layer */
+        st = run_rotate_tma(pl, n_rot, n_ins, layer_ptrs, layer_repl, stream, &slot);
     else
         st = run_rotate(pl, 0, n_rot, n_ins, layer_ptrs, layer_repl, stream, &slot);
     if (st != LEYLINE_OK) return st;
@@ -590,6 +690,7 @@ extern "C" LEYLINE_API leyline_status leyline_plan_prefetch(leyline_plan_t* pl) 
 extern "C" LEYLINE_API leyline_status leyline_plan_kernel_ms(const leyline_plan_t* pl, float* ms) try {
     g_last_error.clear();
     if (!pl || !ms || !pl->ev_start) return LEYLINE_E_INVALID;
+    CU(cudaEventSynchronize(static_cast<cudaEvent_t>(pl->ev_stop))); /* returns at once when the launch has finished */
     CU(cudaEventElapsedTime(ms, static_cast<cudaEvent_t>(pl->ev_start), static_cast<cudaEvent_t>(pl->ev_stop)));
     return LEYLINE_OK;
 } LEYLINE_CATCH_STATUS
@@ -603,6 +704,26 @@ extern "C" LEYLINE_API leyline_status leyline_plan_trig_table_device(const leyli
     cudaStream_t stream = static_cast<cudaStream_t>(pl->last_stream);
     CU(cudaMemcpyAsync(out, blob_at<float>(pl, pl->off_trig), bytes, cudaMemcpyDeviceToHost, stream));
     CU(cudaStreamSynchronize(stream));
+    return LEYLINE_OK;
+} LEYLINE_CATCH_STATUS
+
+/* Measurement aid (leyline.h): the a5 access pattern on a contiguous buffer, nothing else. */
+extern "C" LEYLINE_API leyline_status leyline_probe_band_update(void* dev_buf, int64_t n_rows, int64_t row_stride_bytes,
+                                                                int32_t band_offset_bytes, int32_t band_bytes,
+                                                                int32_t ctas_per_sm, void* cuda_stream) try {
+    g_last_error.clear();
+    if (!dev_buf || n_rows < 0 || row_stride_bytes < 16 || (row_stride_bytes & 15) || band_offset_bytes < 0 ||
+        (band_offset_bytes & 15) || band_bytes < 16 || (band_bytes & 15) || band_offset_bytes + (int64_t)band_bytes > row_stride_bytes ||
+        (reinterpret_cast<uintptr_t>(dev_buf) & 15) || ctas_per_sm < 0 || ctas_per_sm > 32)
+        return LEYLINE_E_INVALID;
+    if (n_rows == 0) return LEYLINE_OK;
+    int dev = 0;
+    leyline_status st = device_info(&dev);
+    if (st != LEYLINE_OK) return st;
+    const int per_sm = ctas_per_sm > 0 ? ctas_per_sm : 8;
+    k_probe_band_update<8><<<(unsigned)(g_dev.sms * per_sm), kThreads, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+        static_cast<uint8_t*>(dev_buf), n_rows, row_stride_bytes, band_offset_bytes, band_bytes / 16);
+    CU(cudaGetLastError());
     return LEYLINE_OK;
 } LEYLINE_CATCH_STATUS
 

@@ -357,3 +357,21 @@ def test_gpu_chunker_parameter_extremes(mn, mx, bits):
     np.testing.assert_array_equal(end, o_end)
     np.testing.assert_array_equal(kind, o_kind)
     np.testing.assert_array_equal(hsh, o_hash)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("mn,mx,bits", [(64, 4096, 12), (2048, 4096, 16), (1, 3000, 9), (16, 256, 6)])
+def test_gpu_chunker_long_unanchored_sequences(mn, mx, bits):
+    """No anchors at all, four sequences of ~200 K tokens: hard stops are ~200 K positions apart and candidates up to
+    65 K, so "next set bit" walks the second bitmap level over many words, chains are thousands of chunks long (the
+    doubling needs most of its rounds) and max_size cuts dominate where the mask rarely fires."""
+    rng = np.random.default_rng(mn + mx + bits)
+    lens = [200003, 199999, 1, 180000]
+    t = rng.integers(0, 32000, size=sum(lens)).astype(np.int32)
+    so = [0, *np.cumsum(lens).tolist()]
+    c, end, hsh, kind, _ = gpu_chunk(t, so, [], SEED, mn, mx, bits)
+    o_end, o_hash, o_kind = OC.chunk(SEED, mn, mx, bits, t, so, [])
+    assert c == len(o_end)
+    np.testing.assert_array_equal(end, o_end)
+    np.testing.assert_array_equal(kind, o_kind)
+    np.testing.assert_array_equal(hsh, o_hash)

@@ -681,3 +681,58 @@ def test_device_trig_table_matches_the_host_evaluation():
         assert ((d <= 1) & same_sign | (np.abs(dev.astype(np.float64) - want) < 1e-45)).all()
         assert (d == 0).mean() > 0.9999, (cfg, float((d == 0).mean()))
         plan.close()
+
+
+# ----------------------------------------------------------------------------- a5 with 2-D TMA boxes (k_rotate_band_tma)
+
+TMA = {"rotate_kernel": 2}
+
+
+@pytest.mark.parametrize("cfg", [2, 3, "3m", 5])
+def test_rotate_only_tma_full_size(cfg):
+    """leyline_tuning.rotate_kernel = 2: the band of a page as one 2-D TMA box (64 rows x 128 B bf16 / 64 B fp8, pitch =
+    row stride), loaded into shared memory, rotated there and stored back.  Every layer, whole pools."""
+    from paper_2606_01065_b200 import binding as B
+    w = synth.config(cfg, pool_factor=2.0)
+    run_and_compare(w, O.ROTATE_ONLY, tuning=TMA)
+    B.leyline_set_tuning(**TMA)
+    try:
+        with __import__("test_plan_host").make_plan(w, B.ROTATE_ONLY) as plan:
+            assert plan.info.mover == 3 and plan.info.rot_tile_rows == 64
+    finally:
+        B.leyline_set_tuning()
+
+
+@pytest.mark.parametrize("page", [16, 32, 64, 256])
+@pytest.mark.parametrize("dtype", [synth.DT_BF16, synth.DT_FP8])
+@pytest.mark.parametrize("pairing", [synth.NEOX, synth.INTERLEAVED])
+def test_rotate_only_tma_ragged(page, dtype, pairing):
+    """Segments that start and end inside pages (ragged first / last tiles move row by row), several requests, growth
+    and shrink, replacement inserts in the same launch, a request of one token and an empty one."""
+    w = synth.Workload("tma_ragged", 3, [3000, 1, 0, 2777], page, dtype=dtype, pairing=pairing, inv_freq=synth.yarn_inv_freq(),
+                       directives=[(0, 5, 5, 40, 0, 0), (0, 100, 900, 3, 0, 0), (0, 1500, 1501, 333, 0, 0),
+                                   (0, 2990, 3000, 0, 0, 0), (1, 0, 1, 0, 0, 0),
+                                   (3, 0, 17, 500, 0, 0), (3, 1000, 1700, 0, 0, 0), (3, 2776, 2777, 2, 0, 0)],
+                       seed=12, pool_factor=3.0, extra_pages=80).finalize()
+    run_and_compare(w, O.ROTATE_ONLY, tuning=TMA)
+    run_and_compare(w, O.ROTATE_ONLY, tuning=dict(TMA, stages=6, layer_group=2))
+
+
+def test_rotate_only_tma_other_geometries():
+    """Two heads of 64 behind an MLA latent (256-B band), the narrowest band (32 B, fp8), per-layer pairing, caller-
+    prefilled replacement slots, more layers than one launch holds (64 tensor maps per launch), and pools whose pages
+    are smaller than a box row count (falls back to the strided kernel)."""
+    rng = np.random.default_rng(64)
+    run_and_compare(heads_workload("tma_heads", 2, 64, 512, synth.DT_BF16, synth.NEOX, 1.0e4), O.ROTATE_ONLY, tuning=TMA)
+    run_and_compare(heads_workload("tma_narrow", 1, 32, 16, synth.DT_FP8, synth.NEOX, 1.0e4), O.ROTATE_ONLY, tuning=TMA)
+    w = tiny_workload(rng, P=16, n_req=3)
+    w.n_layers = 5
+    w.layer_pairing = [synth.NEOX, synth.INTERLEAVED, synth.INTERLEAVED, synth.NEOX, synth.INTERLEAVED]
+    run_and_compare(w, O.ROTATE_ONLY, tuning=TMA)
+    run_and_compare(tiny_workload(rng, P=16), O.ROTATE_ONLY, tuning=TMA, inserts_prefilled=True)
+    w = tiny_workload(rng, P=16, n_req=2)
+    w.n_layers = 130
+    run_and_compare(w, O.ROTATE_ONLY, tuning=TMA)
+    run_and_compare(tiny_workload(rng, P=4), O.ROTATE_ONLY, tuning=TMA)
+    for _ in range(6):
+        run_and_compare(fuzz_workload(rng), O.ROTATE_ONLY, tuning=TMA, prefetch=bool(rng.integers(0, 2)))

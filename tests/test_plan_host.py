@@ -291,6 +291,14 @@ def test_alias_rule_refuses_plans_that_would_overwrite_live_kv():
     assert status(B.INPLACE_MOVE, [(0, 9, 10, 0, 0, A)], [10], pages=shared) == B.E_ALIAS
     assert status(B.INPLACE_MOVE, [], [10], pages=shared) == B.OK
     assert status(B.INPLACE_MOVE, edit1, [10], pages=np.array([0, 1, 2, 3, 3], np.int32)) == B.E_ALIAS   # twice in one request
+    # leyline_tuning.skip_alias_check = 1: the caller vouches for its tables, nothing is checked (and nothing is cheaper)
+    B.leyline_set_tuning(skip_alias_check=1)
+    try:
+        assert status(B.FRESH, grow, [10, 1, 12, 13, 14]) == B.OK
+        assert status(B.INPLACE_MOVE, edit1, [10], pages=shared) == B.OK
+        assert status(B.ROTATE_ONLY, grow, [40, 41, 42, 43, 44, 45, 46, 47, 40]) == B.OK
+    finally:
+        B.leyline_set_tuning()
     del keep
 
 
@@ -335,7 +343,7 @@ def test_plan_ex_takes_its_tuning_per_call():
     w = synth.config(2, pool_factor=2.2)
     d, keep = B.make_desc(w.n_layers, w.latent_dim, w.rope_dim, w.page_size, w.dtype, w.pairing, w.row_bytes, w.n_slots, w.inv_freq)
     args = (d, B.FRESH, w.seq_lens, w.pt_offsets, w.pages, w.directives, w.free_pages)
-    with B.leyline_plan_ex(*args) as p0, B.leyline_plan_ex(*args, B.Tuning(1, 7, 0, 0, 0, 0, 0, 0)) as p1:
+    with B.leyline_plan_ex(*args) as p0, B.leyline_plan_ex(*args, B.Tuning(1, 7, 0, 0, 0, 0, 0, 0, 0)) as p1:
         assert (p0.info.mover, p0.info.tile_rows) == (2, 32) and (p1.info.mover, p1.info.tile_rows) == (1, 7)
     B.leyline_set_tuning(kernel=1, tile_rows=5)
     try:
@@ -345,7 +353,7 @@ def test_plan_ex_takes_its_tuning_per_call():
     finally:
         B.leyline_set_tuning()
     with pytest.raises(B.LeylineError) as ei:
-        B.leyline_plan_ex(*args, B.Tuning(9, 0, 0, 0, 0, 0, 0, 0))
+        B.leyline_plan_ex(*args, B.Tuning(9, 0, 0, 0, 0, 0, 0, 0, 0))
     assert ei.value.status == B.E_INVALID
     del keep
 
@@ -514,3 +522,37 @@ int main(void) {
     # tokens 5..61 removed, 11 inserted, 9 downstream tokens moved by -46; token-level FRESH keeps slots [0, 5)
     assert "L_new=25 consumed=20 released=66 rows_moved=9 rows_inserted=11" in out, out
     assert "sm_100a" in out
+
+
+def test_tma_rotate_tiles_are_whole_boxes_inside_one_page():
+    """leyline_tuning.rotate_kernel = 2 (k_rotate_band_tma): ROTATE_ONLY tiles are at most min(page, 64) rows, never
+    straddle a page of the OLD table (so their rows are consecutive slots: one 2-D box), and every interior tile of a
+    segment is a whole box.  Pages below 16 rows and wide bands fall back to the other kernels."""
+    for P, box in ((16, 16), (64, 64), (256, 64)):
+        w = synth.Workload("t", 1, [5000, 777], P, inv_freq=synth.yarn_inv_freq(),
+                           directives=[(0, 300, 1100, 77, 0, 0), (0, 3000, 3001, 600, 0, 0), (1, 770, 777, 0, 0, 0)],
+                           seed=2, pool_factor=3.0, extra_pages=4).finalize()
+        B.leyline_set_tuning(rotate_kernel=2)
+        try:
+            plan = make_plan(w, B.ROTATE_ONLY)
+        finally:
+            B.leyline_set_tuning()
+        with plan:
+            assert plan.info.mover == 3 and plan.info.rot_tile_rows == box
+            bm = oracle_plan(w, B.ROTATE_ONLY)
+            assert_plan_equal(plan, bm, B.ROTATE_ONLY)
+            check_tiles_cover(plan, bm, w, B.ROTATE_ONLY)
+            rot = plan.tiles[:plan.info.n_move_tiles]
+            for t in rot:
+                assert 1 <= t.n_rows <= box and t.src_pos // P == (t.src_pos + t.n_rows - 1) // P
+                assert t.src_pos // box == (t.src_pos + t.n_rows - 1) // box          # aligned to the box grid
+            assert sum(1 for t in rot if t.n_rows == box) >= len(rot) - 2 * len(plan.segments)
+    w = synth.config(1, pool_factor=2.5)                                              # token-level slots: no boxes
+    B.leyline_set_tuning(rotate_kernel=2)
+    try:
+        with make_plan(w, B.ROTATE_ONLY) as plan:
+            assert plan.info.mover == 1
+        with make_plan(synth.config("gqa", pool_factor=2.0), B.ROTATE_ONLY) as plan:
+            assert plan.info.mover == 2                                               # wide band: whole rows on the bulk mover
+    finally:
+        B.leyline_set_tuning()

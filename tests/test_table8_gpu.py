@@ -76,7 +76,8 @@ def test_table8_row(name, d, mode):
                 pool[1 + r] = to_storage(k, O.BF16)[0]
             olds.append(pool.reshape(-1))
             pools.append(torch.from_numpy(olds[-1].copy()).to("cuda:0"))
-        plan = B.leyline_plan(desc, mode, seq_lens, pt_offsets, pages, dirs, free)
+        # the dummy slot is aliased on purpose (never read or written here): the caller vouches for its tables
+        plan = B.leyline_plan_ex(desc, mode, seq_lens, pt_offsets, pages, dirs, free, B.Tuning(skip_alias_check=1))
         idx = torch.empty(int(plan.info.total_new_tokens), dtype=torch.int32, device="cuda:0")
         if mode == O.ROTATE_ONLY:
             B.leyline_rotate_inplace(plan, pools, None, idx)
