@@ -259,7 +259,7 @@ def time_discovery(dev, with_oracle: bool, n_sessions: int = 16, prompt_len: int
     microbenchmark -- 16 sessions x ~17 K-token prompts, anchors every ~600 tokens -- against
     the oracle's sequential chunker on the host, for the default chunk parameters (16, 256, 6) and for long chunks
     (64, 4096, 12).  The input is 1 MB, so the call is bound by its chain of dependent small launches, not by bytes:
-    `launch_bound_ms` = launches x the measured cost of one tiny dependent launch on this stream."""
+    `launch_bound_ms` = launches x the per-launch cost of the same call on a 48-token input."""
     import torch
     from paper_2606_01065_b200 import binding as B
     rng = np.random.default_rng(17)
@@ -288,12 +288,19 @@ def time_discovery(dev, with_oracle: bool, n_sessions: int = 16, prompt_len: int
         torch.cuda.synchronize()
         return e0.elapsed_time(e1) / reps
 
-    keys, vals = torch.zeros(1, dtype=torch.int64, device=dev), torch.zeros(1, dtype=torch.int64, device=dev)
-    launch_ms = timed(lambda: B.leyline_registry_clear(keys, vals, 1), 200)      # one tiny kernel per call, back to back
-    rounds = int(np.ceil(np.log2(n + 1)))
-    launches = 1 + 5 + rounds + 4          # memset; flags, seq_ends, signature, level1, next; doubling; count, scan, emit, hash
-    out = {"tokens": n, "tiny_launch_us": launch_ms * 1e3, "launches_per_call": launches,
-           "launch_bound_ms": launches * launch_ms}
+    # cost of one small dependent launch of this call chain: the same call on a 48-token input (every kernel is one
+    # block, so its time is launches x launch cost), divided by its launch count
+    n_small = 48
+    launches_of = lambda m: 1 + 5 + int(np.ceil(np.log2(m + 1))) + 4   # memset; flags, seq_ends, signature, level1, next; doubling; count, scan, emit, hash
+    off_small = torch.tensor([0, n_small], dtype=torch.int64, device=dev)
+    prm0 = B.CdcParams(0x5EED, 16, 256, 6, 0)
+    small_ms = timed(lambda: B.leyline_cdc_chunk(prm0, td, n_small, off_small, 1, an, len(anchors), end, hsh, kind, n_small, cnt), 50)
+    launch_ms = small_ms / launches_of(n_small)
+    launches = launches_of(n)
+    out = {"tokens": n, "small_launch_us": launch_ms * 1e3, "launches_per_call": launches,
+           "launch_bound_ms": launches * launch_ms,
+           "bound": "launch latency: the input is 1 MB, the call is a chain of dependent small launches (scratch "
+                    "allocation included); launch_bound_ms = launches_per_call x the per-launch cost of the same call on 48 tokens"}
     for name, (mn, mx, bits) in (("min16_max256_bits6", (16, 256, 6)), ("min64_max4096_bits12", (64, 4096, 12))):
         prm = B.CdcParams(0x5EED, mn, mx, bits, 0)
         gpu_ms = timed(lambda: B.leyline_cdc_chunk(prm, td, n, off, n_sessions, an, len(anchors), end, hsh, kind, n, cnt), reps)

@@ -736,3 +736,20 @@ def test_rotate_only_tma_other_geometries():
     run_and_compare(tiny_workload(rng, P=4), O.ROTATE_ONLY, tuning=TMA)
     for _ in range(6):
         run_and_compare(fuzz_workload(rng), O.ROTATE_ONLY, tuning=TMA, prefetch=bool(rng.integers(0, 2)))
+
+
+@pytest.mark.parametrize("seed", [101, 202])
+def test_hazard_mover_random_batches_all_layers(seed):
+    """More race coverage for k_move_bulk<HAZARD> at full concurrency (148 CTAs, every layer compared, whole pools):
+    config-4-shaped batches with other directive draws -- 48 requests x 8 K tokens x 24 layers, 1-5 directives each,
+    spans log-uniform 16-4096, replacements up to 512 rows (more growth than config 4), Delta of both signs."""
+    rng = np.random.default_rng(seed)
+    n_req, L = 48, 8192
+    dirs = []
+    for r in range(n_req):
+        for (s0, e0, rl) in synth.random_directives(rng, L, int(rng.integers(1, 6)), 16, 4096, 512):
+            dirs.append((r, s0, e0, rl, 0, synth.AMORTIZE))
+    w = synth.Workload(f"hazard_batch_{seed}", 24, [L] * n_req, 64, inv_freq=synth.yarn_inv_freq(64, 10000.0, 40.0, 4096),
+                       directives=dirs, seed=seed, pool_factor=1.3).finalize()
+    assert any(d[3] > d[2] - d[1] for d in dirs) and any(d[3] < d[2] - d[1] for d in dirs)
+    run_and_compare(w, O.INPLACE_MOVE)
