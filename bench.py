@@ -291,21 +291,26 @@ def time_discovery(dev, with_oracle: bool, n_sessions: int = 16, prompt_len: int
     # cost of one small dependent launch of this call chain: the same call on a 48-token input (every kernel is one
     # block, so its time is launches x launch cost), divided by its launch count
     n_small = 48
-    launches_of = lambda m: 1 + 5 + int(np.ceil(np.log2(m + 1))) + 4   # memset; flags, seq_ends, signature, level1, next; doubling; count, scan, emit, hash
+    def launches_of(m, mn):      # front, next; doubling rounds (seeds behind every hard stop: <= (m-1)/min_size + 1 chunks to cover); count+scan, emit
+        far, rounds, reach = (m - 1) // mn + 1, 0, 1
+        while reach <= far:
+            reach, rounds = reach << 1, rounds + 1
+        return 2 + rounds + 2
     off_small = torch.tensor([0, n_small], dtype=torch.int64, device=dev)
     prm0 = B.CdcParams(0x5EED, 16, 256, 6, 0)
     small_ms = timed(lambda: B.leyline_cdc_chunk(prm0, td, n_small, off_small, 1, an, len(anchors), end, hsh, kind, n_small, cnt), 50)
-    launch_ms = small_ms / launches_of(n_small)
-    launches = launches_of(n)
-    out = {"tokens": n, "small_launch_us": launch_ms * 1e3, "launches_per_call": launches,
-           "launch_bound_ms": launches * launch_ms,
+    launch_ms = small_ms / launches_of(n_small, 16)
+    out = {"tokens": n, "small_launch_us": launch_ms * 1e3,
            "bound": "launch latency: the input is 1 MB, the call is a chain of dependent small launches (scratch "
-                    "allocation included); launch_bound_ms = launches_per_call x the per-launch cost of the same call on 48 tokens"}
+                    "allocation included, programmatic dependent launch); launch_bound_ms = launches_per_call x the "
+                    "per-launch cost of the same call on 48 tokens"}
     for name, (mn, mx, bits) in (("min16_max256_bits6", (16, 256, 6)), ("min64_max4096_bits12", (64, 4096, 12))):
         prm = B.CdcParams(0x5EED, mn, mx, bits, 0)
         gpu_ms = timed(lambda: B.leyline_cdc_chunk(prm, td, n, off, n_sessions, an, len(anchors), end, hsh, kind, n, cnt), reps)
         c = int(cnt.item())
-        line = {"chunks": c, "gpu_ms": gpu_ms, "gpu_Mtok_per_s": n / gpu_ms / 1e3, "over_launch_bound": gpu_ms / (launches * launch_ms)}
+        launches = launches_of(n, mn)
+        line = {"chunks": c, "gpu_ms": gpu_ms, "gpu_Mtok_per_s": n / gpu_ms / 1e3, "launches_per_call": launches,
+                "launch_bound_ms": launches * launch_ms, "over_launch_bound": gpu_ms / (launches * launch_ms)}
         if with_oracle:      # part of the cpu_baseline leg: the oracle's sequential chunker timed on the host beside it
             from oracle import cdc as OC
             t0 = time.perf_counter()

@@ -4,26 +4,32 @@
  * registry.  Readings D1-D5 of DESIGN.md fix the constants the paper leaves open.
  *
  * The sequential definition (one rolling hash, one open chunk) is restated so that every step is data-parallel:
- *   k_cdc_flags      per token: gear value G(t) (D1), "anchor" and "last token of its sequence" flags
- *   k_cdc_signature  per position: h_i as the 64-term window sum  sum_j G(t_{i-j}) << j  cut at the last reset (D2
- *                    in closed form: the shift drops a token out of the 64-bit word after 64 steps); the "hash
- *                    candidate" and "hard stop" (anchor / sequence end) predicates go into two BITMAPS, one ballot per
- *                    32 positions, with a second level (one bit per non-empty word) built by k_cdc_level1
+ *   k_cdc_front      everything that is a function of a 64-token window, one launch: gear value G(t) (D1), "anchor" /
+ *                    "last token of its sequence" flags, h_i as the 64-term window sum  sum_j G(t_{i-j}) << j  cut at the
+ *                    last reset (D2 in closed form: the shift drops a token out of the 64-bit word after 64 steps), the
+ *                    "hash candidate" and "hard stop" (anchor / sequence end) predicates as two-level BITMAPS (one
+ *                    ballot per 32 positions, one bit per non-empty word above it), and the chain SEEDS: a chunk starts
+ *                    for certain at every sequence start and behind every hard stop
  *   k_cdc_next       per position s: where a chunk that STARTS at s would end (D3) = min(next hard stop >= s,
  *                    s + max_size - 1, next candidate >= s + min_size - 1); "next set bit at or after i" is a
  *                    find-first-set in the position's word, else in the level-1 word: O(1) loads per position for
  *                    every legal (min_size, max_size, mask_bits), so the pass is linear in n
- *   k_cdc_reach      pointer doubling over s -> next(s): marks the starts actually reached from the sequence starts;
- *                    a round that sets no new mark proves the longest per-sequence chain is covered, and every later
- *                    round returns at once (ceil(log2(longest chain)) working rounds, not ceil(log2 n))
- *   k_cdc_count / k_cdc_scan / k_cdc_emit   ordered compaction of the marked starts
- *   k_cdc_hash       content hash per chunk (D4).  FNV-1a is a serial recurrence (x = (x ^ byte) * prime), so its
- *                    floor is the LONGEST chunk: 4 dependent 64-bit multiplies per token, <= 4 * max_size in a row
+ *   k_cdc_reach      pointer doubling over s -> next(s): marks the starts actually reached from the seeds.  Between two
+ *                    seeds every chunk but the last holds >= min_size tokens, so ceil(log2(n / min_size + 2)) rounds
+ *                    always suffice; a round that sets no new mark proves every chain is covered, and every later
+ *                    round returns at once
+ *   k_cdc_count_scan ordered compaction of the marked starts: marks per block, scanned by the block that finishes last
+ *   k_cdc_emit       chunk end, kind and content hash (D4).  FNV-1a is a serial recurrence (x = (x ^ byte) * prime), so
+ *                    the floor is the LONGEST chunk: 4 dependent 64-bit multiplies per token, <= 4 * max_size in a row
+ * The call is a chain of R + 4 small dependent launches on ~1 MB of input (R = the doubling rounds), so it is bound by
+ * the launch-to-launch gap: every kernel is launched with programmatic stream serialisation (PDL) and lets its successor
+ * be scheduled while it runs.  No memset, no intermediate host step.
  * Integer work throughout; results are bit-exact against the CPU oracle.
  */
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <cstring>
 #include <string>
 
 #include "leyline_cdc.h"
@@ -32,7 +38,8 @@
 namespace {
 
 constexpr int kT = 256;
-constexpr uint8_t F_ANCHOR = 1, F_SEQ_END = 2;
+constexpr uint8_t F_ANCHOR = 1, F_SEQ_END = 2, F_RESET = 3 /* either: a hard stop, and the signature restarts behind it */,
+                  F_SEQ_START = 4 /* shared-memory only: a non-empty sequence starts here */;
 
 thread_local std::string g_cdc_error;
 bool ok(cudaError_t e) {
@@ -50,63 +57,104 @@ __device__ __forceinline__ uint64_t gear_of(uint64_t seed, int32_t token) { /* D
     return z ^ (z >> 31);
 }
 
-__global__ void __launch_bounds__(kT) k_cdc_flags(const int32_t* __restrict__ tokens, int64_t n, const int32_t* __restrict__ anchors,
-                                                  int n_anchors, uint64_t seed, uint64_t* __restrict__ gear, uint8_t* __restrict__ flags) {
-    for (int64_t i = blockIdx.x * (int64_t)kT + threadIdx.x; i < n; i += (int64_t)gridDim.x * kT) {
-        const int32_t t = tokens[i];
-        int lo = 0, hi = n_anchors; /* first anchor >= t */
-        while (lo < hi) {
-            const int mid = (lo + hi) >> 1;
-            if (__ldg(anchors + mid) < t) lo = mid + 1; else hi = mid;
-        }
-        gear[i] = gear_of(seed, t);
-        flags[i] = (lo < n_anchors && __ldg(anchors + lo) == t) ? F_ANCHOR : 0;
-    }
+/* Programmatic dependent launch (sm_90+): every kernel of the call lets its successor be scheduled at once
+ * (launch_dependents) and then waits until its predecessor has completed and flushed (wait).  The call is a chain of ~20
+ * small dependent launches on 1 MB of input, so what it costs is the launch-to-launch gap, and this is what hides it. */
+__device__ __forceinline__ void pdl_enter() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
-/* the last token of every non-empty sequence (runs after k_cdc_flags on the same stream).  Offsets live on the device
- * and cannot be validated by the host: anything outside [0, n] is ignored here rather than followed. */
-__global__ void __launch_bounds__(kT) k_cdc_seq_ends(const int64_t* __restrict__ seq_offsets, int n_seqs, int64_t n,
-                                                     uint8_t* __restrict__ flags, uint8_t* __restrict__ mark) {
-    for (int s = blockIdx.x * kT + threadIdx.x; s < n_seqs; s += gridDim.x * kT) {
-        const int64_t b = seq_offsets[s], e = seq_offsets[s + 1];
-        if (e > b && b >= 0 && e <= n) {
-            flags[e - 1] |= F_SEQ_END; /* one writer per byte: sequences do not share tokens */
-            mark[b] = 1;               /* a chunk starts at every sequence start */
-        }
-    }
-}
+constexpr int kSigSpan = 1024;              /* positions per block pass = one level-1 bitmap word */
+constexpr int kSigHalo = 63;                /* D2: h_i depends on the last 64 tokens */
 
-/* D2 + the two predicates of D3 as bitmaps.  Word w of hard0 / cand0 covers positions [32w, 32w + 32): a warp handles 32
- * consecutive positions and lane 0 stores the ballot, so every word (also the tail, where positions >= n read as 0) is
- * written exactly once and nothing is modified in place. */
-__global__ void __launch_bounds__(kT) k_cdc_signature(const uint64_t* __restrict__ gear, const uint8_t* __restrict__ flags, int64_t n,
-                                                      int64_t n_padded, int mask_bits, uint32_t* __restrict__ hard0,
-                                                      uint32_t* __restrict__ cand0) {
-    for (int64_t i = blockIdx.x * (int64_t)kT + threadIdx.x; i < n_padded; i += (int64_t)gridDim.x * kT) {
-        bool hard = false, cand = false;
-        if (i < n) {
-            uint64_t h = gear[i];
-            for (int j = 1; j < 64; ++j) {
-                const int64_t k = i - j;
-                if (k < 0 || flags[k]) break; /* the signature was reset after token k (anchor or end of a sequence) */
-                h += gear[k] << j;
+/* k_cdc_front: everything that is a function of a 64-token window, in ONE launch.  A block pass covers the 1024 positions
+ * of one level-1 word v plus a 63-token halo in front of it:
+ *   - gear value G(t) (D1) and the reset flags of those 1087 positions go to shared memory: "anchor" by bisection of the
+ *     sorted anchor ids, "last token of a non-empty sequence" by bisection of the sequence offsets;
+ *   - the chain seeds (mark[i], every position written exactly once): position i starts a chunk for certain when a
+ *     sequence starts there or when position i - 1 is a hard stop (an anchor or a sequence end, D3).  With these seeds the pointer doubling only has to cover the chunks
+ *     between two hard stops, all of which but the last hold >= min_size tokens;
+ *   - h_i as the 64-term window sum  sum_j G(t_{i-j}) << j  cut at the last reset (D2 in closed form), the "hash
+ *     candidate" and "hard stop" predicates as two bitmaps (one ballot per 32 positions) and their level-1 words (one
+ *     bit per non-empty level-0 word).
+ * Offsets live on the device and cannot be validated by the host: the bisections only ever index [0, n_seqs], and nothing
+ * at or past n is written. */
+__global__ void __launch_bounds__(kT) k_cdc_front(const int32_t* __restrict__ tokens, int64_t n, const int32_t* __restrict__ anchors,
+                                                  int n_anchors, uint64_t seed, const int64_t* __restrict__ seq_offsets, int n_seqs,
+                                                  int mask_bits, int64_t n_super, uint8_t* __restrict__ flags, uint8_t* __restrict__ mark,
+                                                  uint32_t* __restrict__ hard0, uint32_t* __restrict__ cand0,
+                                                  uint32_t* __restrict__ hard1, uint32_t* __restrict__ cand1,
+                                                  int32_t* __restrict__ progress, int n_progress) {
+    __shared__ uint64_t s_gear[kSigSpan + kSigHalo];
+    __shared__ uint8_t s_flag[kSigSpan + kSigHalo];
+    __shared__ uint32_t s_nonzero[2][kSigSpan / 32];
+    pdl_enter();
+    if (blockIdx.x == 0)
+        for (int k = threadIdx.x; k < n_progress; k += kT) progress[k] = 0;
+    const int64_t first = seq_offsets[0];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int64_t v = blockIdx.x; v < n_super; v += gridDim.x) {
+        const int64_t base = v * kSigSpan - kSigHalo;
+        for (int k = threadIdx.x; k < kSigSpan + kSigHalo; k += kT) {
+            const int64_t i = base + k;
+            uint64_t g = 0;
+            uint8_t f = F_SEQ_END; /* outside [0, n): a reset, so that no window reaches across it */
+            if (i >= 0 && i < n) {
+                const int32_t t = tokens[i];
+                int lo = 0, hi = n_anchors; /* first anchor >= t */
+                while (lo < hi) {
+                    const int mid = (lo + hi) >> 1;
+                    if (__ldg(anchors + mid) < t) lo = mid + 1; else hi = mid;
+                }
+                const bool anchor = lo < n_anchors && __ldg(anchors + lo) == t;
+                int a = 0, b = n_seqs + 1; /* first offset > i */
+                while (a < b) {
+                    const int mid = (a + b) >> 1;
+                    if (__ldg(seq_offsets + mid) <= i) a = mid + 1; else b = mid;
+                }
+                const bool seq_end = a >= 1 && a <= n_seqs && __ldg(seq_offsets + a) == i + 1; /* [.., i + 1) is non-empty: offsets[a-1] <= i */
+                const bool seq_start = a >= 1 && a <= n_seqs && __ldg(seq_offsets + a - 1) == i; /* [i, offsets[a]) is non-empty */
+                g = gear_of(seed, t);
+                f = (uint8_t)((anchor ? F_ANCHOR : 0) | (seq_end ? F_SEQ_END : 0));
+                if (k >= kSigHalo) flags[i] = f;
+                if (seq_start) f |= F_SEQ_START;
             }
-            hard = flags[i] != 0;
-            cand = mask_bits == 0 || (h >> (64 - mask_bits)) == 0;
+            s_gear[k] = g;
+            s_flag[k] = f;
         }
-        const unsigned hb = __ballot_sync(0xFFFFFFFFu, hard), cb = __ballot_sync(0xFFFFFFFFu, cand);
-        if ((threadIdx.x & 31) == 0) { hard0[i >> 5] = hb; cand0[i >> 5] = cb; }
-    }
-}
-
-/* level 1: bit b of word v <=> level-0 word 32v + b is non-zero (both bitmaps in one pass) */
-__global__ void __launch_bounds__(kT) k_cdc_level1(const uint32_t* __restrict__ hard0, const uint32_t* __restrict__ cand0, int64_t n_words,
-                                                   int64_t n_words_padded, uint32_t* __restrict__ hard1, uint32_t* __restrict__ cand1) {
-    for (int64_t w = blockIdx.x * (int64_t)kT + threadIdx.x; w < n_words_padded; w += (int64_t)gridDim.x * kT) {
-        const unsigned hb = __ballot_sync(0xFFFFFFFFu, w < n_words && hard0[w] != 0);
-        const unsigned cb = __ballot_sync(0xFFFFFFFFu, w < n_words && cand0[w] != 0);
-        if ((threadIdx.x & 31) == 0) { hard1[w >> 5] = hb; cand1[w >> 5] = cb; }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < kSigSpan / kT; ++q) {
+            const int w_in = warp * (kSigSpan / kT) + q;      /* level-0 word inside this span */
+            const int k = kSigHalo + w_in * 32 + lane;
+            const int64_t i = base + k;
+            bool hard = false, cand = false;
+            if (i < n) {
+                uint64_t h = s_gear[k];
+                for (int j = 1; j < 64; ++j) {
+                    if (s_flag[k - j] & F_RESET) break; /* the signature was reset after that token (anchor, end of a sequence, or i - j < 0) */
+                    h += s_gear[k - j] << j;
+                }
+                hard = (s_flag[k] & F_RESET) != 0;
+                cand = mask_bits == 0 || (h >> (64 - mask_bits)) == 0;
+                /* chain seed: a sequence starts here, or the token in front is a hard stop the chains can reach */
+                mark[i] = ((s_flag[k] & F_SEQ_START) || (i >= 1 && i - 1 >= first && (s_flag[k - 1] & F_RESET))) ? 1 : 0;
+            }
+            const unsigned hb = __ballot_sync(0xFFFFFFFFu, hard), cb = __ballot_sync(0xFFFFFFFFu, cand);
+            if (lane == 0) {
+                hard0[v * 32 + w_in] = hb;
+                cand0[v * 32 + w_in] = cb;
+                s_nonzero[0][w_in] = hb != 0;
+                s_nonzero[1][w_in] = cb != 0;
+            }
+        }
+        __syncthreads();
+        if (warp == 0) {
+            const unsigned h1 = __ballot_sync(0xFFFFFFFFu, s_nonzero[0][lane] != 0), c1 = __ballot_sync(0xFFFFFFFFu, s_nonzero[1][lane] != 0);
+            if (lane == 0) { hard1[v] = h1; cand1[v] = c1; }
+        }
+        __syncthreads();
     }
 }
 
@@ -138,6 +186,7 @@ __global__ void __launch_bounds__(kT) k_cdc_next(const uint8_t* __restrict__ fla
                                                  const uint32_t* __restrict__ hard1, const uint32_t* __restrict__ cand0,
                                                  const uint32_t* __restrict__ cand1, int64_t n, int min_size, int max_size,
                                                  int32_t* __restrict__ nxt, uint8_t* __restrict__ kind) {
+    pdl_enter();
     for (int64_t s = blockIdx.x * (int64_t)kT + threadIdx.x; s <= n; s += (int64_t)gridDim.x * kT) {
         if (s == n) { nxt[s] = (int32_t)n; break; } /* terminal: the chain stops here */
         const int64_t i_max = min(s + max_size - 1, n - 1); /* the last token of the pool ends a chunk in any case */
@@ -162,11 +211,14 @@ __global__ void __launch_bounds__(kT) k_cdc_next(const uint8_t* __restrict__ fla
 
 /* One round of pointer doubling: jump_in = next applied 2^k times.  Every marked start marks the start 2^k chunks
  * ahead; marks only ever land on starts of the true chain, so reading a mark set in this same round is harmless.
- * progress[0] (the previous round's) == 0: that round set no new mark, so every chain is complete (a sequence's k-th
- * round is the only one that can mark its chunks 2^k .. 2^(k+1) - 1) and this round has nothing to do. */
+ * After rounds 0 .. k-1 exactly the starts less than 2^k chunks behind a seed are marked.  progress_prev == 0: round
+ * k-1 set no new mark, so the start 2^(k-1) chunks behind every seed was already marked, i.e. lies within 2^(k-1) chunks
+ * of a LATER seed: no start is 2^(k-1) or more chunks behind its nearest seed, every chain is complete and this round
+ * (and every later one) has nothing to do. */
 __global__ void __launch_bounds__(kT) k_cdc_reach(const int32_t* __restrict__ jump_in, int32_t* __restrict__ jump_out, int64_t n,
                                                   uint8_t* __restrict__ mark, const int32_t* __restrict__ progress_prev,
                                                   int32_t* __restrict__ progress) {
+    pdl_enter();
     if (progress_prev && *progress_prev == 0) return;
     bool any = false;
     for (int64_t s = blockIdx.x * (int64_t)kT + threadIdx.x; s <= n; s += (int64_t)gridDim.x * kT) {
@@ -182,8 +234,14 @@ __global__ void __launch_bounds__(kT) k_cdc_reach(const int32_t* __restrict__ ju
 constexpr int kItems = 8;                 /* consecutive positions per thread */
 constexpr int kBlockSpan = kT * kItems;   /* positions per block */
 
-__global__ void __launch_bounds__(kT) k_cdc_count(const uint8_t* __restrict__ mark, int64_t n, int32_t* __restrict__ block_count) {
+/* Marks per block, and -- by the block that finishes last (a ticket from `done`, zeroed by k_cdc_front) -- the
+ * exclusive scan of those counts and the total: n / 2048 entries (512 for a million tokens), a strip per thread. */
+__global__ void __launch_bounds__(kT) k_cdc_count_scan(const uint8_t* __restrict__ mark, int64_t n, int32_t* __restrict__ block_count,
+                                                       int32_t* __restrict__ done, int64_t* __restrict__ n_chunks) {
     __shared__ int s_warp[kT / 32];
+    __shared__ int s_strip[kT];
+    __shared__ bool s_last;
+    pdl_enter();
     const int64_t base = blockIdx.x * (int64_t)kBlockSpan + threadIdx.x * kItems;
     int c = 0;
 #pragma unroll
@@ -196,33 +254,28 @@ __global__ void __launch_bounds__(kT) k_cdc_count(const uint8_t* __restrict__ ma
         int tot = 0;
         for (int w = 0; w < kT / 32; ++w) tot += s_warp[w];
         block_count[blockIdx.x] = tot;
+        __threadfence();
+        s_last = atomicAdd(done, 1) == (int)gridDim.x - 1;
     }
-}
-
-/* exclusive scan of the block counts by ONE block (n / 2048 entries: 512 for a million tokens); also the total */
-__global__ void __launch_bounds__(1024) k_cdc_scan(int32_t* __restrict__ block_count, int n_blocks, int64_t* __restrict__ n_chunks) {
-    __shared__ int s_part[1024];
-    __shared__ int s_carry;
-    if (threadIdx.x == 0) s_carry = 0;
     __syncthreads();
-    for (int base = 0; base < n_blocks; base += 1024) {
-        const int i = base + threadIdx.x;
-        const int v = i < n_blocks ? block_count[i] : 0;
-        s_part[threadIdx.x] = v;
+    if (!s_last) return;
+    __threadfence(); /* the other blocks' counts, published before their tickets */
+    const int n_blocks = (int)gridDim.x;
+    const int per = (n_blocks + kT - 1) / kT, b0 = threadIdx.x * per, b1 = min(b0 + per, n_blocks);
+    volatile int32_t* counts = block_count;
+    int sum = 0;
+    for (int i = b0; i < b1; ++i) sum += counts[i];
+    s_strip[threadIdx.x] = sum;
+    __syncthreads();
+    for (int o = 1; o < kT; o <<= 1) { /* Hillis-Steele inclusive scan of the strip sums */
+        const int add = threadIdx.x >= o ? s_strip[threadIdx.x - o] : 0;
         __syncthreads();
-        for (int o = 1; o < 1024; o <<= 1) { /* Hillis-Steele inclusive scan */
-            const int add = threadIdx.x >= o ? s_part[threadIdx.x - o] : 0;
-            __syncthreads();
-            s_part[threadIdx.x] += add;
-            __syncthreads();
-        }
-        const int carry = s_carry;
-        if (i < n_blocks) block_count[i] = carry + s_part[threadIdx.x] - v;
-        __syncthreads();
-        if (threadIdx.x == 1023) s_carry = carry + s_part[1023];
+        s_strip[threadIdx.x] += add;
         __syncthreads();
     }
-    if (threadIdx.x == 0) *n_chunks = s_carry;
+    int run = s_strip[threadIdx.x] - sum;
+    for (int i = b0; i < b1; ++i) { const int v = counts[i]; counts[i] = run; run += v; }
+    if (threadIdx.x == kT - 1) *n_chunks = s_strip[kT - 1];
 }
 
 __device__ __forceinline__ uint64_t fnv1a_tokens(const int32_t* __restrict__ tokens, int64_t b, int64_t e) { /* D4 */
@@ -238,12 +291,16 @@ __device__ __forceinline__ uint64_t fnv1a_tokens(const int32_t* __restrict__ tok
     return x ? x : 1ull;
 }
 
-/* chunk c = the c-th marked start in position order: end, kind */
-__global__ void __launch_bounds__(kT) k_cdc_emit(const uint8_t* __restrict__ mark, const int32_t* __restrict__ nxt,
-                                                 const uint8_t* __restrict__ kind, int64_t n, const int32_t* __restrict__ block_offset,
-                                                 int64_t capacity, int64_t* __restrict__ chunk_end, int32_t* __restrict__ chunk_kind,
-                                                 int32_t* __restrict__ chunk_start) {
+/* chunk c = the c-th marked start in position order: end, kind and content hash (D4).  FNV-1a is a serial recurrence
+ * (x = (x ^ byte) * prime), so the floor of this kernel is the LONGEST chunk: 4 dependent 64-bit multiplies per token, at
+ * most 4 * max_size in a row, by the thread that owns the chunk's start. */
+__global__ void __launch_bounds__(kT) k_cdc_emit(const int32_t* __restrict__ tokens, const uint8_t* __restrict__ mark,
+                                                 const int32_t* __restrict__ nxt, const uint8_t* __restrict__ kind, int64_t n,
+                                                 const int32_t* __restrict__ block_offset, int64_t capacity,
+                                                 int64_t* __restrict__ chunk_end, int32_t* __restrict__ chunk_kind,
+                                                 uint64_t* __restrict__ chunk_hash) {
     __shared__ int s_warp[kT / 32];
+    pdl_enter();
     const int64_t base = blockIdx.x * (int64_t)kBlockSpan + threadIdx.x * kItems;
     int c = 0;
 #pragma unroll
@@ -263,21 +320,14 @@ __global__ void __launch_bounds__(kT) k_cdc_emit(const uint8_t* __restrict__ mar
         const int64_t s = base + k;
         if (s < n && mark[s]) {
             if (before < capacity) {
-                chunk_end[before] = nxt[s];
+                const int64_t e = nxt[s];
+                chunk_end[before] = e;
                 if (chunk_kind) chunk_kind[before] = kind[s];
-                chunk_start[before] = (int32_t)s;
+                if (chunk_hash) chunk_hash[before] = fnv1a_tokens(tokens, s, e);
             }
             ++before;
         }
     }
-}
-
-__global__ void __launch_bounds__(kT) k_cdc_hash(const int32_t* __restrict__ tokens, const int32_t* __restrict__ chunk_start,
-                                                 const int64_t* __restrict__ chunk_end, const int64_t* __restrict__ n_chunks,
-                                                 int64_t capacity, uint64_t* __restrict__ chunk_hash) {
-    const int64_t m = *n_chunks < capacity ? *n_chunks : capacity;
-    for (int64_t c = blockIdx.x * (int64_t)kT + threadIdx.x; c < m; c += (int64_t)gridDim.x * kT)
-        chunk_hash[c] = fnv1a_tokens(tokens, chunk_start[c], chunk_end[c]);
 }
 
 /* ---- registry (D5) ---- */
@@ -331,6 +381,23 @@ __global__ void __launch_bounds__(kT) k_reg_lookup(const uint64_t* __restrict__ 
     }
 }
 
+/* cudaLaunchKernelEx with the programmatic-stream-serialisation attribute: the kernel may be scheduled while its
+ * predecessor on the stream still runs; its pdl_enter() waits for that predecessor to complete before touching memory. */
+template <class... KArgs, class... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), unsigned grid, unsigned block, cudaStream_t stream, Args... args) {
+    cudaLaunchConfig_t cfg;
+    std::memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(block, 1, 1);
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 unsigned grid_for(int64_t n, int per_block = kT) {
     int64_t b = (n + per_block - 1) / per_block;
     if (b < 1) b = 1;
@@ -358,54 +425,51 @@ extern "C" LEYLINE_API leyline_status leyline_cdc_chunk(const leyline_cdc_params
         CU(cudaMemsetAsync(dev_n_chunks, 0, sizeof(int64_t), stream));
         return LEYLINE_OK;
     }
-    /* scratch: gear u64[n] | jumpA i32[n+1] | jumpB i32[n+1] | nxt i32[n+1] | start i32[n] | blocks i32 | bitmaps (two
-     * levels x two predicates) | progress i32[rounds] | flags, kind, mark */
+    /* scratch: jumpA i32[n+1] | jumpB i32[n+1] | nxt i32[n+1] | blocks i32 | bitmaps (two levels x two predicates) |
+     * progress i32[rounds] + the compaction's ticket | flags, kind, mark.  Every byte that is read is written by a kernel
+     * of this call first (k_cdc_front zeroes the counters), so there is no memset. */
     auto up = [](int64_t x) { return (x + 255) / 256 * 256; };
     const int64_t n_blocks = (n + kBlockSpan - 1) / kBlockSpan;
-    const int64_t n_words = (n + 31) / 32, n_words_padded = (n_words + 31) / 32 * 32, n_words1 = n_words_padded / 32;
-    int rounds = 0; /* the chain has at most n links: ceil(log2(n + 1)) doubling rounds reach all of it */
-    for (int64_t reach = 1; reach <= n; reach <<= 1) ++rounds;
-    const int64_t o_gear = 0, o_ja = o_gear + up(n * 8), o_jb = o_ja + up((n + 1) * 4), o_nxt = o_jb + up((n + 1) * 4),
-                  o_start = o_nxt + up((n + 1) * 4), o_blk = o_start + up(n * 4), o_h0 = o_blk + up(n_blocks * 4),
-                  o_c0 = o_h0 + up(n_words_padded * 4), o_h1 = o_c0 + up(n_words_padded * 4), o_c1 = o_h1 + up((n_words1 + 1) * 4),
-                  o_prog = o_c1 + up((n_words1 + 1) * 4), o_flags = o_prog + up((rounds + 1) * 4), o_kind = o_flags + up(n + 1),
-                  o_mark = o_kind + up(n + 1), total = o_mark + up(n + 1);
+    const int64_t n_super = (n + kSigSpan - 1) / kSigSpan, n_words_padded = n_super * 32;
+    /* Doubling rounds: seeds sit behind every hard stop, and between two seeds every chunk but the last holds >= min_size
+     * tokens, so no start is more than (n - 1) / min_size + 1 chunks behind its seed; rounds 0 .. R-1 reach 2^R - 1. */
+    int rounds = 0;
+    for (int64_t reach = 1, far = (n - 1) / p->min_size + 1; reach <= far; reach <<= 1) ++rounds;
+    const int n_counters = rounds + 1; /* progress[0 .. rounds), then the compaction's ticket */
+    const int64_t o_ja = 0, o_jb = o_ja + up((n + 1) * 4), o_nxt = o_jb + up((n + 1) * 4), o_blk = o_nxt + up((n + 1) * 4),
+                  o_h0 = o_blk + up(n_blocks * 4), o_c0 = o_h0 + up(n_words_padded * 4), o_h1 = o_c0 + up(n_words_padded * 4),
+                  o_c1 = o_h1 + up((n_super + 1) * 4), o_prog = o_c1 + up((n_super + 1) * 4), o_flags = o_prog + up(n_counters * 4),
+                  o_kind = o_flags + up(n + 1), o_mark = o_kind + up(n + 1), total = o_mark + up(n + 1);
     uint8_t* ws = nullptr;
     CU(cudaMallocAsync(reinterpret_cast<void**>(&ws), (size_t)total, stream));
-    uint64_t* gear = reinterpret_cast<uint64_t*>(ws + o_gear);
     int32_t* ja = reinterpret_cast<int32_t*>(ws + o_ja);
     int32_t* jb = reinterpret_cast<int32_t*>(ws + o_jb);
     int32_t* nxt = reinterpret_cast<int32_t*>(ws + o_nxt);
-    int32_t* start = reinterpret_cast<int32_t*>(ws + o_start);
     int32_t* blk = reinterpret_cast<int32_t*>(ws + o_blk);
     uint32_t *hard0 = reinterpret_cast<uint32_t*>(ws + o_h0), *cand0 = reinterpret_cast<uint32_t*>(ws + o_c0),
              *hard1 = reinterpret_cast<uint32_t*>(ws + o_h1), *cand1 = reinterpret_cast<uint32_t*>(ws + o_c1);
     int32_t* progress = reinterpret_cast<int32_t*>(ws + o_prog);
     uint8_t *flags = ws + o_flags, *kind = ws + o_kind, *mark = ws + o_mark;
     leyline_status st = LEYLINE_OK;
-    auto fail = [&]() { cudaFreeAsync(ws, stream); return LEYLINE_E_CUDA; };
-    /* progress | flags | kind | mark are contiguous: one memset (flags must be 0 where k_cdc_flags does not write) */
-    if (!ok(cudaMemsetAsync(progress, 0, (size_t)(total - o_prog), stream))) return fail();
-    k_cdc_flags<<<grid_for(n), kT, 0, stream>>>(dev_tokens, n, dev_anchor_ids, n_anchor_ids, p->seed, gear, flags);
-    k_cdc_seq_ends<<<grid_for(n_seqs), kT, 0, stream>>>(dev_seq_offsets, n_seqs, n, flags, mark);
-    k_cdc_signature<<<grid_for(n_words * 32), kT, 0, stream>>>(gear, flags, n, n_words * 32, p->mask_bits, hard0, cand0);
-    k_cdc_level1<<<grid_for(n_words_padded), kT, 0, stream>>>(hard0, cand0, n_words, n_words_padded, hard1, cand1);
-    k_cdc_next<<<grid_for(n + 1), kT, 0, stream>>>(flags, hard0, hard1, cand0, cand1, n, p->min_size, p->max_size, nxt, kind);
+    bool launched = true;
+    auto go = [&](cudaError_t e) { launched = launched && ok(e); };
+    go(launch_pdl(k_cdc_front, grid_for(n_super, 1), kT, stream, dev_tokens, n, dev_anchor_ids, (int)n_anchor_ids, p->seed,
+                  dev_seq_offsets, (int)n_seqs, (int)p->mask_bits, n_super, flags, mark, hard0, cand0, hard1, cand1, progress, n_counters));
+    go(launch_pdl(k_cdc_next, grid_for(n + 1), kT, stream, (const uint8_t*)flags, (const uint32_t*)hard0, (const uint32_t*)hard1,
+                  (const uint32_t*)cand0, (const uint32_t*)cand1, n, (int)p->min_size, (int)p->max_size, nxt, kind));
     const int32_t* jin = nxt;
     int32_t* jout = ja;
     for (int r = 0; r < rounds; ++r) {
-        k_cdc_reach<<<grid_for(n + 1), kT, 0, stream>>>(jin, jout, n, mark, r ? progress + r - 1 : nullptr, progress + r);
+        go(launch_pdl(k_cdc_reach, grid_for(n + 1), kT, stream, jin, jout, n, mark, (const int32_t*)(r ? progress + r - 1 : nullptr),
+                      progress + r));
         jin = jout;
         jout = (jout == ja) ? jb : ja;
     }
-    k_cdc_count<<<(unsigned)n_blocks, kT, 0, stream>>>(mark, n, blk);
-    k_cdc_scan<<<1, 1024, 0, stream>>>(blk, (int)n_blocks, dev_n_chunks);
-    if (capacity > 0) {
-        k_cdc_emit<<<(unsigned)n_blocks, kT, 0, stream>>>(mark, nxt, kind, n, blk, capacity, dev_chunk_end, dev_chunk_kind, start);
-        if (dev_chunk_hash)
-            k_cdc_hash<<<grid_for(capacity < n ? capacity : n, kT), kT, 0, stream>>>(dev_tokens, start, dev_chunk_end, dev_n_chunks,
-                                                                                  capacity, dev_chunk_hash);
-    }
+    go(launch_pdl(k_cdc_count_scan, (unsigned)n_blocks, kT, stream, (const uint8_t*)mark, n, blk, progress + rounds, dev_n_chunks));
+    if (capacity > 0)
+        go(launch_pdl(k_cdc_emit, (unsigned)n_blocks, kT, stream, dev_tokens, (const uint8_t*)mark, (const int32_t*)nxt,
+                      (const uint8_t*)kind, n, (const int32_t*)blk, capacity, dev_chunk_end, dev_chunk_kind, dev_chunk_hash));
+    if (!launched) st = LEYLINE_E_CUDA;
     if (!ok(cudaGetLastError())) st = LEYLINE_E_CUDA;
     if (!ok(cudaFreeAsync(ws, stream))) st = LEYLINE_E_CUDA;
     return st;

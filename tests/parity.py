@@ -139,13 +139,30 @@ def compare_layer(w: synth.Workload, bm: O.BatchMap, mode: int, old_pool: np.nda
     return stats
 
 
+_PINNED = {"bufs": [], "cap": 0}
+
+
+def _pinned_buffers(nbytes: int, count: int):
+    """`count` pinned host buffers of at least `nbytes` bytes, kept from test to test (page-locking costs about as much
+    as the copies it speeds up, so it is done once per size class, grow-only)."""
+    import torch
+    if _PINNED["cap"] < nbytes or len(_PINNED["bufs"]) < count:
+        _PINNED["bufs"] = []          # drop the old arena before pinning a larger one
+        _PINNED["cap"] = 0
+        _PINNED["bufs"] = [torch.empty(nbytes, dtype=torch.uint8, pin_memory=True) for _ in range(count)]
+        _PINNED["cap"] = nbytes
+    return _PINNED["bufs"][:count]
+
+
 def compare_all_layers(w: synth.Workload, bm: O.BatchMap, mode: int, cache, layers=None, inserts_prefilled: bool = False,
                        checksums=None, max_workers: int | None = None) -> list:
     """Every layer of a device cache against the oracle, whole pool, one layer at a time (SURVEY.md section 7 "never hold
     a whole cache on the host").  The pristine layer is REGENERATED from its seed into a device scratch buffer (the
     generator is counter-based and seeded per layer, so this reproduces the bytes the splice started from; `checksums`,
-    taken before the splice, prove it), so in-place modes need no host snapshot of the cache.  The oracle (GIL-free C)
-    and the numpy comparisons of different layers run on a thread pool, sized to the host's cores and free memory."""
+    taken before the splice, prove it), so in-place modes need no host snapshot of the cache.  Layers cross PCIe through
+    a small ring of pinned bounce buffers (a pageable `.cpu()` runs at ~2 GB/s on the GPU box, pinned at ~55 GB/s); the
+    oracle (GIL-free C) and the numpy comparisons of different layers run on a thread pool, sized to the host's cores
+    and free memory."""
     import os
     import threading
     from concurrent.futures import ThreadPoolExecutor
@@ -159,10 +176,22 @@ def compare_all_layers(w: synth.Workload, bm: O.BatchMap, mode: int, cache, laye
     if max_workers:
         nw = min(nw, max_workers)
     scratch = torch.empty(w.layer_bytes, dtype=torch.uint8, device=cache.device)
+    n_sets = 3 if w.layer_bytes <= (1 << 30) else 2          # pinning costs time too: fewer, when a layer is > 1 GiB
+    pins = _pinned_buffers(w.layer_bytes, 2 * n_sets)
+    free_sets = list(range(n_sets))
+    set_lock = threading.Condition()
     gate = threading.Semaphore(nw + 1)            # layers resident on the host at once
     stats = [None] * len(layers)
 
-    def work(i, l, old, new, repl, scale):
+    def work(i, l, k, landed, repl, scale):
+        try:
+            landed.synchronize()                   # both copies of this layer have reached the pinned buffers
+            old = pins[2 * k][: w.layer_bytes].numpy().copy()
+            new = pins[2 * k + 1][: w.layer_bytes].numpy().copy()
+        finally:
+            with set_lock:
+                free_sets.append(k)
+                set_lock.notify()
         try:
             stats[i] = compare_layer(w, bm, mode, old, new, repl, scale, layer=l, inserts_prefilled=inserts_prefilled)
         finally:
@@ -172,14 +201,20 @@ def compare_all_layers(w: synth.Workload, bm: O.BatchMap, mode: int, cache, laye
         futs = []
         for i, l in enumerate(layers):
             gate.acquire()
+            with set_lock:
+                while not free_sets:
+                    set_lock.wait()
+                k = free_sets.pop()
             scale = synth.fill_layer_(scratch, w, cache.layer_ids[l])
             assert scale == cache.scales[l]
             if checksums is not None:
                 assert int(layer_checksum(scratch)) == checksums[l], f"layer {l}: regenerated bytes differ from the cache's"
-            old = scratch.cpu().numpy()
-            new = cache.pools[l].cpu().numpy()
+            pins[2 * k][: w.layer_bytes].copy_(scratch, non_blocking=True)
+            pins[2 * k + 1][: w.layer_bytes].copy_(cache.pools[l], non_blocking=True)
+            landed = torch.cuda.Event()
+            landed.record()
             repl = None if inserts_prefilled else cache.repl[l].cpu().numpy()
-            futs.append(ex.submit(work, i, l, old, new, repl, scale))
+            futs.append(ex.submit(work, i, l, k, landed, repl, scale))
         for f in futs:
             f.result()
     return stats
