@@ -4,8 +4,9 @@
  * The K_pe arithmetic is Eq. (1) of the paper: K_pe_new = R(C) K_pe, applied per RoPE pair
  *   a' = a cos(phi) - b sin(phi),  b' = b cos(phi) + a sin(phi),  phi = C * theta_i,
  * in fp32 with FMA and one round-to-nearest-even on store (the paper's default AKASHA_PIC_ROTATION_FP32=1,
- * PAPER.md:163, :650).  cos/sin come from the plan's table (fp64 product and trig, rounded once to fp32).
- * No fast-math, no flush-to-zero.
+ * PAPER.md:163, :650).  cos/sin come from the launch's table (fp64 product and trig, kept as an fp32 hi + lo pair); on
+ * bf16 caches an output whose two products cancel is redone with compensated fp32 arithmetic (rot_comp), so every stored
+ * code is within one of the exact result's.  No fast-math, no flush-to-zero.
  */
 #ifndef LEYLINE_DEVICE_COMMON_CUH_
 #define LEYLINE_DEVICE_COMMON_CUH_
@@ -78,10 +79,18 @@ __device__ __forceinline__ int4 ld_stream(const void* p) { /* read-only for the 
                  : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
     return r;
 }
-__device__ __forceinline__ int4 ld_coherent(const void* p) { /* the buffer is also written by this kernel */
+/* the buffer is also written by this kernel.  HALF_LINE: ask L2 to fetch 64 bytes, not the 128-byte line, on a miss --
+ * for bands that are half a line (fp8 MLA: 64 of every 576 bytes), where the other half is latent nobody reads
+ * (measured on B200: a5 on config 5 2.86 -> 3.31 TB/s; SASS: LDG.E.NA.LTC64B.128) */
+template <bool HALF_LINE = false>
+__device__ __forceinline__ int4 ld_coherent(const void* p) {
     int4 r;
-    asm volatile("ld.global.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
-                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p) : "memory");
+    if (HALF_LINE)
+        asm volatile("ld.global.L1::no_allocate.L2::64B.v4.s32 {%0,%1,%2,%3}, [%4];"
+                     : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p) : "memory");
+    else
+        asm volatile("ld.global.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
+                     : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p) : "memory");
     return r;
 }
 __device__ __forceinline__ void st_stream(void* p, const int4& v) {
@@ -173,89 +182,227 @@ __device__ __forceinline__ void load_floats(const float* __restrict__ p, float* 
     }
 }
 
-template <int DT>
-__device__ __forceinline__ int4 rotate_chunk_neox(const int4& mine, const int4& other, const float* __restrict__ cs,
-                                                  const float* __restrict__ sn, float sgn) {
-    constexpr int N = Codec<DT>::kElems;
-    float m[N], o[N], c[N], s[N];
-    Codec<DT>::unpack(mine, m);
-    Codec<DT>::unpack(other, o);
-    load_floats(cs, c, N);
-    load_floats(sn, s, N);
-#pragma unroll
-    for (int e = 0; e < N; ++e) m[e] = __fmaf_rn(o[e], sgn * s[e], m[e] * c[e]);
-    return Codec<DT>::pack(m);
+/* ---- the cos/sin table of a launch ----
+ * Row g (one per distinct non-zero shift) = [cos_hi | sin_hi | cos_lo | sin_lo], H floats each: hi = the fp64 value
+ * rounded to fp32, lo = (fp64 value - hi) rounded to fp32, so hi + lo carries ~48 bits of cos / sin (k_index writes it). */
+constexpr int kTrigParts = 4;
+__device__ __forceinline__ const float* trig_row_of(const float* __restrict__ trig, int32_t g, int H) {
+    return trig + (int64_t)g * kTrigParts * H;
 }
 
+/* ---- THE rotation arithmetic: x*c + y*t, one output element (a' = a c + b (-s), b' = b c + a s) ----
+ * The same function of (x, y, cos, sin) in every kernel, so every mode and mover stores the same bits:
+ *   plain form   p = fl(x c_hi), r = fl(y t_hi + p) (fma): two fp32 roundings plus the roundings of cos / sin themselves,
+ *                absolute error <= ~1.7 * 2^-24 * (|x c| + |y t|) whatever the size of the result;
+ *   on bf16 caches, when |r| < 2^-12 |p| -- the two products cancel -- the compensated form instead:
+ *                q = fl(y t_hi), e = y t_hi - q exactly (fma), r1 = fl(x c_hi + q) (one rounding of the exact sum), and
+ *                the terms left out so far, e + x c_lo + y t_lo, are added last: error ~2^-24 |r| + 2^-47 (|x c| + |y t|).
+ * Without cancellation the plain form's error is below 2^-11 |r|, so the stored bf16 code is at most one from the
+ * oracle's single rounding of the exact value (the fp32 -> bf16 double rounding); with the fix-up the same holds where the
+ * result cancels, and the tolerance needs no cancellation floor (DESIGN.md T).  About one output in 10^4 takes the
+ * compensated form, so cos_lo / sin_lo are fetched only then.  e4m3 codes are 2^-3 apart in relative terms and 2^-9 in
+ * absolute ones: there the plain form is already within one code. */
 template <int DT>
-__device__ __forceinline__ int4 rotate_chunk_interleaved(const int4& mine, const float* __restrict__ cs,
-                                                         const float* __restrict__ sn) {
-    constexpr int N = Codec<DT>::kElems;
-    float m[N], c[N / 2], s[N / 2], r[N];
-    Codec<DT>::unpack(mine, m);
-    load_floats(cs, c, N / 2);
-    load_floats(sn, s, N / 2);
-#pragma unroll
-    for (int q = 0; q < N / 2; ++q) {
-        const float a = m[2 * q], b = m[2 * q + 1];
-        r[2 * q] = __fmaf_rn(b, -s[q], a * c[q]);
-        r[2 * q + 1] = __fmaf_rn(a, s[q], b * c[q]);
+struct Comp { static constexpr bool value = DT == LEYLINE_BF16; };
+
+__device__ __forceinline__ bool cancels(float r, float p) { return fabsf(r) * 4096.0f < fabsf(p); }
+
+__device__ __forceinline__ float rot_plain(float x, float ch, float y, float th, bool& any) {
+    const float p = __fmul_rn(x, ch);
+    const float r = __fmaf_rn(y, th, p);
+    any |= cancels(r, p);
+    return r;
+}
+__device__ __forceinline__ float rot_comp(float x, float ch, float cl, float y, float th, float tl) {
+    const float q = __fmul_rn(y, th);
+    const float e = __fmaf_rn(y, th, -q);
+    const float r1 = __fmaf_rn(x, ch, q);
+    return __fadd_rn(r1, __fmaf_rn(x, cl, __fmaf_rn(y, tl, e)));
+}
+/* the rare path for one output: r = the plain result already formed from (x, y); cl_at / tl_at -> the lo parts */
+__device__ __forceinline__ float rot_fix(float r, float x, float ch, const float* __restrict__ cl_at, float y, float th,
+                                         const float* __restrict__ tl_at, float tl_sign) {
+    if (cancels(r, __fmul_rn(x, ch))) r = rot_comp(x, ch, __ldg(cl_at), y, th, tl_sign * __ldg(tl_at));
+    return r;
+}
+
+/* cos / sin registers of one pair column (see rotate_chunk_pair): the hi parts, and the lo parts when LO */
+template <int N, bool LO>
+struct PairTrig {
+    float c[N], s[N], cl[LO ? N : 1], sl[LO ? N : 1];
+};
+
+/* NeoX: elements [q*N, q*N+N) of the head's cos / sin.  Interleaved: c[0..N/2) / s[0..N/2) belong to chunk q (pairs
+ * q*N/2 ..), c[N/2..N) / s[N/2..N) to chunk q + half (pairs (q+half)*N/2 ..). */
+template <int PAIRING, int N>
+__device__ __forceinline__ void load_pair_part(const float* __restrict__ cos_row, const float* __restrict__ sin_row, int q, int half,
+                                               float* c, float* s) {
+    if (PAIRING == LEYLINE_ROPE_NEOX) {
+        load_floats(cos_row + q * N, c, N);
+        load_floats(sin_row + q * N, s, N);
+    } else {
+        load_floats(cos_row + q * (N / 2), c, N / 2);
+        load_floats(sin_row + q * (N / 2), s, N / 2);
+        load_floats(cos_row + (q + half) * (N / 2), c + N / 2, N / 2);
+        load_floats(sin_row + (q + half) * (N / 2), s + N / 2, N / 2);
     }
-    return Codec<DT>::pack(r);
+}
+template <int PAIRING, int N, bool LO>
+__device__ __forceinline__ void load_pair_trig(const float* __restrict__ trig_row, int H, int q, int half, PairTrig<N, LO>& t) {
+    load_pair_part<PAIRING, N>(trig_row, trig_row + H, q, half, t.c, t.s);
+    if (LO) load_pair_part<PAIRING, N>(trig_row + 2 * H, trig_row + 3 * H, q, half, t.cl, t.sl);
 }
 
 /* ---- the rotation of a PAIR of 16-byte chunks held by one thread (no lane exchange) ----
- * NeoX: `lo` = elements [q*N, q*N+N) of a head's first half, `hi` = the same elements of its second half;
- *       c / s = cos / sin of those N pairs (trig_row + q*N, trig_row + H + q*N).
- * Interleaved: `lo` = chunk q of the head, `hi` = chunk q + half; each holds N/2 whole pairs;
- *       c[0..N/2) / s[0..N/2) belong to lo (pairs q*N/2 ..), c[N/2..N) / s[N/2..N) to hi (pairs (q+half)*N/2 ..).
- * Same fp32 expressions as rotate_chunk_neox / rotate_chunk_interleaved: a' = fma(b, -s, a*c), b' = fma(a, s, b*c). */
-/* The fp32 arithmetic of one (lo, hi) chunk pair: N elements each, cos / sin as described above. */
-template <int PAIRING, int N>
-__device__ __forceinline__ void rotate_pair_f32(float* a, float* b, const float* c, const float* s) {
-    if (PAIRING == LEYLINE_ROPE_NEOX) {
-#pragma unroll
-        for (int e = 0; e < N; ++e) {
-            const float x = a[e], y = b[e];
-            a[e] = __fmaf_rn(y, -s[e], x * c[e]);
-            b[e] = __fmaf_rn(x, s[e], y * c[e]);
-        }
-    } else {
-#pragma unroll
-        for (int q = 0; q < N / 2; ++q) {
-            const float x0 = a[2 * q], y0 = a[2 * q + 1], x1 = b[2 * q], y1 = b[2 * q + 1];
-            a[2 * q] = __fmaf_rn(y0, -s[q], x0 * c[q]);
-            a[2 * q + 1] = __fmaf_rn(x0, s[q], y0 * c[q]);
-            b[2 * q] = __fmaf_rn(y1, -s[N / 2 + q], x1 * c[N / 2 + q]);
-            b[2 * q + 1] = __fmaf_rn(x1, s[N / 2 + q], y1 * c[N / 2 + q]);
-        }
-    }
-}
-
+ * NeoX: `lo` = elements [q*N, q*N+N) of a head's first half, `hi` = the same elements of its second half (N pairs).
+ * Interleaved: `lo` = chunk q of the head, `hi` = chunk q + half; each holds N/2 whole pairs.
+ * t = the hi parts of the column's cos / sin; trig_row / q / half locate the lo parts for the rare compensated outputs.
+ * lo_at / hi_at: where the INPUT chunks can be read again (the global or shared memory they were loaded from, not yet
+ * overwritten): the rare path re-reads them instead of keeping eight more registers alive in every kernel's main loop. */
 template <int DT, int PAIRING>
-__device__ __forceinline__ void rotate_chunk_pair(int4& lo, int4& hi, const float* c, const float* s) {
+__device__ __forceinline__ bool rotate_chunk_pair_plain(int4& lo, int4& hi, const PairTrig<Codec<DT>::kElems, false>& t) {
     constexpr int N = Codec<DT>::kElems;
     float a[N], b[N];
     Codec<DT>::unpack(lo, a);
     Codec<DT>::unpack(hi, b);
-    rotate_pair_f32<PAIRING, N>(a, b, c, s);
+    bool any = false;
+    if (PAIRING == LEYLINE_ROPE_NEOX) {
+#pragma unroll
+        for (int e = 0; e < N; ++e) {
+            const float x = a[e], y = b[e];
+            a[e] = rot_plain(x, t.c[e], y, -t.s[e], any);
+            b[e] = rot_plain(y, t.c[e], x, t.s[e], any);
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < N / 2; ++k) {
+            const float x0 = a[2 * k], y0 = a[2 * k + 1], x1 = b[2 * k], y1 = b[2 * k + 1];
+            a[2 * k] = rot_plain(x0, t.c[k], y0, -t.s[k], any);
+            a[2 * k + 1] = rot_plain(y0, t.c[k], x0, t.s[k], any);
+            b[2 * k] = rot_plain(x1, t.c[N / 2 + k], y1, -t.s[N / 2 + k], any);
+            b[2 * k + 1] = rot_plain(y1, t.c[N / 2 + k], x1, t.s[N / 2 + k], any);
+        }
+    }
+    lo = Codec<DT>::pack(a);
+    hi = Codec<DT>::pack(b);
+    return any;
+}
+
+/* the rare path: the whole chunk pair again from its inputs, every output through the plain form and the fix-up; cos /
+ * sin come from the table */
+template <int DT, int PAIRING>
+__device__ __forceinline__ void rotate_chunk_pair_careful(int4& lo, int4& hi, const float* __restrict__ trig_row, int H, int q, int half,
+                                                          const int4 lo_in, const int4 hi_in) {
+    constexpr int N = Codec<DT>::kElems;
+    float x[N], y[N];
+    Codec<DT>::unpack(lo_in, x);
+    Codec<DT>::unpack(hi_in, y);
+    const float* __restrict__ sn = trig_row + H;
+    const float* __restrict__ cl = trig_row + 2 * H;
+    const float* __restrict__ sl = trig_row + 3 * H;
+    bool unused = false;
+    float a[N], b[N];
+    if (PAIRING == LEYLINE_ROPE_NEOX) {
+#pragma unroll
+        for (int e = 0; e < N; ++e) {
+            const int i = q * N + e;
+            const float c = __ldg(trig_row + i), s = __ldg(sn + i);
+            a[e] = rot_fix(rot_plain(x[e], c, y[e], -s, unused), x[e], c, cl + i, y[e], -s, sl + i, -1.0f);
+            b[e] = rot_fix(rot_plain(y[e], c, x[e], s, unused), y[e], c, cl + i, x[e], s, sl + i, 1.0f);
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < N / 2; ++k) {
+            const int i0 = q * (N / 2) + k, i1 = (q + half) * (N / 2) + k;
+            const float c0 = __ldg(trig_row + i0), s0 = __ldg(sn + i0), c1 = __ldg(trig_row + i1), s1 = __ldg(sn + i1);
+            a[2 * k] = rot_fix(rot_plain(x[2 * k], c0, x[2 * k + 1], -s0, unused), x[2 * k], c0, cl + i0, x[2 * k + 1], -s0, sl + i0, -1.0f);
+            a[2 * k + 1] = rot_fix(rot_plain(x[2 * k + 1], c0, x[2 * k], s0, unused), x[2 * k + 1], c0, cl + i0, x[2 * k], s0, sl + i0, 1.0f);
+            b[2 * k] = rot_fix(rot_plain(y[2 * k], c1, y[2 * k + 1], -s1, unused), y[2 * k], c1, cl + i1, y[2 * k + 1], -s1, sl + i1, -1.0f);
+            b[2 * k + 1] = rot_fix(rot_plain(y[2 * k + 1], c1, y[2 * k], s1, unused), y[2 * k + 1], c1, cl + i1, y[2 * k], s1, sl + i1, 1.0f);
+        }
+    }
     lo = Codec<DT>::pack(a);
     hi = Codec<DT>::pack(b);
 }
 
-/* cos / sin registers for pair column q of a head (see rotate_chunk_pair): N floats each. */
 template <int DT, int PAIRING>
-__device__ __forceinline__ void load_pair_trig(const float* __restrict__ trig_row, int H, int q, int half, float* c, float* s) {
-    constexpr int N = Codec<DT>::kElems;
+__device__ __forceinline__ void rotate_chunk_pair(int4& lo, int4& hi, const PairTrig<Codec<DT>::kElems, false>& t,
+                                                  const float* __restrict__ trig_row, int H, int q, int half,
+                                                  const int4* lo_at, const int4* hi_at) {
+    if (rotate_chunk_pair_plain<DT, PAIRING>(lo, hi, t) && Comp<DT>::value)
+        rotate_chunk_pair_careful<DT, PAIRING>(lo, hi, trig_row, H, q, half, *lo_at, *hi_at);
+}
+
+/* The fp32 master band (k_rotate_master): fp32 inputs, always the compensated form (N pairs as for rotate_chunk_pair). */
+template <int PAIRING, int N>
+__device__ __forceinline__ void rotate_pair_master(float* a, float* b, const PairTrig<N, true>& t) {
     if (PAIRING == LEYLINE_ROPE_NEOX) {
-        load_floats(trig_row + q * N, c, N);
-        load_floats(trig_row + H + q * N, s, N);
+#pragma unroll
+        for (int e = 0; e < N; ++e) {
+            const float x = a[e], y = b[e];
+            a[e] = rot_comp(x, t.c[e], t.cl[e], y, -t.s[e], -t.sl[e]);
+            b[e] = rot_comp(y, t.c[e], t.cl[e], x, t.s[e], t.sl[e]);
+        }
     } else {
-        load_floats(trig_row + q * (N / 2), c, N / 2);
-        load_floats(trig_row + H + q * (N / 2), s, N / 2);
-        load_floats(trig_row + (q + half) * (N / 2), c + N / 2, N / 2);
-        load_floats(trig_row + H + (q + half) * (N / 2), s + N / 2, N / 2);
+#pragma unroll
+        for (int k = 0; k < N / 2; ++k) {
+            const float x0 = a[2 * k], y0 = a[2 * k + 1], x1 = b[2 * k], y1 = b[2 * k + 1];
+            a[2 * k] = rot_comp(x0, t.c[k], t.cl[k], y0, -t.s[k], -t.sl[k]);
+            a[2 * k + 1] = rot_comp(y0, t.c[k], t.cl[k], x0, t.s[k], t.sl[k]);
+            b[2 * k] = rot_comp(x1, t.c[N / 2 + k], t.cl[N / 2 + k], y1, -t.s[N / 2 + k], -t.sl[N / 2 + k]);
+            b[2 * k + 1] = rot_comp(y1, t.c[N / 2 + k], t.cl[N / 2 + k], x1, t.s[N / 2 + k], t.sl[N / 2 + k]);
+        }
     }
+}
+
+/* ---- one 16-byte chunk per thread (k_move_rows, k_rotate_band_tma) ----
+ * NeoX (pair i <-> i+H): `mine` holds N elements of one half, `other` the same elements of the other half (fetched from
+ * the partner lane); sgn = -1 for the first half (a' = a c - b s), +1 for the second (b' = b c + a s).
+ * `first` = index of the chunk's first pair in the head's cos / sin. */
+template <int DT>
+__device__ __forceinline__ int4 rotate_chunk_neox(const int4& mine, const int4& other, const float* __restrict__ trig_row, int H,
+                                                  int first, float sgn) {
+    constexpr int N = Codec<DT>::kElems;
+    float m[N], o[N], c[N], s[N], r[N];
+    Codec<DT>::unpack(mine, m);
+    Codec<DT>::unpack(other, o);
+    load_floats(trig_row + first, c, N);
+    load_floats(trig_row + H + first, s, N);
+    bool any = false;
+#pragma unroll
+    for (int e = 0; e < N; ++e) r[e] = rot_plain(m[e], c[e], o[e], sgn * s[e], any);
+    if (Comp<DT>::value && any) {
+#pragma unroll
+        for (int e = 0; e < N; ++e)
+            r[e] = rot_fix(r[e], m[e], c[e], trig_row + 2 * H + first + e, o[e], sgn * s[e], trig_row + 3 * H + first + e, sgn);
+    }
+    return Codec<DT>::pack(r);
+}
+
+/* Interleaved (pair 2i <-> 2i+1): both elements of a pair sit in `mine`; `first` = index of the chunk's first pair. */
+template <int DT>
+__device__ __forceinline__ int4 rotate_chunk_interleaved(const int4& mine, const float* __restrict__ trig_row, int H, int first) {
+    constexpr int N = Codec<DT>::kElems;
+    float m[N], c[N / 2], s[N / 2], r[N];
+    Codec<DT>::unpack(mine, m);
+    load_floats(trig_row + first, c, N / 2);
+    load_floats(trig_row + H + first, s, N / 2);
+    bool any = false;
+#pragma unroll
+    for (int k = 0; k < N / 2; ++k) {
+        r[2 * k] = rot_plain(m[2 * k], c[k], m[2 * k + 1], -s[k], any);
+        r[2 * k + 1] = rot_plain(m[2 * k + 1], c[k], m[2 * k], s[k], any);
+    }
+    if (Comp<DT>::value && any) {
+#pragma unroll
+        for (int k = 0; k < N / 2; ++k) {
+            const float* cl = trig_row + 2 * H + first + k;
+            const float* sl = trig_row + 3 * H + first + k;
+            r[2 * k] = rot_fix(r[2 * k], m[2 * k], c[k], cl, m[2 * k + 1], -s[k], sl, -1.0f);
+            r[2 * k + 1] = rot_fix(r[2 * k + 1], m[2 * k + 1], c[k], cl, m[2 * k], s[k], sl, 1.0f);
+        }
+    }
+    return Codec<DT>::pack(r);
 }
 
 __device__ __forceinline__ int4 shfl_xor_int4(const int4& v, int lane_mask) {
@@ -274,11 +421,10 @@ __device__ __forceinline__ int4 rotate_band_chunk(const int4& mine, int j, int n
         const int4 other = shfl_xor_int4(mine, half);
         if (!active) return mine;
         const int jj = j & (half - 1);
-        const float sgn = j < half ? -1.0f : 1.0f;
-        return rotate_chunk_neox<DT>(mine, other, trig_row + jj * N, trig_row + H + jj * N, sgn);
+        return rotate_chunk_neox<DT>(mine, other, trig_row, H, jj * N, j < half ? -1.0f : 1.0f);
     } else {
         if (!active) return mine;
-        return rotate_chunk_interleaved<DT>(mine, trig_row + j * (N / 2), trig_row + H + j * (N / 2));
+        return rotate_chunk_interleaved<DT>(mine, trig_row, H, j * (N / 2));
     }
 }
 

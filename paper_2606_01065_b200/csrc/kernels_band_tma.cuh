@@ -120,7 +120,7 @@ k_rotate_band_tma(const __grid_constant__ MoveParams p, const __grid_constant__ 
             const BandStageInfo info = s_info[stage];
             if (info.n_rows == 0) break;
             uint8_t* stage_mem = smem + (size_t)stage * stage_bytes;
-            const float* __restrict__ trig_row = p.trig + (int64_t)info.trig * 2 * p.H;
+            const float* __restrict__ trig_row = trig_row_of(p.trig, info.trig, p.H);
             if (lane_exchange) {
                 /* thread <-> 16-byte chunk of the dense stage, consecutive lanes on consecutive chunks */
                 const int total = info.n_rows * p.band_chunks;
@@ -143,9 +143,9 @@ k_rotate_band_tma(const __grid_constant__ MoveParams p, const __grid_constant__ 
                     const int head = col / half, q = col - head * half;
                     int4* band = reinterpret_cast<int4*>(stage_mem + (size_t)r * band_bytes) + head * p.head_chunks + q;
                     int4 lo = band[0], hi = band[half];
-                    float c[N], sn[N];
-                    load_pair_trig<DT, PAIRING>(trig_row, p.H, q, half, c, sn);
-                    rotate_chunk_pair<DT, PAIRING>(lo, hi, c, sn);
+                    PairTrig<N, false> tr;
+                    load_pair_trig<PAIRING>(trig_row, p.H, q, half, tr);
+                    rotate_chunk_pair<DT, PAIRING>(lo, hi, tr, trig_row, p.H, q, half, band, band + half);
                     band[0] = lo;
                     band[half] = hi;
                 }

@@ -89,7 +89,7 @@ __device__ __forceinline__ void named_bar_sync(int id, int n_threads) {
  * round-robin over stages, and a last warp that watches the stages land in order. */
 constexpr int kBulkConsumerWarps = 4;
 constexpr int kBulkWideConsumerWarps = 12; /* default when the band is most of the row (measured: 8 -> 12 is +9 % on GQA) */
-constexpr int kBulkMaxConsumerWarps = 16;
+constexpr int kBulkMaxConsumerWarps = 12; /* more never helped (measured), and the launch bound caps the registers per thread */
 constexpr int kBulkHazardWarps = 4;
 constexpr int kBulkMaxThreadsWS = 32 * (1 + kBulkMaxConsumerWarps);
 constexpr int kBulkMaxThreadsHazard = kBulkMaxThreadsWS + 32 * (kBulkHazardWarps + 1);
@@ -231,6 +231,16 @@ k_move_bulk(const __grid_constant__ MoveParams p, const int n_stages, const int 
 
     /* ---------------- consumers: rotate the K_pe band in shared memory, then warp 1 stores the runs ---------------- */
     const int cwarp = warp - 1;
+    const int half = p.head_chunks >> 1;  /* pair columns per head */
+    const int cols = p.n_heads * half;    /* pair columns per row */
+    /* unit u = (row u / cols, column u % cols), units strided by n_consumers: when cols divides n_consumers a thread
+     * keeps its column, and with it its cos / sin registers */
+    const bool fixed_col = n_consumers % cols == 0;
+    const int my_u = cwarp * 32 + lane, my_r0 = my_u / cols, my_col = my_u - my_r0 * cols;
+    const int my_q = my_col % half, my_chunk = (my_col / half) * p.head_chunks + my_q;
+    const int rows_per_pass = n_consumers / cols;
+    PairTrig<N, false> tr;
+    int have_trig = -1;
     for (int it = 0;; ++it) {
         const int stage = it % n_stages;
         mbar_wait(&s_full[stage], (uint32_t)((it / n_stages) & 1));
@@ -241,20 +251,37 @@ k_move_bulk(const __grid_constant__ MoveParams p, const int n_stages, const int 
         if (info.trig >= 0) {
             /* a unit = (row, pair column): chunk q of a head's first half and its partner q + half, both rotated by
              * this thread (rotate_chunk_pair), so no two threads touch the same bytes */
-            const float* __restrict__ trig_row = p.trig + (int64_t)info.trig * 2 * p.H;
-            const int half = p.head_chunks >> 1;
-            const int cols = p.n_heads * half;
             const int total = n_rows * cols;
-            for (int u = cwarp * 32 + lane; u < total; u += n_consumers) {
-                const int r = u / cols, col = u - r * cols;
-                const int head = col / half, q = col - head * half;
-                int4* band = reinterpret_cast<int4*>(stage_mem + (size_t)r * row_bytes + band0) + head * p.head_chunks + q;
-                int4 lo = band[0], hi = band[half];
-                float c[N], sn[N];
-                load_pair_trig<DT, PAIRING>(trig_row, p.H, q, half, c, sn);
-                rotate_chunk_pair<DT, PAIRING>(lo, hi, c, sn);
-                band[0] = lo;
-                band[half] = hi;
+            if (fixed_col) {
+                /* the thread's pair column is the same for all of its units: its cos / sin stay in registers and are
+                 * reloaded only when the tile belongs to another segment (the table reads through L1 were as many
+                 * bytes as the band itself) */
+                const float* __restrict__ trig_row = trig_row_of(p.trig, info.trig, p.H);
+                if (info.trig != have_trig) {
+                    load_pair_trig<PAIRING>(trig_row, p.H, my_q, half, tr);
+                    have_trig = info.trig;
+                }
+                int4* band = reinterpret_cast<int4*>(stage_mem + (size_t)my_r0 * row_bytes + band0) + my_chunk;
+                const size_t step = (size_t)rows_per_pass * row_bytes / 16;
+                for (int r = my_r0; r < n_rows; r += rows_per_pass, band += step) {
+                    int4 lo = band[0], hi = band[half];
+                    rotate_chunk_pair<DT, PAIRING>(lo, hi, tr, trig_row, p.H, my_q, half, band, band + half);
+                    band[0] = lo;
+                    band[half] = hi;
+                }
+            } else {
+                const float* __restrict__ trig_row = trig_row_of(p.trig, info.trig, p.H);
+                for (int u = cwarp * 32 + lane; u < total; u += n_consumers) {
+                    const int r = u / cols, col = u - r * cols;
+                    const int head = col / half, q = col - head * half;
+                    int4* band = reinterpret_cast<int4*>(stage_mem + (size_t)r * row_bytes + band0) + head * p.head_chunks + q;
+                    int4 lo = band[0], hi = band[half];
+                    PairTrig<N, false> t1;
+                    load_pair_trig<PAIRING>(trig_row, p.H, q, half, t1);
+                    rotate_chunk_pair<DT, PAIRING>(lo, hi, t1, trig_row, p.H, q, half, band, band + half);
+                    band[0] = lo;
+                    band[half] = hi;
+                }
             }
             fence_proxy_async_smem(); /* generic-proxy writes -> visible to the bulk store's async-proxy reads */
         }

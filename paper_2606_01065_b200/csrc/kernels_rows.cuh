@@ -53,8 +53,12 @@ __global__ void __launch_bounds__(kThreads) k_index(const IndexParams a, const I
             const int g = u / tp.H, i = u - g * tp.H;
             double sn, cs;
             sincos((double)tp.shifts[g] * (double)tp.inv_freq[i], &sn, &cs);
-            tp.out[(int64_t)g * 2 * tp.H + i] = (float)cs;
-            tp.out[(int64_t)g * 2 * tp.H + tp.H + i] = (float)sn;
+            const float ch = (float)cs, sh = (float)sn; /* hi: the value rounded once to fp32; lo: what that rounding dropped */
+            float* row = tp.out + (int64_t)g * kTrigParts * tp.H;
+            row[i] = ch;
+            row[tp.H + i] = sh;
+            row[2 * tp.H + i] = (float)(cs - (double)ch);
+            row[3 * tp.H + i] = (float)(sn - (double)sh);
         }
     }
 }
@@ -111,7 +115,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_move_rows(const __grid_constant
         }
 
         /* rotate (tile-uniform branch: C = 0 segments, head copies and inserts are byte copies, G19) */
-        if (t.trig >= 0) band = rotate_band_chunk<DT, PAIRING>(band, bj, NB, p.trig + (int64_t)t.trig * 2 * p.H, p.H, has_band);
+        if (t.trig >= 0) band = rotate_band_chunk<DT, PAIRING>(band, bj, NB, trig_row_of(p.trig, t.trig, p.H), p.H, has_band);
 
         if (HAZARD) {
             /* rule M2: publish "loaded", then wait for the tiles whose source rows this tile overwrites.
@@ -151,15 +155,20 @@ __global__ void __launch_bounds__(kThreads, 3) k_move_rows(const __grid_constant
  * 1152-B bf16 MLA row), so the kernel is a strided gather/scatter: what matters is many independent 16-byte
  * accesses in flight and few instructions around them.  A work unit is a (row, pair column): the 16-byte chunk q
  * of a head's first half and its partner chunk q + half, both held by ONE thread, so no lane exchange, no shared
- * memory and no barrier is needed.  One block handles one (tile, layer) item = kRotUnroll units per thread, all
+ * memory and no barrier is needed.  One block handles one (tile, layer) item = kRotUnroll (4) units per thread, all
  * loads issued before the first store; items are assigned round-robin (static), no atomics.
  * FIXED: the pair columns per row divide the block size, so a thread keeps one column (cos/sin stay in registers). */
-constexpr int kRotUnroll = 4;
-static_assert(kRotUnitsPerItem == kThreads * kRotUnroll, "the planner sizes ROTATE_ONLY tiles to <= this many units");
+static_assert(rot_units_per_item(2) == kThreads * kRotUnrollBf16 && rot_units_per_item(1) == kThreads * kRotUnrollFp8,
+              "the planner sizes ROTATE_ONLY tiles to <= the units a block holds");
 
+#ifndef LEYLINE_ROT_BF16_CTAS
+#define LEYLINE_ROT_BF16_CTAS 2
+#endif
 template <int DT, int PAIRING, bool FIXED>
-__global__ void __launch_bounds__(kThreads, DT == LEYLINE_FP8_E4M3 ? 2 : 3) k_rotate_band(const __grid_constant__ MoveParams p) {
+__global__ void __launch_bounds__(kThreads, DT == LEYLINE_FP8_E4M3 ? 2 : LEYLINE_ROT_BF16_CTAS) k_rotate_band(const __grid_constant__ MoveParams p) {
     constexpr int N = Codec<DT>::kElems;
+    constexpr int kRotUnroll = DT == LEYLINE_BF16 ? kRotUnrollBf16 : kRotUnrollFp8;
+    constexpr bool HALF_LINE = DT == LEYLINE_FP8_E4M3; /* fp8 rows are 4.5 lines: a narrow band shares its line with latent */
     const int tid = threadIdx.x;
     const int half = p.head_chunks >> 1;   /* pair columns per head */
     const int cols = p.n_heads * half;     /* pair columns per row */
@@ -196,17 +205,18 @@ __global__ void __launch_bounds__(kThreads, DT == LEYLINE_FP8_E4M3 ? 2 : 3) k_ro
         for (; item < p.n_items; item += gridDim.x) {
             const DevTile t = p.tiles[p.tile_begin + (int)(item / p.n_layers)];
             uint8_t* __restrict__ base = p.dst[(int)(item % p.n_layers)];
-            const float* __restrict__ trig_row = p.trig + (int64_t)t.trig * 2 * p.H;
+            const float* __restrict__ trig_row = trig_row_of(p.trig, t.trig, p.H);
             const int total = t.n_rows * cols;
             for (int u = tid; u < total; u += kThreads) {
                 const int r = u / cols, col = u - r * cols;
                 const int head = col / half, q = col - head * half;
                 uint8_t* a = base + slot_of(p.tabs, t.src_tab, t.src_pos + r, p.page_shift) * p.stride + band0 +
                              (int64_t)(head * p.head_chunks + q) * 16;
-                int4 lo = ld_coherent(a), hi = ld_coherent(a + half * 16);
-                float c[N], s[N];
-                load_pair_trig<DT, PAIRING>(trig_row, p.H, q, half, c, s);
-                rotate_chunk_pair<DT, PAIRING>(lo, hi, c, s);
+                int4 lo = ld_coherent<HALF_LINE>(a), hi = ld_coherent<HALF_LINE>(a + half * 16);
+                PairTrig<N, false> t1;
+                load_pair_trig<PAIRING>(trig_row, p.H, q, half, t1);
+                rotate_chunk_pair<DT, PAIRING>(lo, hi, t1, trig_row, p.H, q, half, reinterpret_cast<const int4*>(a),
+                                               reinterpret_cast<const int4*>(a) + half);
                 st_stream(a, lo);
                 st_stream(a + half * 16, hi);
             }
@@ -222,23 +232,29 @@ __global__ void __launch_bounds__(kThreads, DT == LEYLINE_FP8_E4M3 ? 2 : 3) k_ro
             addr[k] = nullptr;
             if (cur.slot[k] >= 0) {
                 addr[k] = base + (int64_t)cur.slot[k] * p.stride + band0 + (int64_t)chunk[k] * 16;
-                lo[k] = ld_coherent(addr[k]);
-                hi[k] = ld_coherent(addr[k] + half * 16);
+                lo[k] = ld_coherent<HALF_LINE>(addr[k]);
+                hi[k] = ld_coherent<HALF_LINE>(addr[k] + half * 16);
             }
         }
         const long long next = item + gridDim.x;
         const bool more = next < p.n_items;
         if (more) resolve(next, nxt);
-        const float* __restrict__ trig_row = p.trig + (int64_t)cur.trig * 2 * p.H;
-        float c[N], s[N];
-        if (FIXED) load_pair_trig<DT, PAIRING>(trig_row, p.H, qs[0], half, c, s);
+        const float* __restrict__ trig_row = trig_row_of(p.trig, cur.trig, p.H);
+        PairTrig<N, false> tr;
+        if (FIXED) load_pair_trig<PAIRING>(trig_row, p.H, qs[0], half, tr);
 #pragma unroll
         for (int k = 0; k < kRotUnroll; ++k) {
             if (addr[k]) {
-                if (!FIXED) load_pair_trig<DT, PAIRING>(trig_row, p.H, qs[k], half, c, s);
-                rotate_chunk_pair<DT, PAIRING>(lo[k], hi[k], c, s);
-                st_stream(addr[k], lo[k]);
-                st_stream(addr[k] + half * 16, hi[k]);
+                if (!FIXED) load_pair_trig<PAIRING>(trig_row, p.H, qs[k], half, tr);
+                int4 lo_out = lo[k], hi_out = hi[k];
+                const bool redo = rotate_chunk_pair_plain<DT, PAIRING>(lo_out, hi_out, tr);
+                st_stream(addr[k], lo_out);          /* never waits for the test */
+                st_stream(addr[k] + half * 16, hi_out);
+                if (redo && Comp<DT>::value) {       /* about one unit in 1000: again from its inputs, with the fix-up */
+                    rotate_chunk_pair_careful<DT, PAIRING>(lo_out, hi_out, trig_row, p.H, qs[k], half, lo[k], hi[k]);
+                    st_stream(addr[k], lo_out);
+                    st_stream(addr[k] + half * 16, hi_out);
+                }
             }
         }
         if (!more) break;
@@ -297,7 +313,7 @@ __global__ void __launch_bounds__(kThreads) k_rotate_master(const __grid_constan
         const int layer = (int)(item % p.n_layers);
         uint8_t* __restrict__ pool = p.dst[layer];
         float* __restrict__ master = reinterpret_cast<float*>(const_cast<uint8_t*>(p.src[layer]));
-        const float* __restrict__ trig_row = p.trig + (int64_t)t.trig * 2 * p.H;
+        const float* __restrict__ trig_row = trig_row_of(p.trig, t.trig, p.H);
         const int total = t.n_rows * cols;
         for (int u = tid; u < total; u += kThreads) {
             const int r = u / cols, col = u - r * cols;
@@ -306,15 +322,16 @@ __global__ void __launch_bounds__(kThreads) k_rotate_master(const __grid_constan
             const int64_t slot = slot_of(p.tabs, t.src_tab, t.src_pos + r, p.page_shift);
             float4* mlo = reinterpret_cast<float4*>(master + slot * band_elems + (int64_t)chunk * N);
             float4* mhi = mlo + half * (N / 4);
-            float a[N], b[N], c[N], s[N];
+            float a[N], b[N];
+            PairTrig<N, true> tr;
 #pragma unroll
             for (int k = 0; k < N / 4; ++k) {
                 const float4 x = mlo[k], y = mhi[k];
                 a[4 * k] = x.x; a[4 * k + 1] = x.y; a[4 * k + 2] = x.z; a[4 * k + 3] = x.w;
                 b[4 * k] = y.x; b[4 * k + 1] = y.y; b[4 * k + 2] = y.z; b[4 * k + 3] = y.w;
             }
-            load_pair_trig<LEYLINE_BF16, PAIRING>(trig_row, p.H, q, half, c, s);
-            rotate_pair_f32<PAIRING, N>(a, b, c, s);
+            load_pair_trig<PAIRING>(trig_row, p.H, q, half, tr);
+            rotate_pair_master<PAIRING, N>(a, b, tr);
 #pragma unroll
             for (int k = 0; k < N / 4; ++k) {
                 mlo[k] = make_float4(a[4 * k], a[4 * k + 1], a[4 * k + 2], a[4 * k + 3]);
@@ -355,9 +372,10 @@ __global__ void __launch_bounds__(kThreads) k_rotate_master(const __grid_constan
 /* The access pattern of a5 with everything else taken away (leyline_probe_band_update): `band_chunks` 16-byte chunks at
  * byte `band0` of every `stride`-byte row of ONE contiguous buffer are read, changed (one integer add) and written back
  * in place.  No page table, no tiles, no rotation; consecutive lanes take consecutive chunks of a row (full-line
- * requests), U independent loads per thread are issued before the first store.  What this reaches is what the memory
- * system gives ANY kernel on that pattern; bench.py reports it next to k_rotate_band. */
-template <int U>
+ * requests), U independent loads per thread are issued before the first store; HALF_LINE as in k_rotate_band (the host
+ * picks it when the band is not a whole number of 128-byte lines).  What this reaches is what the memory system gives
+ * ANY kernel on that pattern; bench.py reports it next to k_rotate_band. */
+template <int U, bool HALF_LINE>
 __global__ void __launch_bounds__(kThreads) k_probe_band_update(uint8_t* __restrict__ base, const long long n_rows, const long long stride,
                                                                 const int band0, const int band_chunks) {
     const long long total = n_rows * band_chunks;
@@ -372,7 +390,7 @@ __global__ void __launch_bounds__(kThreads) k_probe_band_update(uint8_t* __restr
             if (u < total) {
                 const long long r = u / band_chunks;
                 a[k] = base + r * stride + band0 + (int)(u - r * band_chunks) * 16;
-                v[k] = ld_coherent(a[k]);
+                v[k] = ld_coherent<HALF_LINE>(a[k]);
             }
         }
 #pragma unroll

@@ -154,10 +154,10 @@ int choose_tile_rows(const leyline_cache_desc& c, int E, const leyline_tuning& t
     return (int)std::max<int64_t>(1, std::min(want, cap));
 }
 
-/* Rows per k_rotate_band work item: as many as fill the block's kRotUnitsPerItem (row, pair column) units. */
+/* Rows per k_rotate_band work item: as many as fill the block's rot_units_per_item (row, pair column) units. */
 int choose_rot_tile_rows(const leyline_cache_desc& c, int E, const leyline_tuning& t) {
     const int64_t cols = (int64_t)heads_of(c) * ((int64_t)c.rope_dim * E / 32);
-    int64_t cap = std::max<int64_t>(1, leyline::kRotUnitsPerItem / cols);
+    int64_t cap = std::max<int64_t>(1, leyline::rot_units_per_item(E) / cols);
     int64_t want = t.tile_rows > 0 ? t.tile_rows : cap;
     return (int)std::max<int64_t>(1, std::min(want, cap));
 }

@@ -35,9 +35,14 @@ static_assert(sizeof(DevTile) == 48, "DevTile layout");
 enum : int32_t { TILE_SRC_REPL = 1, TILE_DST_TOKEN = 2,
                  TILE_DST_IS_SRC = 4 /* rows are written back to the slots they were read from (in-place rotation) */ };
 
-/* k_rotate_band (a5): (row, pair column) units one block handles = 256 threads x 4; ROTATE_ONLY tiles hold at most
- * this many units, i.e. rot_tile_rows = kRotUnitsPerItem / (rope_heads * head_chunks / 2) rows. */
-constexpr int kRotUnitsPerItem = 1024;
+/* k_rotate_band (a5): (row, pair column) units one block handles = 256 threads x the units a thread keeps in flight;
+ * ROTATE_ONLY tiles hold at most this many units, i.e. rot_tile_rows = rot_units_per_item / (rope_heads * head_chunks / 2)
+ * rows. */
+#ifndef LEYLINE_ROT_BF16_UNROLL
+#define LEYLINE_ROT_BF16_UNROLL 6
+#endif
+constexpr int kRotUnrollBf16 = LEYLINE_ROT_BF16_UNROLL, kRotUnrollFp8 = 4;
+constexpr int rot_units_per_item(int elem_bytes) { return 256 * (elem_bytes == 2 ? kRotUnrollBf16 : kRotUnrollFp8); }
 
 /* k_rotate_band_tma (a5 on paged pools): the band of up to kRotTmaBoxRows consecutive slots is one 2-D TMA box. */
 constexpr int kRotTmaBoxRows = 64;

@@ -140,7 +140,7 @@ leyline_status upload_tables(leyline_plan_s* pl, int dev, cudaStream_t stream) {
     pl->off_slot_runs = place((int64_t)pl->slot_runs.size() * sizeof(IdxRun));
     pl->off_page_runs = place((int64_t)pl->page_runs.size() * sizeof(IdxRun));
     const int64_t upload_bytes = off > 0 ? off : 256;
-    pl->off_trig = place((int64_t)pl->trig_shifts.size() * 2 * (int64_t)pl->inv_freq.size() * sizeof(float));
+    pl->off_trig = place((int64_t)pl->trig_shifts.size() * kTrigParts * (int64_t)pl->inv_freq.size() * sizeof(float)); /* cos, sin: hi and lo parts */
     pl->blob_bytes = off > 0 ? off : 256;
     const int64_t n_flags = pl->mode == LEYLINE_INPLACE_MOVE ? pl->info.n_tiles * pl->desc.n_layers : 0;
     pl->scratch_bytes = 256 + align_up(n_flags * (int64_t)sizeof(int32_t), 256);
@@ -700,9 +700,11 @@ extern "C" LEYLINE_API leyline_status leyline_plan_trig_table_device(const leyli
     g_last_error.clear();
     if (!pl || (!out && !pl->trig_shifts.empty()) || !pl->trig_ready || !pl->d_blob) return LEYLINE_E_INVALID;
     if (pl->trig_shifts.empty()) return LEYLINE_OK;
-    const size_t bytes = pl->trig_shifts.size() * 2 * pl->inv_freq.size() * sizeof(float);
+    /* the hi parts [cos | sin] of every row: the fp64 values rounded once to fp32, which is what the host query evaluates */
+    const size_t row = 2 * pl->inv_freq.size() * sizeof(float);
     cudaStream_t stream = static_cast<cudaStream_t>(pl->last_stream);
-    CU(cudaMemcpyAsync(out, blob_at<float>(pl, pl->off_trig), bytes, cudaMemcpyDeviceToHost, stream));
+    CU(cudaMemcpy2DAsync(out, row, blob_at<float>(pl, pl->off_trig), kTrigParts / 2 * row, row, pl->trig_shifts.size(),
+                         cudaMemcpyDeviceToHost, stream));
     CU(cudaStreamSynchronize(stream));
     return LEYLINE_OK;
 } LEYLINE_CATCH_STATUS
@@ -721,7 +723,9 @@ extern "C" LEYLINE_API leyline_status leyline_probe_band_update(void* dev_buf, i
     leyline_status st = device_info(&dev);
     if (st != LEYLINE_OK) return st;
     const int per_sm = ctas_per_sm > 0 ? ctas_per_sm : 8;
-    k_probe_band_update<8><<<(unsigned)(g_dev.sms * per_sm), kThreads, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+    const bool half_line = ((row_stride_bytes | band_offset_bytes | band_bytes) & 127) != 0; /* bands that share lines with bytes nobody reads */
+    auto probe = half_line ? k_probe_band_update<8, true> : k_probe_band_update<8, false>;
+    probe<<<(unsigned)(g_dev.sms * per_sm), kThreads, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
         static_cast<uint8_t*>(dev_buf), n_rows, row_stride_bytes, band_offset_bytes, band_bytes / 16);
     CU(cudaGetLastError());
     return LEYLINE_OK;

@@ -4,8 +4,10 @@ The bar (BASELINE.json north_star):
   * bit-exact: new sequence lengths, page-table rows, token-level slot list, released list, free ids consumed,
     segments, every pool byte outside rotated K_pe bands (moved latent, C = 0 segments, replacement rows, and
     every byte the mode never writes -- other requests, free pool, prefix pages, released pages);
-  * rotated bf16 K_pe: ordinal distance <= 2 bf16 ulp, or |g - o| <= 2^-20 * rho where the result cancels
-    (rho = norm of the input pair; fp32 rounding error does not shrink with the result);
+  * rotated bf16 K_pe: ordinal distance <= 2 bf16 ulp for EVERY element (north_star's bound as written, +0 == -0).
+    Round 1 needed a cancellation floor |g - o| <= 2^-20 * rho here (plain fp32 arithmetic has an absolute error of
+    ~2^-24 * rho, which is many bf16 steps where a cos - b sin cancels: about one element in 10^6); since round 2 the
+    kernels redo such outputs with compensated fp32 arithmetic and the floor is gone.  Measured: never more than 1;
   * rotated fp8 K_pe: ordinal distance <= 1 e4m3 code (+0 == -0).
 """
 from __future__ import annotations
@@ -111,25 +113,9 @@ def compare_layer(w: synth.Workload, bm: O.BatchMap, mode: int, old_pool: np.nda
     if w.dtype == synth.DT_BF16:
         gbits, obits = gb.view(np.uint16), ob.view(np.uint16)
         dist = np.abs(_bf16_ord(gbits) - _bf16_ord(obits))
-        bad = dist > 2
-        n_floor = 0
-        if bad.any():
-            # cancellation floor: |g - o| <= 2^-20 * rho, rho = norm of the INPUT pair
-            ib = np.ascontiguousarray(old_pool.reshape(-1, stride)[old_s, band0:]).view(np.uint16)
-            x = _bf16_val(ib).reshape(len(old_s), w.rope_heads, w.rope_dim)      # pairs live inside a head
-            H = w.rope_dim // 2
-            if pairing == synth.NEOX:
-                rho_h = np.sqrt(x[..., :H] ** 2 + x[..., H:] ** 2)
-                rho = np.concatenate([rho_h, rho_h], axis=-1)
-            else:
-                rho_h = np.sqrt(x[..., 0::2] ** 2 + x[..., 1::2] ** 2)
-                rho = np.repeat(rho_h, 2, axis=-1)
-            rho = rho.reshape(len(old_s), -1)
-            err = np.abs(_bf16_val(gbits) - _bf16_val(obits))
-            floor_ok = err <= (2.0 ** -20) * rho
-            n_floor = int((bad & floor_ok).sum())
-            really_bad = bad & ~floor_ok
-            assert not really_bad.any(), f"{int(really_bad.sum())} rotated bf16 elements beyond 2 ulp and the 2^-20 rho floor"
+        n_floor = 0                    # kept in the statistics: the cancellation floor of round 1 no longer exists
+        assert dist.max() <= 2, (f"layer {layer}: {int((dist > 2).sum())} rotated bf16 elements beyond 2 ulp "
+                                 f"(max ordinal distance {int(dist.max())})")
         stats.update(rotated_elems=int(dist.size), max_ord=int(dist.max()), frac_equal=float((dist == 0).mean()),
                      n_floor=n_floor)
     else:
@@ -176,7 +162,7 @@ def compare_all_layers(w: synth.Workload, bm: O.BatchMap, mode: int, cache, laye
     if max_workers:
         nw = min(nw, max_workers)
     scratch = torch.empty(w.layer_bytes, dtype=torch.uint8, device=cache.device)
-    n_sets = 3 if w.layer_bytes <= (1 << 30) else 2          # pinning costs time too: fewer, when a layer is > 1 GiB
+    n_sets = min(len(layers), 3 if w.layer_bytes <= (1 << 30) else 2)    # pinning costs time too: fewer, when a layer is > 1 GiB
     pins = _pinned_buffers(w.layer_bytes, 2 * n_sets)
     free_sets = list(range(n_sets))
     set_lock = threading.Condition()

@@ -326,10 +326,10 @@ def test_gpu_master_chain_matches_oracle(n):
             assert (np.abs(g_m - o_m) <= 4 * 2.0 ** -24 * np.concatenate([rho, rho], axis=1) + 1e-30).all()
             g_p, o_p = pools[l].cpu().numpy().reshape(-1, ch.stride), sync_p[l].reshape(-1, ch.stride)
             np.testing.assert_array_equal(g_p[:, :DC * 2], o_p[:, :DC * 2])                     # latent untouched
-            # tolerance T of DESIGN.md: 1 bf16 code, or the cancellation floor 2^-20 * rho where the result is tiny
-            far = np.abs(_bf16_ord(g_p[:, DC * 2:].copy().view(np.uint16)) - _bf16_ord(o_p[:, DC * 2:].copy().view(np.uint16))) > 1
-            gv, ov = from_storage(g_p, O.BF16)[:, DC:], from_storage(o_p, O.BF16)[:, DC:]
-            assert (np.abs(gv - ov)[far] <= (2.0 ** -20 * np.concatenate([rho, rho], axis=1))[far]).all()
+            # the master is rotated with compensated fp32 arithmetic (accurate relative to the result), so the band --
+            # one RNE of the master -- is within 1 bf16 code of the oracle's everywhere: no cancellation floor
+            dist = np.abs(_bf16_ord(g_p[:, DC * 2:].copy().view(np.uint16)) - _bf16_ord(o_p[:, DC * 2:].copy().view(np.uint16)))
+            assert dist.max() <= 1
         plan.close()
         S += d
     del keep
