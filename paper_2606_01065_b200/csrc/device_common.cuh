@@ -202,8 +202,11 @@ __device__ __forceinline__ const float* trig_row_of(const float* __restrict__ tr
  * result cancels, and the tolerance needs no cancellation floor (DESIGN.md T).  About one output in 10^4 takes the
  * compensated form, so cos_lo / sin_lo are fetched only then.  e4m3 codes are 2^-3 apart in relative terms and 2^-9 in
  * absolute ones: there the plain form is already within one code. */
+#ifndef LEYLINE_COMPENSATE
+#define LEYLINE_COMPENSATE 1 /* 0: experiment builds only (what the tests report without the fix-up) */
+#endif
 template <int DT>
-struct Comp { static constexpr bool value = DT == LEYLINE_BF16; };
+struct Comp { static constexpr bool value = DT == LEYLINE_BF16 && LEYLINE_COMPENSATE != 0; };
 
 __device__ __forceinline__ bool cancels(float r, float p) { return fabsf(r) * 4096.0f < fabsf(p); }
 

@@ -753,3 +753,96 @@ def test_hazard_mover_random_batches_all_layers(seed):
                        directives=dirs, seed=seed, pool_factor=1.3).finalize()
     assert any(d[3] > d[2] - d[1] for d in dirs) and any(d[3] < d[2] - d[1] for d in dirs)
     run_and_compare(w, O.INPLACE_MOVE)
+
+
+# ----------------------------------------------------------------------------- the rotation arithmetic itself
+
+def _band_by_position(w, cache, idx, n_tok):
+    """K_pe band bytes of every layer in NEW logical order ([layer][token][band bytes])."""
+    slots = idx[:n_tok].long()
+    band0 = w.latent_dim * w.elem_bytes
+    return torch.stack([p.view(-1, w.row_bytes)[slots, band0:] for p in cache.pools]).cpu().numpy()
+
+
+@pytest.mark.parametrize("dtype", [synth.DT_BF16, synth.DT_FP8])
+@pytest.mark.parametrize("pairing", [synth.NEOX, synth.INTERLEAVED])
+def test_every_mode_and_mover_stores_the_same_bits(dtype, pairing):
+    """One function of (a, b, cos, sin) in every kernel (device_common.cuh, rot_plain / rot_comp): FRESH, INPLACE_MOVE and
+    ROTATE_ONLY, through the bulk mover, the row mover, the strided band kernel and the TMA band kernel, must leave
+    bit-identical K_pe at every new position -- not merely results that each sit within tolerance of the oracle."""
+    w = synth.Workload("same_bits", 3, [3000, 1, 2777], 16, dtype=dtype, pairing=pairing, inv_freq=synth.yarn_inv_freq(),
+                       directives=[(0, 5, 5, 40, 0, 0), (0, 100, 900, 3, 0, 0), (0, 1500, 1501, 333, 0, 0),
+                                   (2, 0, 17, 500, 0, 0), (2, 1000, 1700, 0, 0, 0), (2, 2776, 2777, 2, 0, 0)],
+                       seed=19, pool_factor=3.0, extra_pages=80).finalize()
+    from paper_2606_01065_b200 import binding as B
+    from paper_2606_01065_b200 import harness
+    ref = None
+    for mode, tuning in ((O.FRESH, {"kernel": 2}), (O.FRESH, {"kernel": 1}), (O.INPLACE_MOVE, {"kernel": 2}),
+                         (O.INPLACE_MOVE, {"kernel": 1}), (O.ROTATE_ONLY, {"rotate_kernel": 1}), (O.ROTATE_ONLY, {"rotate_kernel": 2})):
+        B.leyline_set_tuning(**tuning)
+        try:
+            cache = harness.DeviceCache(w, "cuda:0")
+            plan, pt, idx = harness.run_workload(cache, mode)
+            torch.cuda.synchronize()
+        finally:
+            B.leyline_set_tuning()
+        got = _band_by_position(w, cache, idx, int(plan.info.total_new_tokens))
+        plan.close()
+        if ref is None:
+            ref = got
+        else:
+            np.testing.assert_array_equal(got, ref, err_msg=f"mode {MODE_NAME[mode]} tuning {tuning}")
+
+
+@pytest.mark.parametrize("mode,tuning", [(O.FRESH, {"kernel": 2}), (O.FRESH, {"kernel": 1}), (O.INPLACE_MOVE, {"kernel": 2}),
+                                         (O.ROTATE_ONLY, {"rotate_kernel": 1}), (O.ROTATE_ONLY, {"rotate_kernel": 2})])
+@pytest.mark.parametrize("pairing", [synth.NEOX, synth.INTERLEAVED])
+def test_cancelling_pairs_stay_within_one_code(mode, tuning, pairing):
+    """Inputs built so that a cos - b sin (or b cos + a sin) nearly cancels in EVERY pair of every downstream row: for the
+    segment's shift C the stored pair is (r sin phi, r cos phi) / (r cos phi, -r sin phi) rounded to bf16, phi = C theta_i,
+    so one output is what the input rounding left over, 2^-9 rho and less.  Plain fp32 arithmetic (absolute error
+    ~2^-24 rho) is several bf16 codes off on the deepest of these; the kernels' compensated form must stay within ONE
+    code of the oracle on all of them -- the path that one element in 10^4 of ordinary data takes, taken here by most."""
+    from paper_2606_01065_b200 import binding as B
+    from paper_2606_01065_b200 import harness
+    L, s0, e0, rl = 4096 + 37, 700, 1900, 333
+    w = synth.Workload("cancel", 2, [L], 16, pairing=pairing, inv_freq=synth.yarn_inv_freq(),
+                       directives=[(0, s0, e0, rl, 0, 0)], seed=23, pool_factor=3.0, extra_pages=40).finalize()
+    C = rl - (e0 - s0)
+    H = w.rope_dim // 2
+    phi = float(C) * w.inv_freq.astype(np.float64)
+    rng = np.random.default_rng(5)
+    n_down = L - e0
+    r = np.exp(rng.uniform(np.log(0.05), np.log(8.0), size=(w.n_layers, n_down, H)))
+    flip = rng.integers(0, 2, size=(w.n_layers, n_down, H)).astype(bool)
+    a = np.where(flip, r * np.cos(phi), r * np.sin(phi))      # flip: b' = b cos + a sin cancels; else a' = a cos - b sin
+    b = np.where(flip, -r * np.sin(phi), r * np.cos(phi))
+    band = np.concatenate([a, b], axis=-1) if pairing == synth.NEOX else np.stack([a, b], axis=-1).reshape(w.n_layers, n_down, 2 * H)
+    B.leyline_set_tuning(**tuning)
+    try:
+        cache = harness.DeviceCache(w, "cuda:0")
+        old_slots = torch.from_numpy(w.pages.astype(np.int64)[np.arange(e0, L) // 16] * 16 + np.arange(e0, L) % 16).to("cuda:0")
+        for l in range(w.n_layers):
+            rows = cache.pools[l].view(torch.bfloat16).view(-1, w.row_elems)
+            rows[old_slots, w.latent_dim:] = torch.from_numpy(band[l]).to("cuda:0").to(torch.bfloat16)
+        old = [p.cpu().numpy() for p in cache.pools]
+        plan, pt, idx = harness.run_workload(cache, mode)
+        torch.cuda.synchronize()
+    finally:
+        B.leyline_set_tuning()
+    bm = oracle_plan(w, mode)
+    assert_plan_equal(plan, bm, mode)
+    deep = 0
+    for l in range(w.n_layers):
+        st = compare_layer(w, bm, mode, old[l], cache.pools[l].cpu().numpy(), cache.repl[l].cpu().numpy(), 1.0, layer=l)
+        assert st["max_ord"] <= 1, st
+        # how deep the cancellation goes on this input: the oracle's own output against the pair's norm
+        want = O.splice_layer(w.dtype, pairing, w.latent_dim, w.rope_dim, w.row_bytes, w.inv_freq, 1.0, old[l],
+                              cache.repl[l].cpu().numpy(), bm, n_heads=w.rope_heads).reshape(-1, w.row_bytes)
+        new_s, _ = __import__("parity").rotated_rows(w, bm, mode)
+        out = (want[new_s, w.latent_dim * 2:].copy().view(np.uint16).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+        x, y = (out[:, :H], out[:, H:]) if pairing == synth.NEOX else (out[:, 0::2], out[:, 1::2])
+        rho = np.sqrt(x * x + y * y)
+        deep += int((np.minimum(np.abs(x), np.abs(y)) < 2.0 ** -13 * rho).sum())
+    plan.close()
+    assert deep > 1000, f"the constructed input does not cancel deeply enough to exercise the compensated form ({deep})"

@@ -142,9 +142,10 @@ def check_tiles_cover(plan, bm, w, mode):
     seen = {}
     for t_i, t in enumerate(tiles):
         is_repl = bool(t.flags & B.TILE_SRC_REPL)
-        if mode == B.ROTATE_ONLY and not is_repl:     # a5 work items: <= 1024 (row, pair column) units per block
-            assert 1 <= t.n_rows <= plan.info.rot_tile_rows
-            assert (plan.info.rot_tile_rows * w.rope_heads * (w.rope_dim * w.elem_bytes // 32) <= 1024 or plan.info.rot_tile_rows == 1
+        if mode == B.ROTATE_ONLY and not is_repl:     # a5 work items: the (row, pair column) units one block holds =
+            assert 1 <= t.n_rows <= plan.info.rot_tile_rows     # 256 threads x 6 (bf16) / 4 (fp8) units in flight
+            units = 1536 if w.elem_bytes == 2 else 1024
+            assert (plan.info.rot_tile_rows * w.rope_heads * (w.rope_dim * w.elem_bytes // 32) <= units or plan.info.rot_tile_rows == 1
                     or plan.info.mover == 2)
         else:
             assert 1 <= t.n_rows <= plan.info.tile_rows <= 64
