@@ -104,6 +104,11 @@ class ClockSampler:
                                           "-i", str(self.index), "-lms", "20"], stdout=subprocess.PIPE, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
+            # nvidia-smi initialises NVML for some hundred ms and holds driver locks meanwhile, which stalls this
+            # process's CUDA calls: wait for its first sample so that none of that falls into a timed region
+            t0 = time.perf_counter()
+            while not self.rows and self.proc.poll() is None and time.perf_counter() - t0 < 3.0:
+                time.sleep(0.01)
         except Exception:
             self.proc = None
 

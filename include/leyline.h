@@ -256,10 +256,12 @@ LEYLINE_API leyline_status leyline_plan_tiles(const leyline_plan_t* plan, leylin
 LEYLINE_API leyline_status leyline_plan_trig_shifts(const leyline_plan_t* plan, int64_t* out /*[n_trig]*/);
 /* The table itself, [n_trig][2][rope_dim/2] fp32: cos then sin of C_g * theta_i (fp64 product and trig, rounded once),
  * evaluated on the HOST by this call (libm).  The launches never upload it: the index kernel of every launch evaluates
- * the same expression in fp64 on the device (CUDA's sincos, <= 2 ulp of fp64 before the one rounding to fp32), which
- * takes the 32 fp64 sincos per distinct shift off the host's critical path (hundreds of shifts per call in the paper's
- * chunk workload).  leyline_plan_trig_table_device copies the device's table back (after the plan has
- * been launched and its stream synchronised; LEYLINE_E_INVALID before that) so that the two can be compared. */
+ * the same expression in fp64 on the device (CUDA's sincos, <= 2 ulp of fp64), which takes the 32 fp64 sincos per
+ * distinct shift off the host's critical path (hundreds of shifts per call in the paper's chunk workload),
+ * and keeps every value as an fp32 hi + lo pair: hi is the value rounded once to fp32 -- what this call returns -- and
+ * lo what that rounding dropped, used only where an output's two products cancel (bf16 caches).
+ * leyline_plan_trig_table_device copies the device's hi parts back (after the plan has been launched and its stream
+ * synchronised; LEYLINE_E_INVALID before that) so that the two evaluations can be compared. */
 LEYLINE_API leyline_status leyline_plan_trig_table(const leyline_plan_t* plan, float* out);
 LEYLINE_API leyline_status leyline_plan_trig_table_device(const leyline_plan_t* plan, float* out);
 
