@@ -499,6 +499,9 @@ def extra_workloads(peak: float, device_index: int, skip=()):
         torch.cuda.synchronize()
         for m in modes:
             out[f"{key}_{m}"] = extra_line(cache, w, m, peak, device_index)
+        if key == "appB":    # the paper's own shape: what ONE call costs a server (plan + upload + kernels, idle GPU)
+            for m in modes:
+                out[f"{key}_{m}_single_call_idle_gpu"] = time_single_calls(cache, w, MODES[m])
         del cache
         gc.collect()
         torch.cuda.empty_cache()

@@ -375,3 +375,41 @@ def test_gpu_chunker_long_unanchored_sequences(mn, mx, bits):
     np.testing.assert_array_equal(end, o_end)
     np.testing.assert_array_equal(kind, o_kind)
     np.testing.assert_array_equal(hsh, o_hash)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("offsets", [[5, 3, 900, 20], [-7, 10**12, 4], [0, 0, 0, 0], [123, 123], [2000, 0]])
+def test_gpu_chunker_survives_garbage_device_offsets(offsets):
+    """The sequence offsets live on the device, so the host cannot validate them (leyline_cdc.h asks for ascending
+    offsets from 0 to n_tokens).  Whatever they hold, the call must stay inside its buffers: nothing at or past
+    `capacity` is written (canaries on both sides of every output), the count stays within [0, n_tokens], reported ends
+    are non-decreasing positions in (0, n_tokens], and a well-formed call right behind it is unaffected."""
+    import torch
+    from paper_2606_01065_b200 import binding as B
+    dev = torch.device("cuda:0")
+    rng = np.random.default_rng(len(offsets))
+    n, cap, pad = 2000, 300, 64
+    t = random_prompt(rng, n, anchor_every=40)
+    td = torch.from_numpy(t).to(dev)
+    off = torch.tensor(offsets, dtype=torch.int64, device=dev)
+    an = torch.tensor(sorted(ANCHORS), dtype=torch.int32, device=dev)
+    end = torch.full((cap + 2 * pad,), -7, dtype=torch.int64, device=dev)
+    hsh = torch.full((cap + 2 * pad,), -7, dtype=torch.int64, device=dev)
+    kind = torch.full((cap + 2 * pad,), -7, dtype=torch.int32, device=dev)
+    cnt = torch.full((3,), -7, dtype=torch.int64, device=dev)
+    B.leyline_cdc_chunk(B.CdcParams(SEED, MIN, MAX, BITS, 0), td, n, off, len(offsets) - 1, an, len(ANCHORS),
+                        end[pad:], hsh[pad:], kind[pad:], cap, cnt[1:])
+    torch.cuda.synchronize()
+    for buf in (end, hsh, kind):
+        assert bool((buf[:pad] == -7).all()) and bool((buf[pad + cap:] == -7).all())
+    assert int(cnt[0]) == -7 and int(cnt[2]) == -7
+    c = int(cnt[1])
+    assert 0 <= c <= n
+    e = end[pad:pad + min(c, cap)].cpu().numpy()
+    assert ((e > 0) & (e <= n)).all() and (np.diff(e) >= 0).all()
+    # the library is still in working order
+    c2, end2, hsh2, kind2, _ = gpu_chunk(t, None, ANCHORS, SEED, MIN, MAX, BITS)
+    o_end, o_hash, o_kind = OC.chunk(SEED, MIN, MAX, BITS, t, None, ANCHORS)
+    assert c2 == len(o_end)
+    np.testing.assert_array_equal(end2, o_end)
+    np.testing.assert_array_equal(hsh2, o_hash)
