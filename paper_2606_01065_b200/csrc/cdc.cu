@@ -29,7 +29,6 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include <cstring>
 #include <string>
 
 #include "leyline_cdc.h"
@@ -385,8 +384,7 @@ __global__ void __launch_bounds__(kT) k_reg_lookup(const uint64_t* __restrict__ 
  * predecessor on the stream still runs; its pdl_enter() waits for that predecessor to complete before touching memory. */
 template <class... KArgs, class... Args>
 cudaError_t launch_pdl(void (*kernel)(KArgs...), unsigned grid, unsigned block, cudaStream_t stream, Args... args) {
-    cudaLaunchConfig_t cfg;
-    std::memset(&cfg, 0, sizeof(cfg));
+    cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid, 1, 1);
     cfg.blockDim = dim3(block, 1, 1);
     cfg.stream = stream;

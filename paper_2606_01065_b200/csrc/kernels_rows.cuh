@@ -155,9 +155,13 @@ __global__ void __launch_bounds__(kThreads, 3) k_move_rows(const __grid_constant
  * 1152-B bf16 MLA row), so the kernel is a strided gather/scatter: what matters is many independent 16-byte
  * accesses in flight and few instructions around them.  A work unit is a (row, pair column): the 16-byte chunk q
  * of a head's first half and its partner chunk q + half, both held by ONE thread, so no lane exchange, no shared
- * memory and no barrier is needed.  One block handles one (tile, layer) item = kRotUnroll (4) units per thread, all
- * loads issued before the first store; items are assigned round-robin (static), no atomics.
- * FIXED: the pair columns per row divide the block size, so a thread keeps one column (cos/sin stay in registers). */
+ * memory and no barrier is needed.  One block handles one (tile, layer) item = kRotUnroll units per thread (6 on bf16,
+ * 4 on fp8; two CTAs per SM either way), all loads issued before the first store; items are assigned round-robin
+ * (static), no atomics.  The plain result of a unit is stored at once; the rare unit with an output that cancels is then
+ * redone from its inputs (still in registers) with the compensated form and stored again (device_common.cuh).
+ * FIXED: the pair columns per row divide the block size, so a thread keeps one column (cos/sin stay in registers).
+ * LEYLINE_ROT_BF16_CTAS / LEYLINE_ROT_BF16_UNROLL are build-time knobs kept for measurements (3 x 4,
+ * 2 x 4, 2 x 5, 2 x 6 and 2 x 8 were timed; 2 x 6 is the default). */
 static_assert(rot_units_per_item(2) == kThreads * kRotUnrollBf16 && rot_units_per_item(1) == kThreads * kRotUnrollFp8,
               "the planner sizes ROTATE_ONLY tiles to <= the units a block holds");
 
