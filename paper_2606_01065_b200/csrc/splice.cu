@@ -44,6 +44,7 @@ struct PinnedBuf { void* p = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; 
 std::mutex g_pin_mu;
 std::vector<PinnedBuf> g_pin_pool;
 constexpr size_t kPinMinBytes = 256 << 10, kPinMaxPooled = 32;
+constexpr int kPinPrefill = 5;
 
 PinnedBuf pin_acquire(size_t bytes, int dev) {
     {
@@ -57,17 +58,31 @@ PinnedBuf pin_acquire(size_t bytes, int dev) {
         }
         (void)cudaGetLastError(); /* cudaErrorNotReady from a busy buffer is not an error */
     }
-    PinnedBuf b;
     size_t cap = kPinMinBytes;
     while (cap < bytes) cap <<= 1;
-    if (cudaHostAlloc(&b.p, cap, cudaHostAllocDefault) != cudaSuccess ||
-        cudaEventCreateWithFlags(&b.ev, cudaEventDisableTiming) != cudaSuccess) {
-        (void)cudaGetLastError();
-        if (b.p) cudaFreeHost(b.p);
-        return PinnedBuf{}; /* caller falls back to a pageable source */
+    auto make = [&](PinnedBuf& b) {
+        if (cudaHostAlloc(&b.p, cap, cudaHostAllocDefault) != cudaSuccess ||
+            cudaEventCreateWithFlags(&b.ev, cudaEventDisableTiming) != cudaSuccess) {
+            (void)cudaGetLastError();
+            if (b.p) cudaFreeHost(b.p);
+            b = PinnedBuf{};
+            return false;
+        }
+        b.cap = cap;
+        b.device = dev;
+        return true;
+    };
+    PinnedBuf b;
+    if (!make(b)) return PinnedBuf{}; /* caller falls back to a pageable source */
+    /* cudaHostAlloc waits for the device and takes milliseconds: when this size class runs dry, stock it for the calls
+     * that follow (a server keeps a few plans in flight), so that the stall is paid once, not once per concurrent plan */
+    for (int extra = 0; extra < kPinPrefill; ++extra) {
+        PinnedBuf e;
+        if (!make(e)) break;
+        std::lock_guard<std::mutex> lk(g_pin_mu);
+        if (g_pin_pool.size() >= kPinMaxPooled) { cudaEventDestroy(e.ev); cudaFreeHost(e.p); break; }
+        g_pin_pool.push_back(e);
     }
-    b.cap = cap;
-    b.device = dev;
     return b;
 }
 
@@ -83,6 +98,7 @@ void pin_release(PinnedBuf b, cudaStream_t stream) {
 /* ---- device memory for the plan tables ----
  * A pool of its own: allocations made on the copy stream (leyline_plan_prefetch) must never pick up a dependency
  * on the work of the stream that freed the previous plan's tables, which the default pool is allowed to insert. */
+constexpr size_t kPlanPoolReserveBytes = 128u << 20;
 struct PlanPool { int device = -1; cudaMemPool_t pool = nullptr; cudaStream_t copy_stream = nullptr; };
 std::deque<PlanPool> g_plan_pools; /* deque: references stay valid as devices are added */
 
@@ -108,6 +124,15 @@ PlanPool* plan_pool(int dev) {
         cudaMemPoolDestroy(pp.pool);
         return nullptr;
     }
+    /* Growing the pool (cuMemCreate + map) stalls every stream of the device for tens of ms, and it would happen at some
+     * later call, whenever one more plan is in flight than ever before: reserve once, now.  The block goes straight back
+     * to the pool, which keeps it (release threshold above) and carves the plans' tables out of it. */
+    void* reserve = nullptr;
+    if (cudaMallocFromPoolAsync(&reserve, kPlanPoolReserveBytes, pp.pool, pp.copy_stream) == cudaSuccess) {
+        cudaFreeAsync(reserve, pp.copy_stream);
+        cudaStreamSynchronize(pp.copy_stream);
+    }
+    (void)cudaGetLastError();
     g_plan_pools.push_back(pp);
     return &g_plan_pools.back();
 }
