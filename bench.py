@@ -321,9 +321,17 @@ def time_discovery(dev, with_oracle: bool, n_sessions: int = 16, prompt_len: int
         prm = B.CdcParams(0x5EED, mn, mx, bits, 0)
         gpu_ms = timed(lambda: B.leyline_cdc_chunk(prm, td, n, off, n_sessions, an, len(anchors), end, hsh, kind, n, cnt), reps)
         c = int(cnt.item())
+        one = []                      # ONE call on an idle GPU, synchronised on both sides (what a server's request path sees)
+        for _ in range(12):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            B.leyline_cdc_chunk(prm, td, n, off, n_sessions, an, len(anchors), end, hsh, kind, n, cnt)
+            torch.cuda.synchronize()
+            one.append((time.perf_counter() - t0) * 1e6)
         launches = launches_of(n, mn)
         line = {"chunks": c, "gpu_ms": gpu_ms, "gpu_Mtok_per_s": n / gpu_ms / 1e3, "launches_per_call": launches,
-                "launch_bound_ms": launches * launch_ms, "over_launch_bound": gpu_ms / (launches * launch_ms)}
+                "launch_bound_ms": launches * launch_ms, "over_launch_bound": gpu_ms / (launches * launch_ms),
+                "one_synchronised_call_us": float(np.median(one[2:]))}
         if with_oracle:      # part of the cpu_baseline leg: the oracle's sequential chunker timed on the host beside it
             from oracle import cdc as OC
             t0 = time.perf_counter()

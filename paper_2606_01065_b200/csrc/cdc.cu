@@ -439,7 +439,12 @@ extern "C" LEYLINE_API leyline_status leyline_cdc_chunk(const leyline_cdc_params
                   o_c1 = o_h1 + up((n_super + 1) * 4), o_prog = o_c1 + up((n_super + 1) * 4), o_flags = o_prog + up(n_counters * 4),
                   o_kind = o_flags + up(n + 1), o_mark = o_kind + up(n + 1), total = o_mark + up(n + 1);
     uint8_t* ws = nullptr;
-    CU(cudaMallocAsync(reinterpret_cast<void**>(&ws), (size_t)total, stream));
+    /* from the library's own pool: the default pool hands its memory back to the driver at every synchronisation, and the
+     * next call would pay for mapping it again (measured: one synchronised call 515 -> 124 us) */
+    if (cudaMemPool_t pool = static_cast<cudaMemPool_t>(leyline::scratch_mem_pool()))
+        CU(cudaMallocFromPoolAsync(reinterpret_cast<void**>(&ws), (size_t)total, pool, stream));
+    else
+        CU(cudaMallocAsync(reinterpret_cast<void**>(&ws), (size_t)total, stream));
     int32_t* ja = reinterpret_cast<int32_t*>(ws + o_ja);
     int32_t* jb = reinterpret_cast<int32_t*>(ws + o_jb);
     int32_t* nxt = reinterpret_cast<int32_t*>(ws + o_nxt);

@@ -756,6 +756,13 @@ extern "C" LEYLINE_API leyline_status leyline_probe_band_update(void* dev_buf, i
     return LEYLINE_OK;
 } LEYLINE_CATCH_STATUS
 
+void* leyline::scratch_mem_pool() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+    PlanPool* pp = plan_pool(dev);
+    return pp ? static_cast<void*>(pp->pool) : nullptr;
+}
+
 void leyline::plan_release_device(leyline_plan_s* pl) {
     if (pl->ev_start) cudaEventDestroy(static_cast<cudaEvent_t>(pl->ev_start));
     if (pl->ev_stop) cudaEventDestroy(static_cast<cudaEvent_t>(pl->ev_stop));
