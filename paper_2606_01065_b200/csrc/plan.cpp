@@ -271,8 +271,7 @@ struct ShiftIndex {
 
 /* per-thread scratch that keeps its capacity from plan to plan (same reason as PlanBuffers) */
 struct Scratch {
-    std::vector<uint8_t> stamp;           /* alias checks: stamp[page] == gen (seen, owner not edited) / gen + 1 (seen, owner edited) */
-    uint8_t gen = 0;
+    std::vector<uint64_t> seen;           /* alias checks: two bits per pool page (see the alias pass) */
     std::vector<int32_t> dir_begin, old_tab_off, token_lists, dist, slot_ids;
     std::vector<int64_t> first_edit;
     std::vector<DevTile> insert_tiles;
@@ -396,32 +395,32 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
      *   - a page listed twice, where one of its owners has directives, is refused for the in-place modes (FRESH never
      *     writes a request's own pages, so shared prefix pages are fine there);
      *   - a consumed free id that is a live page (or a slot of one), or that was already consumed, is refused. */
-    /* One byte per pool page, stamped with this plan's generation (no clearing between plans; plain stores where no
-     * answer is needed): this pass touches every live page, i.e. every TOKEN of a token-level pool. */
-    if (S.stamp.size() < (size_t)pool_pages || S.gen >= 253) {
-        S.stamp.assign((size_t)pool_pages, 0);
-        S.gen = 0;
-    }
-    S.gen = (uint8_t)(S.gen + 2); /* gen: seen; gen + 1: seen and owned by a request with directives */
-    const uint8_t gen = S.gen;
-    uint8_t* const stamp = S.stamp.data();
+    /* Two bits per pool page, as two bitmaps cleared per plan (17 KB each for a 137 K-slot token-level pool: they stay
+     * in L1, where one byte per page did not): `seen` = listed by some request or consumed
+     * from the free list, `edited` = listed by a request that has directives.  The pass touches every live page, i.e.
+     * every TOKEN of a token-level pool. */
     const bool inplace_mode = mode != LEYLINE_FRESH;
     const bool check_alias = tuning.skip_alias_check == 0;
+    const size_t bm_words = check_alias ? ((size_t)pool_pages + 63) / 64 : 0;
+    S.seen.assign(2 * bm_words, 0); /* word pairs: [2w] = seen, [2w + 1] = edited, so that a page touches one cache line */
+    uint64_t* const seen = S.seen.data();
     bool alias = false;
     for (int32_t r = 0; r < n_requests && check_alias; ++r) {
         const int32_t* row = pl->tabs.data() + S.old_tab_off[(size_t)r];
         const int64_t need = S.old_tab_off[(size_t)r + 1] - S.old_tab_off[(size_t)r];
         if (!inplace_mode) {
-            for (int64_t p = 0; p < need; ++p) stamp[row[p]] = gen;
+            for (int64_t p = 0; p < need; ++p) seen[((uint32_t)row[p] >> 6) * 2] |= 1ull << (row[p] & 63);
             continue;
         }
         const bool has_dirs = S.dir_begin[(size_t)r + 1] > S.dir_begin[(size_t)r];
-        const uint8_t mine = (uint8_t)(gen + (has_dirs ? 1 : 0));
-        uint32_t bad = 0;
+        const uint64_t mine = has_dirs ? ~0ull : 0ull;
+        uint64_t bad = 0;
         for (int64_t p = 0; p < need; ++p) {
-            const uint8_t was = stamp[row[p]];
-            bad |= (uint32_t)((was == gen + 1) | ((was == gen) & has_dirs)); /* listed before, and one owner is edited */
-            stamp[row[p]] = was == gen + 1 ? was : mine;
+            uint64_t* const w = seen + ((uint32_t)row[p] >> 6) * 2;
+            const uint64_t bit = 1ull << (row[p] & 63);
+            bad |= (w[1] & bit) | (w[0] & bit & mine); /* listed before, and one owner is edited */
+            w[0] |= bit;
+            w[1] |= bit & mine;
         }
         alias = alias || bad != 0;
     }
@@ -445,8 +444,9 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
         for (int64_t q = 0; q < count; ++q) {
             if (ids[q] < 0 || ids[q] >= free_limit) { badfree = true; continue; }
             if (!check_alias) continue;
-            alias = alias || stamp[ids[q]] >= gen; /* live, or consumed before */
-            stamp[ids[q]] = gen;
+            const uint64_t bit = 1ull << (ids[q] & 63);
+            alias = alias || (seen[((uint32_t)ids[q] >> 6) * 2] & bit) != 0; /* live, or consumed before */
+            seen[((uint32_t)ids[q] >> 6) * 2] |= bit;
         }
         pl->new_pages.insert(pl->new_pages.end(), ids, ids + count);
         consumed += count;
@@ -516,7 +516,8 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
                     const int32_t* ids = free_ids + consumed;
                     for (int64_t q = 0; q < s.length; ++q) {
                         if (ids[q] < 0 || ids[q] >= free_limit) { badfree = true; continue; }
-                        alias = alias || (check_alias && stamp[ids[q] >> pshift] >= gen); /* a slot of a live page */
+                        const int32_t pg = ids[q] >> pshift;
+                        alias = alias || (check_alias && ((seen[((uint32_t)pg >> 6) * 2] >> (pg & 63)) & 1ull)); /* a slot of a live page */
                     }
                     S.token_lists.insert(S.token_lists.end(), ids, ids + s.length);
                     consumed += s.length;
