@@ -321,6 +321,32 @@ int occupancy(const void* fn, int smem) {
     return blocks;
 }
 
+/* Static shared memory of a kernel and the dynamic size it was last opted in for (per host thread and device): asking the
+ * runtime for both on every launch cost ~8 us of a ~25 us call. */
+struct SmemCache { const void* fn; int device; int static_bytes; int dyn_set; };  /* dyn_set: -1 until opted in */
+thread_local SmemCache g_smem[32];
+thread_local int g_smem_n = 0;
+
+leyline_status smem_entry(const void* fn, SmemCache** out) {
+    for (int i = 0; i < g_smem_n; ++i)
+        if (g_smem[i].fn == fn && g_smem[i].device == g_dev.device) { *out = &g_smem[i]; return LEYLINE_OK; }
+    cudaFuncAttributes fa;
+    CU(cudaFuncGetAttributes(&fa, fn));
+    if (g_smem_n == 32) g_smem_n = 0; /* more kernel variants than slots: start over */
+    g_smem[g_smem_n] = {fn, g_dev.device, (int)fa.sharedSizeBytes, -1};
+    *out = &g_smem[g_smem_n++];
+    return LEYLINE_OK;
+}
+/* Opt the kernel in for ALL the dynamic shared memory the device allows, once: the attribute belongs to the function, not
+ * to this thread, so a per-launch size cached here could be lowered behind our back by another thread's launch. */
+leyline_status smem_opt_in(SmemCache* e) {
+    const int dyn_bytes = g_dev.smem_optin - e->static_bytes;
+    if (e->dyn_set == dyn_bytes) return LEYLINE_OK;
+    CU(cudaFuncSetAttribute(e->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_bytes));
+    e->dyn_set = dyn_bytes;
+    return LEYLINE_OK;
+}
+
 /* Layers that one launch can serve: same pairing convention ("per layer"; G20), at most kMaxLayers.
  * `flag_base` numbers the launch's layers uniquely inside the call (hazard-flag column). */
 struct LayerChunk { int pairing; int flag_base; std::vector<int> layers; };
@@ -474,14 +500,15 @@ leyline_status run_rotate_tma(leyline_plan_s* pl, int64_t tile_count, int64_t in
     for (const LayerChunk& lc : layer_chunks(pl, kBandTmaLayers)) {
         const int nl = (int)lc.layers.size();
         BandKernel fn = pl->desc.dtype == LEYLINE_BF16 ? pick_band_dt<LEYLINE_BF16>(lc.pairing) : pick_band_dt<LEYLINE_FP8_E4M3>(lc.pairing);
-        cudaFuncAttributes fa;
-        CU(cudaFuncGetAttributes(&fa, reinterpret_cast<const void*>(fn)));
-        int stages = (g_dev.smem_optin - (int)fa.sharedSizeBytes - 1024) / stage_bytes;
+        SmemCache* sc = nullptr;
+        leyline_status sst = smem_entry(reinterpret_cast<const void*>(fn), &sc);
+        if (sst != LEYLINE_OK) return sst;
+        int stages = (g_dev.smem_optin - sc->static_bytes - 1024) / stage_bytes;
         if (pl->tuning.stages > 0 && stages > pl->tuning.stages) stages = pl->tuning.stages;
         if (stages > kBandMaxStages) stages = kBandMaxStages;
         if (stages < kBandStoresInFlight + 2) { g_last_error = "TMA band kernel: too few shared-memory stages"; return LEYLINE_E_UNSUPPORTED; }
         const int smem = stages * stage_bytes;
-        CU(cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        if ((sst = smem_opt_in(sc)) != LEYLINE_OK) return sst;
         if (*ticket_slot >= 32) { g_last_error = "too many launches for one plan"; return LEYLINE_E_UNSUPPORTED; }
         MoveParams mp;
         fill_params(pl, mp, 0, tile_count, lc, nullptr, layer_ptrs, layer_repl, (*ticket_slot)++);
@@ -521,14 +548,15 @@ leyline_status run_tiles_bulk(leyline_plan_s* pl, bool hazard, int32_t tile_begi
     for (const LayerChunk& lc : layer_chunks(pl)) {
         const int nl = (int)lc.layers.size();
         BulkKernel fn = pick_bulk(pl, lc.pairing, hazard);
-        cudaFuncAttributes fa;
-        CU(cudaFuncGetAttributes(&fa, reinterpret_cast<const void*>(fn)));
-        int stages = (g_dev.smem_optin - (int)fa.sharedSizeBytes - 1024) / stage_bytes;
+        SmemCache* sc = nullptr;
+        leyline_status sst = smem_entry(reinterpret_cast<const void*>(fn), &sc);
+        if (sst != LEYLINE_OK) return sst;
+        int stages = (g_dev.smem_optin - sc->static_bytes - 1024) / stage_bytes;
         if (pl->tuning.stages > 0 && stages > pl->tuning.stages) stages = pl->tuning.stages;
         if (stages > kBulkMaxStages) stages = kBulkMaxStages;
         if (stages < 3) { g_last_error = "bulk kernel: tile does not fit three shared-memory stages"; return LEYLINE_E_UNSUPPORTED; }
         const int smem = stages * stage_bytes;
-        CU(cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        if ((sst = smem_opt_in(sc)) != LEYLINE_OK) return sst;
         if (*ticket_slot >= 32) { g_last_error = "too many launches for one plan"; return LEYLINE_E_UNSUPPORTED; }
         MoveParams mp;
         fill_params(pl, mp, tile_begin, tile_count, lc, layer_src, layer_dst, layer_repl, (*ticket_slot)++);
