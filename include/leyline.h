@@ -170,7 +170,8 @@ typedef struct leyline_tuning_s {
     int32_t stages;        /* bulk / TMA-band kernels: shared-memory stages per CTA, 0 = as many as fit (bulk: at most 8) */
     int32_t layer_group;   /* bulk / TMA-band kernels: layers per work item (one stage each), 0 = default */
     int32_t consumer_warps;/* bulk kernel only: warps that rotate the band in shared memory, 0 = default (4 for MLA's
-                              narrow band, more when the band is most of the row), at most 16 */
+                              narrow band, 12 when the band is most of the row); values up to 16 are accepted, at most 12 are used
+                              (more never helped and the launch bound caps the registers per thread) */
     int32_t rotate_kernel; /* a5 on a narrow band (MLA): 0 = auto, 1 = k_rotate_band (strided 16-byte loads / stores through
                               registers), 2 = k_rotate_band_tma (the band of a page as one 2-D TMA box staged through shared
                               memory; pages of >= 16 rows, else falls back to 1) */
