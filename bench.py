@@ -468,7 +468,8 @@ def run_e2e(cache, w, steps: int, warmup: int = 1):
 # (key, synth config, modes) of SURVEY.md section 8(d)'s table that ride along with the headline as `extras`
 EXTRA_WORKLOADS = [("cfg2", "2", ("fresh", "inplace", "rotate_only"), 2.0),
                    ("cfg5", "5", ("fresh", "inplace", "rotate_only"), 2.0),
-                   ("cfg4", "4", ("inplace",), 1.25),
+                   ("cfg4", "4", ("inplace", "rotate_only"), 1.25),
+                   ("cfg4", "4", ("fresh",), 2.0),          # 147 GB of pools: runs when that much device memory is free
                    ("gqa", "gqa", ("fresh", "inplace", "rotate_only"), 2.0),
                    ("mha96", "mha96", ("fresh", "inplace", "rotate_only"), 2.0),
                    ("appB", "appB", ("fresh", "rotate_only"), 2.0)]
