@@ -272,6 +272,7 @@ struct ShiftIndex {
 /* per-thread scratch that keeps its capacity from plan to plan (same reason as PlanBuffers) */
 struct Scratch {
     std::vector<uint64_t> seen;           /* alias checks: two bits per pool page (see the alias pass) */
+    std::vector<uint64_t> slot_seen;      /* ROTATE_ONLY: a bit per pool slot, consumed free slots */
     std::vector<int32_t> dir_begin, old_tab_off, token_lists, dist, slot_ids;
     std::vector<int64_t> first_edit;
     std::vector<DevTile> insert_tiles;
@@ -531,9 +532,24 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
     if (nofree) return LEYLINE_E_NOFREE;
     if (badfree) return LEYLINE_E_RANGE;
     if (mode == LEYLINE_ROTATE_ONLY && check_alias && !alias && S.token_lists.size() > 1) { /* the same free slot handed out twice */
-        S.slot_ids = S.token_lists;
-        std::sort(S.slot_ids.begin(), S.slot_ids.end());
-        alias = std::adjacent_find(S.slot_ids.begin(), S.slot_ids.end()) != S.slot_ids.end();
+        const size_t n_ids = S.token_lists.size(), words = ((size_t)desc->pool_slots + 63) / 64;
+        if (words <= 64 * n_ids) {
+            /* a bit per pool slot: clearing it costs less than sorting the ids (19 K inserted rows on config 4: the
+             * sort was 250 of the plan's 360 us) unless the pool is huge and the ids are few */
+            S.slot_seen.assign(words, 0);
+            uint64_t dup = 0;
+            for (size_t q = 0; q < n_ids; ++q) {
+                const uint32_t id = (uint32_t)S.token_lists[q];
+                const uint64_t bit = 1ull << (id & 63);
+                dup |= S.slot_seen[id >> 6] & bit;
+                S.slot_seen[id >> 6] |= bit;
+            }
+            alias = dup != 0;
+        } else {
+            S.slot_ids = S.token_lists;
+            std::sort(S.slot_ids.begin(), S.slot_ids.end());
+            alias = std::adjacent_find(S.slot_ids.begin(), S.slot_ids.end()) != S.slot_ids.end();
+        }
     }
     if (alias) return LEYLINE_E_ALIAS;
     if (mode != LEYLINE_ROTATE_ONLY) n_released = (int64_t)pl->released.size();

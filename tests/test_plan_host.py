@@ -282,6 +282,17 @@ def test_alias_rule_refuses_plans_that_would_overwrite_live_kv():
     assert status(B.ROTATE_ONLY, grow, [40, 41, 42, 43, 44, 45, 46, 47, 13]) == B.E_ALIAS
     assert status(B.ROTATE_ONLY, grow, [40, 41, 42, 43, 44, 45, 46, 47, 40]) == B.E_ALIAS
     assert status(B.ROTATE_ONLY, grow, [40, 41, 42, 43, 44, 45, 46, 47, 48]) == B.OK
+    # the same in a pool of 2^22 slots, where the planner finds duplicates by sorting the few ids instead of a bit per slot
+    big, keep_big = B.make_desc(1, 512, 64, 4, 0, 0, 1152, 1 << 22, inv)
+    for free, want in (([40, 41, 42, 43, 44, 45, 46, 47, 40], B.E_ALIAS), ([40, 41, 42, 43, 4000000, 45, 46, 47, 4000000], B.E_ALIAS),
+                       ([40, 41, 42, 43, 44, 45, 46, 47, 4000000], B.OK)):
+        try:
+            B.leyline_plan(big, B.ROTATE_ONLY, seq, pto, pages, grow, np.asarray(free, np.int32)).close()
+            got = B.OK
+        except B.LeylineError as e:
+            got = e.status
+        assert got == want
+    del keep_big
     # a page shared by two requests (a common prefix): fine for FRESH, which never writes a request's own pages ...
     shared = np.array([0, 1, 2, 0, 4], np.int32)
     edit1 = [(1, 5, 6, 0, 0, A)]
