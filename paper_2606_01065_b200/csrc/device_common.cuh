@@ -82,10 +82,13 @@ __device__ __forceinline__ int4 ld_stream(const void* p) { /* read-only for the 
 /* the buffer is also written by this kernel.  HALF_LINE: ask L2 to fetch 64 bytes, not the 128-byte line, on a miss --
  * for bands that are half a line (fp8 MLA: 64 of every 576 bytes), where the other half is latent nobody reads
  * (measured on B200: a5 on config 5 2.86 -> 3.31 TB/s; SASS: LDG.E.NA.LTC64B.128) */
+#ifndef LEYLINE_L2_HALF_LINE
+#define LEYLINE_L2_HALF_LINE 1 /* 0: measurement builds only (the default 128-byte fetch on half-line bands) */
+#endif
 template <bool HALF_LINE = false>
 __device__ __forceinline__ int4 ld_coherent(const void* p) {
     int4 r;
-    if (HALF_LINE)
+    if (HALF_LINE && LEYLINE_L2_HALF_LINE)
         asm volatile("ld.global.L1::no_allocate.L2::64B.v4.s32 {%0,%1,%2,%3}, [%4];"
                      : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p) : "memory");
     else
