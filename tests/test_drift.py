@@ -286,6 +286,55 @@ def test_master_replacement_rows_are_widened_exactly():
         np.testing.assert_array_equal(ch.masters[l][ch.idx[:S]].astype(np.float64), from_storage(rows, O.BF16)[:, DC:])
 
 
+@pytest.mark.parametrize("pairing", [O.NEOX, O.INTERLEAVED])
+@pytest.mark.parametrize("n_heads,dr", [(1, 64), (2, 64), (4, 64), (2, 96), (4, 96)])
+def test_master_option_in_either_pairing_and_with_several_heads(pairing, n_heads, dr):
+    """Pins the branches of ora_rotate_master_layer that the NeoX / one-head chain above never reaches: the INTERLEAVED
+    pair indices (2i, 2i+1) and the per-head offset h * Dr of a full-width K band (d = 64 and 96,
+    2 and 4 heads).  Pin: textbook complex-exponential RoPE (helpers.rope_complex, per head) at the FINAL position
+    (a re-anchored band is fresh RoPE), master to (N + 2) * 2^-23, stored band == torch's fp32 -> bf16 of
+    the master bit for bit.  A swapped (ia, ib) rotates by -phi, a dropped h * Dr leaves heads 1.. unrotated (and head 0
+    rotated n_heads times): both fail the first assertion."""
+    rng = np.random.default_rng(31 * n_heads + dr + pairing)
+    inv = synth.rope_inv_freq(dr, 10000.0)
+    band, n_slots, n_steps = n_heads * dr, 2048, 3
+    stride = (DC + band) * 2
+    s0, tail = 200, 40                                           # scratch region [0, s0), then `tail` tracked tokens
+    L = s0 + tail
+    raw = rng.standard_normal((L, n_heads, dr))
+    k0 = rope_complex(raw, np.arange(L)[:, None], inv, pairing)  # every head at its token's position
+    rows = np.concatenate([rng.standard_normal((L, DC)), k0.reshape(L, band)], axis=1)
+    order = rng.permutation(n_slots).astype(np.int32)
+    idx = order[:L].copy()
+    pool = np.zeros((n_slots, stride), np.uint8)
+    pool[idx] = to_storage(rows, O.BF16)
+    pool = pool.reshape(-1)
+    master = np.zeros((n_slots, band), np.float32)
+    master[idx] = k0.reshape(L, band).astype(np.float32)
+    repl_rows = to_storage(rng.standard_normal((1024, DC + band)), O.BF16)
+    S, total = s0, 0
+    for d in (37, -150, 301)[:n_steps]:
+        live = np.zeros(n_slots, bool)
+        live[idx] = True
+        free = order[~live[order]]
+        bm = O.plan_batch(O.ROTATE_ONLY, 1, [len(idx)], np.array([0, len(idx)], np.int64), idx,
+                          [(0, 0, S, S + d, 0, O.AMORTIZE)], free)
+        assert bm.status == O.OK
+        O.rotate_master_layer(pairing, DC, dr, stride, inv, pool, master, repl_rows.reshape(-1), bm, n_heads=n_heads)
+        idx = bm.requests[0].slot_new.astype(np.int32)
+        S, total = S + d, total + d
+    assert len(idx) == S + tail
+    got = master[idx[-tail:]].astype(np.float64).reshape(tail, n_heads, dr)
+    ref = rope_complex(raw[s0:], (np.arange(s0, L) + total)[:, None], inv, pairing)
+    assert np.abs(got - ref).max() <= (n_steps + 2) * 2.0 ** -23 * np.abs(ref).max()
+    stored = pool.reshape(n_slots, stride)[idx[-tail:], DC * 2:].copy().view(np.uint16)
+    np.testing.assert_array_equal(stored, bf16_bits_of_f32(master[idx[-tail:]]))
+    # the replacement rows of the last turn: byte copy into the pool, band widened exactly into every head of the master
+    new_rows = pool.reshape(n_slots, stride)[idx[:S]]
+    np.testing.assert_array_equal(new_rows, repl_rows[:S])
+    np.testing.assert_array_equal(master[idx[:S]].astype(np.float64), from_storage(new_rows, O.BF16)[:, DC:])
+
+
 @pytest.mark.gpu
 @pytest.mark.parametrize("n", [1, 20, 100])
 def test_gpu_master_chain_matches_oracle(n):
