@@ -64,6 +64,46 @@ LEYLINE_API leyline_status leyline_cdc_chunk(const leyline_cdc_params* params, c
                                  int32_t* dev_chunk_kind, int64_t capacity, int64_t* dev_n_chunks, void* cuda_stream);
 
 /*
+ * leyline_cdc_chunk_noalloc -- leyline_cdc_chunk for callers that cannot allocate device memory.
+ *
+ * Who needs it: leyline_cdc_chunk borrows its working memory (~15 B per token) from a stream-ordered pool inside the
+ * call.  That is not an option for a host that has already given the whole GPU to its own KV-cache allocator and
+ * must never see the driver asked for more (an inference server after start-up: the request can fail, and growing a
+ * pool stalls the device), for a process held to a fixed device-memory budget, or for code that may not take the
+ * allocator's lock where it runs.  This entry point makes no cudaMalloc / cudaFree / pool call at all, on any call.
+ *
+ * How: the working memory is a fixed 8 MiB array that is part of the library's device image.  Every GPU on which
+ * the library's device code gets loaded carries those 8 MiB until the process exits, whether this call is used or not.
+ * The size does not grow, so the call has a limit:
+ *
+ *   n_tokens <= LEYLINE_CDC_NOALLOC_MAX_TOKENS, else LEYLINE_E_UNSUPPORTED and nothing is launched
+ *   (leyline_cdc_last_error() says which limit was hit).  Split a larger batch at sequence boundaries, or use
+ *   leyline_cdc_chunk.
+ *
+ * Arguments, outputs and results are exactly leyline_cdc_chunk's (same kernels; bit-identical output).  The caller
+ * still owns and passes every input and output buffer.
+ *
+ * Rules that follow from the one shared array:
+ *   - The first call on each device looks up the array's address on that device (the device must be current, as for
+ *     any launch on `cuda_stream`) and may make the runtime load the library's device code there.  Make that first
+ *     call during start-up, before any stream capture begins on that device.  Later calls only launch kernels.
+ *   - All calls on one device use the same array, and it keeps the previous call's contents.  The call itself resets
+ *     what has to start from zero, so calls of any sizes may follow each other on ONE stream.  Two calls that can
+ *     overlap on the GPU (different streams without an ordering between them, or two host threads feeding different
+ *     streams) overwrite each other's tables: order them yourself, or use leyline_cdc_chunk for one of them.
+ *   - At most 64 device ordinals.
+ */
+#define LEYLINE_CDC_NOALLOC_MAX_TOKENS 524288
+LEYLINE_API leyline_status leyline_cdc_chunk_noalloc(const leyline_cdc_params* params, const int32_t* dev_tokens, int64_t n_tokens,
+                                         const int64_t* dev_seq_offsets, int32_t n_seqs, const int32_t* dev_anchor_ids,
+                                         int32_t n_anchor_ids, int64_t* dev_chunk_end, uint64_t* dev_chunk_hash,
+                                         int32_t* dev_chunk_kind, int64_t capacity, int64_t* dev_n_chunks, void* cuda_stream);
+
+/* Message of the last error a leyline_cdc_chunk_noalloc call returned on this thread ("" if none); valid until the
+ * thread's next call into this header. */
+LEYLINE_API const char* leyline_cdc_last_error(void);
+
+/*
  * Registry (D5): an open-addressing table in caller-owned device memory, `capacity` a power of two:
  * dev_keys uint64 [capacity] (0 = empty) and dev_vals int64 [capacity].  Keep it at most half full.
  *   clear   empties the table.

@@ -114,6 +114,9 @@ def _load() -> C.CDLL:
     # discovery side (include/leyline_cdc.h)
     L.leyline_cdc_chunk.restype = C.c_int
     L.leyline_cdc_chunk.argtypes = [C.POINTER(CdcParams), vp, i64, vp, i32, vp, i32, vp, vp, vp, i64, vp, vp]
+    L.leyline_cdc_chunk_noalloc.restype = C.c_int
+    L.leyline_cdc_chunk_noalloc.argtypes = L.leyline_cdc_chunk.argtypes
+    L.leyline_cdc_last_error.restype = C.c_char_p
     L.leyline_registry_clear.restype = C.c_int
     L.leyline_registry_clear.argtypes = [vp, vp, i64, vp]
     L.leyline_registry_insert.restype = C.c_int
@@ -372,6 +375,23 @@ def leyline_cdc_chunk(params: CdcParams, tokens, n_tokens: int, seq_offsets, n_s
                                 _dev_ptr(anchor_ids), n_anchor_ids, _dev_ptr(chunk_end), _dev_ptr(chunk_hash),
                                 _dev_ptr(chunk_kind), capacity, _dev_ptr(n_chunks), _stream_handle(stream))
     _check(st, "leyline_cdc_chunk")
+
+
+CDC_NOALLOC_MAX_TOKENS = 524288      # leyline_cdc.h: LEYLINE_CDC_NOALLOC_MAX_TOKENS
+
+
+def leyline_cdc_chunk_noalloc(params: CdcParams, tokens, n_tokens: int, seq_offsets, n_seqs: int, anchor_ids,
+                              n_anchor_ids: int, chunk_end, chunk_hash, chunk_kind, capacity: int, n_chunks, stream=None):
+    """leyline_cdc.h: leyline_cdc_chunk_noalloc.  Same arguments and results as ``leyline_cdc_chunk``, for callers that
+    may not allocate device memory (a server whose own allocator owns the GPU, a fixed memory budget): the working
+    tables sit in an 8 MiB array inside the library instead of a pool, so ``n_tokens`` is limited to
+    ``CDC_NOALLOC_MAX_TOKENS`` (LeylineError with the library's message beyond it).  Calls share that array: keep them
+    on one stream, or order them; make the first call on a device before any stream capture."""
+    st = _lib.leyline_cdc_chunk_noalloc(C.byref(params), _dev_ptr(tokens), n_tokens, _dev_ptr(seq_offsets), n_seqs,
+                                        _dev_ptr(anchor_ids), n_anchor_ids, _dev_ptr(chunk_end), _dev_ptr(chunk_hash),
+                                        _dev_ptr(chunk_kind), capacity, _dev_ptr(n_chunks), _stream_handle(stream))
+    if st != OK:
+        raise LeylineError(st, "leyline_cdc_chunk_noalloc", _lib.leyline_cdc_last_error().decode())
 
 
 def leyline_registry_clear(keys, vals, capacity: int, stream=None):

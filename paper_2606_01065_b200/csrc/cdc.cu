@@ -510,3 +510,165 @@ extern "C" LEYLINE_API leyline_status leyline_registry_lookup(const uint64_t* de
     CU(cudaGetLastError());
     return LEYLINE_OK;
 } LEYLINE_CATCH_STATUS
+
+/* ===================================================================================================================
+ * leyline_cdc_chunk_noalloc -- the chunker for callers that must not allocate device memory (leyline_cdc.h).
+ *
+ * leyline_cdc_chunk takes its ~15 B / token of working memory from a stream-ordered pool on every call.  Some hosts of
+ * this library cannot do that: a serving engine that has handed the whole GPU to its own KV-cache allocator at start-up
+ * and treats any later driver allocation as a bug (it can fail, and growing a pool stalls the device); a process that
+ * runs under a fixed memory budget set by a scheduler; code that runs between two points where the allocator's lock may
+ * not be taken.  For them the working memory below is part of the library's image: it exists from the moment the module
+ * is loaded on a GPU until the process exits, on EVERY GPU that loads the library, used or not.  That is why it is kept
+ * small (8 MiB) and why the entry point has a hard size limit instead of growing.
+ *
+ * The launch chain is the one leyline_cdc_chunk runs (same kernels, same order, same arguments); only where the scratch
+ * lives differs.  It is written out again here rather than shared so that the allocating path stays as it was.
+ * =================================================================================================================== */
+
+#include <mutex>
+
+constexpr size_t kNoAllocScratchBytes = size_t(8) << 20;
+/* File-scope device array.  In HOST code this name is only a handle the runtime knows the symbol by, not a device
+ * address -- passing it to a kernel would hand the kernel a host address.  Host code gets the real address once per
+ * device from cudaGetSymbolAddress (noalloc_scratch_on_current_device below) and passes that. */
+static __device__ __align__(256) unsigned char g_cdc_noalloc_scratch[kNoAllocScratchBytes];
+
+namespace {
+
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mutex;
+uint8_t* g_noalloc_ptr[kNoAllocMaxDevices] = {};   /* device address of g_cdc_noalloc_scratch, per device ordinal */
+
+/* Bytes of scratch the chain needs for n tokens, and where each table starts (same layout as leyline_cdc_chunk). */
+struct NoAllocLayout {
+    int64_t ja, jb, nxt, blk, h0, c0, h1, c1, prog, flags, kind, mark, total;
+    int64_t n_blocks, n_super;
+    int rounds, n_counters;
+};
+NoAllocLayout noalloc_layout(int64_t n, int min_size) {
+    auto up = [](int64_t x) { return (x + 255) / 256 * 256; };
+    NoAllocLayout L;
+    L.n_blocks = (n + kBlockSpan - 1) / kBlockSpan;
+    L.n_super = (n + kSigSpan - 1) / kSigSpan;
+    const int64_t n_words_padded = L.n_super * 32;
+    L.rounds = 0;
+    for (int64_t reach = 1, far = (n - 1) / min_size + 1; reach <= far; reach <<= 1) ++L.rounds;
+    L.n_counters = L.rounds + 1;
+    L.ja = 0;
+    L.jb = L.ja + up((n + 1) * 4);
+    L.nxt = L.jb + up((n + 1) * 4);
+    L.blk = L.nxt + up((n + 1) * 4);
+    L.h0 = L.blk + up(L.n_blocks * 4);
+    L.c0 = L.h0 + up(n_words_padded * 4);
+    L.h1 = L.c0 + up(n_words_padded * 4);
+    L.c1 = L.h1 + up((L.n_super + 1) * 4);
+    L.prog = L.c1 + up((L.n_super + 1) * 4);
+    L.flags = L.prog + up(L.n_counters * 4);
+    L.kind = L.flags + up(n + 1);
+    L.mark = L.kind + up(n + 1);
+    L.total = L.mark + up(n + 1);
+    return L;
+}
+
+/* Set-up, once per device, with that device current: ask the runtime where g_cdc_noalloc_scratch lives on it.  The
+ * query makes the runtime load this library's device code on that GPU if it has not yet (that is when the 8 MiB are
+ * placed), so the first call on a device should be made outside any stream capture.  Nothing is allocated here. */
+leyline_status noalloc_scratch_on_current_device(uint8_t** out) {
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNoAllocMaxDevices) {
+        g_cdc_error = "leyline_cdc_chunk_noalloc: device ordinal " + std::to_string(dev) + " is beyond the " +
+                      std::to_string(kNoAllocMaxDevices) + " devices this entry point keeps an address for";
+        return LEYLINE_E_UNSUPPORTED;
+    }
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        void* p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_cdc_noalloc_scratch));
+        if (!p) { g_cdc_error = "cudaGetSymbolAddress returned a null address for the static scratch"; return LEYLINE_E_CUDA; }
+        g_noalloc_ptr[dev] = static_cast<uint8_t*>(p);
+    }
+    *out = g_noalloc_ptr[dev];
+    return LEYLINE_OK;
+}
+
+}  // namespace
+
+extern "C" LEYLINE_API leyline_status leyline_cdc_chunk_noalloc(const leyline_cdc_params* p, const int32_t* dev_tokens, int64_t n,
+                                                    const int64_t* dev_seq_offsets, int32_t n_seqs,
+                                                    const int32_t* dev_anchor_ids, int32_t n_anchor_ids,
+                                                    int64_t* dev_chunk_end, uint64_t* dev_chunk_hash,
+                                                    int32_t* dev_chunk_kind, int64_t capacity, int64_t* dev_n_chunks,
+                                                    void* cuda_stream) try {
+    g_cdc_error.clear();
+    if (!p || p->reserved_ != 0 || p->min_size < 1 || p->max_size < p->min_size || p->max_size > 4096 ||
+        p->mask_bits < 0 || p->mask_bits > 32) {
+        g_cdc_error = "leyline_cdc_chunk_noalloc: bad leyline_cdc_params";
+        return LEYLINE_E_INVALID;
+    }
+    if (n < 0 || n_seqs < 0 || n_anchor_ids < 0 || capacity < 0) {
+        g_cdc_error = "leyline_cdc_chunk_noalloc: negative size";
+        return LEYLINE_E_INVALID;
+    }
+    if (n > LEYLINE_CDC_NOALLOC_MAX_TOKENS) {
+        g_cdc_error = "leyline_cdc_chunk_noalloc: n_tokens = " + std::to_string(n) + " exceeds LEYLINE_CDC_NOALLOC_MAX_TOKENS = " +
+                      std::to_string((long long)LEYLINE_CDC_NOALLOC_MAX_TOKENS) +
+                      " (the static scratch is fixed at 8 MiB; split the batch or use leyline_cdc_chunk)";
+        return LEYLINE_E_UNSUPPORTED;
+    }
+    if (!dev_n_chunks || !dev_seq_offsets || (n > 0 && (!dev_tokens || n_seqs < 1)) || (capacity > 0 && !dev_chunk_end) ||
+        (n_anchor_ids > 0 && !dev_anchor_ids)) {
+        g_cdc_error = "leyline_cdc_chunk_noalloc: NULL argument";
+        return LEYLINE_E_INVALID;
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (n == 0) {
+        CU(cudaMemsetAsync(dev_n_chunks, 0, sizeof(int64_t), stream));
+        return LEYLINE_OK;
+    }
+    const NoAllocLayout L = noalloc_layout(n, p->min_size);
+    if (L.total > (int64_t)kNoAllocScratchBytes) { /* cannot happen for n <= the stated maximum; kept as the real guard */
+        g_cdc_error = "leyline_cdc_chunk_noalloc: " + std::to_string(L.total) + " B of scratch needed, the static array holds " +
+                      std::to_string(kNoAllocScratchBytes);
+        return LEYLINE_E_UNSUPPORTED;
+    }
+    uint8_t* ws = nullptr;
+    if (leyline_status st = noalloc_scratch_on_current_device(&ws)) return st;
+    /* The array still holds whatever the previous call (any size, any parameters) left in it.  Nothing has to be
+     * cleared by hand: every table entry the chain reads for THIS n is written by an earlier kernel of this same chain,
+     * and the only values that must start at zero -- the doubling rounds' progress words and the compaction's ticket --
+     * are zeroed by k_cdc_front itself. */
+    int32_t* ja = reinterpret_cast<int32_t*>(ws + L.ja);
+    int32_t* jb = reinterpret_cast<int32_t*>(ws + L.jb);
+    int32_t* nxt = reinterpret_cast<int32_t*>(ws + L.nxt);
+    int32_t* blk = reinterpret_cast<int32_t*>(ws + L.blk);
+    uint32_t *hard0 = reinterpret_cast<uint32_t*>(ws + L.h0), *cand0 = reinterpret_cast<uint32_t*>(ws + L.c0),
+             *hard1 = reinterpret_cast<uint32_t*>(ws + L.h1), *cand1 = reinterpret_cast<uint32_t*>(ws + L.c1);
+    int32_t* progress = reinterpret_cast<int32_t*>(ws + L.prog);
+    uint8_t *flags = ws + L.flags, *kind = ws + L.kind, *mark = ws + L.mark;
+    bool launched = true;
+    auto go = [&](cudaError_t e) { launched = launched && ok(e); };
+    go(launch_pdl(k_cdc_front, grid_for(L.n_super, 1), kT, stream, dev_tokens, n, dev_anchor_ids, (int)n_anchor_ids, p->seed,
+                  dev_seq_offsets, (int)n_seqs, (int)p->mask_bits, L.n_super, flags, mark, hard0, cand0, hard1, cand1, progress,
+                  L.n_counters));
+    go(launch_pdl(k_cdc_next, grid_for(n + 1), kT, stream, (const uint8_t*)flags, (const uint32_t*)hard0, (const uint32_t*)hard1,
+                  (const uint32_t*)cand0, (const uint32_t*)cand1, n, (int)p->min_size, (int)p->max_size, nxt, kind));
+    const int32_t* jin = nxt;
+    int32_t* jout = ja;
+    for (int r = 0; r < L.rounds; ++r) {
+        go(launch_pdl(k_cdc_reach, grid_for(n + 1), kT, stream, jin, jout, n, mark,
+                      (const int32_t*)(r ? progress + r - 1 : nullptr), progress + r));
+        jin = jout;
+        jout = (jout == ja) ? jb : ja;
+    }
+    go(launch_pdl(k_cdc_count_scan, (unsigned)L.n_blocks, kT, stream, (const uint8_t*)mark, n, blk, progress + L.rounds, dev_n_chunks));
+    if (capacity > 0)
+        go(launch_pdl(k_cdc_emit, (unsigned)L.n_blocks, kT, stream, dev_tokens, (const uint8_t*)mark, (const int32_t*)nxt,
+                      (const uint8_t*)kind, n, (const int32_t*)blk, capacity, dev_chunk_end, dev_chunk_kind, dev_chunk_hash));
+    if (!launched) return LEYLINE_E_CUDA;
+    CU(cudaGetLastError());
+    return LEYLINE_OK;
+} LEYLINE_CATCH_STATUS
+
+extern "C" LEYLINE_API const char* leyline_cdc_last_error(void) { return g_cdc_error.c_str(); }
