@@ -221,13 +221,14 @@ def time_splice(cache, w, mode: int, steps: int, warmup: int, world: int = 1, ch
     e1.record()
     barrier(world)
     ms = e0.elapsed_time(e1) / steps
-    ms_chunk = None
+    ms_chunk = ms_best = None
     if chunk and marks:
         ev = [e0, *marks]
-        ms_chunk = float(np.median([ev[j].elapsed_time(ev[j + 1]) / chunk for j in range(len(ev) - 1)]))
+        per = [ev[j].elapsed_time(ev[j + 1]) / chunk for j in range(len(ev) - 1)]
+        ms_chunk, ms_best = float(np.median(per)), float(np.min(per))
     retire(0)
     del keep
-    return {"ms_per_step": ms, "ms_per_step_median_chunk": ms_chunk, "kernel_ms": float(np.mean(kms)), "kernel_ms_min": float(np.min(kms)), "bytes": nbytes,
+    return {"ms_per_step": ms, "ms_per_step_median_chunk": ms_chunk, "ms_per_step_best_chunk": ms_best, "kernel_ms_median": float(np.median(kms)), "kernel_ms": float(np.mean(kms)), "kernel_ms_min": float(np.min(kms)), "bytes": nbytes,
             "plan_host_us": float(np.median(host_us)), "launches_per_step": launches,
             "n_directives": len(w.directives), "rows_moved": int(info.rows_moved), "rows_inserted": int(info.rows_inserted),
             "mover": int(info.mover), "tile_rows": int(info.tile_rows)}
@@ -392,16 +393,55 @@ def cpu_baseline(pools, repls, scales, w, mode: int, bytes_per_layer: int, budge
             "seconds": t_total, "host_cpus": os.cpu_count()}
 
 
+def pcie_peak(dev, nbytes: int = 1 << 30, reps: int = 3):
+    """What the link gives plain copies, measured in this run: one pinned host -> device and one device -> host
+    cudaMemcpyAsync of `nbytes` each, alone and then both at once on two streams (one copy per direction in flight).
+    `both_GBps` (bytes of both directions / the time until both are done) is the bound `e2e` is read against."""
+    import torch
+    h_src = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    h_dst = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    d_dst = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    d_src = torch.zeros(nbytes, dtype=torch.uint8, device=dev)
+    h_src.zero_()
+    s_in, s_out = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+
+    def run(h2d: bool, d2h: bool) -> float:
+        best = float("inf")
+        for _ in range(reps + 1):                 # the first pass is the warm-up
+            torch.cuda.synchronize()
+            ev = []
+            for on, st, dst, src in ((h2d, s_in, d_dst, h_src), (d2h, s_out, h_dst, d_src)):
+                if on:
+                    with torch.cuda.stream(st):
+                        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        a.record()
+                        dst.copy_(src, non_blocking=True)
+                        b.record()
+                        ev.append((a, b))
+            torch.cuda.synchronize()
+            first = ev[0][0]                      # both streams start right behind the same synchronize
+            best = min(best, max(max(first.elapsed_time(b), a.elapsed_time(b)) for a, b in ev))
+        return best * 1e-3
+
+    one_in, one_out, both = run(True, False), run(False, True), run(True, True)
+    return {"h2d_alone_GBps": nbytes / one_in / 1e9, "d2h_alone_GBps": nbytes / one_out / 1e9,
+            "both_GBps": 2 * nbytes / both / 1e9, "bytes_each_way": nbytes,
+            "how": "pinned cudaMemcpyAsync, one per direction, two streams, CUDA events, best of %d" % reps}
+
+
 def run_e2e(cache, w, steps: int, warmup: int = 1):
     """Same metric through the public API with HOST buffers: the cache lives in pinned host memory and the library is
     handed those host pointers (include/leyline.h: layer pointers may be device memory or device-accessible pinned
     host memory).  The kernels gather the rows to move straight from host memory and scatter the spliced rows
     straight back over PCIe, so only the bytes the method needs cross the link: per step host -> device = the rows
-    read + the plan tables, device -> host = the rows written + the page table and slot list read back."""
+    read + the plan tables, device -> host = the rows written + the page table and slot list read back.
+    `pcie_peak` is the link's own rate for plain pinned copies in both directions at once, measured here; `frac` =
+    value / pcie_peak.both_GBps."""
     import torch
     from paper_2606_01065_b200 import binding as B
     L = cache.n_layers
     dev = cache.device
+    link = pcie_peak(dev)
     host_pool = [torch.empty(w.layer_bytes, dtype=torch.uint8, pin_memory=True) for _ in range(L)]
     host_repl = [torch.empty(cache.repl[l].numel(), dtype=torch.uint8, pin_memory=True) for l in range(L)]
     for l in range(L):
@@ -412,16 +452,24 @@ def run_e2e(cache, w, steps: int, warmup: int = 1):
     pools, repl = B.layer_pointers(host_pool), B.layer_pointers(host_repl)
     dirs = B.pack_directives(w.directives)
     sizes = {}
+    # the step's small results (new page table, slot list) land in buffers a scheduler would hold for the session:
+    # device side for the kernels, pinned host side for the read-back; sized once from the first plan
+    plan0 = B.leyline_plan(desc, B.FRESH, w.seq_lens, w.pt_offsets, w.pages, dirs, w.free_pages)
+    n_pt, n_idx = int(plan0.info.total_new_pages), int(plan0.info.total_new_tokens)
+    plan0.close()
+    pt = torch.empty(n_pt, dtype=torch.int32, device=dev)
+    idx = torch.empty(n_idx, dtype=torch.int32, device=dev)
+    pt_host = torch.empty(n_pt, dtype=torch.int32, pin_memory=True)
+    idx_host = torch.empty(n_idx, dtype=torch.int32, pin_memory=True)
 
     def step():
         plan = B.leyline_plan(desc, B.FRESH, w.seq_lens, w.pt_offsets, w.pages, dirs, w.free_pages)
         plan.prefetch()
         info = plan.info
-        pt = torch.empty(int(info.total_new_pages), dtype=torch.int32, device=dev)
-        idx = torch.empty(int(info.total_new_tokens), dtype=torch.int32, device=dev)
         B.leyline_splice(plan, pools, pools, repl, pt, idx)
-        pt_host, idx_host = pt.cpu(), idx.cpu()          # the step's result that the scheduler reads
-        torch.cuda.synchronize()
+        pt_host.copy_(pt, non_blocking=True)             # the step's result that the scheduler reads
+        idx_host.copy_(idx, non_blocking=True)
+        torch.cuda.synchronize()                         # ... and it reads it: the step ends when the result is on the host
         sizes.update(read=int(info.bytes_read), written=int(info.bytes_written), small=pt_host.numel() * 4 + idx_host.numel() * 4,
                      tables=int(info.n_tiles) * 48 + int(info.total_new_pages) * 8)
         plan.close()
@@ -455,13 +503,17 @@ def run_e2e(cache, w, steps: int, warmup: int = 1):
     plan.close()
     same = all(bool((host_pool[l].to(dev) == cache.pools[l]).all()) for l in (0, L - 1))
     del keep
-    return {"value": (sizes["read"] + sizes["written"]) / dt / 1e9, "unit": UNIT,
+    value = (sizes["read"] + sizes["written"]) / dt / 1e9
+    return {"value": value, "unit": UNIT,
             "h2d_bytes_per_step": sizes["read"] + sizes["tables"], "d2h_bytes_per_step": sizes["written"] + sizes["small"],
             "ms_per_step": dt * 1e3, "steps": steps, "matches_device_resident_result": same,
+            "pcie_peak": link, "frac": value / link["both_GBps"],
             "swap_in": {"ms_per_step": dt_swap * 1e3, "h2d_GBps": sizes["read"] / dt_swap / 1e9,
+                        "frac_of_h2d_alone": sizes["read"] / dt_swap / 1e9 / link["h2d_alone_GBps"],
                         "note": "host-resident source spliced into the device pool: moved rows cross PCIe once"},
             "note": "cache in pinned host memory, spliced in place over PCIe by the same kernels (host pointers through the "
-                    "C ABI); host wall clock around synchronised steps; PCIe-bound by construction"}
+                    "C ABI); host wall clock around synchronised steps; bound = pcie_peak.both_GBps (plain pinned copies, "
+                    "both directions at once, measured in this run)"}
 
 
 
@@ -594,6 +646,79 @@ def pattern_reference(device, n_rows: int = 4 << 20):
     return out
 
 
+def sustained_line(cache, w, mode: int, ms_per_step: float, device_index: int, seconds: float = 3.2):
+    """The headline step back to back for >= 3 s (median and best, clocks under load): the same
+    time_splice as the headline, cut into 32 chunks whose median and best are reported beside the plain mean."""
+    steps = int(max(64, np.ceil(seconds * 1e3 / max(ms_per_step, 1e-3))))
+    sampler = ClockSampler(device_index)
+    sampler.start()
+    x = time_splice(cache, w, mode, steps, 3, chunk=max(1, steps // 32))
+    clocks = sampler.stop()
+    gbs = lambda ms: x["bytes"] / ms / 1e6
+    return {"steps": steps, "seconds": steps * x["ms_per_step"] * 1e-3, "ms_per_step_mean": x["ms_per_step"],
+            "ms_per_step_median": x["ms_per_step_median_chunk"], "ms_per_step_best": x["ms_per_step_best_chunk"],
+            "GBps_mean": gbs(x["ms_per_step"]), "GBps_median": gbs(x["ms_per_step_median_chunk"]),
+            "GBps_best": gbs(x["ms_per_step_best_chunk"]), "kernel_ms_mean": x["kernel_ms"], "kernel_ms_median": x["kernel_ms_median"],
+            "kernel_ms_best": x["kernel_ms_min"], "mover_GBps_mean": gbs(x["kernel_ms"]), "mover_GBps_best": gbs(x["kernel_ms_min"]),
+            "chunks": 32, "clocks": clocks}
+
+
+SUMMARY_KEYS = {"cfg2": "2", "cfg3": "3", "cfg3m": "3m", "cfg4": "4", "cfg5": "5", "gqa": "g", "mha96": "m", "appB": "B"}
+SUMMARY_MODES = {"fresh": "f", "inplace": "i", "rotate_only": "r"}
+
+
+def summary_of(out: dict, peak: float) -> dict:
+    """Every (workload, mode) of SURVEY.md 8(d) in a few characters each, as the LAST key of the line, so that a
+    truncated record of this line still shows them.  Row = [mover GB/s, fraction of the copy peak, us per directive of
+    the step, host plan us, SM MHz under load, 1 if any throttle reason was seen].  Keys: workload (2 3 3m 4 5 = BASELINE
+    configs, g = gqa, m = mha96, B = App. B shape) + mode (f fresh, i in place, r rotate only)."""
+    def us(x):
+        return round(x, 1) if x < 100 else int(round(x))
+
+    def row(gbs, frac, us_dir, plan_us, clocks):
+        c = clocks or {}
+        return [int(round(gbs)), round(frac, 2), us(us_dir), int(round(plan_us)), int(c.get("sm_mhz") or 0),
+                int(bool([r for r in c.get("reasons") or [] if r != "nvidia-smi unavailable"]))]
+
+    rf = out["roofline"]
+    sm = {"cols": "kGBps,frac,us/dir,plan_us,MHz,thr",
+          "3f": row(rf["achieved"], rf["frac"], out["us_per_directive"], out["plan_host_us"], out.get("clocks"))}
+    ex = out.get("extras") if isinstance(out.get("extras"), dict) else {}
+    for key, x in ex.items():
+        wl, _, md = key.partition("_")
+        if wl not in SUMMARY_KEYS or md not in SUMMARY_MODES or not isinstance(x, dict):
+            continue
+        k = SUMMARY_KEYS[wl] + SUMMARY_MODES[md]
+        sm[k] = "skip" if "skipped" in x else row(x["kernel_GBps"], x["frac"], x["us_per_directive"], x["plan_host_us"], x.get("clocks"))
+    for m in ("fresh", "rotate_only"):          # the paper's own shape: one call on an idle GPU, us (median)
+        one = ex.get(f"appB_{m}_single_call_idle_gpu")
+        if one:
+            sm["B" + SUMMARY_MODES[m] + "1"] = int(round(one["median_us"]))
+    su = out.get("sustained")
+    if su:   # [seconds, median GB/s, best GB/s, mover GB/s mean, MHz, thr]
+        c = su.get("clocks") or {}
+        sm["sus"] = [round(su["seconds"], 1), int(round(su["GBps_median"])), int(round(su["GBps_best"])), int(round(su["mover_GBps_mean"])),
+                     int(c.get("sm_mhz") or 0), int(bool(c.get("reasons")))]
+    e = out.get("e2e") or {}
+    if e.get("value"):
+        sm["e2e"] = [round(e["value"], 1), round(e.get("frac") or 0, 2)]
+    pp = ex.get("a5_pattern_probe") or {}
+    if pp:   # a5's ceiling: the pattern probe, GB/s read+write (bf16 128 of 1152 B, fp8 64 of 576 B)
+        sm["a5p"] = [int(round(pp[k]["GBps"])) for k in ("bf16_128_of_1152", "fp8_64_of_576") if k in pp]
+    sm["peak"] = int(round(peak))
+    return sm
+
+
+def kernel_name(mover: int, rotate_only: bool) -> str:
+    """leyline_plan_info.mover -> the kernel that moves the bytes (2 = bulk mover, 3 = the 2-D TMA band variant chosen
+    with --rotate-kernel 2; otherwise the register-staged kernels)."""
+    if mover == 2:
+        return "k_move_bulk"
+    if mover == 3:
+        return "k_rotate_band_tma"
+    return "k_rotate_band" if rotate_only else "k_move_rows"
+
+
 def run_stub(args):
     """--stub-step-ms: the N-replica launch and timing contract with a host sleep in place of the splice (no GPU, no
     library): barrier, K timed steps, MAX over ranks of the step time, SUM of the units, one JSON line from rank 0."""
@@ -642,7 +767,7 @@ def run_ours(args):
     value = R.sum_over_ranks(float(r["bytes"]), world, dev) / (ms * 1e-3) / 1e9     # whole job: all replicas' bytes / slowest rank's time
     peak, peak_src = peaks()
     kernel_gbs = r["bytes"] / (r["kernel_ms"] * 1e-3) / 1e9
-    kname = "k_move_bulk" if r["mover"] == 2 else ("k_rotate_band" if mode == B.ROTATE_ONLY else "k_move_rows")
+    kname = kernel_name(r["mover"], mode == B.ROTATE_ONLY)
     traffic, traffic_src = ncu_traffic(args.workload, args.mode, kname)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -662,7 +787,7 @@ def run_ours(args):
         "clocks": clocks,
         "roofline": {"bound": "hbm", "achieved": kernel_gbs, "peak": peak, "unit": UNIT, "frac": kernel_gbs / peak,
                      "traffic": traffic, "traffic_source": traffic_src, "algorithmic_bytes": r["bytes"],
-                     "kernel": kname + (" (in-place K_pe rotation)" if kname == "k_rotate_band" else " (fused gather-rotate-scatter + insert)"),
+                     "kernel": kname + (" (in-place K_pe rotation)" if kname.startswith("k_rotate_band") else " (fused gather-rotate-scatter + insert)"),
                      "tile_rows": r["tile_rows"],
                      "kernel_ms": r["kernel_ms"], "kernel_ms_best": r["kernel_ms_min"],
                      "peak_source": peak_src, "frac_of_8TBps_nominal": kernel_gbs / 8000.0},
@@ -678,6 +803,7 @@ def run_ours(args):
                 cache.w = wl
                 extras[name] = extra_line(cache, wl, md, peak, local)
             cache.w = w
+            out["sustained"] = sustained_line(cache, w, mode, r["ms_per_step"], local)
             extras["single_call_idle_gpu"] = time_single_calls(cache, w, mode)
             extras["discovery_cdc"] = time_discovery(cache.device, with_oracle=not args.no_cpu_baseline)
             out["extras"] = extras
@@ -690,7 +816,7 @@ def run_ours(args):
     if not args.no_e2e and mode == B.FRESH:
         # every replica runs its own end-to-end leg (host pools over its own PCIe link); whole job = all bytes / slowest
         try:
-            e = run_e2e(cache, w, steps=min(args.steps, 3))
+            e = run_e2e(cache, w, steps=5)
         except Exception as ex:   # e.g. the host cannot pin that much memory: say so instead of inventing a number
             e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
                  "error": f"{type(ex).__name__}: {ex}"}
@@ -718,6 +844,12 @@ def run_ours(args):
         out["extras"] = "N = 1 only (supplementary workloads; they do not depend on the replica count)"
     R.finish(world)
     if rank == 0:
+        # order of the line: contract keys, roofline, cpu_baseline, e2e, sustained, then the long `extras`, and the compact
+        # `summary` of every SURVEY.md 8(d) row as the very last key
+        ex = out.pop("extras", None)
+        if ex is not None:
+            out["extras"] = ex
+        out["summary"] = summary_of(out, peak)
         print(json.dumps(out))
 
 
