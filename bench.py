@@ -47,7 +47,7 @@ def parse_args():
     ap.add_argument("--stages", type=int, default=0, help="leyline_tuning.stages (bulk kernel)")
     ap.add_argument("--layer-group", type=int, default=0, help="leyline_tuning.layer_group (bulk kernel)")
     ap.add_argument("--consumer-warps", type=int, default=0, help="leyline_tuning.consumer_warps (bulk kernel)")
-    ap.add_argument("--rotate-kernel", type=int, default=0, help="leyline_tuning.rotate_kernel (0 auto, 1 strided registers, 2 TMA boxes)")
+    ap.add_argument("--rotate-kernel", type=int, default=0, help="leyline_tuning.rotate_kernel (0 auto, 1 strided registers, 2 TMA boxes, 3 flat passes)")
     ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="process-group backend for --gpus N > 1")
     ap.add_argument("--stub-step-ms", type=float, default=0.0,
                     help="TEST ONLY (tests/test_replicas_gloo.py): replace the splice by a host sleep of this many ms "
@@ -709,13 +709,21 @@ def summary_of(out: dict, peak: float) -> dict:
     return sm
 
 
+def build_flags() -> str:
+    from paper_2606_01065_b200 import build as _b
+    return _b.built_with()
+
+
 def kernel_name(mover: int, rotate_only: bool) -> str:
     """leyline_plan_info.mover -> the kernel that moves the bytes (2 = bulk mover, 3 = the 2-D TMA band variant chosen
-    with --rotate-kernel 2; otherwise the register-staged kernels)."""
+    with --rotate-kernel 2, 4 = the band kernel over flat passes (short segments, or --rotate-kernel 3); otherwise the
+    register-staged kernels)."""
     if mover == 2:
         return "k_move_bulk"
     if mover == 3:
         return "k_rotate_band_tma"
+    if mover == 4:
+        return "k_rotate_band_flat"
     return "k_rotate_band" if rotate_only else "k_move_rows"
 
 
@@ -778,6 +786,7 @@ def run_ours(args):
                    "rows_inserted_per_layer": r["rows_inserted"], "bytes_read_plus_written": r["bytes"],
                    "cache_flush": "none needed: each step streams %.2f GB, far larger than the 126 MB L2" % (r["bytes"] / 1e9),
                    "replicas": world, "multi_gpu": "replicas only (the path has no exchange step)",
+                   "build_knobs": " ".join(f for f in build_flags().split() if f.startswith("-D")) or "none (default build)",
                    "throughput": "pipelined steady state: the host plan and table upload of step n+1 overlap the kernels of "
                                  "step n; extras.single_call_idle_gpu is one call on an idle GPU"},
         "us_per_directive": ms * 1e3 / max(1, r["n_directives"]),

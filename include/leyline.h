@@ -152,7 +152,9 @@ typedef struct {
     int64_t mover;             /* a3/a4 kernel this plan launches: 1 = k_move_rows, 2 = k_move_bulk (see leyline_tuning).
                                   ROTATE_ONLY: 1 = k_rotate_band (strided band kernel), 2 = the band is at least half of
                                   the row (full-width K), so whole rows stream through k_move_bulk and are written back
-                                  to the slots they were read from, 3 = k_rotate_band_tma (2-D TMA boxes of the band) */
+                                  to the slots they were read from, 3 = k_rotate_band_tma (2-D TMA boxes of the band),
+                                  4 = k_rotate_band_flat (k_rotate_band's arithmetic with consecutive short tiles packed
+                                  into full block passes; chosen when the rotated segments are short) */
 } leyline_plan_info;
 
 typedef struct leyline_plan_s leyline_plan_t;
@@ -174,7 +176,8 @@ typedef struct leyline_tuning_s {
                               (more never helped and the launch bound caps the registers per thread) */
     int32_t rotate_kernel; /* a5 on a narrow band (MLA): 0 = auto, 1 = k_rotate_band (strided 16-byte loads / stores through
                               registers), 2 = k_rotate_band_tma (the band of a page as one 2-D TMA box staged through shared
-                              memory; pages of >= 16 rows, else falls back to 1) */
+                              memory; pages of >= 16 rows, else falls back to 1), 3 = k_rotate_band_flat whenever the
+                              geometry allows it (auto picks it only when it saves a fifth of the work items or more) */
     int32_t skip_alias_check; /* 1: the caller guarantees what the alias rule checks (free ids disjoint from live pages and
                               from each other, no page shared with a request edited in place); LEYLINE_E_ALIAS is then
                               never returned and the planner skips its pass over every live page */

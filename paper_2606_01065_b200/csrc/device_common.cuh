@@ -33,7 +33,8 @@ struct MoveParams {
     long long n_items;            /* tiles in this launch * layers in this launch */
     long long n_copy_items;       /* k_rotate_band only: replacement-insert tiles * layers, handled after the rotations */
     int32_t copy_tile_begin;      /* k_rotate_band only: first insert tile */
-    int32_t pad0_;
+    int32_t n_rot_tiles;          /* k_rotate_band_flat only: rotate tiles [tile_begin, tile_begin + n_rot_tiles) */
+    const RotPass* passes;        /* k_rotate_band_flat only: one entry per pass; n_items = passes * layers */
     int64_t stride;               /* row stride in bytes */
     int32_t tile_begin;           /* first tile of this launch in the plan's list */
     int32_t n_layers;             /* layers in this launch */

@@ -296,6 +296,141 @@ __global__ void __launch_bounds__(kThreads, DT == LEYLINE_FP8_E4M3 ? 2 : LEYLINE
     }
 }
 
+/* ------------------------------------------------------------------ a5 on short segments ---- */
+
+/* k_rotate_band with the work cut differently (same arithmetic, same loads and stores per unit): a tile never crosses
+ * a segment, so when the rotated segments are short -- the paper's own workload is hundreds of ~130-token chunks per
+ * call -- a (tile, layer) item fills a third of the block's units and the memory system sees a
+ * third of the requests it could have in flight.  Here the rows of all rotate tiles, in tile order, are one flat row
+ * space, and an item is (pass, layer): pass b = flat rows [b * R, (b + 1) * R), R = the rows a block holds, whatever tiles
+ * they fall in.  p.passes[b] names the tile of the pass's first row and that row's offset in it; a thread walks forward
+ * from there over the tiles' row counts (its units are ascending in row, so the walk never restarts; a block spans a
+ * handful of tiles at most).  Every unit carries its own cos/sin row, reloaded only when the tile's rotation changes.
+ * Geometry: the FIXED case only (the pair columns of a row divide the block), which is every narrow band; the planner
+ * picks this kernel (plan.cpp) and falls back to k_rotate_band otherwise.  Inserts ride behind as in k_rotate_band. */
+template <int DT, int PAIRING>
+__global__ void __launch_bounds__(kThreads, DT == LEYLINE_FP8_E4M3 ? 2 : LEYLINE_ROT_BF16_CTAS) k_rotate_band_flat(const __grid_constant__ MoveParams p) {
+    constexpr int N = Codec<DT>::kElems;
+    constexpr int kRotUnroll = DT == LEYLINE_BF16 ? kRotUnrollBf16 : kRotUnrollFp8;
+    constexpr bool HALF_LINE = DT == LEYLINE_FP8_E4M3;
+    const int tid = threadIdx.x;
+    const int half = p.head_chunks >> 1;   /* pair columns per head */
+    const int cols = p.n_heads * half;     /* pair columns per row; divides kThreads */
+    const int64_t band0 = (int64_t)p.lat_chunks * 16;
+    const int r0 = tid / cols, col = tid - r0 * cols;
+    const int head = col / half, q = col - head * half;
+    const int64_t chunk_off = band0 + (int64_t)(head * p.head_chunks + q) * 16;
+    const int rstep = kThreads / cols;     /* rows between a thread's consecutive units */
+    const int tile_end = p.tile_begin + p.n_rot_tiles;
+
+    struct Item { int32_t slot[kRotUnroll]; int32_t trig[kRotUnroll]; int32_t layer; };
+    auto resolve = [&](long long item, Item& it) {
+        const long long pass = item / p.n_layers;
+        it.layer = (int)(item - pass * p.n_layers);
+        const RotPass rp = p.passes[pass];
+        int j = p.tile_begin + rp.tile;
+        int off = rp.row_off + r0;                                   /* row of unit 0, counted from tile j's first row */
+        int n = j < tile_end ? p.tiles[j].n_rows : 0;
+        int held = -1, t_tab = 0, t_trig = -1;                       /* the tile whose fields are in registers */
+        int64_t t_pos = 0;
+#pragma unroll
+        for (int k = 0; k < kRotUnroll; ++k) {
+            while (j < tile_end && off >= n) {
+                off -= n;
+                ++j;
+                n = j < tile_end ? p.tiles[j].n_rows : 0;
+            }
+            if (j < tile_end) {
+                if (held != j) {
+                    const DevTile& t = p.tiles[j];
+                    t_pos = t.src_pos; t_tab = t.src_tab; t_trig = t.trig;
+                    held = j;
+                }
+                it.slot[k] = (int32_t)slot_of(p.tabs, t_tab, t_pos + off, p.page_shift);
+                it.trig[k] = t_trig;
+            } else {
+                it.slot[k] = -1;                                     /* behind the last rotated row */
+                it.trig[k] = -1;
+            }
+            off += rstep;
+        }
+    };
+
+    long long item = blockIdx.x;
+    Item cur, nxt;
+    if (item < p.n_items) resolve(item, cur);
+    while (item < p.n_items) {
+        uint8_t* __restrict__ base = p.dst[cur.layer];
+        int4 lo[kRotUnroll], hi[kRotUnroll];
+        uint8_t* addr[kRotUnroll];
+#pragma unroll
+        for (int k = 0; k < kRotUnroll; ++k) {
+            addr[k] = nullptr;
+            if (cur.slot[k] >= 0) {
+                addr[k] = base + (int64_t)cur.slot[k] * p.stride + chunk_off;
+                lo[k] = ld_coherent<HALF_LINE>(addr[k]);
+                hi[k] = ld_coherent<HALF_LINE>(addr[k] + half * 16);
+            }
+        }
+        const long long next = item + gridDim.x;
+        const bool more = next < p.n_items;
+        if (more) resolve(next, nxt);                                /* the next item's look-ups run under this item's loads */
+        const float* __restrict__ trig_row = nullptr;
+        PairTrig<N, false> tr;
+        int have = -2;
+#pragma unroll
+        for (int k = 0; k < kRotUnroll; ++k) {
+            if (addr[k]) {
+                if (cur.trig[k] != have) {                           /* a new segment: this column's cos/sin of its shift */
+                    have = cur.trig[k];
+                    trig_row = trig_row_of(p.trig, have, p.H);
+                    load_pair_trig<PAIRING>(trig_row, p.H, q, half, tr);
+                }
+                int4 lo_out = lo[k], hi_out = hi[k];
+                const bool redo = rotate_chunk_pair_plain<DT, PAIRING>(lo_out, hi_out, tr);
+                st_stream(addr[k], lo_out);
+                st_stream(addr[k] + half * 16, hi_out);
+                if (redo && Comp<DT>::value) {
+                    rotate_chunk_pair_careful<DT, PAIRING>(lo_out, hi_out, trig_row, p.H, q, half, lo[k], hi[k]);
+                    st_stream(addr[k], lo_out);
+                    st_stream(addr[k] + half * 16, hi_out);
+                }
+            }
+        }
+        if (!more) break;
+        cur = nxt;
+        item = next;
+    }
+
+    /* a4 in the same launch, as in k_rotate_band */
+    const int row_chunks = p.lat_chunks + p.band_chunks;
+    for (long long ci = blockIdx.x; ci < p.n_copy_items; ci += gridDim.x) {
+        const DevTile t = p.tiles[p.copy_tile_begin + (int)(ci / p.n_layers)];
+        const int layer = (int)(ci % p.n_layers);
+        const uint8_t* __restrict__ src = p.repl[layer] + t.src_pos * p.stride;
+        uint8_t* __restrict__ dst = p.dst[layer];
+        const int shift = (t.flags & TILE_DST_TOKEN) ? 0 : p.page_shift;
+        const int n_chunks = t.n_rows * row_chunks;
+        for (int c0 = tid; c0 < n_chunks; c0 += kThreads * 4) {
+            int4 v[4];
+            uint8_t* out[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int c = c0 + k * kThreads;
+                out[k] = nullptr;
+                if (c < n_chunks) {
+                    const int r = c / row_chunks, cc = c - r * row_chunks;
+                    v[k] = ld_stream(src + (int64_t)r * p.stride + cc * 16);
+                    out[k] = dst + slot_of(p.tabs, t.dst_tab, t.dst_pos + r, shift) * p.stride + cc * 16;
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (out[k]) st_stream(out[k], v[k]);
+        }
+    }
+}
+
 /* ------------------------------------------------------------------ a5 with an fp32 master band ---- */
 
 /* Chained splices round the bf16 K_pe once per turn and the error random-walks (Table 6; the paper's

@@ -100,7 +100,7 @@ leyline_status check_tuning(const leyline_tuning* t) {
     if (t->kernel < 0 || t->kernel > 2 || t->tile_rows < 0 || t->tile_rows > 64 || t->ctas_per_sm < 0 ||
         t->ctas_per_sm > 32 || t->stages < 0 || t->stages > 32 || t->layer_group < 0 ||
         t->layer_group > LEYLINE_MAX_LAYERS_PER_LAUNCH || t->consumer_warps < 0 || t->consumer_warps > 16 ||
-        t->rotate_kernel < 0 || t->rotate_kernel > 2 || t->skip_alias_check < 0 || t->skip_alias_check > 1)
+        t->rotate_kernel < 0 || t->rotate_kernel > 3 || t->skip_alias_check < 0 || t->skip_alias_check > 1)
         return LEYLINE_E_INVALID;
     return LEYLINE_OK;
 }
@@ -720,6 +720,29 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
     in.rot_tile_rows = pl->rot_tile_rows;
     in.mover = pl->use_bulk ? 2 : 1; /* ROTATE_ONLY: 2 = the rotation itself runs on the bulk mover (wide bands) */
     if (mode == LEYLINE_ROTATE_ONLY && !pl->rotate_with_bulk) in.mover = pl->rotate_with_tma ? 3 : 1;
+    /* a5 on short segments (the paper's own workload: hundreds of ~130-token chunks per call): a tile
+     * never crosses a segment, so k_rotate_band's one-tile items would fill a fraction of a block's units.  The flat
+     * kernel packs consecutive tiles into full passes instead; it is chosen when that saves a fifth of the items or more
+     * (tuning.rotate_kernel: 1 = never, 3 = always). */
+    if (mode == LEYLINE_ROTATE_ONLY && !pl->rotate_with_bulk && !pl->rotate_with_tma && TR_ROT > 0 && !tiles.empty()) {
+        const int64_t cols = (int64_t)pl->n_heads * (pl->head_chunks / 2);
+        const bool fixed = cols <= 256 && 256 % cols == 0 && leyline::rot_units_per_item(E) % cols == 0 &&
+                           (int64_t)TR_ROT * cols == leyline::rot_units_per_item(E);
+        const int64_t n_passes = (in.rows_rotated + TR_ROT - 1) / TR_ROT;
+        const bool pays = n_passes * 5 <= (int64_t)tiles.size() * 4;
+        if (fixed && tuning.rotate_kernel != 1 && (tuning.rotate_kernel == 3 || pays)) {
+            pl->rotate_flat = true;
+            pl->rot_passes.reserve((size_t)n_passes);
+            int64_t next_start = 0, row0 = 0; /* flat row at which the next pass starts / the current tile starts */
+            for (size_t j = 0; j < tiles.size(); ++j) {
+                const int64_t n = tiles[j].n_rows;
+                for (; next_start < row0 + n; next_start += TR_ROT)
+                    pl->rot_passes.push_back({(int32_t)j, (int32_t)(next_start - row0)});
+                row0 += n;
+            }
+            in.mover = 4;
+        }
+    }
 
     if (!S.dist.empty()) { /* how far back (in tiles) a waiting tile's dependencies sit: a launch hint (sampled) */
         std::nth_element(S.dist.begin(), S.dist.begin() + (long)(S.dist.size() / 2), S.dist.end());

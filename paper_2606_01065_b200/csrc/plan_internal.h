@@ -44,6 +44,15 @@ enum : int32_t { TILE_SRC_REPL = 1, TILE_DST_TOKEN = 2,
 constexpr int kRotUnrollBf16 = LEYLINE_ROT_BF16_UNROLL, kRotUnrollFp8 = 4;
 constexpr int rot_units_per_item(int elem_bytes) { return 256 * (elem_bytes == 2 ? kRotUnrollBf16 : kRotUnrollFp8); }
 
+/* k_rotate_band_flat (a5 when the rotated segments are short): the rows of ALL rotate tiles, in tile order, form one
+ * flat row space; pass b covers flat rows [b * rot_tile_rows, (b + 1) * rot_tile_rows) whatever tiles they fall in.
+ * RotPass says where pass b starts: the tile that holds its first row and that row's offset inside the tile. */
+struct RotPass {
+    int32_t tile;
+    int32_t row_off;
+};
+static_assert(sizeof(RotPass) == 8, "RotPass layout");
+
 /* k_rotate_band_tma (a5 on paged pools): the band of up to kRotTmaBoxRows consecutive slots is one 2-D TMA box. */
 constexpr int kRotTmaBoxRows = 64;
 constexpr bool kRotateTmaByDefault = false; /* decided by measurement */
@@ -83,6 +92,7 @@ struct leyline_plan_s {
     int32_t dep_distance_median = -1;   /* INPLACE_MOVE: median of (tile index - dep_hi) over tiles that wait, -1 if none */
     bool rotate_with_bulk = false;      /* ROTATE_ONLY on a band that is most of the row: the rotation runs on k_move_bulk, in place */
     bool rotate_with_tma = false;       /* ROTATE_ONLY on a narrow band in pages of >= 16 rows: k_rotate_band_tma (2-D TMA boxes) */
+    bool rotate_flat = false;           /* ROTATE_ONLY, narrow band, short segments: k_rotate_band_flat over rot_passes */
     bool use_bulk = false;              /* a3/a4 run on k_move_bulk (TMA bulk copies) instead of k_move_rows */
     leyline_tuning tuning{};
 
@@ -93,6 +103,7 @@ struct leyline_plan_s {
     std::vector<int64_t> seg_begin;     /* segments of request r: [seg_begin[r], seg_begin[r+1]) */
     std::vector<leyline_segment> segments;
     std::vector<leyline::DevTile> tiles;   /* move tiles first, then insert tiles; ticket order */
+    std::vector<leyline::RotPass> rot_passes; /* rotate_flat: start of every block pass in the flat row space of the rotate tiles */
     std::vector<int64_t> trig_shifts;
                                         /* the cos/sin table [n_trig][2][H] of C * theta_i is evaluated in fp64 on the
                                            device by the launch's index kernel (and by the host only for the query) */
@@ -104,7 +115,7 @@ struct leyline_plan_s {
     /* device side (owned by splice.cu; created on first launch, freed by leyline_plan_destroy) */
     void* d_blob = nullptr;             /* tiles | trig (device-computed) | shifts | inv_freq | tabs | slot_runs | page_runs */
     int64_t off_tiles = 0, off_trig = 0, off_shifts = 0, off_inv_freq = 0, off_tabs = 0, off_slot_runs = 0, off_page_runs = 0,
-            blob_bytes = 0;
+            off_rot_passes = 0, blob_bytes = 0;
     void* d_scratch = nullptr;          /* tail of d_blob: [0,256) ticket counters; then hazard flags [n_move_tiles * n_layers] int32 */
     int64_t scratch_bytes = 0;
     int device = -1;

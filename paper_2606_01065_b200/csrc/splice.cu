@@ -164,6 +164,7 @@ leyline_status upload_tables(leyline_plan_s* pl, int dev, cudaStream_t stream) {
     pl->off_tabs = place((int64_t)pl->tabs.size() * sizeof(int32_t));
     pl->off_slot_runs = place((int64_t)pl->slot_runs.size() * sizeof(IdxRun));
     pl->off_page_runs = place((int64_t)pl->page_runs.size() * sizeof(IdxRun));
+    pl->off_rot_passes = place((int64_t)pl->rot_passes.size() * sizeof(leyline::RotPass));
     const int64_t upload_bytes = off > 0 ? off : 256;
     pl->off_trig = place((int64_t)pl->trig_shifts.size() * kTrigParts * (int64_t)pl->inv_freq.size() * sizeof(float)); /* cos, sin: hi and lo parts */
     pl->blob_bytes = off > 0 ? off : 256;
@@ -180,6 +181,7 @@ leyline_status upload_tables(leyline_plan_s* pl, int dev, cudaStream_t stream) {
     put(pl->off_tabs, pl->tabs.data(), pl->tabs.size() * sizeof(int32_t));
     put(pl->off_slot_runs, pl->slot_runs.data(), pl->slot_runs.size() * sizeof(IdxRun));
     put(pl->off_page_runs, pl->page_runs.data(), pl->page_runs.size() * sizeof(IdxRun));
+    put(pl->off_rot_passes, pl->rot_passes.data(), pl->rot_passes.size() * sizeof(leyline::RotPass));
     PlanPool* pp = plan_pool(dev);
     const size_t total = (size_t)(pl->blob_bytes + pl->scratch_bytes);
     const cudaError_t e = pp ? cudaMallocFromPoolAsync(&pl->d_blob, total, pp->pool, stream) : cudaMallocAsync(&pl->d_blob, total, stream);
@@ -299,6 +301,13 @@ MoveKernel pick_rotate(const leyline_plan_s* pl, int pairing) {
     const int cols = pl->n_heads * (pl->head_chunks / 2);
     const bool fixed = cols <= kThreads && kThreads % cols == 0;
     return pl->desc.dtype == LEYLINE_BF16 ? pick_rotate_dt<LEYLINE_BF16>(pairing, fixed) : pick_rotate_dt<LEYLINE_FP8_E4M3>(pairing, fixed);
+}
+/* a5 on short segments (plan.cpp sets rotate_flat only for the FIXED geometry) */
+MoveKernel pick_rotate_flat(const leyline_plan_s* pl, int pairing) {
+    const bool neox = pairing == LEYLINE_ROPE_NEOX;
+    if (pl->desc.dtype == LEYLINE_BF16)
+        return neox ? k_rotate_band_flat<LEYLINE_BF16, LEYLINE_ROPE_NEOX> : k_rotate_band_flat<LEYLINE_BF16, LEYLINE_ROPE_INTERLEAVED>;
+    return neox ? k_rotate_band_flat<LEYLINE_FP8_E4M3, LEYLINE_ROPE_NEOX> : k_rotate_band_flat<LEYLINE_FP8_E4M3, LEYLINE_ROPE_INTERLEAVED>;
 }
 
 }  // namespace
@@ -420,14 +429,33 @@ leyline_status run_tiles(leyline_plan_s* pl, bool hazard, int smem, int max_ctas
 leyline_status run_rotate(leyline_plan_s* pl, int32_t tile_begin, int64_t tile_count, int64_t insert_count,
                           void* const* layer_ptrs, const void* const* layer_repl, cudaStream_t stream, int* ticket_slot) {
     if (tile_count + insert_count <= 0) return LEYLINE_OK;
+    const bool flat = pl->rotate_flat && tile_begin == 0 && tile_count == pl->info.n_move_tiles && tile_count > 0;
     for (const LayerChunk& lc : layer_chunks(pl)) {
-        MoveKernel fn = pick_rotate(pl, lc.pairing);
+        MoveKernel fn = flat ? pick_rotate_flat(pl, lc.pairing) : pick_rotate(pl, lc.pairing);
         MoveParams mp;
         fill_params(pl, mp, tile_begin, tile_count, lc, nullptr, layer_ptrs, layer_repl, *ticket_slot);
         mp.n_copy_items = insert_count * (long long)lc.layers.size();   /* a4 rides in the same launch */
         mp.copy_tile_begin = tile_begin + (int32_t)tile_count;
         const int per_sm = occupancy(reinterpret_cast<const void*>(fn), 0);
         long long grid = (long long)g_dev.sms * per_sm * 8;
+        if (flat) {
+            /* items are (pass, layer): full block passes.  Resident blocks only, each with an equal share of the items, so
+             * that every block's look-ups for item n+1 run under the loads of item n (a block with ONE item has nothing
+             * to hide its tile -> page table -> slot chain behind) */
+            mp.passes = blob_at<leyline::RotPass>(pl, pl->off_rot_passes);
+            mp.n_rot_tiles = (int32_t)tile_count;
+            mp.n_items = (long long)pl->rot_passes.size() * (long long)lc.layers.size();
+#ifndef LEYLINE_FLAT_OVERSUBSCRIBE
+#define LEYLINE_FLAT_OVERSUBSCRIBE 0
+#endif
+            const long long resident = (long long)g_dev.sms * per_sm * (LEYLINE_FLAT_OVERSUBSCRIBE ? LEYLINE_FLAT_OVERSUBSCRIBE : 1);
+            grid = mp.n_items;
+            if (mp.n_items > resident) {
+                const long long share = (mp.n_items + resident - 1) / resident;
+                grid = (mp.n_items + share - 1) / share;
+            }
+            if (grid < 1) grid = 1;
+        }
         const long long most = mp.n_items > mp.n_copy_items ? mp.n_items : mp.n_copy_items;
         if (grid > most) grid = most;
         fn<<<(unsigned)grid, kThreads, 0, stream>>>(mp);

@@ -741,6 +741,76 @@ def test_rotate_only_tma_other_geometries():
         run_and_compare(fuzz_workload(rng), O.ROTATE_ONLY, tuning=TMA, prefetch=bool(rng.integers(0, 2)))
 
 
+FLAT = {"rotate_kernel": 3}
+
+
+def test_rotate_flat_is_chosen_for_short_segments_only():
+    """Auto: the paper's own shape (185 chunks of ~130 tokens, token-level slots) runs on
+    k_rotate_band_flat (plan.info.mover == 4), configs with long segments keep k_rotate_band; rotate_kernel = 1 / 3 force
+    either.  Full size, every layer, whole pools, against the oracle, in each case."""
+    from paper_2606_01065_b200 import binding as B
+    mk = __import__("test_plan_host").make_plan
+    appb = synth.config("appB", pool_factor=2.0)
+    with mk(appb, B.ROTATE_ONLY) as plan:
+        assert plan.info.mover == 4 and plan.info.rot_tile_rows == 384
+    with mk(synth.config(2, pool_factor=1.25), B.ROTATE_ONLY) as plan:
+        assert plan.info.mover == 1
+    for tuning, mover in (({"rotate_kernel": 1}, 1), (FLAT, 4)):
+        B.leyline_set_tuning(**tuning)
+        try:
+            with mk(appb, B.ROTATE_ONLY) as plan:
+                assert plan.info.mover == mover
+            with mk(synth.config(2, pool_factor=1.25), B.ROTATE_ONLY) as plan:
+                assert plan.info.mover == mover
+        finally:
+            B.leyline_set_tuning()
+    run_and_compare(appb, O.ROTATE_ONLY)                       # auto = flat
+    run_and_compare(appb, O.ROTATE_ONLY, tuning={"rotate_kernel": 1})
+    run_and_compare(synth.config(2, pool_factor=1.25), O.ROTATE_ONLY, tuning=FLAT)
+
+
+@pytest.mark.parametrize("cfg", [3, 5])
+def test_rotate_flat_full_size(cfg):
+    """rotate_kernel = 3 on the long-segment configs (bf16: 384-row passes of 4 pair columns; fp8: 512-row passes of 2):
+    passes that start and end inside tiles, every layer, whole pools."""
+    run_and_compare(synth.config(cfg, pool_factor=1.25), O.ROTATE_ONLY, tuning=FLAT)
+
+
+@pytest.mark.parametrize("page", [1, 16, 64])
+@pytest.mark.parametrize("dtype", [synth.DT_BF16, synth.DT_FP8])
+@pytest.mark.parametrize("pairing", [synth.NEOX, synth.INTERLEAVED])
+def test_rotate_flat_ragged(page, dtype, pairing):
+    """Passes that span several short segments with different rotations, a pass that ends behind the last rotated row,
+    several requests, growth and shrink, replacement inserts in the same launch, a request of one token and an empty one."""
+    w = synth.Workload("flat_ragged", 3, [3000, 1, 0, 2777, 150, 97, 260], page, dtype=dtype, pairing=pairing, inv_freq=synth.yarn_inv_freq(),
+                       directives=[(0, 5, 5, 40, 0, 0), (0, 100, 900, 3, 0, 0), (0, 1500, 1501, 333, 0, 0),
+                                   (0, 2990, 3000, 0, 0, 0), (1, 0, 1, 0, 0, 0),
+                                   (3, 0, 17, 500, 0, 0), (3, 1000, 1700, 0, 0, 0), (3, 2776, 2777, 2, 0, 0),
+                                   (4, 0, 30, 0, 0, 0), (5, 3, 3, 9, 0, 0), (6, 10, 20, 0, 0, 0), (6, 100, 101, 7, 0, 0)],
+                       seed=13, pool_factor=3.0, extra_pages=80).finalize()
+    run_and_compare(w, O.ROTATE_ONLY, tuning=FLAT)
+
+
+def test_rotate_flat_other_geometries():
+    """Two heads of 64 behind an MLA latent (8 pair columns), the narrowest band (32 B fp8: one pair column), per-layer
+    pairing (two launches over the same passes), caller-prefilled replacement slots, more layers than one launch
+    holds, and fuzzed workloads."""
+    from paper_2606_01065_b200 import binding as B
+    rng = np.random.default_rng(65)
+    run_and_compare(heads_workload("flat_heads", 2, 64, 512, synth.DT_BF16, synth.NEOX, 1.0e4), O.ROTATE_ONLY, tuning=FLAT)
+    run_and_compare(heads_workload("flat_narrow", 1, 32, 16, synth.DT_FP8, synth.NEOX, 1.0e4), O.ROTATE_ONLY, tuning=FLAT)
+    w = tiny_workload(rng, P=16, n_req=3)
+    w.n_layers = 5
+    w.layer_pairing = [synth.NEOX, synth.INTERLEAVED, synth.INTERLEAVED, synth.NEOX, synth.INTERLEAVED]
+    run_and_compare(w, O.ROTATE_ONLY, tuning=FLAT)
+    run_and_compare(tiny_workload(rng, P=16), O.ROTATE_ONLY, tuning=FLAT, inserts_prefilled=True)
+    w = tiny_workload(rng, P=1, n_req=2)
+    w.n_layers = 130
+    run_and_compare(w, O.ROTATE_ONLY, tuning=FLAT)
+    for _ in range(8):
+        run_and_compare(fuzz_workload(rng), O.ROTATE_ONLY, tuning=FLAT, prefetch=bool(rng.integers(0, 2)))
+
+
 @pytest.mark.parametrize("seed", [101, 202])
 def test_hazard_mover_random_batches_all_layers(seed):
     """More race coverage for k_move_bulk<HAZARD> at full concurrency (148 CTAs, every layer compared, whole pools):
@@ -771,7 +841,8 @@ def _band_by_position(w, cache, idx, n_tok):
 @pytest.mark.parametrize("pairing", [synth.NEOX, synth.INTERLEAVED])
 def test_every_mode_and_mover_stores_the_same_bits(dtype, pairing):
     """One function of (a, b, cos, sin) in every kernel (device_common.cuh, rot_plain / rot_comp): FRESH, INPLACE_MOVE and
-    ROTATE_ONLY, through the bulk mover, the row mover, the strided band kernel and the TMA band kernel, must leave
+    ROTATE_ONLY, through the bulk mover, the row mover, the strided band kernel (tile items and flat passes) and the TMA
+    band kernel, must leave
     bit-identical K_pe at every new position -- not merely results that each sit within tolerance of the oracle."""
     w = synth.Workload("same_bits", 3, [3000, 1, 2777], 16, dtype=dtype, pairing=pairing, inv_freq=synth.yarn_inv_freq(),
                        directives=[(0, 5, 5, 40, 0, 0), (0, 100, 900, 3, 0, 0), (0, 1500, 1501, 333, 0, 0),
@@ -781,7 +852,8 @@ def test_every_mode_and_mover_stores_the_same_bits(dtype, pairing):
     from paper_2606_01065_b200 import harness
     ref = None
     for mode, tuning in ((O.FRESH, {"kernel": 2}), (O.FRESH, {"kernel": 1}), (O.INPLACE_MOVE, {"kernel": 2}),
-                         (O.INPLACE_MOVE, {"kernel": 1}), (O.ROTATE_ONLY, {"rotate_kernel": 1}), (O.ROTATE_ONLY, {"rotate_kernel": 2})):
+                         (O.INPLACE_MOVE, {"kernel": 1}), (O.ROTATE_ONLY, {"rotate_kernel": 1}), (O.ROTATE_ONLY, {"rotate_kernel": 2}),
+                         (O.ROTATE_ONLY, {"rotate_kernel": 3})):
         B.leyline_set_tuning(**tuning)
         try:
             cache = harness.DeviceCache(w, "cuda:0")
@@ -798,7 +870,8 @@ def test_every_mode_and_mover_stores_the_same_bits(dtype, pairing):
 
 
 @pytest.mark.parametrize("mode,tuning", [(O.FRESH, {"kernel": 2}), (O.FRESH, {"kernel": 1}), (O.INPLACE_MOVE, {"kernel": 2}),
-                                         (O.ROTATE_ONLY, {"rotate_kernel": 1}), (O.ROTATE_ONLY, {"rotate_kernel": 2})])
+                                         (O.ROTATE_ONLY, {"rotate_kernel": 1}), (O.ROTATE_ONLY, {"rotate_kernel": 2}),
+                                         (O.ROTATE_ONLY, {"rotate_kernel": 3})])
 @pytest.mark.parametrize("pairing", [synth.NEOX, synth.INTERLEAVED])
 def test_cancelling_pairs_stay_within_one_code(mode, tuning, pairing):
     """Inputs built so that a cos - b sin (or b cos + a sin) nearly cancels in EVERY pair of every downstream row: for the

@@ -568,3 +568,38 @@ def test_tma_rotate_tiles_are_whole_boxes_inside_one_page():
             assert plan.info.mover == 2                                               # wide band: whole rows on the bulk mover
     finally:
         B.leyline_set_tuning()
+
+
+def test_flat_rotate_kernel_is_chosen_by_the_planner_for_short_segments():
+    """k_rotate_band_flat (plan.info.mover == 4) is a host decision: auto picks it when packing the rotate tiles into full
+    block passes saves a fifth of the work items (the paper's App. B shape: 228 tiles -> 62 passes), keeps k_rotate_band on
+    long segments, never overrides the wide-band (bulk) or TMA choice; rotate_kernel = 1 / 3 force either; the tiles,
+    segments and maps of the plan are the same whichever kernel runs them."""
+    appb, cfg2 = synth.config("appB", pool_factor=2.0), synth.config(2, pool_factor=1.25)
+    with make_plan(appb, B.ROTATE_ONLY) as plan:
+        assert plan.info.mover == 4 and plan.info.rot_tile_rows == 384
+        n_passes = -(-int(plan.info.rows_rotated) // 384)
+        assert n_passes * 5 <= int(plan.info.n_move_tiles) * 4
+        auto_tiles = [(t.src_pos, t.dst_pos, t.n_rows, t.trig) for t in plan.tiles]
+    with make_plan(cfg2, B.ROTATE_ONLY) as plan:
+        assert plan.info.mover == 1
+    with make_plan(synth.config(5, pool_factor=1.25), B.ROTATE_ONLY) as plan:
+        assert plan.info.mover == 1 and plan.info.rot_tile_rows == 512
+    for rk, mover in ((1, 1), (3, 4)):
+        B.leyline_set_tuning(rotate_kernel=rk)
+        try:
+            with make_plan(appb, B.ROTATE_ONLY) as plan:
+                assert plan.info.mover == mover
+                assert [(t.src_pos, t.dst_pos, t.n_rows, t.trig) for t in plan.tiles] == auto_tiles
+                assert_plan_equal(plan, oracle_plan(appb, B.ROTATE_ONLY), B.ROTATE_ONLY)
+            with make_plan(cfg2, B.ROTATE_ONLY) as plan:
+                assert plan.info.mover == mover
+            with make_plan(synth.config("gqa", pool_factor=2.0), B.ROTATE_ONLY) as plan:
+                assert plan.info.mover == 2                                           # wide band stays on the bulk mover
+            with make_plan(synth.config(2, pool_factor=2.0), B.FRESH) as plan:
+                assert plan.info.mover == 2                                           # not a ROTATE_ONLY plan: untouched
+        finally:
+            B.leyline_set_tuning()
+    with pytest.raises(B.LeylineError):
+        B.leyline_set_tuning(rotate_kernel=4)
+    B.leyline_set_tuning()
