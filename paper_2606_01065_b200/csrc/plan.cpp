@@ -27,24 +27,6 @@ using leyline::DevTile;
 using leyline::IdxRun;
 using leyline::ReleasedRun;
 
-#ifdef LEYLINE_PLAN_TIMING /* development aid: per-phase wall time of leyline_plan, printed at exit */
-#include <chrono>
-#include <cstdio>
-namespace {
-struct PhaseClock {
-    double acc[8] = {0};
-    std::chrono::steady_clock::time_point t;
-    void start() { t = std::chrono::steady_clock::now(); }
-    void lap(int i) { auto n = std::chrono::steady_clock::now(); acc[i] += std::chrono::duration<double, std::micro>(n - t).count(); t = n; }
-    ~PhaseClock() { for (int i = 0; i < 8; ++i) std::fprintf(stderr, "phase %d: %.0f us total\n", i, acc[i]); }
-} g_phase;
-}
-#define PHASE_START() g_phase.start()
-#define PHASE(i) g_phase.lap(i)
-#else
-#define PHASE_START()
-#define PHASE(i)
-#endif
 
 namespace {
 
@@ -284,7 +266,6 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
                          const int64_t* pt_offsets, const int32_t* pages, int32_t n_directives,
                          const leyline_directive* directives, const int32_t* free_ids, int64_t n_free,
                          const leyline_tuning& tuning, leyline_plan_t** out) {
-    PHASE_START();
     int E = 2, pshift = 0;
     leyline_status st = check_desc(desc, &E, &pshift);
     if (st != LEYLINE_OK) return st;
@@ -324,7 +305,6 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
     if (st != LEYLINE_OK) return st;
     if (tuning.kernel == 1 && !row_kernel_ok(*desc, E)) return LEYLINE_E_UNSUPPORTED; /* forced row kernel on a band it does not cover */
 
-    PHASE(0); /* validation */
     PlanGuard guard{new leyline_plan_s()};
     leyline_plan_s* pl = guard.p;
     take_buffers(pl);
@@ -390,7 +370,6 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
         S.old_tab_off[(size_t)n_requests] = (int32_t)pl->tabs.size();
     }
 
-    PHASE(1); /* plan object, tabs */
     /* Alias rule (after rule V; first failure wins): the kernels write rows in place (INPLACE_MOVE, ROTATE_ONLY) or
      * into consumed free pages (FRESH, growth), so
      *   - a page listed twice, where one of its owners has directives, is refused for the in-place modes (FRESH never
@@ -425,7 +404,6 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
         }
         alias = alias || bad != 0;
     }
-    PHASE(2); /* alias bitmaps */
     pl->old_seq_lens.assign(seq_lens, seq_lens + n_requests);
     pl->new_seq_lens.resize((size_t)n_requests);
     pl->forget_trim.resize((size_t)n_requests);
@@ -528,7 +506,6 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
         }
         pl->new_pt_offsets[(size_t)r + 1] = (int64_t)pl->new_pages.size();
     }
-    PHASE(3); /* pass 1 */
     if (nofree) return LEYLINE_E_NOFREE;
     if (badfree) return LEYLINE_E_RANGE;
     if (mode == LEYLINE_ROTATE_ONLY && check_alias && !alias && S.token_lists.size() > 1) { /* the same free slot handed out twice */
@@ -697,7 +674,6 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
             t.dep_hi = hi;
         }
     }
-    PHASE(4); /* pass 2 */
     if (mode != LEYLINE_ROTATE_ONLY && !pl->new_pages.empty())
         pl->page_runs.push_back({0, (int64_t)pl->new_pages.size(), new_tab_base, 0, 2});
 
@@ -749,7 +725,6 @@ leyline_status plan_impl(const leyline_cache_desc* desc, int32_t mode, int32_t n
         pl->dep_distance_median = S.dist[S.dist.size() / 2];
     }
     tiles.insert(tiles.end(), inserts.begin(), inserts.end());
-    PHASE(5); /* info, insert tiles appended */
     *out = guard.release();
     return LEYLINE_OK;
 }
