@@ -212,8 +212,18 @@ def test_config3m_row_mover_full_size(mode):
     run_and_compare(synth.config("3m", pool_factor=2.0), mode, tuning={"kernel": 1})         # all 61 layers
 
 
+def _release_cached_device_memory():
+    """mem_get_info counts what torch's caching allocator still holds from earlier tests as used: hand it back first, so
+    that "free" means free (without this the 147-GB test took its 12-layer branch whenever it ran behind the 92-GB one)."""
+    import gc
+    gc.collect()
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+
+
 def test_config4_batched_inplace_full_size():
     w = synth.config(4)           # 64 x 16K x 61 layers, one shared pool (~92 GB with the 25 % spare pages)
+    _release_cached_device_memory()
     free, total = torch.cuda.mem_get_info(0)
     if free < w.layer_bytes * w.n_layers * 1.08:
         # a B200 (>= 170 GiB in total) must run this at full size: on such a device a shortage is a failure, not a skip
@@ -226,6 +236,7 @@ def test_config4_batched_fresh_full_size():
     # FRESH on the batched workload needs a second set of pages: 147 GB of pools for all 61 layers, which a 180 GB B200
     # holds; on a smaller or busier device the same plan runs on 12 layers (layers are independent buffers under one plan)
     w = synth.config(4, pool_factor=2.0)
+    _release_cached_device_memory()
     free, total = torch.cuda.mem_get_info(0)
     if free < (w.layer_bytes * (w.n_layers + 1)) * 1.04 + (2 << 30):
         # the 12-layer fallback is for smaller devices only: on a B200 (>= 170 GiB in total) the test fails rather than
