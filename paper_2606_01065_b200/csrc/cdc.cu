@@ -29,6 +29,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <mutex>
 #include <string>
 
 #include "leyline_cdc.h"
@@ -396,6 +397,38 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), unsigned grid, unsigned block, 
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
+/* Scratch of leyline_cdc_chunk comes from a pool of the chunker's own, one per device.  Not the default pool (it hands
+ * its memory back to the driver at every synchronisation: measured 515 -> 124 us per synchronised call), and not the
+ * plan-table pool either: that one forbids internal dependencies so that leyline_plan_prefetch's copy stream never
+ * waits on a user stream, which also means a block freed by a discovery call on a user stream cannot be handed to a
+ * prefetch (or back) -- concurrent discovery and planning kept GROWING it, the 10-40 ms stall its reserve exists to
+ * avoid.  This pool caches up to kCdcPoolKeepBytes between calls (1 M tokens need 16 MB) and trims the rest at the next
+ * synchronisation, so it is bounded. */
+constexpr unsigned long long kCdcPoolKeepBytes = 64ull << 20;
+constexpr int kCdcMaxDevices = 64;
+std::mutex g_cdc_pool_mutex;
+cudaMemPool_t g_cdc_pool[kCdcMaxDevices] = {};
+
+cudaMemPool_t cdc_pool_on_current_device() {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kCdcMaxDevices) { (void)cudaGetLastError(); return nullptr; }
+    std::lock_guard<std::mutex> lock(g_cdc_pool_mutex);
+    if (!g_cdc_pool[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        if (cudaMemPoolCreate(&pool, &props) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+        unsigned long long keep = kCdcPoolKeepBytes;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        (void)cudaGetLastError();
+        g_cdc_pool[dev] = pool;
+    }
+    return g_cdc_pool[dev];
+}
+
 unsigned grid_for(int64_t n, int per_block = kT) {
     int64_t b = (n + per_block - 1) / per_block;
     if (b < 1) b = 1;
@@ -439,9 +472,8 @@ extern "C" LEYLINE_API leyline_status leyline_cdc_chunk(const leyline_cdc_params
                   o_c1 = o_h1 + up((n_super + 1) * 4), o_prog = o_c1 + up((n_super + 1) * 4), o_flags = o_prog + up(n_counters * 4),
                   o_kind = o_flags + up(n + 1), o_mark = o_kind + up(n + 1), total = o_mark + up(n + 1);
     uint8_t* ws = nullptr;
-    /* from the library's own pool: the default pool hands its memory back to the driver at every synchronisation, and the
-     * next call would pay for mapping it again (measured: one synchronised call 515 -> 124 us) */
-    if (cudaMemPool_t pool = static_cast<cudaMemPool_t>(leyline::scratch_mem_pool()))
+    /* from the chunker's own pool (cdc_pool_on_current_device above); the default pool only if that cannot be created */
+    if (cudaMemPool_t pool = cdc_pool_on_current_device())
         CU(cudaMallocFromPoolAsync(reinterpret_cast<void**>(&ws), (size_t)total, pool, stream));
     else
         CU(cudaMallocAsync(reinterpret_cast<void**>(&ws), (size_t)total, stream));
@@ -525,8 +557,6 @@ extern "C" LEYLINE_API leyline_status leyline_registry_lookup(const uint64_t* de
  * The launch chain is the one leyline_cdc_chunk runs (same kernels, same order, same arguments); only where the scratch
  * lives differs.  It is written out again here rather than shared so that the allocating path stays as it was.
  * =================================================================================================================== */
-
-#include <mutex>
 
 constexpr size_t kNoAllocScratchBytes = size_t(8) << 20;
 /* File-scope device array.  In HOST code this name is only a handle the runtime knows the symbol by, not a device

@@ -135,9 +135,6 @@ struct leyline_plan_s {
 namespace leyline {
 /* implemented in splice.cu; plan.cpp calls it from leyline_plan_destroy (not part of the ABI, not exported) */
 void plan_release_device(leyline_plan_s* plan);
-/* the library's own stream-ordered memory pool on the current device (a cudaMemPool_t; it keeps what is freed into it,
- * so that a call's scratch is not handed back to the driver at every synchronisation), or nullptr */
-void* scratch_mem_pool();
 }  // namespace leyline
 
 #endif /* LEYLINE_PLAN_INTERNAL_H_ */

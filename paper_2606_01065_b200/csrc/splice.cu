@@ -45,6 +45,11 @@ std::mutex g_pin_mu;
 std::vector<PinnedBuf> g_pin_pool;
 constexpr size_t kPinMinBytes = 256 << 10, kPinMaxPooled = 32;
 constexpr int kPinPrefill = 5;
+/* The pool is bounded in BYTES as well as in buffers: only small size classes are stocked ahead (a plan with tens of MB
+ * of tables would otherwise pin six times that in one call, six device-stalling cudaHostAlloc calls back to back), the
+ * pool keeps at most kPinMaxPooledBytes, and a buffer of more than kPinMaxKeptCap is freed when its copy is done. */
+constexpr size_t kPinPrefillMaxCap = size_t(4) << 20, kPinMaxPooledBytes = size_t(256) << 20, kPinMaxKeptCap = size_t(64) << 20;
+size_t g_pin_pool_bytes = 0; /* sum of cap over g_pin_pool, under g_pin_mu */
 
 PinnedBuf pin_acquire(size_t bytes, int dev) {
     {
@@ -53,6 +58,7 @@ PinnedBuf pin_acquire(size_t bytes, int dev) {
             PinnedBuf b = g_pin_pool[i];
             if (b.cap >= bytes && b.device == dev && cudaEventQuery(b.ev) == cudaSuccess) {
                 g_pin_pool.erase(g_pin_pool.begin() + (long)i);
+                g_pin_pool_bytes -= b.cap;
                 return b;
             }
         }
@@ -76,20 +82,32 @@ PinnedBuf pin_acquire(size_t bytes, int dev) {
     if (!make(b)) return PinnedBuf{}; /* caller falls back to a pageable source */
     /* cudaHostAlloc waits for the device and takes milliseconds: when this size class runs dry, stock it for the calls
      * that follow (a server keeps a few plans in flight), so that the stall is paid once, not once per concurrent plan */
-    for (int extra = 0; extra < kPinPrefill; ++extra) {
+    for (int extra = 0; extra < kPinPrefill && cap <= kPinPrefillMaxCap; ++extra) {
         PinnedBuf e;
         if (!make(e)) break;
         std::lock_guard<std::mutex> lk(g_pin_mu);
-        if (g_pin_pool.size() >= kPinMaxPooled) { cudaEventDestroy(e.ev); cudaFreeHost(e.p); break; }
+        if (g_pin_pool.size() >= kPinMaxPooled || g_pin_pool_bytes + cap > kPinMaxPooledBytes) {
+            cudaEventDestroy(e.ev);
+            cudaFreeHost(e.p);
+            break;
+        }
         g_pin_pool.push_back(e);
+        g_pin_pool_bytes += cap;
     }
     return b;
 }
 
 void pin_release(PinnedBuf b, cudaStream_t stream) {
     cudaEventRecord(b.ev, stream);
-    std::lock_guard<std::mutex> lk(g_pin_mu);
-    if (g_pin_pool.size() < kPinMaxPooled) { g_pin_pool.push_back(b); return; }
+    {
+        std::lock_guard<std::mutex> lk(g_pin_mu);
+        if (g_pin_pool.size() < kPinMaxPooled && b.cap <= kPinMaxKeptCap && g_pin_pool_bytes + b.cap <= kPinMaxPooledBytes) {
+            g_pin_pool.push_back(b);
+            g_pin_pool_bytes += b.cap;
+            return;
+        }
+    }
+    /* over the bound, or an oversized buffer: freed once its copy has finished (outside the lock) */
     cudaEventSynchronize(b.ev);
     cudaEventDestroy(b.ev);
     cudaFreeHost(b.p);
@@ -811,13 +829,6 @@ extern "C" LEYLINE_API leyline_status leyline_probe_band_update(void* dev_buf, i
     CU(cudaGetLastError());
     return LEYLINE_OK;
 } LEYLINE_CATCH_STATUS
-
-void* leyline::scratch_mem_pool() {
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
-    PlanPool* pp = plan_pool(dev);
-    return pp ? static_cast<void*>(pp->pool) : nullptr;
-}
 
 void leyline::plan_release_device(leyline_plan_s* pl) {
     if (pl->ev_start) cudaEventDestroy(static_cast<cudaEvent_t>(pl->ev_start));
